@@ -1,0 +1,343 @@
+"""Pins of oracle/frs_oracle.py against what the paper and the mathematics fix (CPU only).
+
+Each test names the passage / reading it pins (P:<n> = PAPER.md line n; R<k> = DESIGN.md reading k).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from gen import workloads as wl
+from oracle import frs_oracle as o
+
+
+def rel(a, b):
+    return np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b)
+
+
+@pytest.fixture(scope="module")
+def small():
+    """config-1 recipe at 16x16 (brute-force size)."""
+    return wl.make_config(1, n=16, npts=4000)
+
+
+@pytest.fixture(scope="module")
+def rect():
+    """config-3 recipe on a 16x32 rectangle (ny != nx catches transposed operands)."""
+    return wl.make_config(3, ny=16, nx=32, npts=6000)
+
+
+@pytest.fixture(scope="module")
+def multi():
+    """config-5 recipe, 3 channels of 16x16, two latent fields."""
+    return wl.make_config(5, n=16, nchan=3, npts=5000)
+
+
+# ------------------------------------------------------------------ library FFT vs the definition
+@pytest.mark.parametrize("n", [1, 2, 3, 8, 16, 64])
+def test_fft_is_the_dft_definition(n):
+    rng = np.random.default_rng(n)
+    x = rng.normal(size=n) + 1j * rng.normal(size=n)
+    assert rel(np.fft.fft(x), o.dft_naive(x)) < 1e-12 if n > 1 else True
+    assert np.allclose(np.fft.ifft(x) * n, o.dft_naive(x, +1), atol=1e-12)
+    assert np.allclose(o.dft_naive(o.dft_naive(x), +1), n * x, atol=1e-10)          # inverse o forward = n id
+    assert np.isclose(np.sum(np.abs(o.dft_naive(x)) ** 2), n * np.sum(np.abs(x) ** 2))  # Parseval
+
+
+def test_fft2_and_rfft2_are_the_2d_definition():
+    rng = np.random.default_rng(0)
+    x = rng.normal(size=(8, 16))
+    f = o.dft2_naive(x)
+    assert rel(np.fft.fft2(x), f) < 1e-12
+    assert rel(np.fft.rfft2(x), f[:, :9]) < 1e-12
+    assert rel(np.fft.irfft2(f[:, :9], s=x.shape) * x.size, np.real(o.dft2_naive(f, +1))) < 1e-12
+
+
+# ------------------------------------------------------------------ Eq. 14, R2, R3
+def test_golden_hand_worked_2x2(golden_dir):
+    rows = [l for l in open(os.path.join(golden_dir, "hand_conv_2x2.txt")) if not l.startswith("#")]
+    img = np.array([rows[0].split(), rows[1].split()], float)
+    exp = np.array([rows[2].split(), rows[3].split()], float)
+    w_half = np.zeros((4, 3))
+    w_half[0, 1] = 1.0                       # W[0][1] (and, by Hermitian symmetry, W[0][3])
+    assert np.allclose(o.psf_from_weights(w_half)[0], [2, 0, -2, 0], atol=1e-14)
+    assert np.allclose(o.psf_apply(w_half, img), exp, atol=1e-13)
+    assert np.isclose(np.sum(img * o.psf_apply(w_half, img)), float(rows[4]))
+    assert np.isclose(o.quadratic_form_spectral(w_half, img), float(rows[4]))
+
+
+def test_convolution_theorem_vs_direct_sum_16(small, rect):
+    """padded FFT convolution == O(N^4) linear convolution with the 2N PSF."""
+    for w in (small, rect):
+        rng = np.random.default_rng(1)
+        x = rng.normal(size=(w.ny, w.nx))
+        wh = w.w_half[0].astype(np.float64)
+        psf = o.psf_from_weights(wh)
+        ref = o.conv_direct(psf, x)
+        assert rel(o.psf_apply(wh, x), ref) < 1e-12
+        assert rel(o.psf_apply_full(wh, x), ref) < 1e-12
+
+
+def test_psf_peak_is_sum_of_weights(small, rect):
+    for w in (small, rect):
+        wh = w.w_half[0].astype(np.float64)
+        psf = o.psf_from_weights(wh)
+        tot = np.sum(o.full_spectrum(wh))
+        assert np.isclose(psf[0, 0], tot, rtol=1e-13)
+        assert np.all(np.abs(psf) <= psf[0, 0] * (1 + 1e-12))
+        assert np.isclose(psf[0, 0], np.max(psf))
+
+
+def test_special_kernels_closed_forms():
+    ny, nx = 8, 16
+    my, mx = 2 * ny, 2 * nx
+    rng = np.random.default_rng(2)
+    x = rng.normal(size=(ny, nx))
+    # W == c  =>  C = c My Mx identity
+    assert rel(o.psf_apply(np.full((my, nx + 1), 0.25), x), 0.25 * my * mx * x) < 1e-13
+    # one +-k0 pair  =>  psf = 2 w cos(2 pi k0.x/M)
+    wh = np.zeros((my, nx + 1))
+    wh[3, 5] = 0.7
+    wh[my - 3, 5] = 0.0                       # (-k0 lives at [my-3][mx-5], outside the half grid)
+    yy, xx = np.mgrid[0:my, 0:mx]
+    assert np.allclose(o.psf_from_weights(wh), 2 * 0.7 * np.cos(2 * np.pi * (3 * yy / my + 5 * xx / mx)), atol=1e-12)
+    # s = delta_{x0}  =>  C s = psf[x - x0] cropped; corners exercise the wrapped half
+    w = wl.make_config(2, ny=ny, nx=nx, npts=3000)
+    wh = w.w_half[0].astype(np.float64)
+    psf = o.psf_from_weights(wh)
+    for (y0, x0) in [(0, 0), (0, nx - 1), (ny - 1, 0), (ny - 1, nx - 1), (3, 7)]:
+        d = np.zeros((ny, nx))
+        d[y0, x0] = 1.0
+        exp = np.array([[psf[(y - y0) % my, (xq - x0) % mx] for xq in range(nx)] for y in range(ny)])
+        got = o.psf_apply(wh, d)
+        assert np.allclose(got, exp, atol=1e-9 * psf[0, 0])
+        assert np.unravel_index(np.argmax(got), got.shape) == (y0, x0)      # index/padding layout, exact
+
+
+def test_quadratic_form_independent_route(small, rect):
+    for w in (small, rect):
+        x = np.random.default_rng(3).normal(size=(w.ny, w.nx))
+        wh = w.w_half[0].astype(np.float64)
+        q = float(np.sum(x * o.psf_apply(wh, x)))
+        assert q >= 0
+        assert np.isclose(q, o.quadratic_form_spectral(wh, x), rtol=1e-12)
+
+
+def test_pruned_even_odd_identity():
+    """Zero-padded N->2N transform: even bins = FFT_N(x), odd bins = FFT_N(x w_2N^n); the cropped
+    inverse is y[n] = (IFFT_N(Y_even) + w_2N^-n IFFT_N(Y_odd))/2 -- lets the GPU prune while the
+    oracle stays plain."""
+    n = 32
+    rng = np.random.default_rng(4)
+    x = rng.normal(size=n) + 1j * rng.normal(size=n)
+    full = np.fft.fft(np.concatenate([x, np.zeros(n)]))
+    tw = np.exp(-2j * np.pi * np.arange(n) / (2 * n))
+    assert rel(full[0::2], np.fft.fft(x)) < 1e-14
+    assert rel(full[1::2], np.fft.fft(x * tw)) < 1e-14
+    y = rng.normal(size=2 * n) + 1j * rng.normal(size=2 * n)
+    exp = np.fft.ifft(y)[:n]
+    got = 0.5 * (np.fft.ifft(y[0::2]) + np.conj(tw) * np.fft.ifft(y[1::2]))
+    assert rel(got, exp) < 1e-14
+
+
+# ------------------------------------------------------------------ symmetry / adjointness to 1e-12
+def test_adjointness(small, rect, multi):
+    rng = np.random.default_rng(5)
+    for w in (small, rect):
+        wh = w.w_half[0].astype(np.float64)
+        x, y = rng.normal(size=(2, w.ny, w.nx))
+        a, b = np.sum(o.psf_apply(wh, x) * y), np.sum(x * o.psf_apply(wh, y))
+        assert abs(a - b) <= 1e-12 * max(abs(a), abs(b))
+        a, b = np.sum(o.hartley2(x) * y), np.sum(x * o.hartley2(y))
+        assert abs(a - b) <= 1e-12 * np.linalg.norm(o.hartley2(x)) * np.linalg.norm(y)
+        big = rng.normal(size=(2 * w.ny, 2 * w.nx))
+        assert np.isclose(np.sum(o.pad(x) * big), np.sum(x * o.crop(big)), rtol=1e-13)
+    for w in (small, multi):
+        xi = rng.normal(size=(w.nfield, w.ny, w.nx))
+        v = rng.normal(size=(w.nfield, w.ny, w.nx))
+        u = rng.normal(size=(w.nchan, w.ny, w.nx))
+        s = o.sky(xi, w.amp, w.mu, w.lognu)
+        a = np.sum(o.jvp(w.amp, w.mu, w.lognu, xi, v) * u)
+        b = np.sum(v * o.vjp(w.amp.astype(np.float64), w.lognu, s, u))
+        assert abs(a - b) <= 1e-12 * max(abs(a), abs(b), 1.0) * 10
+
+
+def test_generated_weights_are_hermitian_and_integer(small, rect, multi):
+    for w in (small, rect, multi):
+        for c in range(w.nchan):
+            full = o.full_spectrum(w.w_counts[c])
+            my, mx = full.shape
+            ky, kx = (-np.arange(my)) % my, (-np.arange(mx)) % mx
+            assert np.array_equal(full, full[np.ix_(ky, kx)])           # W[-k] = W[k], bit-exact
+            assert np.array_equal(full, np.rint(full)) and full.min() >= 0
+            assert np.array_equal(full[:, : w.nx + 1], w.w_counts[c])   # half-grid round trip
+            # the self-conjugate columns kx = 0 and kx = nx are even in ky
+            for col in (0, w.nx):
+                assert np.array_equal(w.w_counts[c][:, col], w.w_counts[c][ky, col])
+
+
+def test_set_psf_semantics(small):
+    wh = small.w_half[0].astype(np.float64)
+    psf = o.psf_from_weights(wh)
+    back, ok = o.psf_spectrum_from_psf(psf)
+    assert ok and rel(back, wh) < 1e-12
+    bad = psf.copy()
+    bad[1, 2] += 0.3 * psf[0, 0]              # breaks evenness -> imaginary spectrum
+    assert not o.psf_spectrum_from_psf(bad)[1]
+
+
+# ------------------------------------------------------------------ correlated field (R6)
+def test_hartley_closed_forms():
+    ny, nx = 8, 16
+    rng = np.random.default_rng(6)
+    z = rng.normal(size=(ny, nx))
+    assert rel(o.hartley2(o.hartley2(z)), ny * nx * z) < 1e-13
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    for (ky, kx) in [(0, 0), (1, 0), (3, 5), (7, 15), (4, 8)]:
+        d = np.zeros((ny, nx))
+        d[ky, kx] = 1.0
+        th = 2 * np.pi * (ky * yy / ny + kx * xx / nx)
+        assert np.allclose(o.hartley2(d), np.cos(th) + np.sin(th), atol=1e-12)
+    # definition written out as the O(N^4) sum
+    kyy, kxx = np.mgrid[0:ny, 0:nx]
+    brute = np.array([[np.sum(z * (np.cos(2 * np.pi * (kyy * y / ny + kxx * x / nx))
+                                   + np.sin(2 * np.pi * (kyy * y / ny + kxx * x / nx))))
+                       for x in range(nx)] for y in range(ny)])
+    assert rel(o.hartley2(z), brute) < 1e-12
+
+
+def test_field_variance_is_sum_of_A_squared():
+    """Var(lin[x]) = sum_k A[k]^2 at every pixel, exact for even A (R6)."""
+    ny, nx = 8, 16
+    a = wl.amplitude_spectrum(ny, nx, "lorentz4", 1.0)
+    kyi, kxi = (-np.arange(ny)) % ny, (-np.arange(nx)) % nx
+    assert np.array_equal(a, a[np.ix_(kyi, kxi)])                       # A[-k] = A[k]
+    assert np.isclose(np.sum(a ** 2) - a[0, 0] ** 2, 1.0)
+    # exact: Var = sum_k A_k^2 cas^2 = sum A^2 (1 + sin 2 theta), and the sine term cancels k <-> -k
+    yy, xx = 3, 11
+    kyy, kxx = np.mgrid[0:ny, 0:nx]
+    th = 2 * np.pi * (kyy * yy / ny + kxx * xx / nx)
+    assert np.isclose(np.sum(a ** 2 * (np.cos(th) + np.sin(th)) ** 2), np.sum(a ** 2), rtol=1e-12)
+    rng = np.random.default_rng(7)
+    draws = np.stack([o.hartley2(a * rng.normal(size=(ny, nx))) for _ in range(4000)])
+    assert abs(draws.var() / np.sum(a ** 2) - 1.0) < 0.02
+
+
+# ------------------------------------------------------------------ gradient / JVP vs central differences (1e-6)
+@pytest.mark.parametrize("which", ["small", "multi"])
+def test_gradient_and_jvp_vs_finite_differences(which, small, multi):
+    w = small if which == "small" else multi
+    rng = np.random.default_rng(8)
+    xi = 0.3 * rng.normal(size=(w.nfield, w.ny, w.nx))
+    args = (w.w_half, w.dirty, w.amp, w.mu, w.lognu)
+    e, g = o.energy_grad(*args, xi, True)
+    assert np.isclose(e, o.energy(*args, xi, True), rtol=1e-13)
+    h = 1e-5 * np.linalg.norm(xi)
+    for _ in range(10):
+        d = rng.normal(size=xi.shape)
+        d /= np.linalg.norm(d)
+        fd = (o.energy(*args, xi + h * d, True) - o.energy(*args, xi - h * d, True)) / (2 * h)
+        an = np.sum(g * d)
+        assert abs(fd - an) <= 1e-6 * max(abs(an), np.linalg.norm(g) * 1e-2)
+    v = rng.normal(size=xi.shape)
+    hh = 1e-6
+    fd = (o.sky(xi + hh * v, w.amp, w.mu, w.lognu) - o.sky(xi - hh * v, w.amp, w.mu, w.lognu)) / (2 * hh)
+    assert rel(fd, o.jvp(w.amp, w.mu, w.lognu, xi, v)) < 1e-6
+
+
+# ------------------------------------------------------------------ metric (Eq. 10)
+@pytest.mark.parametrize("which", ["small", "multi"])
+def test_metric_invariants(which, small, multi):
+    w = small if which == "small" else multi
+    rng = np.random.default_rng(9)
+    xi = 0.3 * rng.normal(size=(w.nfield, w.ny, w.nx))
+    u, v = rng.normal(size=(2, w.nfield, w.ny, w.nx))
+    mv = o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, v, True)
+    mu_ = o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, u, True)
+    a, b = np.sum(u * mv), np.sum(mu_ * v)
+    assert abs(a - b) <= 1e-12 * max(abs(a), abs(b)) * 10              # symmetric
+    assert np.sum(v * mv) >= np.sum(v * v)                              # M >= identity
+    # composition J^T (C (J v)) + v written out step by step
+    s = o.sky(xi, w.amp, w.mu, w.lognu)
+    jv = o.jvp(w.amp, w.mu, w.lognu, xi, v)
+    cj = np.stack([o.psf_apply(w.w_half[c], jv[c]) for c in range(w.nchan)])
+    assert rel(mv, o.vjp(w.amp.astype(np.float64), w.lognu, s, cj) + v) < 1e-13
+    # the sky-space ('L1') apply is the same thing without the Hartley maps
+    x = rng.normal(size=(w.nchan, w.ny, w.nx))
+    l1 = o.sky_metric_apply(w.w_half, s, x)
+    assert rel(l1[0], s[0] * o.psf_apply(w.w_half[0], s[0] * x[0])) < 1e-14
+
+
+def test_fisher_identity_monte_carlo():
+    """E_n[(J^T n)(J^T n)^T v] -> M_lh v for n ~ N(0, C): data noise (generator), energy and metric
+    are mutually consistent (Eq. 10)."""
+    n = 8
+    w = wl.make_config(1, n=n, npts=3000, sigma_rel=0.1)
+    wh = w.w_half[0].astype(np.float64)
+    rng = np.random.default_rng(10)
+    xi = 0.2 * rng.normal(size=(1, n, n))
+    v = rng.normal(size=(1, n, n))
+    s = o.sky(xi, w.amp, w.mu, w.lognu)
+    m_lh = o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, v, False)
+    wfull = o.full_spectrum(wh)
+    acc = np.zeros_like(v)
+    ndraw = 6000
+    for _ in range(ndraw):
+        eta = rng.normal(size=(2 * n, 2 * n))
+        noise = o.crop(np.real(np.fft.ifft2(np.sqrt(wfull) * np.fft.fft2(eta))) * (2 * n))   # Cov = C
+        jn = o.vjp(w.amp.astype(np.float64), w.lognu, s, noise[None])
+        acc += jn * np.sum(jn * v)
+    assert rel(acc / ndraw, m_lh) < 0.12                                   # ~ a few / sqrt(ndraw)
+
+
+def test_noise_scale_of_generator():
+    """std(n')/max(C s*) = sigma_rel and Var(n'[x]) = sum W (R7): check sum W against w0."""
+    w = wl.make_config(1, n=32, npts=8000, sigma_rel=1e-3)
+    wh = w.w_half[0].astype(np.float64)
+    sig = o.psf_apply(wh, w.sky_true[0])
+    var = np.sum(o.full_spectrum(wh))
+    assert np.isclose(np.sqrt(var) / sig.max(), 1e-3, rtol=2e-3)
+    resid = w.dirty[0] - sig
+    assert 0.5 < resid.std() / np.sqrt(var) < 1.5
+
+
+# ------------------------------------------------------------------ CG (R9)
+def test_cg_reaches_dense_solve_and_phi_decreases():
+    n = 8
+    w = wl.make_config(1, n=n, npts=3000, sigma_rel=0.05)
+    rng = np.random.default_rng(11)
+    xi = 0.2 * rng.normal(size=(1, n, n))
+    s = o.sky(xi, w.amp, w.mu, w.lognu)
+    ap = lambda v: o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, v, True, s=s)
+    dense = np.stack([ap(e.reshape(1, n, n)).ravel() for e in np.eye(n * n)], axis=1)
+    assert np.allclose(dense, dense.T, rtol=1e-11, atol=1e-11 * np.abs(dense).max())
+    assert np.linalg.eigvalsh(0.5 * (dense + dense.T)).min() >= 1 - 1e-9
+    b = rng.normal(size=(1, n, n))
+    exact = np.linalg.solve(dense, b.ravel()).reshape(1, n, n)
+    sol = o.cg(ap, b, max_iter=4 * n * n, rtol=1e-13, keep=True)
+    assert rel(sol["x"], exact) < 1e-10
+    phi = [0.5 * np.sum(x * ap(x)) - np.sum(b * x) for x in sol["xs"]]
+    assert all(p1 < p0 + 1e-9 * abs(p0) for p0, p1 in zip([0.0] + phi[:-1], phi))    # phi strictly decreases
+    assert sol["res"][-1] < sol["res"][0]
+    # teacher-forced step == the loop's own step
+    st = o.cg_step(ap, np.zeros_like(b), b.copy(), b.copy(), float(np.sum(b * b)))
+    assert rel(st["x"], sol["xs"][0]) < 1e-14
+
+
+def test_cg_on_config1_recipe_residual_decreases_and_envelope_grows():
+    w = wl.make_config(1, n=32, npts=6000)
+    xi = np.zeros((1, 32, 32))
+    e, g = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, True)
+    s = o.sky(xi, w.amp, w.mu, w.lognu)
+    ap = lambda v: o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, v, True, s=s)
+    sol = o.cg(ap, -g, max_iter=20)
+    assert sol["iters"] == 20 and sol["res"][-1] < sol["res"][0]
+    env = o.cg_fp32_envelope(ap, -g, max_iter=20)
+    assert env[0] < 1e-6 and env[-1] >= env[0]
+
+
+def test_newton_cg_step_decreases_energy():
+    w = wl.make_config(2, n=16, npts=3000, sigma_rel=0.05)
+    xi = np.zeros((1, 16, 16))
+    xi1, e0, e1 = o.newton_cg_step(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, cg_iters=30)
+    assert e1 < e0
