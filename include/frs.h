@@ -1,0 +1,131 @@
+/* frs.h -- C ABI of the fast-resolve hot path on B200 (sm_100a).
+ *
+ * The library evaluates the PSF-convolution likelihood of fast-resolve (arXiv 2406.09144),
+ *     E(s) = 1/2 s^T (PSF * s) - j^T s,        s = exp(correlated field),
+ * its gradient and its Fisher-metric-vector product, and solves M x = b by conjugate gradients.
+ * Citations `P:<n>` are lines of the paper text; `R<k>` are the
+ * readings listed in DESIGN.md for points the paper leaves open.
+ *
+ * Conventions (all calls)
+ *   - frs_ctx owns the PSF spectrum, dirty image, amplitude spectra, the cached sky of the current
+ *     position and all scratch.  The caller owns every array it passes; set_* calls COPY.
+ *   - Unless a name ends in `_host`, array arguments are DEVICE pointers to contiguous float32,
+ *     16-byte aligned, on the ctx's device.  Scalars documented "host" are host pointers.
+ *   - Layout: images [nchan][ny][nx] row-major (x fastest); latent arrays [nfield][ny][nx] indexed
+ *     by harmonic mode (ky, kx) in DFT order; PSF half spectrum [nchan][2ny][nx+1].
+ *   - Calls enqueue work on the ctx's stream and return; they synchronise only where a host output
+ *     is requested (documented per call).  One ctx per stream; a ctx is not thread-safe.
+ *   - Input and output arrays of one call must not overlap unless stated.
+ *   - Return value: 0 on success, a negative FRS_E* code otherwise.  No exceptions cross the ABI.
+ *   - ny, nx: powers of two in [32, 4096]; nchan >= 1; nfield in {1, 2}.
+ */
+#ifndef FRS_H
+#define FRS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct frs_ctx frs_ctx;
+
+#define FRS_OK 0
+#define FRS_EINVAL (-1)     /* bad size, NULL or misaligned pointer */
+#define FRS_ESTATE (-2)     /* call order: e.g. metric_apply before a position / PSF was set */
+#define FRS_ENOTPSD (-3)    /* PSF spectrum has a significant negative or imaginary part */
+#define FRS_ECUDA (-4)      /* CUDA runtime error; text via frs_last_error */
+#define FRS_EBREAKDOWN (-5) /* CG met <p, M p> <= 0 */
+
+/* Create a context for images of ny x nx pixels, nchan frequency channels, on CUDA device `device`,
+ * enqueuing on `stream` (a cudaStream_t; NULL = the legacy default stream).  The number of latent
+ * fields is fixed later by frs_set_amplitude.  Allocates all tables; scratch is allocated lazily. */
+int frs_create(int ny, int nx, int nchan, int device, void* stream, frs_ctx** out);
+void frs_destroy(frs_ctx* ctx);
+/* Text of the last error of this ctx (never NULL; owned by the ctx). */
+const char* frs_last_error(const frs_ctx* ctx);
+/* Library version / build string (static storage). */
+const char* frs_version(void);
+
+/* ---- setup (untimed) ---------------------------------------------------------------------- */
+
+/* PSF given in image space: psf [nchan][2ny][2nx], origin at [0][0], negative offsets wrapped
+ * (R2).  Computes W = DFT(psf)/(4 ny nx) with a direct O(M^2 log M) transform on the device and
+ * requires max|Im W| <= 1e-5 max W and min Re W >= -1e-5 max W, else FRS_ENOTPSD (R4; P:191:
+ * a covariance kernel must be real and positive).  Stores max(Re W, 0).  Synchronises. */
+int frs_set_psf(frs_ctx* ctx, const float* psf);
+/* PSF given as its real, non-negative half spectrum W [nchan][2ny][nx+1] (the gridded, Hermitian-
+ * symmetrised visibility weights; P:180 'FFT[I^PSF]', R3: (C x)[n] = sum_k W[k] xhat[k] e^{+2 pi i k.n/M},
+ * so the PSF peak equals sum W).  Negative entries -> FRS_ENOTPSD.  Synchronises. */
+int frs_set_psf_weights(frs_ctx* ctx, const float* w_half);
+/* Dirty image j = I^D [nchan][ny][nx]  (Eq. 6, Eq. 8).  For major cycles pass
+ * j_eff = d_i + C s_{i-1} (Eq. 21, R13). */
+int frs_set_dirty(frs_ctx* ctx, const float* j);
+/* Correlated-field model (R6): amplitude spectra A [nfield][ny][nx] (real >= 0, even in k) and
+ * offsets mu [nfield] (HOST pointer).  nfield = 1: s = exp(mu + H[A xi]);  nfield = 2:
+ * s_c = exp(tau_0 + lognu_c tau_1).  Invalidates the cached position. */
+int frs_set_amplitude(frs_ctx* ctx, int nfield, const float* amp, const float* mu_host);
+/* ln(nu_c / nu_0) per channel, HOST pointer [nchan]; only used when nfield == 2. */
+int frs_set_channel_lognu(frs_ctx* ctx, const float* lognu_host);
+
+/* ---- hot path -------------------------------------------------------------------------------- */
+
+/* s = exp(correlated field of xi): sets the position, caches s inside the ctx and, if `sky` is
+ * not NULL, also writes it there [nchan][ny][nx]  (R6). */
+int frs_sky_forward(frs_ctx* ctx, const float* xi, float* sky);
+/* y = C x: zero-pad, FFT, multiply by W, inverse FFT, crop (Eq. 14). x, y [nchan][ny][nx]. */
+int frs_psf_apply(frs_ctx* ctx, const float* x, float* y);
+/* 'L1 apply', the headline operator: y = s . C (s . x) at the cached position -- the likelihood
+ * Fisher metric in log-sky coordinates (Eq. 10, R8).  Needs a prior frs_sky_forward /
+ * frs_energy_grad / frs_set_sky. */
+int frs_sky_metric_apply(frs_ctx* ctx, const float* x, float* y);
+/* Set the cached sky directly (copy), bypassing the correlated-field model. */
+int frs_set_sky(frs_ctx* ctx, const float* sky);
+/* E = sum_c 1/2 <s_c, C_c s_c> - <j_c, s_c> (+ 1/2 <xi, xi> if with_prior) and its gradient
+ * grad [nfield][ny][nx] = J^T (C s - j) (+ xi)   (Eq. 9 with N' = R', R1, R8).
+ * d_energy: device double (may be NULL); h_energy: host double (may be NULL; non-NULL makes the
+ * call synchronise).  Sets the position to xi. */
+int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_energy, double* h_energy, float* grad);
+/* 'L2 apply': out = J^T C J v (+ v if with_prior) at the cached position -- the MGVI metric
+ * (R8).  v, out [nfield][ny][nx]. */
+int frs_metric_apply(frs_ctx* ctx, const float* v, int with_prior, float* out);
+/* Solve M x = b by textbook CG (R9).  x: in = x0, out = solution.  Runs until max_iter or
+ * ||r|| <= rtol ||b|| (rtol = 0: exactly max_iter iterations, fully asynchronous until the end).
+ * h_iters (host, may be NULL): iterations done.  h_resnorm (host, may be NULL): final ||r||.
+ * d_res_history (DEVICE double [max_iter+1], may be NULL): ||r_k||.  Synchronises at the end. */
+int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior,
+                 int* h_iters, double* h_resnorm, double* d_res_history);
+/* CG state of the last frs_cg_solve / frs_cg_step (device pointers owned by the ctx,
+ * [nfield][ny][nx] each; d_scal: double[8] = rr, pq, rr_new, alpha, beta, breakdown, bb, -). */
+int frs_cg_state(frs_ctx* ctx, float** r, float** p, float** q, double** d_scal);
+/* One CG iteration on caller-visible state (teacher-forced parity, R9): given x, and the ctx's
+ * r, p and rr (loaded with frs_cg_load), computes q = M p, alpha, x, r, beta, p. */
+int frs_cg_load(frs_ctx* ctx, const float* r, const float* p, double rr_host);
+int frs_cg_step(frs_ctx* ctx, float* x, int with_prior);
+
+/* ---- host-buffer entry points (end-to-end measurements: copies are part of the call) -------- */
+
+/* y = s . C (s . x) with x, y in HOST memory (pinned or pageable), [nchan][ny][nx].
+ * Copies x to the device, runs frs_sky_metric_apply, copies y back, synchronises. */
+int frs_sky_metric_apply_host(frs_ctx* ctx, const float* x_host, float* y_host);
+/* y = C x with HOST buffers. */
+int frs_psf_apply_host(frs_ctx* ctx, const float* x_host, float* y_host);
+
+/* ---- instrumentation ---------------------------------------------------------------------------- */
+
+/* Number of kernels this ctx has launched since creation (monotone). */
+long long frs_launch_count(const frs_ctx* ctx);
+/* When enabled, every FFT pass is bracketed by CUDA events on the ctx's stream.  frs_profile_read
+ * synchronises and returns accumulated milliseconds and launch counts per pass kind:
+ * 0 rows_fwd (conv), 1 conv_cols, 2 rows_inv, 3 rows_fwd (Hartley), 4 hart_cols.  Resets on read. */
+int frs_profile_enable(frs_ctx* ctx, int on);
+int frs_profile_read(frs_ctx* ctx, double ms[5], long long launches[5]);
+
+/* ---- self-test of host-replayable index logic (no GPU needed) -------------------------------- */
+
+/* Replays the register/shared-memory FFT stage logic thread by thread on the CPU for an n-point
+ * transform (n a power of two in [16, 4096]); in/out: interleaved complex float [n]. */
+int frs_selftest_fft_host(int n, int inverse, const float* in, float* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FRS_H */

@@ -1,0 +1,8 @@
+"""fast-resolve hot path on B200: thin Python binding of libfrs.so (see include/frs.h).
+
+The package only marshals arguments (torch tensors -> device pointers); every step of the path
+runs in the CUDA kernels of libfrs.so.  There is no CPU fallback: if the library is missing or no
+CUDA device is present, calls raise.
+"""
+from .binding import (FrsError, Context, lib, load_library, selftest_fft_host, EXPORTS,  # noqa: F401
+                      FRS_OK, FRS_EINVAL, FRS_ESTATE, FRS_ENOTPSD, FRS_ECUDA, FRS_EBREAKDOWN)

@@ -1,0 +1,256 @@
+"""ctypes binding of include/frs.h -- argument marshalling only (same names as the C ABI)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libfrs.so")
+
+FRS_OK, FRS_EINVAL, FRS_ESTATE, FRS_ENOTPSD, FRS_ECUDA, FRS_EBREAKDOWN = 0, -1, -2, -3, -4, -5
+_CODES = {-1: "FRS_EINVAL", -2: "FRS_ESTATE", -3: "FRS_ENOTPSD", -4: "FRS_ECUDA", -5: "FRS_EBREAKDOWN"}
+
+_vp, _i, _f, _d = C.c_void_p, C.c_int, C.c_float, C.c_double
+# name -> (restype, argtypes): every symbol include/frs.h declares
+EXPORTS = {
+    "frs_create": (_i, [_i, _i, _i, _i, _vp, C.POINTER(_vp)]),
+    "frs_destroy": (None, [_vp]),
+    "frs_last_error": (C.c_char_p, [_vp]),
+    "frs_version": (C.c_char_p, []),
+    "frs_set_psf": (_i, [_vp, _vp]),
+    "frs_set_psf_weights": (_i, [_vp, _vp]),
+    "frs_set_dirty": (_i, [_vp, _vp]),
+    "frs_set_amplitude": (_i, [_vp, _i, _vp, C.POINTER(_f)]),
+    "frs_set_channel_lognu": (_i, [_vp, C.POINTER(_f)]),
+    "frs_sky_forward": (_i, [_vp, _vp, _vp]),
+    "frs_psf_apply": (_i, [_vp, _vp, _vp]),
+    "frs_sky_metric_apply": (_i, [_vp, _vp, _vp]),
+    "frs_set_sky": (_i, [_vp, _vp]),
+    "frs_energy_grad": (_i, [_vp, _vp, _i, _vp, C.POINTER(_d), _vp]),
+    "frs_metric_apply": (_i, [_vp, _vp, _i, _vp]),
+    "frs_cg_solve": (_i, [_vp, _vp, _vp, _i, _f, _i, C.POINTER(_i), C.POINTER(_d), _vp]),
+    "frs_cg_state": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp)]),
+    "frs_cg_load": (_i, [_vp, _vp, _vp, _d]),
+    "frs_cg_step": (_i, [_vp, _vp, _i]),
+    "frs_sky_metric_apply_host": (_i, [_vp, _vp, _vp]),
+    "frs_psf_apply_host": (_i, [_vp, _vp, _vp]),
+    "frs_launch_count": (C.c_longlong, [_vp]),
+    "frs_profile_enable": (_i, [_vp, _i]),
+    "frs_profile_read": (_i, [_vp, C.POINTER(_d), C.POINTER(C.c_longlong)]),
+    "frs_selftest_fft_host": (_i, [_i, _i, _vp, _vp]),
+}
+
+_lib = None
+
+
+class FrsError(RuntimeError):
+    def __init__(self, code, msg=""):
+        self.code = code
+        super().__init__(f"{_CODES.get(code, code)}: {msg}")
+
+
+def load_library(path=LIB_PATH):
+    """dlopen libfrs.so and declare every prototype.  Raises if the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not built -- run `python -m paper_2406_09144_b200.build` "
+                                "(there is no CPU fallback)")
+    lib_ = C.CDLL(path)
+    for name, (res, args) in EXPORTS.items():
+        fn = getattr(lib_, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = lib_
+    return lib_
+
+
+def lib():
+    return load_library()
+
+
+def selftest_fft_host(x, inverse=False):
+    """CPU replay of the kernels' FFT stage logic (complex64 [n])."""
+    x = np.ascontiguousarray(x, dtype=np.complex64)
+    out = np.empty_like(x)
+    rc = lib().frs_selftest_fft_host(x.shape[0], int(inverse), x.ctypes.data, out.ctypes.data)
+    if rc != 0:
+        raise FrsError(rc, "selftest")
+    return out
+
+
+def _ptr(t, dtype=None, numel=None, name="tensor"):
+    if t is None:
+        return None
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"{name}: expected dtype {dtype}, got {t.dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+class Context:
+    """frs_ctx wrapper.  Methods mirror the C calls and take torch CUDA float32 tensors."""
+
+    def __init__(self, ny, nx, nchan=1, device=0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the fast-resolve hot path has no CPU fallback")
+        self.torch = torch
+        self.ny, self.nx, self.nchan, self.nfield = ny, nx, nchan, 0
+        self.device = torch.device("cuda", device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        self._h = _vp()
+        rc = lib().frs_create(ny, nx, nchan, device, _vp(stream.cuda_stream), C.byref(self._h))
+        if rc != 0:
+            raise FrsError(rc, "frs_create")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().frs_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        if rc != 0:
+            raise FrsError(rc, lib().frs_last_error(self._h).decode())
+
+    @property
+    def npix(self):
+        return self.ny * self.nx
+
+    @property
+    def f32(self):
+        return self.torch.float32
+
+    def new_image(self):
+        return self.torch.empty((self.nchan, self.ny, self.nx), dtype=self.f32, device=self.device)
+
+    def new_latent(self):
+        return self.torch.empty((self.nfield, self.ny, self.nx), dtype=self.f32, device=self.device)
+
+    # ---- setup
+    def set_psf(self, psf):
+        self._ck(lib().frs_set_psf(self._h, _ptr(psf, self.f32, self.nchan * 4 * self.npix, "psf")))
+
+    def set_psf_weights(self, w_half):
+        self._ck(lib().frs_set_psf_weights(
+            self._h, _ptr(w_half, self.f32, self.nchan * 2 * self.ny * (self.nx + 1), "w_half")))
+
+    def set_dirty(self, j):
+        self._ck(lib().frs_set_dirty(self._h, _ptr(j, self.f32, self.nchan * self.npix, "dirty")))
+
+    def set_amplitude(self, amp, mu):
+        nfield = amp.shape[0]
+        mu_arr = (_f * nfield)(*[float(m) for m in mu])
+        self._ck(lib().frs_set_amplitude(self._h, nfield, _ptr(amp, self.f32, nfield * self.npix, "amp"), mu_arr))
+        self.nfield = nfield
+
+    def set_channel_lognu(self, lognu):
+        arr = (_f * self.nchan)(*[float(v) for v in lognu])
+        self._ck(lib().frs_set_channel_lognu(self._h, arr))
+
+    def set_sky(self, sky):
+        self._ck(lib().frs_set_sky(self._h, _ptr(sky, self.f32, self.nchan * self.npix, "sky")))
+
+    # ---- hot path
+    def sky_forward(self, xi, sky=None):
+        self._ck(lib().frs_sky_forward(self._h, _ptr(xi, self.f32, self.nfield * self.npix, "xi"),
+                                       _ptr(sky, self.f32, self.nchan * self.npix, "sky")))
+        return sky
+
+    def psf_apply(self, x, y):
+        self._ck(lib().frs_psf_apply(self._h, _ptr(x, self.f32, self.nchan * self.npix, "x"),
+                                     _ptr(y, self.f32, self.nchan * self.npix, "y")))
+        return y
+
+    def sky_metric_apply(self, x, y):
+        self._ck(lib().frs_sky_metric_apply(self._h, _ptr(x, self.f32, self.nchan * self.npix, "x"),
+                                            _ptr(y, self.f32, self.nchan * self.npix, "y")))
+        return y
+
+    def energy_grad(self, xi, grad, with_prior=True, d_energy=None, host_energy=True):
+        h = _d(0.0)
+        self._ck(lib().frs_energy_grad(self._h, _ptr(xi, self.f32, self.nfield * self.npix, "xi"), int(with_prior),
+                                       _ptr(d_energy, self.torch.float64, 1, "d_energy"),
+                                       C.byref(h) if host_energy else None,
+                                       _ptr(grad, self.f32, self.nfield * self.npix, "grad")))
+        return h.value if host_energy else None
+
+    def metric_apply(self, v, out, with_prior=True):
+        self._ck(lib().frs_metric_apply(self._h, _ptr(v, self.f32, self.nfield * self.npix, "v"), int(with_prior),
+                                        _ptr(out, self.f32, self.nfield * self.npix, "out")))
+        return out
+
+    def cg_solve(self, b, x, max_iter, rtol=0.0, with_prior=True, res_history=None):
+        it, rn = _i(0), _d(0.0)
+        if res_history is not None and res_history.numel() < max_iter + 1:
+            raise ValueError("res_history needs max_iter + 1 doubles")
+        self._ck(lib().frs_cg_solve(self._h, _ptr(b, self.f32, self.nfield * self.npix, "b"),
+                                    _ptr(x, self.f32, self.nfield * self.npix, "x"), int(max_iter), float(rtol),
+                                    int(with_prior), C.byref(it), C.byref(rn),
+                                    _ptr(res_history, self.torch.float64, None, "res_history")))
+        return it.value, rn.value
+
+    def cg_load(self, r, p, rr):
+        self._ck(lib().frs_cg_load(self._h, _ptr(r, self.f32, self.nfield * self.npix, "r"),
+                                   _ptr(p, self.f32, self.nfield * self.npix, "p"), float(rr)))
+
+    def cg_step(self, x, with_prior=True):
+        self._ck(lib().frs_cg_step(self._h, _ptr(x, self.f32, self.nfield * self.npix, "x"), int(with_prior)))
+
+    def cg_read_state(self):
+        """Copies of the ctx-owned r, p, q (torch) and the scalar block (numpy float64[8]:
+        rr, pq, rr_new, alpha, beta, breakdown, bb, -) after a cg_step / cg_solve."""
+        r, p, q, s = _vp(), _vp(), _vp(), _vp()
+        self._ck(lib().frs_cg_state(self._h, C.byref(r), C.byref(p), C.byref(q), C.byref(s)))
+        n = self.nfield * self.npix
+        self.stream.synchronize()
+        rt = self.torch.cuda.cudart()
+        outs = []
+        for ptr in (r, p, q):
+            t = self.new_latent()
+            rc = rt.cudaMemcpy(t.data_ptr(), ptr.value, n * 4, 3)
+            if int(rc) != 0:
+                raise FrsError(FRS_ECUDA, f"cudaMemcpy {rc}")
+            outs.append(t)
+        sc = self.torch.zeros(8, dtype=self.torch.float64, device=self.device)
+        rc = rt.cudaMemcpy(sc.data_ptr(), s.value, 64, 3)
+        if int(rc) != 0:
+            raise FrsError(FRS_ECUDA, f"cudaMemcpy {rc}")
+        return outs[0], outs[1], outs[2], sc.cpu().numpy()
+
+    # ---- host-buffer entry points (torch CPU tensors, ideally pinned)
+    def sky_metric_apply_host(self, x_host, y_host):
+        self._ck(lib().frs_sky_metric_apply_host(self._h, _vp(x_host.data_ptr()), _vp(y_host.data_ptr())))
+        return y_host
+
+    def psf_apply_host(self, x_host, y_host):
+        self._ck(lib().frs_psf_apply_host(self._h, _vp(x_host.data_ptr()), _vp(y_host.data_ptr())))
+        return y_host
+
+    # ---- instrumentation
+    def launch_count(self):
+        return int(lib().frs_launch_count(self._h))
+
+    def profile_enable(self, on=True):
+        self._ck(lib().frs_profile_enable(self._h, int(on)))
+
+    def profile_read(self):
+        ms = (_d * 5)()
+        n = (C.c_longlong * 5)()
+        self._ck(lib().frs_profile_read(self._h, ms, n))
+        names = ["conv_rows_fwd", "conv_cols", "conv_rows_inv", "hart_rows", "hart_cols"]
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(names)}

@@ -1,0 +1,185 @@
+// ew_kernels.cuh -- elementwise maps, deterministic single-order reductions and the CG vector
+// updates.  All reductions: fp64 products and sums, one partial per
+// CTA written to a buffer, summed afterwards in a fixed order by one CTA (no float atomics), so a
+// result does not depend on scheduling.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace frs {
+
+constexpr int kEwThreads = 256;
+constexpr int kRedThreads = 256;
+
+__device__ __forceinline__ double block_sum(double x) {
+    __shared__ double red[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) red[w] = x;
+    __syncthreads();
+    double y = 0.0;
+    if (w == 0) {
+        const int nw = blockDim.x >> 5;
+        y = l < nw ? red[l] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) y += __shfl_down_sync(0xffffffffu, y, o);
+    }
+    return y;   // valid in thread 0
+}
+
+// s[c][i] = exp(tau0[i] + lognu[c] tau1[i])   (tau already contains mu; reading R6)
+__global__ void sky_kernel(const float* __restrict__ tau, const float* __restrict__ lognu, float* __restrict__ s,
+                           size_t npix, int nfield, int nchan) {
+    const size_t i4 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i4 * 4 >= npix) return;
+    const float4 t0 = reinterpret_cast<const float4*>(tau)[i4];
+    float4 t1 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (nfield == 2) t1 = reinterpret_cast<const float4*>(tau + npix)[i4];
+    for (int c = 0; c < nchan; ++c) {
+        const float l = nfield == 2 ? lognu[c] : 0.f;
+        float4 o;
+        o.x = expf(fmaf(l, t1.x, t0.x)); o.y = expf(fmaf(l, t1.y, t0.y));
+        o.z = expf(fmaf(l, t1.z, t0.z)); o.w = expf(fmaf(l, t1.w, t0.w));
+        reinterpret_cast<float4*>(s + (size_t)c * npix)[i4] = o;
+    }
+}
+
+// img[c][i] = s[c][i] (lin0[i] + lognu[c] lin1[i])      (J v without the Hartley map)
+__global__ void jvp_combine_kernel(const float* __restrict__ lin, const float* __restrict__ s,
+                                   const float* __restrict__ lognu, float* __restrict__ img,
+                                   size_t npix, int nfield, int nchan) {
+    const size_t i4 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i4 * 4 >= npix) return;
+    const float4 t0 = reinterpret_cast<const float4*>(lin)[i4];
+    float4 t1 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (nfield == 2) t1 = reinterpret_cast<const float4*>(lin + npix)[i4];
+    for (int c = 0; c < nchan; ++c) {
+        const float l = nfield == 2 ? lognu[c] : 0.f;
+        const float4 sv = reinterpret_cast<const float4*>(s + (size_t)c * npix)[i4];
+        float4 o;
+        o.x = sv.x * fmaf(l, t1.x, t0.x); o.y = sv.y * fmaf(l, t1.y, t0.y);
+        o.z = sv.z * fmaf(l, t1.z, t0.z); o.w = sv.w * fmaf(l, t1.w, t0.w);
+        reinterpret_cast<float4*>(img + (size_t)c * npix)[i4] = o;
+    }
+}
+
+// acc[f][i] = sum_c coeff[c][f] img[c][i], channels summed in index order   (J^T without H, A)
+__global__ void vjp_combine_kernel(const float* __restrict__ img, const float* __restrict__ lognu,
+                                   float* __restrict__ acc, size_t npix, int nfield, int nchan) {
+    const size_t i4 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i4 * 4 >= npix) return;
+    float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
+    for (int c = 0; c < nchan; ++c) {
+        const float4 w = reinterpret_cast<const float4*>(img + (size_t)c * npix)[i4];
+        a0.x += w.x; a0.y += w.y; a0.z += w.z; a0.w += w.w;
+        if (nfield == 2) {
+            const float l = lognu[c];
+            a1.x = fmaf(l, w.x, a1.x); a1.y = fmaf(l, w.y, a1.y); a1.z = fmaf(l, w.z, a1.z); a1.w = fmaf(l, w.w, a1.w);
+        }
+    }
+    reinterpret_cast<float4*>(acc)[i4] = a0;
+    if (nfield == 2) reinterpret_cast<float4*>(acc + npix)[i4] = a1;
+}
+
+// partials[blockIdx.x] = sum over this CTA's slice of a[i] b[i]
+__global__ void __launch_bounds__(kRedThreads) dot_partial_kernel(const float* __restrict__ a, const float* __restrict__ b,
+                                                                  size_t n, double* __restrict__ partials) {
+    double acc = 0.0;
+    const size_t n4 = n / 4;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        const float4 x = reinterpret_cast<const float4*>(a)[i], y = reinterpret_cast<const float4*>(b)[i];
+        acc += (double)x.x * y.x + (double)x.y * y.y + (double)x.z * y.z + (double)x.w * y.w;
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+}
+
+// out[k] = scale[k] * sum_{i<n} partials[i*stride + k] for k < nk, fixed order; one CTA.
+// Optional combination for the energy:  energy = 0.5*S0 - S1 + 0.5*prior
+__global__ void __launch_bounds__(kRedThreads) reduce_final_kernel(const double* __restrict__ partials, int n, int stride,
+                                                                   int k, double* __restrict__ out) {
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) acc += partials[(size_t)i * stride + k];
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) *out = acc;
+}
+
+// sc: device scalars.  E = 0.5 sc[kSC] - sc[kJS] + 0.5 with_prior sc[kXX]
+__global__ void energy_final_kernel(const double* __restrict__ sc_sc, const double* __restrict__ sc_js,
+                                    const double* __restrict__ sc_xx, int with_prior, double* __restrict__ e) {
+    *e = 0.5 * (*sc_sc) - (*sc_js) + (with_prior ? 0.5 * (*sc_xx) : 0.0);
+}
+
+// ---- CG (reading R9).  scal[0]=rr, [1]=pq, [2]=rr_new, [3]=alpha, [4]=beta, [5]=breakdown flag
+enum { kRR = 0, kPQ = 1, kRRNew = 2, kAlpha = 3, kBeta = 4, kBreak = 5, kBB = 6, kNScal = 8 };
+
+// r = b - q ; p = r ; partial <r,r>       (q = M x0, or q == nullptr for x0 = 0)
+__global__ void __launch_bounds__(kRedThreads) cg_init_kernel(const float* __restrict__ b, const float* __restrict__ q,
+                                                              float* __restrict__ r, float* __restrict__ p, size_t n,
+                                                              double* __restrict__ partials) {
+    double acc = 0.0;
+    const size_t n4 = n / 4;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        float4 x = reinterpret_cast<const float4*>(b)[i];
+        if (q) {
+            const float4 y = reinterpret_cast<const float4*>(q)[i];
+            x.x -= y.x; x.y -= y.y; x.z -= y.z; x.w -= y.w;
+        }
+        reinterpret_cast<float4*>(r)[i] = x;
+        reinterpret_cast<float4*>(p)[i] = x;
+        acc += (double)x.x * x.x + (double)x.y * x.y + (double)x.z * x.z + (double)x.w * x.w;
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+}
+
+// alpha = rr/pq ; x += alpha p ; r -= alpha q ; partial <r,r>
+__global__ void __launch_bounds__(kRedThreads) cg_update_xr_kernel(float* __restrict__ x, float* __restrict__ r,
+                                                                   const float* __restrict__ p, const float* __restrict__ q,
+                                                                   size_t n, double* __restrict__ scal,
+                                                                   double* __restrict__ partials) {
+    const double pq = scal[kPQ];
+    const double alpha_d = pq > 0.0 ? scal[kRR] / pq : 0.0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        scal[kAlpha] = alpha_d;
+        if (!(pq > 0.0)) scal[kBreak] = 1.0;
+    }
+    const float alpha = (float)alpha_d;
+    double acc = 0.0;
+    const size_t n4 = n / 4;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        float4 xv = reinterpret_cast<float4*>(x)[i], rv = reinterpret_cast<float4*>(r)[i];
+        const float4 pv = reinterpret_cast<const float4*>(p)[i], qv = reinterpret_cast<const float4*>(q)[i];
+        xv.x = fmaf(alpha, pv.x, xv.x); xv.y = fmaf(alpha, pv.y, xv.y); xv.z = fmaf(alpha, pv.z, xv.z); xv.w = fmaf(alpha, pv.w, xv.w);
+        rv.x = fmaf(-alpha, qv.x, rv.x); rv.y = fmaf(-alpha, qv.y, rv.y); rv.z = fmaf(-alpha, qv.z, rv.z); rv.w = fmaf(-alpha, qv.w, rv.w);
+        reinterpret_cast<float4*>(x)[i] = xv;
+        reinterpret_cast<float4*>(r)[i] = rv;
+        acc += (double)rv.x * rv.x + (double)rv.y * rv.y + (double)rv.z * rv.z + (double)rv.w * rv.w;
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+}
+
+// beta = rr_new/rr ; p = r + beta p ; then rr <- rr_new (done by the last-launched thread 0 after use)
+__global__ void __launch_bounds__(kEwThreads) cg_update_p_kernel(float* __restrict__ p, const float* __restrict__ r, size_t n,
+                                                                 const double* __restrict__ scal, double* __restrict__ beta_out) {
+    const double rr = scal[kRR];
+    const double beta_d = rr > 0.0 ? scal[kRRNew] / rr : 0.0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *beta_out = beta_d;
+    const float beta = (float)beta_d;
+    const size_t n4 = n / 4;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        const float4 rv = reinterpret_cast<const float4*>(r)[i];
+        float4 pv = reinterpret_cast<float4*>(p)[i];
+        pv.x = fmaf(beta, pv.x, rv.x); pv.y = fmaf(beta, pv.y, rv.y); pv.z = fmaf(beta, pv.z, rv.z); pv.w = fmaf(beta, pv.w, rv.w);
+        reinterpret_cast<float4*>(p)[i] = pv;
+    }
+}
+
+__global__ void cg_shift_kernel(double* __restrict__ scal, double* __restrict__ hist, int k) {
+    scal[kRR] = scal[kRRNew];
+    if (hist) hist[k] = sqrt(scal[kRRNew]);
+}
+
+}  // namespace frs

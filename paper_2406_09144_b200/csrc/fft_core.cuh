@@ -1,0 +1,215 @@
+// fft_core.cuh -- register-resident Stockham FFT shared by a group of P = N/16 threads.
+//
+// Each thread owns kE = 16 complex elements of an N-point transform in the CANONICAL
+// distribution  reg e  <->  position p + e*P  (p = thread index inside the group).  A stage of
+// radix R does 16/R butterflies per thread fully in registers; between stages the group
+// exchanges through a padded shared-memory buffer (pad 1 float2 per 16 -> conflict-free 64-bit
+// accesses).  Input and output are both in natural order
+// in the canonical distribution, so forward -> pointwise -> inverse needs no reordering.
+//
+// The stage arithmetic is __host__ __device__: csrc/selftest.cu replays it thread by thread on
+// the CPU so that the index maps and twiddle tables are tested without a GPU.
+#pragma once
+#include <cuda_runtime.h>
+
+#define FRS_HD __host__ __device__ __forceinline__
+
+namespace frs {
+
+constexpr int kE = 16;
+constexpr float kSqrtHalf = 0.70710678118654752440f;
+constexpr float kC1 = 0.92387953251128675613f;   // cos(pi/8)
+constexpr float kS1 = 0.38268343236508977173f;   // sin(pi/8)
+
+FRS_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+FRS_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+FRS_HD float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
+FRS_HD float2 cscale(float2 a, float s) { return make_float2(a.x * s, a.y * s); }
+// a * w
+FRS_HD float2 cmul(float2 a, float2 w) {
+    return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.y, w.x, a.x * w.y));
+}
+// a * conj(w)
+FRS_HD float2 cmulc(float2 a, float2 w) {
+    return make_float2(fmaf(a.y, w.y, a.x * w.x), fmaf(a.y, w.x, -(a.x * w.y)));
+}
+template <bool INV> FRS_HD float2 cmul_dir(float2 a, float2 w) { return INV ? cmulc(a, w) : cmul(a, w); }
+// a * (-i) forward, a * (+i) inverse
+template <bool INV> FRS_HD float2 mul_mi(float2 a) {
+    return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+}
+// a * w8^k (forward w8 = exp(-2 pi i/8)); inverse uses the conjugate
+template <int K, bool INV> FRS_HD float2 mul_w8(float2 a) {
+    if (K == 0) return a;
+    if (K == 2) return mul_mi<INV>(a);
+    if (K == 1) return INV ? make_float2((a.x - a.y) * kSqrtHalf, (a.x + a.y) * kSqrtHalf)
+                           : make_float2((a.x + a.y) * kSqrtHalf, (a.y - a.x) * kSqrtHalf);
+    /* K == 3 */ return INV ? make_float2((-a.x - a.y) * kSqrtHalf, (a.x - a.y) * kSqrtHalf)
+                           : make_float2((a.y - a.x) * kSqrtHalf, (-a.x - a.y) * kSqrtHalf);
+}
+// a * w16^K, K in {0,1,2,3,4,6,9}
+template <int K, bool INV> FRS_HD float2 mul_w16(float2 a) {
+    if (K == 0) return a;
+    if (K == 2) return mul_w8<1, INV>(a);
+    if (K == 4) return mul_mi<INV>(a);
+    if (K == 6) return mul_w8<3, INV>(a);
+    float2 w = (K == 1) ? make_float2(kC1, -kS1) : (K == 3) ? make_float2(kS1, -kC1) : make_float2(-kC1, kS1) /*K==9*/;
+    return cmul_dir<INV>(a, w);
+}
+
+// ---- small DFTs, natural order in and out, in place ------------------------------------------
+template <bool INV> FRS_HD void dft2(float2& a, float2& b) {
+    float2 t = a;
+    a = cadd(t, b);
+    b = csub(t, b);
+}
+template <bool INV> FRS_HD void dft4(float2& a0, float2& a1, float2& a2, float2& a3) {
+    float2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = mul_mi<INV>(csub(a1, a3));
+    a0 = cadd(t0, t2);
+    a2 = csub(t0, t2);
+    a1 = cadd(t1, t3);
+    a3 = csub(t1, t3);
+}
+template <bool INV> FRS_HD void dft8(float2 (&t)[8]) {
+    dft4<INV>(t[0], t[2], t[4], t[6]);   // E[k] in t[0],t[2],t[4],t[6]
+    dft4<INV>(t[1], t[3], t[5], t[7]);   // O[k] in t[1],t[3],t[5],t[7]
+    float2 o0 = t[1], o1 = mul_w8<1, INV>(t[3]), o2 = mul_w8<2, INV>(t[5]), o3 = mul_w8<3, INV>(t[7]);
+    float2 e0 = t[0], e1 = t[2], e2 = t[4], e3 = t[6];
+    t[0] = cadd(e0, o0); t[4] = csub(e0, o0);
+    t[1] = cadd(e1, o1); t[5] = csub(e1, o1);
+    t[2] = cadd(e2, o2); t[6] = csub(e2, o2);
+    t[3] = cadd(e3, o3); t[7] = csub(e3, o3);
+}
+template <bool INV> FRS_HD void dft16(float2 (&t)[16]) {
+    // n = 4 n1 + n0, k = k0 + 4 k1:  X[k] = sum_n0 w4^{n0 k1} w16^{n0 k0} sum_n1 w4^{n1 k0} a[4 n1 + n0]
+    dft4<INV>(t[0], t[4], t[8], t[12]);      // n0 = 0: B[0][k0] at t[4 k0 + 0]
+    dft4<INV>(t[1], t[5], t[9], t[13]);
+    dft4<INV>(t[2], t[6], t[10], t[14]);
+    dft4<INV>(t[3], t[7], t[11], t[15]);
+    t[5] = mul_w16<1, INV>(t[5]);  t[6] = mul_w16<2, INV>(t[6]);   t[7] = mul_w16<3, INV>(t[7]);
+    t[9] = mul_w16<2, INV>(t[9]);  t[10] = mul_w16<4, INV>(t[10]); t[11] = mul_w16<6, INV>(t[11]);
+    t[13] = mul_w16<3, INV>(t[13]); t[14] = mul_w16<6, INV>(t[14]); t[15] = mul_w16<9, INV>(t[15]);
+    dft4<INV>(t[0], t[1], t[2], t[3]);       // k0 = 0: X[0 + 4 k1] at t[k1]
+    dft4<INV>(t[4], t[5], t[6], t[7]);       // k0 = 1: X[1 + 4 k1] at t[4 + k1]
+    dft4<INV>(t[8], t[9], t[10], t[11]);
+    dft4<INV>(t[12], t[13], t[14], t[15]);
+    // transpose 4x4: X[k0 + 4 k1] currently at t[4 k0 + k1]
+    float2 s;
+    s = t[1]; t[1] = t[4]; t[4] = s;
+    s = t[2]; t[2] = t[8]; t[8] = s;
+    s = t[3]; t[3] = t[12]; t[12] = s;
+    s = t[6]; t[6] = t[9]; t[9] = s;
+    s = t[7]; t[7] = t[13]; t[13] = s;
+    s = t[11]; t[11] = t[14]; t[14] = s;
+}
+template <int R, bool INV> struct Dft;
+template <bool INV> struct Dft<2, INV> { static FRS_HD void run(float2 (&t)[2]) { dft2<INV>(t[0], t[1]); } };
+template <bool INV> struct Dft<4, INV> { static FRS_HD void run(float2 (&t)[4]) { dft4<INV>(t[0], t[1], t[2], t[3]); } };
+template <bool INV> struct Dft<8, INV> { static FRS_HD void run(float2 (&t)[8]) { dft8<INV>(t); } };
+template <bool INV> struct Dft<16, INV> { static FRS_HD void run(float2 (&t)[16]) { dft16<INV>(t); } };
+
+// ---- plan: radices per transform length ------------------------------------------------------
+// 16:[16] 32:[16,2] 64:[8,8] 128:[16,8] 256:[16,16] 512:[8,8,8] 1024:[16,8,8] 2048:[16,16,8] 4096:[16,16,16]
+FRS_HD constexpr int plan_stages(int n) { return n == 16 ? 1 : (n <= 256 ? 2 : 3); }
+FRS_HD constexpr int plan_radix(int n, int s) {
+    return n == 16   ? 16
+         : n == 32   ? (s == 0 ? 16 : 2)
+         : n == 64   ? 8
+         : n == 128  ? (s == 0 ? 16 : 8)
+         : n == 256  ? 16
+         : n == 512  ? 8
+         : n == 1024 ? (s == 0 ? 16 : 8)
+         : n == 2048 ? (s <= 1 ? 16 : 8)
+                     : 16;
+}
+FRS_HD constexpr int plan_ns(int n, int s) {   // product of the radices before stage s
+    return s == 0 ? 1 : plan_ns(n, s - 1) * plan_radix(n, s - 1);
+}
+// twiddle-table offset (in units of P entries) of stage s, and total rows
+FRS_HD constexpr int plan_tw_rows(int n, int s) { return s == 0 ? 0 : kE - kE / plan_radix(n, s); }
+FRS_HD constexpr int plan_tw_off(int n, int s) { return s <= 1 ? 0 : plan_tw_off(n, s - 1) + plan_tw_rows(n, s - 1); }
+FRS_HD constexpr int plan_tw_total(int n) { return plan_tw_off(n, plan_stages(n) - 1) + plan_tw_rows(n, plan_stages(n) - 1); }
+
+FRS_HD constexpr int xpad(int pos) { return pos + (pos >> 4); }
+// float2 slots of one exchange buffer (holds positions 0..N inclusive: the row passes park X[N] too)
+FRS_HD constexpr int xbuf_len(int n) { return n + (n >> 4) + 8; }
+
+// ---- one stage: twiddle the inputs, butterfly, leave result r of butterfly b in v[b + r*NB] ----
+// NT transforms are advanced together so that each twiddle is fetched once.
+template <int N, int S, bool INV, int NT>
+FRS_HD void stage_compute(float2 (&v)[NT][kE], int p, const float2* __restrict__ tw) {
+    constexpr int R = plan_radix(N, S), NB = kE / R, P = N / kE;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        float2 w[R];
+        if (S > 0) {
+#pragma unroll
+            for (int r = 1; r < R; ++r) w[r] = tw[(plan_tw_off(N, S) + b * (R - 1) + (r - 1)) * P + p];
+        }
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            float2 x[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) x[r] = v[t][b + r * NB];
+            if (S > 0) {
+#pragma unroll
+                for (int r = 1; r < R; ++r) x[r] = cmul_dir<INV>(x[r], w[r]);
+            }
+            Dft<R, INV>::run(x);
+#pragma unroll
+            for (int r = 0; r < R; ++r) v[t][b + r * NB] = x[r];
+        }
+    }
+}
+// scatter the stage's outputs to their Stockham positions in the exchange buffer
+template <int N, int S>
+FRS_HD void stage_scatter(const float2 (&v)[kE], int p, float2* buf) {
+    constexpr int R = plan_radix(N, S), NB = kE / R, P = N / kE, NS = plan_ns(N, S);
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        const int j = p + b * P;
+        const int base = (j / NS) * NS * R + (j % NS);
+#pragma unroll
+        for (int r = 0; r < R; ++r) buf[xpad(base + r * NS)] = v[b + r * NB];
+    }
+}
+// read the canonical distribution back
+template <int N>
+FRS_HD void canon_gather(float2 (&v)[kE], int p, const float2* buf) {
+    constexpr int P = N / kE;
+#pragma unroll
+    for (int e = 0; e < kE; ++e) v[e] = buf[xpad(p + e * P)];
+}
+template <int N>
+FRS_HD void canon_scatter(const float2 (&v)[kE], int p, float2* buf) {
+    constexpr int P = N / kE;
+#pragma unroll
+    for (int e = 0; e < kE; ++e) buf[xpad(p + e * P)] = v[e];
+}
+
+#ifdef __CUDACC__
+// ---- the whole transform for NT simultaneous transforms sharing one twiddle fetch -------------
+// All threads of the CTA must call this (it uses __syncthreads()).  bufs: NT exchange buffers of
+// xbuf_len(N) float2 each, private to the group.
+template <int N, bool INV, int NT, int S>
+__device__ __forceinline__ void group_fft_from(float2 (&v)[NT][kE], int p, float2* bufs, const float2* __restrict__ tw) {
+    if constexpr (S < plan_stages(N)) {
+        stage_compute<N, S, INV, NT>(v, p, tw);
+        if constexpr (S + 1 < plan_stages(N)) {
+#pragma unroll
+            for (int t = 0; t < NT; ++t) stage_scatter<N, S>(v[t], p, bufs + t * xbuf_len(N));
+            __syncthreads();
+#pragma unroll
+            for (int t = 0; t < NT; ++t) canon_gather<N>(v[t], p, bufs + t * xbuf_len(N));
+            __syncthreads();
+        }
+        group_fft_from<N, INV, NT, S + 1>(v, p, bufs, tw);
+    }
+}
+template <int N, bool INV, int NT>
+__device__ __forceinline__ void group_fft(float2 (&v)[NT][kE], int p, float2* bufs, const float2* __restrict__ tw) {
+    group_fft_from<N, INV, NT, 0>(v, p, bufs, tw);
+}
+#endif
+
+}  // namespace frs

@@ -1,0 +1,612 @@
+// frs_api.cu -- the C ABI of include/frs.h: context, setup, and the launch sequences of the hot
+// path.  Every step of the path runs in the kernels of this library;
+// there is no CPU fallback: without a CUDA device frs_create fails with FRS_ECUDA.
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <vector>
+
+#include "../../include/frs.h"
+#include "ew_kernels.cuh"
+#include "launch.h"
+#include "setup.h"
+#include "tables.h"
+
+using namespace frs;
+
+namespace {
+enum PassKind { kPassRowsFwd = 0, kPassConvCols = 1, kPassRowsInv = 2, kPassHartRows = 3, kPassHartCols = 4, kNPass = 5 };
+struct ProfRec { int kind; cudaEvent_t a, b; };
+constexpr int kMaxRedBlocks = 1184;   // 148 SMs x 8
+}  // namespace
+
+struct frs_ctx {
+    int ny = 0, nx = 0, nchan = 0, nfield = 0, device = 0;
+    cudaStream_t stream = nullptr;
+    size_t npix = 0;
+    int ntile = 0, ntile_h = 0;
+    std::map<int, float2*> tw, twist;
+    float *wt = nullptr, *dirty = nullptr, *amp = nullptr, *s = nullptr;
+    float *d_mu = nullptr, *d_lognu = nullptr;
+    float2 *T = nullptr, *Th = nullptr;
+    float *lin = nullptr, *img = nullptr, *acc = nullptr;
+    float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
+    float *hx = nullptr, *hy = nullptr;
+    double *partials = nullptr, *scal = nullptr;   // scal: [0..7] CG, [8] sum s.c, [9] sum j.s, [10] <xi,xi>, [11] E
+    int* flag = nullptr;
+    bool have_psf = false, have_dirty = false, have_amp = false, have_s = false;
+    long long launches = 0;
+    bool profiling = false;
+    std::vector<ProfRec> prof;
+    char err[512] = "no error";
+};
+
+namespace {
+
+int fail(frs_ctx* c, int code, const char* msg) {
+    if (c) snprintf(c->err, sizeof(c->err), "%s", msg);
+    return code;
+}
+int cuda_fail(frs_ctx* c, cudaError_t e, const char* where) {
+    if (c) snprintf(c->err, sizeof(c->err), "CUDA error at %s: %s", where, cudaGetErrorString(e));
+    return FRS_ECUDA;
+}
+#define CK(call)                                                          \
+    do {                                                                  \
+        cudaError_t e_ = (call);                                          \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);          \
+    } while (0)
+#define CKL(call)                                                         \
+    do {                                                                  \
+        int e_ = (call);                                                  \
+        if (e_ != 0) return cuda_fail(ctx, (cudaError_t)e_, #call);       \
+    } while (0)
+#define RET(call)                     \
+    do {                              \
+        int r_ = (call);              \
+        if (r_ != FRS_OK) return r_;  \
+    } while (0)
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1)) == 0; }
+
+struct Prof {
+    frs_ctx* c; int kind; cudaEvent_t a = nullptr, b = nullptr;
+    Prof(frs_ctx* c_, int kind_) : c(c_), kind(kind_) {
+        if (c->profiling) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, c->stream); }
+    }
+    ~Prof() {
+        if (c->profiling) { cudaEventRecord(b, c->stream); c->prof.push_back({kind, a, b}); }
+    }
+};
+
+template <typename T>
+int dev_alloc(frs_ctx* ctx, T** p, size_t count) {
+    if (*p) return FRS_OK;
+    CK(cudaMalloc(reinterpret_cast<void**>(p), count * sizeof(T)));
+    return FRS_OK;
+}
+
+int ensure_tables(frs_ctx* ctx, int n) {
+    if (ctx->tw.count(n)) return FRS_OK;
+    std::vector<float2> tw = build_twiddles(n), ts = build_twist(n);
+    float2 *dtw = nullptr, *dts = nullptr;
+    CK(cudaMalloc(reinterpret_cast<void**>(&dtw), tw.size() * sizeof(float2)));
+    CK(cudaMalloc(reinterpret_cast<void**>(&dts), ts.size() * sizeof(float2)));
+    CK(cudaMemcpy(dtw, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(dts, ts.data(), ts.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    ctx->tw[n] = dtw;
+    ctx->twist[n] = dts;
+    return FRS_OK;
+}
+
+int ensure_scratch(frs_ctx* ctx) {
+    const size_t np = ctx->npix;
+    RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * ctx->ntile * ctx->ny * 2));
+    RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * ctx->ntile_h * ctx->ny * 2));
+    RET(dev_alloc(ctx, &ctx->lin, 2 * np));
+    RET(dev_alloc(ctx, &ctx->acc, 2 * np));
+    RET(dev_alloc(ctx, &ctx->img, (size_t)ctx->nchan * np));
+    RET(dev_alloc(ctx, &ctx->s, (size_t)ctx->nchan * np));
+    return FRS_OK;
+}
+
+int red_blocks(size_t n) {
+    size_t b = (n / 4 + kRedThreads - 1) / kRedThreads;
+    return (int)(b < 1 ? 1 : (b > (size_t)kMaxRedBlocks ? kMaxRedBlocks : b));
+}
+
+// out = sum a.b  -> device double
+int dot(frs_ctx* ctx, const float* a, const float* b, size_t n, double* d_out) {
+    const int nb = red_blocks(n);
+    dot_partial_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(a, b, n, ctx->partials);
+    reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, d_out);
+    ctx->launches += 2;
+    CK(cudaGetLastError());
+    return FRS_OK;
+}
+
+// ---- the three passes of C (Eq. 14) -----------------------------------------------------------
+int conv_rows_fwd(frs_ctx* ctx, const float* in, const float* mul) {
+    Prof pr(ctx, kPassRowsFwd);
+    RowsFwdArgs a{};
+    a.in = in; a.mul = mul; a.out = ctx->T; a.ny = ctx->ny;
+    a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)ctx->ntile * ctx->ny * 2;
+    a.scale = 1.0f;   // yields 2 X[k]; the 1/2 is folded into wt
+    a.tw = ctx->tw[ctx->nx]; a.twist = ctx->twist[ctx->nx];
+    CKL(launch_rows_fwd(ctx->stream, ctx->nx, true, a, ctx->nchan));
+    ctx->launches++;
+    return FRS_OK;
+}
+int conv_cols(frs_ctx* ctx) {
+    Prof pr(ctx, kPassConvCols);
+    ConvColsArgs a{};
+    a.t = ctx->T; a.wt = ctx->wt; a.ntile = ctx->ntile;
+    a.t_bstride = (size_t)ctx->ntile * ctx->ny * 2; a.w_bstride = (size_t)ctx->ntile * 2 * ctx->ny * 2;
+    a.tw = ctx->tw[ctx->ny]; a.twist = ctx->twist[ctx->ny];
+    CKL(launch_conv_cols(ctx->stream, ctx->ny, a, ctx->nchan));
+    ctx->launches++;
+    return FRS_OK;
+}
+int conv_rows_inv(frs_ctx* ctx, float* out, int mode, int* grid_x) {
+    Prof pr(ctx, kPassRowsInv);
+    RowsInvArgs a{};
+    a.t = ctx->T; a.out = out; a.s = ctx->s; a.j = ctx->dirty; a.partials = ctx->partials;
+    a.ny = ctx->ny; a.mode = mode;
+    a.t_bstride = (size_t)ctx->ntile * ctx->ny * 2; a.img_bstride = ctx->npix;
+    a.tw = ctx->tw[ctx->nx]; a.twist = ctx->twist[ctx->nx];
+    CKL(launch_rows_inv(ctx->stream, ctx->nx, a, ctx->nchan, grid_x));
+    ctx->launches++;
+    return FRS_OK;
+}
+
+// out[b] = (mul .) H[ premul . in[b] ] (+ offset[b]) (+ add)     -- 2-D Hartley transform, two passes
+int hartley(frs_ctx* ctx, const float* in, const float* premul, float* out, const float* mul, const float* add,
+            const float* offset_dev, int nb) {
+    {
+        Prof pr(ctx, kPassHartRows);
+        RowsFwdArgs a{};
+        a.in = in; a.mul = premul; a.out = ctx->Th; a.ny = ctx->ny;
+        a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)ctx->ntile_h * ctx->ny * 2;
+        a.scale = 0.5f;
+        a.tw = ctx->tw[ctx->nx / 2]; a.twist = ctx->twist[ctx->nx / 2];
+        CKL(launch_rows_fwd(ctx->stream, ctx->nx / 2, false, a, nb));
+        ctx->launches++;
+    }
+    {
+        Prof pr(ctx, kPassHartCols);
+        HartColsArgs a{};
+        a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = ctx->nx;
+        a.t_bstride = (size_t)ctx->ntile_h * ctx->ny * 2; a.img_bstride = ctx->npix;
+        a.tw = ctx->tw[ctx->ny];
+        CKL(launch_hart_cols(ctx->stream, ctx->ny, a, nb));
+        ctx->launches++;
+    }
+    return FRS_OK;
+}
+
+int ew_grid(size_t npix) { return (int)((npix / 4 + kEwThreads - 1) / kEwThreads); }
+
+int check_hot(frs_ctx* ctx, bool need_s, bool need_model) {
+    if (!ctx) return FRS_EINVAL;
+    if (!ctx->have_psf) return fail(ctx, FRS_ESTATE, "PSF not set (frs_set_psf / frs_set_psf_weights)");
+    if (need_model && !ctx->have_amp) return fail(ctx, FRS_ESTATE, "amplitude spectrum not set (frs_set_amplitude)");
+    if (need_s && !ctx->have_s) return fail(ctx, FRS_ESTATE, "no position set (frs_sky_forward / frs_energy_grad / frs_set_sky)");
+    return ensure_scratch(ctx);
+}
+
+int sky_forward_impl(frs_ctx* ctx, const float* xi) {
+    // tau_f = mu_f + H[A_f xi_f];  s_c = exp(tau_0 + lognu_c tau_1)      (R6)
+    RET(hartley(ctx, xi, ctx->amp, ctx->lin, nullptr, nullptr, ctx->d_mu, ctx->nfield));
+    sky_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->d_lognu, ctx->s, ctx->npix, ctx->nfield, ctx->nchan);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    ctx->have_s = true;
+    return FRS_OK;
+}
+
+int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out) {
+    // lin_f = H[A_f v_f]
+    RET(hartley(ctx, v, ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
+    const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
+    if (simple) {
+        RET(conv_rows_fwd(ctx, ctx->lin, ctx->s));                 // s . lin fused into the row pass
+    } else {
+        jvp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->s, ctx->d_lognu, ctx->img,
+                                                                               ctx->npix, ctx->nfield, ctx->nchan);
+        ctx->launches++;
+        RET(conv_rows_fwd(ctx, ctx->img, nullptr));
+    }
+    RET(conv_cols(ctx));
+    if (simple) {
+        RET(conv_rows_inv(ctx, ctx->acc, kMulS, nullptr));         // acc = s . C(...)
+    } else {
+        RET(conv_rows_inv(ctx, ctx->img, kMulS, nullptr));
+        vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
+                                                                               ctx->nfield, ctx->nchan);
+        ctx->launches++;
+    }
+    // out_f = A_f . H[acc_f] (+ v_f)
+    RET(hartley(ctx, ctx->acc, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield));
+    CK(cudaGetLastError());
+    return FRS_OK;
+}
+
+int cg_alloc(frs_ctx* ctx) {
+    const size_t n = (size_t)ctx->nfield * ctx->npix;
+    RET(dev_alloc(ctx, &ctx->cg_r, 2 * ctx->npix));
+    RET(dev_alloc(ctx, &ctx->cg_p, 2 * ctx->npix));
+    RET(dev_alloc(ctx, &ctx->cg_q, 2 * ctx->npix));
+    (void)n;
+    return FRS_OK;
+}
+
+// one iteration from (x, r, p, scal[kRR]); leaves scal[kRR] = new <r,r>
+int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k) {
+    const size_t n = (size_t)ctx->nfield * ctx->npix;
+    const int nb = red_blocks(n);
+    RET(metric_apply_impl(ctx, ctx->cg_p, with_prior, ctx->cg_q));
+    RET(dot(ctx, ctx->cg_p, ctx->cg_q, n, ctx->scal + kPQ));
+    cg_update_xr_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(x, ctx->cg_r, ctx->cg_p, ctx->cg_q, n, ctx->scal, ctx->partials);
+    reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, ctx->scal + kRRNew);
+    cg_update_p_kernel<<<nb, kEwThreads, 0, ctx->stream>>>(ctx->cg_p, ctx->cg_r, n, ctx->scal, ctx->scal + kBeta);
+    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_hist, k + 1);
+    ctx->launches += 4;
+    CK(cudaGetLastError());
+    return FRS_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+const char* frs_version(void) { return "frs 0.1 (sm_100a; register-Stockham FFT passes)"; }
+
+const char* frs_last_error(const frs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+long long frs_launch_count(const frs_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int frs_create(int ny, int nx, int nchan, int device, void* stream, frs_ctx** out) {
+    if (!out) return FRS_EINVAL;
+    *out = nullptr;
+    if (!pow2_in(ny, 32, 4096) || !pow2_in(nx, 32, 4096) || nchan < 1) return FRS_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return FRS_ECUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return FRS_ECUDA;
+    frs_ctx* ctx = new frs_ctx();
+    ctx->ny = ny; ctx->nx = nx; ctx->nchan = nchan; ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(stream);
+    ctx->npix = (size_t)ny * nx;
+    ctx->ntile = nx / 2 + 1;
+    ctx->ntile_h = nx / 4 + 1;
+    int rc = FRS_OK;
+    auto init = [&]() -> int {
+        RET(ensure_tables(ctx, nx));
+        RET(ensure_tables(ctx, ny));
+        RET(ensure_tables(ctx, nx / 2));
+        RET(dev_alloc(ctx, &ctx->partials, (size_t)1 << 16));
+        RET(dev_alloc(ctx, &ctx->scal, 16));
+        RET(dev_alloc(ctx, &ctx->flag, 4));
+        RET(dev_alloc(ctx, &ctx->d_mu, 2));
+        RET(dev_alloc(ctx, &ctx->d_lognu, (size_t)nchan));
+        CK(cudaMemset(ctx->scal, 0, 16 * sizeof(double)));
+        CK(cudaMemset(ctx->d_mu, 0, 2 * sizeof(float)));
+        CK(cudaMemset(ctx->d_lognu, 0, nchan * sizeof(float)));
+        return FRS_OK;
+    };
+    rc = init();
+    if (rc != FRS_OK) { frs_destroy(ctx); return rc; }
+    *out = ctx;
+    return FRS_OK;
+}
+
+void frs_destroy(frs_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (auto& kv : ctx->tw) cudaFree(kv.second);
+    for (auto& kv : ctx->twist) cudaFree(kv.second);
+    void* ptrs[] = {ctx->wt, ctx->dirty, ctx->amp, ctx->s, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->Th, ctx->lin, ctx->img,
+                    ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    delete ctx;
+}
+
+int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
+    if (!ctx || !w_half || !aligned16(w_half)) return fail(ctx, FRS_EINVAL, "frs_set_psf_weights: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(dev_alloc(ctx, &ctx->wt, (size_t)ctx->nchan * ctx->ntile * 2 * ctx->ny * 2));
+    CK(cudaMemsetAsync(ctx->flag, 0, sizeof(int), ctx->stream));
+    CKL(launch_weights_layout(ctx->stream, w_half, ctx->wt, ctx->ny, ctx->nx, ctx->nchan, ctx->flag));
+    ctx->launches++;
+    int neg = 0;
+    CK(cudaMemcpyAsync(&neg, ctx->flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (neg) { ctx->have_psf = false; return fail(ctx, FRS_ENOTPSD, "PSF weights contain negative or NaN entries"); }
+    ctx->have_psf = true;
+    return FRS_OK;
+}
+
+int frs_set_psf(frs_ctx* ctx, const float* psf) {
+    if (!ctx || !psf || !aligned16(psf)) return fail(ctx, FRS_EINVAL, "frs_set_psf: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    const int my = 2 * ctx->ny, mx = 2 * ctx->nx;
+    RET(dev_alloc(ctx, &ctx->wt, (size_t)ctx->nchan * ctx->ntile * 2 * ctx->ny * 2));
+    // row pass over all 2 ny rows of length 2 nx (no padding), then one DIF step + ny-point column FFTs
+    float2* tmp = nullptr;
+    float* stats = nullptr;
+    const size_t tstride = (size_t)ctx->ntile * my * 2;
+    CK(cudaMalloc(reinterpret_cast<void**>(&tmp), (size_t)ctx->nchan * tstride * sizeof(float2)));
+    int rc = FRS_OK;
+    std::vector<float> hs;
+    int gx = 0;
+    auto body = [&]() -> int {
+        RowsFwdArgs a{};
+        a.in = psf; a.mul = nullptr; a.out = tmp; a.ny = my;
+        a.in_bstride = (size_t)my * mx; a.mul_bstride = 0; a.out_bstride = tstride;
+        a.scale = 0.5f; a.tw = ctx->tw[ctx->nx]; a.twist = ctx->twist[ctx->nx];
+        CKL(launch_rows_fwd(ctx->stream, ctx->nx, false, a, ctx->nchan));
+        PsfColsArgs c{};
+        c.t = nullptr; c.ntile = ctx->ntile;
+        CKL(launch_psf_cols(ctx->stream, ctx->ny, c, ctx->nchan, &gx));   // grid size only
+        CK(cudaMalloc(reinterpret_cast<void**>(&stats), (size_t)ctx->nchan * gx * 3 * sizeof(float)));
+        c.t = tmp; c.wt = ctx->wt; c.stats = stats; c.scale = 1.0f / ((float)my * (float)mx);
+        c.t_bstride = tstride; c.w_bstride = (size_t)ctx->ntile * 2 * ctx->ny * 2;
+        c.tw = ctx->tw[ctx->ny]; c.twist = ctx->twist[ctx->ny];
+        CKL(launch_psf_cols(ctx->stream, ctx->ny, c, ctx->nchan, nullptr));
+        ctx->launches += 2;
+        hs.resize((size_t)ctx->nchan * gx * 3);
+        CK(cudaMemcpyAsync(hs.data(), stats, hs.size() * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        return FRS_OK;
+    };
+    rc = body();
+    cudaFree(tmp);
+    if (stats) cudaFree(stats);
+    if (rc != FRS_OK) return rc;
+    float max_im = 0.f, min_re = 0.f, max_re = 0.f;
+    for (size_t i = 0; i < hs.size(); i += 3) {
+        max_im = fmaxf(max_im, hs[i]); min_re = fminf(min_re, hs[i + 1]); max_re = fmaxf(max_re, hs[i + 2]);
+    }
+    if (!(max_im <= 1e-5f * max_re) || !(min_re >= -1e-5f * max_re)) {
+        ctx->have_psf = false;
+        snprintf(ctx->err, sizeof(ctx->err), "PSF spectrum not real/non-negative: max|Im|=%g min Re=%g max Re=%g", max_im, min_re, max_re);
+        return FRS_ENOTPSD;
+    }
+    ctx->have_psf = true;
+    return FRS_OK;
+}
+
+int frs_set_dirty(frs_ctx* ctx, const float* j) {
+    if (!ctx || !j || !aligned16(j)) return fail(ctx, FRS_EINVAL, "frs_set_dirty: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(dev_alloc(ctx, &ctx->dirty, (size_t)ctx->nchan * ctx->npix));
+    CK(cudaMemcpyAsync(ctx->dirty, j, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    ctx->have_dirty = true;
+    return FRS_OK;
+}
+
+int frs_set_amplitude(frs_ctx* ctx, int nfield, const float* amp, const float* mu_host) {
+    if (!ctx || !amp || !mu_host || !aligned16(amp) || nfield < 1 || nfield > 2)
+        return fail(ctx, FRS_EINVAL, "frs_set_amplitude: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(dev_alloc(ctx, &ctx->amp, 2 * ctx->npix));
+    CK(cudaMemcpyAsync(ctx->amp, amp, (size_t)nfield * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    float mu[2] = {mu_host[0], nfield == 2 ? mu_host[1] : 0.f};
+    CK(cudaMemcpyAsync(ctx->d_mu, mu, sizeof(mu), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->nfield = nfield;
+    ctx->have_amp = true;
+    ctx->have_s = false;
+    return FRS_OK;
+}
+
+int frs_set_channel_lognu(frs_ctx* ctx, const float* lognu_host) {
+    if (!ctx || !lognu_host) return fail(ctx, FRS_EINVAL, "frs_set_channel_lognu: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemcpyAsync(ctx->d_lognu, lognu_host, ctx->nchan * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->have_s = false;
+    return FRS_OK;
+}
+
+int frs_set_sky(frs_ctx* ctx, const float* sky) {
+    if (!ctx || !sky || !aligned16(sky)) return fail(ctx, FRS_EINVAL, "frs_set_sky: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(ensure_scratch(ctx));
+    CK(cudaMemcpyAsync(ctx->s, sky, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    ctx->have_s = true;
+    return FRS_OK;
+}
+
+int frs_sky_forward(frs_ctx* ctx, const float* xi, float* sky) {
+    if (!ctx || !xi || !aligned16(xi) || (sky && !aligned16(sky))) return fail(ctx, FRS_EINVAL, "frs_sky_forward: bad argument");
+    if (!ctx->have_amp) return fail(ctx, FRS_ESTATE, "amplitude spectrum not set (frs_set_amplitude)");
+    CK(cudaSetDevice(ctx->device));
+    RET(ensure_scratch(ctx));
+    RET(sky_forward_impl(ctx, xi));
+    if (sky) CK(cudaMemcpyAsync(sky, ctx->s, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    return FRS_OK;
+}
+
+int frs_psf_apply(frs_ctx* ctx, const float* x, float* y) {
+    if (!ctx || !x || !y || !aligned16(x) || !aligned16(y)) return fail(ctx, FRS_EINVAL, "frs_psf_apply: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, false, false));
+    RET(conv_rows_fwd(ctx, x, nullptr));
+    RET(conv_cols(ctx));
+    RET(conv_rows_inv(ctx, y, kPlain, nullptr));
+    return FRS_OK;
+}
+
+int frs_sky_metric_apply(frs_ctx* ctx, const float* x, float* y) {
+    if (!ctx || !x || !y || !aligned16(x) || !aligned16(y)) return fail(ctx, FRS_EINVAL, "frs_sky_metric_apply: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, false));
+    RET(conv_rows_fwd(ctx, x, ctx->s));
+    RET(conv_cols(ctx));
+    RET(conv_rows_inv(ctx, y, kMulS, nullptr));
+    return FRS_OK;
+}
+
+int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_energy, double* h_energy, float* grad) {
+    if (!ctx || !xi || !grad || !aligned16(xi) || !aligned16(grad)) return fail(ctx, FRS_EINVAL, "frs_energy_grad: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, false, true));
+    if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
+    RET(sky_forward_impl(ctx, xi));
+    RET(conv_rows_fwd(ctx, ctx->s, nullptr));
+    RET(conv_cols(ctx));
+    int gx = 0;
+    RET(conv_rows_inv(ctx, ctx->img, kEnergy, &gx));          // img_c = s_c (C s_c - j_c), partial sums
+    const int np = gx * ctx->nchan;
+    reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, np, 2, 0, ctx->scal + 8);
+    reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, np, 2, 1, ctx->scal + 9);
+    ctx->launches += 2;
+    if (with_prior) RET(dot(ctx, xi, xi, (size_t)ctx->nfield * ctx->npix, ctx->scal + 10));
+    energy_final_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal + 8, ctx->scal + 9, ctx->scal + 10, with_prior, ctx->scal + 11);
+    ctx->launches++;
+    const float* accp = ctx->img;
+    if (!(ctx->nchan == 1 && ctx->nfield == 1)) {
+        vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
+                                                                               ctx->nfield, ctx->nchan);
+        ctx->launches++;
+        accp = ctx->acc;
+    }
+    RET(hartley(ctx, accp, nullptr, grad, ctx->amp, with_prior ? xi : nullptr, nullptr, ctx->nfield));
+    CK(cudaGetLastError());
+    if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    if (h_energy) {
+        CK(cudaMemcpyAsync(h_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    return FRS_OK;
+}
+
+int frs_metric_apply(frs_ctx* ctx, const float* v, int with_prior, float* out) {
+    if (!ctx || !v || !out || !aligned16(v) || !aligned16(out) || v == out) return fail(ctx, FRS_EINVAL, "frs_metric_apply: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, true));
+    return metric_apply_impl(ctx, v, with_prior, out);
+}
+
+int frs_cg_state(frs_ctx* ctx, float** r, float** p, float** q, double** d_scal) {
+    if (!ctx) return FRS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    RET(cg_alloc(ctx));
+    if (r) *r = ctx->cg_r;
+    if (p) *p = ctx->cg_p;
+    if (q) *q = ctx->cg_q;
+    if (d_scal) *d_scal = ctx->scal;
+    return FRS_OK;
+}
+
+int frs_cg_load(frs_ctx* ctx, const float* r, const float* p, double rr_host) {
+    if (!ctx || !r || !p) return fail(ctx, FRS_EINVAL, "frs_cg_load: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    if (!ctx->have_amp) return fail(ctx, FRS_ESTATE, "amplitude spectrum not set");
+    RET(cg_alloc(ctx));
+    const size_t bytes = (size_t)ctx->nfield * ctx->npix * sizeof(float);
+    CK(cudaMemcpyAsync(ctx->cg_r, r, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->cg_p, p, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    double sc[kNScal] = {0};
+    sc[kRR] = rr_host;
+    CK(cudaMemcpyAsync(ctx->scal, sc, sizeof(sc), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return FRS_OK;
+}
+
+int frs_cg_step(frs_ctx* ctx, float* x, int with_prior) {
+    if (!ctx || !x || !aligned16(x)) return fail(ctx, FRS_EINVAL, "frs_cg_step: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, true));
+    RET(cg_alloc(ctx));
+    return cg_iter(ctx, x, with_prior, nullptr, 0);
+}
+
+int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,
+                 double* h_resnorm, double* d_res_history) {
+    if (!ctx || !b || !x || !aligned16(b) || !aligned16(x) || max_iter < 0 || rtol < 0.f || b == x)
+        return fail(ctx, FRS_EINVAL, "frs_cg_solve: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, true));
+    RET(cg_alloc(ctx));
+    const size_t n = (size_t)ctx->nfield * ctx->npix;
+    const int nb = red_blocks(n);
+    CK(cudaMemsetAsync(ctx->scal, 0, kNScal * sizeof(double), ctx->stream));
+    // r0 = b - M x0 ; p0 = r0
+    RET(metric_apply_impl(ctx, x, with_prior, ctx->cg_q));
+    cg_init_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(b, ctx->cg_q, ctx->cg_r, ctx->cg_p, n, ctx->partials);
+    reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, ctx->scal + kRRNew);
+    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_res_history, 0);
+    ctx->launches += 3;
+    double bb = 0.0;
+    if (rtol > 0.f) {
+        RET(dot(ctx, b, b, n, ctx->scal + kBB));
+        CK(cudaMemcpyAsync(&bb, ctx->scal + kBB, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    int it = 0;
+    double sc[kNScal];
+    for (; it < max_iter; ++it) {
+        if (rtol > 0.f) {
+            CK(cudaMemcpyAsync(sc, ctx->scal, sizeof(sc), cudaMemcpyDeviceToHost, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+            if (sc[kRR] <= (double)rtol * (double)rtol * bb || sc[kBreak] != 0.0) break;
+        }
+        RET(cg_iter(ctx, x, with_prior, d_res_history, it));
+    }
+    CK(cudaMemcpyAsync(sc, ctx->scal, sizeof(sc), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (h_iters) *h_iters = it;
+    if (h_resnorm) *h_resnorm = sqrt(sc[kRR]);
+    if (sc[kBreak] != 0.0) return fail(ctx, FRS_EBREAKDOWN, "CG breakdown: <p, M p> <= 0");
+    return FRS_OK;
+}
+
+static int host_apply(frs_ctx* ctx, const float* xh, float* yh, bool with_s) {
+    if (!ctx || !xh || !yh) return fail(ctx, FRS_EINVAL, "host apply: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, with_s, false));
+    const size_t n = (size_t)ctx->nchan * ctx->npix;
+    RET(dev_alloc(ctx, &ctx->hx, n));
+    RET(dev_alloc(ctx, &ctx->hy, n));
+    CK(cudaMemcpyAsync(ctx->hx, xh, n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    RET(conv_rows_fwd(ctx, ctx->hx, with_s ? ctx->s : nullptr));
+    RET(conv_cols(ctx));
+    RET(conv_rows_inv(ctx, ctx->hy, with_s ? kMulS : kPlain, nullptr));
+    CK(cudaMemcpyAsync(yh, ctx->hy, n * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return FRS_OK;
+}
+int frs_sky_metric_apply_host(frs_ctx* ctx, const float* x_host, float* y_host) { return host_apply(ctx, x_host, y_host, true); }
+int frs_psf_apply_host(frs_ctx* ctx, const float* x_host, float* y_host) { return host_apply(ctx, x_host, y_host, false); }
+
+int frs_profile_enable(frs_ctx* ctx, int on) {
+    if (!ctx) return FRS_EINVAL;
+    ctx->profiling = on != 0;
+    return FRS_OK;
+}
+
+int frs_profile_read(frs_ctx* ctx, double ms[5], long long launches[5]) {
+    if (!ctx || !ms || !launches) return FRS_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < kNPass; ++i) { ms[i] = 0.0; launches[i] = 0; }
+    for (auto& r : ctx->prof) {
+        float t = 0.f;
+        cudaEventElapsedTime(&t, r.a, r.b);
+        ms[r.kind] += t;
+        launches[r.kind]++;
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    ctx->prof.clear();
+    return FRS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,114 @@
+// k_setup.cu -- untimed setup: PSF -> weight-spectrum layout (P:180 'FFT[I^PSF]' precomputed)
+#include "launch.h"
+#include "setup.h"
+namespace frs {
+
+// Column pass of the full (not zero-padded) 2NF-point DFT of the row-transformed PSF by one
+// decimation-in-frequency step: even bins = FFT_NF(x[n] + x[n+NF]), odd = FFT_NF((x[n] - x[n+NF]) twist^n).
+template <int NF>
+__global__ void __launch_bounds__(Geo<NF, 2>::THREADS, (Geo<NF, 2>::THREADS >= 512 ? 1 : 2))
+psf_cols_kernel(PsfColsArgs a) {
+    using GEO = Geo<NF, 2>;
+    constexpr int P = GEO::P;
+    extern __shared__ float2 smem[];
+    const int g = threadIdx.x / (2 * P), role = (threadIdx.x / P) & 1, p = threadIdx.x % P;
+    float2* bufs = smem + (size_t)g * 4 * xbuf_len(NF) + role * 2 * xbuf_len(NF);
+    const int m = blockIdx.x * GEO::G + g;
+    const int b = blockIdx.y;
+    const bool live = m < a.ntile;
+    float2 v[2][kE];
+#pragma unroll
+    for (int e = 0; e < kE; ++e) { v[0][e] = make_float2(0.f, 0.f); v[1][e] = make_float2(0.f, 0.f); }
+    if (live) {
+        const float4* tile = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + (size_t)m * 2 * NF;
+#pragma unroll
+        for (int e = 0; e < kE; ++e) {
+            const int n = p + e * P;
+            const float4 x0 = ldg4(tile + n), x1 = ldg4(tile + n + NF);
+            if (!role) {
+                v[0][e] = make_float2(x0.x + x1.x, x0.y + x1.y);
+                v[1][e] = make_float2(x0.z + x1.z, x0.w + x1.w);
+            } else {
+                const float2 w = __ldg(a.twist + n);
+                v[0][e] = cmul(make_float2(x0.x - x1.x, x0.y - x1.y), w);
+                v[1][e] = cmul(make_float2(x0.z - x1.z, x0.w - x1.w), w);
+            }
+        }
+    }
+    group_fft<NF, false, 2>(v, p, bufs, a.tw);
+    float max_im = 0.f, min_re = 0.f, max_re = 0.f;
+    if (live) {
+        float2* w = reinterpret_cast<float2*>(a.wt + b * a.w_bstride) + ((size_t)m * 2 + role) * NF;
+#pragma unroll
+        for (int e = 0; e < kE; ++e) {
+            const float re0 = v[0][e].x * a.scale, re1 = v[1][e].x * a.scale;
+            max_im = fmaxf(max_im, fmaxf(fabsf(v[0][e].y), fabsf(v[1][e].y)) * a.scale);
+            min_re = fminf(min_re, fminf(re0, re1));
+            max_re = fmaxf(max_re, fmaxf(re0, re1));
+            w[p + e * P] = make_float2(0.5f * fmaxf(re0, 0.f), 0.5f * fmaxf(re1, 0.f));
+        }
+    }
+    __shared__ float red[3][32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        max_im = fmaxf(max_im, __shfl_down_sync(0xffffffffu, max_im, o));
+        min_re = fminf(min_re, __shfl_down_sync(0xffffffffu, min_re, o));
+        max_re = fmaxf(max_re, __shfl_down_sync(0xffffffffu, max_re, o));
+    }
+    const int wid = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) { red[0][wid] = max_im; red[1][wid] = min_re; red[2][wid] = max_re; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < (int)(blockDim.x >> 5); ++i) {
+            max_im = fmaxf(max_im, red[0][i]); min_re = fminf(min_re, red[1][i]); max_re = fmaxf(max_re, red[2][i]);
+        }
+        float* s = a.stats + ((size_t)b * gridDim.x + blockIdx.x) * 3;
+        s[0] = max_im; s[1] = min_re; s[2] = max_re;
+    }
+}
+
+template <int NF>
+static int run(cudaStream_t st, const PsfColsArgs& a, int nb, int* grid_x) {
+    using GEO = Geo<NF, 2>;
+    static bool attr = false;
+    if (!attr) { cudaError_t e = set_smem(psf_cols_kernel<NF>, GEO::SMEM); if (e != cudaSuccess) return (int)e; attr = true; }
+    dim3 grid((a.ntile + GEO::G - 1) / GEO::G, nb);
+    if (grid_x) *grid_x = grid.x;
+    if (a.t) psf_cols_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
+    return (int)cudaGetLastError();
+}
+int launch_psf_cols(cudaStream_t st, int nf, const PsfColsArgs& a, int nb, int* grid_x) {
+#define CALL(N) return run<N>(st, a, nb, grid_x)
+    FRS_DISPATCH_NF(nf, CALL)
+#undef CALL
+    return 0;
+}
+
+// w_half [nb][2ny][nx+1]  ->  wt [nb][ntile][2][ny][2] = 0.5 * W[2q+par][2m+c]  (0 beyond kx = nx)
+__global__ void weights_layout_kernel(const float* __restrict__ w_half, float* __restrict__ wt, int ny, int nx,
+                                      int* __restrict__ neg_flag) {
+    const int ntile = nx / 2 + 1;
+    const size_t per = (size_t)ntile * 2 * ny * 2;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= per) return;
+    const int b = blockIdx.y;
+    const int c = i & 1;
+    const int q = (i >> 1) % ny;
+    const int par = ((i >> 1) / ny) & 1;
+    const int m = (int)((i >> 1) / ny / 2);
+    const int kx = 2 * m + c, ky = 2 * q + par;
+    float v = 0.f;
+    if (kx <= nx) {
+        v = w_half[(size_t)b * (2 * ny) * (nx + 1) + (size_t)ky * (nx + 1) + kx];
+        if (!(v >= 0.f)) atomicExch(neg_flag, 1);
+    }
+    wt[(size_t)b * per + i] = 0.5f * v;
+}
+int launch_weights_layout(cudaStream_t st, const float* w_half, float* wt, int ny, int nx, int nb, int* neg_flag) {
+    const size_t per = (size_t)(nx / 2 + 1) * 2 * ny * 2;
+    dim3 grid((unsigned)((per + 255) / 256), nb);
+    weights_layout_kernel<<<grid, 256, 0, st>>>(w_half, wt, ny, nx, neg_flag);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace frs

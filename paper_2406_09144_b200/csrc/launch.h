@@ -1,0 +1,50 @@
+// launch.h -- size-dispatching launchers of the FFT passes (one translation unit per pass so the
+// template instantiations compile in parallel).  Return cudaError_t as int.
+#pragma once
+#include <cuda_runtime.h>
+#include "kernels.cuh"
+
+namespace frs {
+
+// valid transform lengths
+inline bool valid_nf(int nf) { return nf >= 16 && nf <= 4096 && (nf & (nf - 1)) == 0; }
+
+// rows: number of image rows (even).  nf: complex transform length (PAD: nf = nx; else nf = nx/2).
+int launch_rows_fwd(cudaStream_t st, int nf, bool pad, const RowsFwdArgs& a, int nb);
+int launch_conv_cols(cudaStream_t st, int nf, const ConvColsArgs& a, int nb);
+int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* grid_x);
+int rows_inv_grid_x(int nf, int ny);
+int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb);
+
+struct PsfColsArgs {
+    const float2* t;      // [nb][ntile][2 NF][2]  row-transformed PSF, all 2 NF rows
+    float* wt;            // [nb][ntile][2][NF][2]
+    float* stats;         // [nb][gridDim.x][3]: max |Im W|, min Re W, max Re W   (unscaled by fold)
+    int ntile;
+    float scale;          // 1 / (My Mx)
+    size_t t_bstride, w_bstride;
+    const float2* tw;
+    const float2* twist;
+};
+int launch_psf_cols(cudaStream_t st, int nf, const PsfColsArgs& a, int nb, int* grid_x);
+
+#define FRS_DISPATCH_NF(nf, CALL)                 \
+    switch (nf) {                                 \
+        case 16: { CALL(16); } break;             \
+        case 32: { CALL(32); } break;             \
+        case 64: { CALL(64); } break;             \
+        case 128: { CALL(128); } break;           \
+        case 256: { CALL(256); } break;           \
+        case 512: { CALL(512); } break;           \
+        case 1024: { CALL(1024); } break;         \
+        case 2048: { CALL(2048); } break;         \
+        case 4096: { CALL(4096); } break;         \
+        default: return (int)cudaErrorInvalidValue; \
+    }
+
+template <typename K>
+inline cudaError_t set_smem(K kernel, int bytes) {
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+}  // namespace frs

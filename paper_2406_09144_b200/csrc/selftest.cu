@@ -1,0 +1,56 @@
+// selftest.cu -- CPU replay of the register/shared-memory FFT logic of fft_core.cuh, thread by
+// thread, with the "shared memory" exchange emulated by a host array.  Lets the index maps, plans
+// and twiddle tables be tested where there is no GPU (tests/test_host_logic.py).
+#include <vector>
+#include "../../include/frs.h"
+#include "fft_core.cuh"
+#include "tables.h"
+
+namespace frs {
+struct Regs { float2 v[1][kE]; };
+
+template <int N, bool INV, int S>
+static void emu_from(std::vector<Regs>& regs, std::vector<float2>& buf, const float2* tw) {
+    constexpr int P = N / kE;
+    if constexpr (S < plan_stages(N)) {
+        for (int p = 0; p < P; ++p) stage_compute<N, S, INV, 1>(regs[p].v, p, tw);
+        if constexpr (S + 1 < plan_stages(N)) {
+            for (int p = 0; p < P; ++p) stage_scatter<N, S>(regs[p].v[0], p, buf.data());
+            for (int p = 0; p < P; ++p) canon_gather<N>(regs[p].v[0], p, buf.data());
+        }
+        emu_from<N, INV, S + 1>(regs, buf, tw);
+    }
+}
+template <int N>
+static int emu(int inverse, const float2* in, float2* out) {
+    constexpr int P = N / kE;
+    std::vector<float2> tw = build_twiddles(N);
+    std::vector<Regs> regs(P);
+    std::vector<float2> buf(xbuf_len(N));
+    for (int p = 0; p < P; ++p)
+        for (int e = 0; e < kE; ++e) regs[p].v[0][e] = in[p + e * P];
+    if (inverse) emu_from<N, true, 0>(regs, buf, tw.data());
+    else emu_from<N, false, 0>(regs, buf, tw.data());
+    for (int p = 0; p < P; ++p)
+        for (int e = 0; e < kE; ++e) out[p + e * P] = regs[p].v[0][e];
+    return 0;
+}
+}  // namespace frs
+
+extern "C" int frs_selftest_fft_host(int n, int inverse, const float* in, float* out) {
+    if (!in || !out) return FRS_EINVAL;
+    const float2* i2 = reinterpret_cast<const float2*>(in);
+    float2* o2 = reinterpret_cast<float2*>(out);
+    switch (n) {
+        case 16: return frs::emu<16>(inverse, i2, o2);
+        case 32: return frs::emu<32>(inverse, i2, o2);
+        case 64: return frs::emu<64>(inverse, i2, o2);
+        case 128: return frs::emu<128>(inverse, i2, o2);
+        case 256: return frs::emu<256>(inverse, i2, o2);
+        case 512: return frs::emu<512>(inverse, i2, o2);
+        case 1024: return frs::emu<1024>(inverse, i2, o2);
+        case 2048: return frs::emu<2048>(inverse, i2, o2);
+        case 4096: return frs::emu<4096>(inverse, i2, o2);
+        default: return FRS_EINVAL;
+    }
+}

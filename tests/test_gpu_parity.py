@@ -1,0 +1,395 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded fp32-rounded inputs.  Tolerances (BASELINE.json north_star): relative L2 <= 1e-5 for sky,
+convolution and gradient, <= 1e-4 after 20 CG iterations; exact for index/padding layouts."""
+import numpy as np
+import pytest
+
+from gen import workloads as wl
+from oracle import frs_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+def rel(a, b):
+    a = np.asarray(a, np.float64)
+    b = np.asarray(b, np.float64)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+@pytest.fixture(scope="module")
+def frs():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2406_09144_b200 as m
+    m.load_library()
+    return m
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def make_ctx(frs, w, with_model=True):
+    ctx = frs.Context(w.ny, w.nx, w.nchan)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    if with_model:
+        ctx.set_amplitude(dev(w.amp), w.mu)
+        ctx.set_channel_lognu(w.lognu)
+    return ctx
+
+
+_CACHE = {}
+
+
+def workload(key):
+    if key not in _CACHE:
+        kind = key[0]
+        if kind == "c1":
+            _CACHE[key] = wl.make_config(1)
+        elif kind == "c1b":
+            _CACHE[key] = wl.make_config(1, sigma_rel=0.1)
+        elif kind == "rect":
+            _CACHE[key] = wl.make_config(3, ny=key[1], nx=key[2])
+        elif kind == "sq":
+            _CACHE[key] = wl.make_config(key[1], n=key[2])
+        elif kind == "multi":
+            _CACHE[key] = wl.make_config(5, n=key[1], nchan=key[2])
+    return _CACHE[key]
+
+
+SHAPES = [("rect", 32, 32), ("rect", 64, 128), ("rect", 256, 64), ("sq", 2, 512), ("rect", 32, 1024), ("rect", 2048, 32)]
+
+
+# ---------------------------------------------------------------------------------- convolution (Eq. 14)
+@pytest.mark.parametrize("key", SHAPES)
+def test_psf_apply_matches_oracle(frs, key):
+    w = workload(key)
+    ctx = make_ctx(frs, w, with_model=False)
+    rng = np.random.default_rng(1)
+    x = rng.normal(size=(1, w.ny, w.nx)).astype(np.float32)
+    y = ctx.new_image()
+    ctx.psf_apply(dev(x), y)
+    ref = o.psf_apply(w.w_half[0], x[0])
+    assert rel(y.cpu().numpy()[0], ref) <= TOL
+    # truth-like positive input with point sources
+    ctx.psf_apply(dev(w.sky_true), y)
+    assert rel(y.cpu().numpy()[0], o.psf_apply(w.w_half[0], w.sky_true[0])) <= TOL
+
+
+def test_index_and_padding_layout_exact(frs):
+    """Integer-valued weights and delta images: results are small integers, compared exactly
+    (corner deltas exercise the wrapped half of the PSF and the crop)."""
+    ny, nx = 64, 128
+    w = wl.make_config(1, ny=ny, nx=nx, npts=300)
+    counts = w.w_counts.astype(np.float32)                        # small integers
+    assert counts.max() <= 8
+    ctx = frs.Context(ny, nx, 1)
+    ctx.set_psf_weights(dev(counts))
+    psf = np.rint(o.psf_from_weights(counts[0].astype(np.float64)))
+    y = ctx.new_image()
+    for (y0, x0) in [(0, 0), (0, nx - 1), (ny - 1, 0), (ny - 1, nx - 1), (17, 93)]:
+        d = np.zeros((1, ny, nx), np.float32)
+        d[0, y0, x0] = 1.0
+        ctx.psf_apply(dev(d), y)
+        got = y.cpu().numpy()[0].astype(np.float64)
+        exp = np.array([[psf[(a - y0) % (2 * ny), (b - x0) % (2 * nx)] for b in range(nx)] for a in range(ny)])
+        assert np.unravel_index(np.argmax(got), got.shape) == (y0, x0)
+        assert np.array_equal(np.rint(got), exp)
+        assert np.max(np.abs(got - exp)) < 2e-2                     # fp32 rounding of sums up to ~600
+
+
+def test_psf_apply_linearity_zero_and_symmetry(frs):
+    w = workload(("rect", 64, 128))
+    ctx = make_ctx(frs, w, with_model=False)
+    import torch
+    z = torch.zeros((1, w.ny, w.nx), device="cuda")
+    y = ctx.new_image()
+    ctx.psf_apply(z, y)
+    assert float(y.abs().max()) == 0.0
+    rng = np.random.default_rng(2)
+    a, b = rng.normal(size=(2, 1, w.ny, w.nx)).astype(np.float32)
+    ya, yb = ctx.new_image(), ctx.new_image()
+    ctx.psf_apply(dev(a), ya)
+    ctx.psf_apply(dev(b), yb)
+    lhs = float((ya.double() * dev(b).double()).sum())
+    rhs = float((dev(a).double() * yb.double()).sum())
+    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), abs(rhs), float(ya.double().norm() * np.linalg.norm(b)) * 1e-1)
+
+
+def test_set_psf_from_image_space_psf(frs):
+    w = workload(("rect", 64, 128))
+    psf = o.psf_from_weights(w.w_half[0].astype(np.float64)).astype(np.float32)
+    ctx = frs.Context(w.ny, w.nx, 1)
+    ctx.set_psf(dev(psf[None]))
+    x = np.random.default_rng(3).normal(size=(1, w.ny, w.nx)).astype(np.float32)
+    y = ctx.new_image()
+    ctx.psf_apply(dev(x), y)
+    ref = o.psf_apply(o.psf_spectrum_from_psf(psf.astype(np.float64))[0], x[0])
+    assert rel(y.cpu().numpy()[0], ref) <= 3e-5      # W itself went through an fp32 transform here
+    bad = psf.copy()
+    bad[1, 2] += 0.3 * psf[0, 0]
+    with pytest.raises(frs.FrsError) as e:
+        ctx.set_psf(dev(bad[None]))
+    assert e.value.code == frs.FRS_ENOTPSD
+
+
+def test_error_behaviour(frs):
+    import torch
+    with pytest.raises(frs.FrsError):
+        frs.Context(48, 64)
+    ctx = frs.Context(64, 64, 1)
+    x = torch.zeros((1, 64, 64), device="cuda")
+    with pytest.raises(frs.FrsError) as e:
+        ctx.psf_apply(x, ctx.new_image())                         # PSF not set
+    assert e.value.code == frs.FRS_ESTATE
+    neg = torch.full((1, 128, 65), -1.0, device="cuda")
+    with pytest.raises(frs.FrsError) as e:
+        ctx.set_psf_weights(neg)
+    assert e.value.code == frs.FRS_ENOTPSD
+    ctx.set_psf_weights(neg.abs())
+    with pytest.raises(frs.FrsError) as e:
+        ctx.sky_metric_apply(x, ctx.new_image())                  # no position
+    assert e.value.code == frs.FRS_ESTATE
+    with pytest.raises(ValueError):
+        ctx.psf_apply(torch.zeros((1, 64, 32), device="cuda"), ctx.new_image())
+
+
+# ---------------------------------------------------------------------------------- sky, L1 apply
+@pytest.mark.parametrize("key", [("c1",), ("rect", 64, 128), ("sq", 2, 512), ("multi", 64, 3)])
+def test_sky_forward_and_sky_metric_apply(frs, key):
+    w = workload(key)
+    ctx = make_ctx(frs, w)
+    rng = np.random.default_rng(4)
+    xi = (0.5 * rng.normal(size=(w.nfield, w.ny, w.nx))).astype(np.float32)
+    s = ctx.new_image()
+    ctx.sky_forward(dev(xi), s)
+    s_ref = o.sky(xi, w.amp, w.mu, w.lognu)
+    assert rel(s.cpu().numpy(), s_ref) <= TOL
+    x = rng.normal(size=(w.nchan, w.ny, w.nx)).astype(np.float32)
+    y = ctx.new_image()
+    ctx.sky_metric_apply(dev(x), y)
+    s32 = s.cpu().numpy()                      # teacher-forced on the GPU's own fp32 sky
+    ref = o.sky_metric_apply(w.w_half, s32, x)
+    for c in range(w.nchan):
+        assert rel(y.cpu().numpy()[c], ref[c]) <= TOL
+    # host-buffer entry point gives the same numbers
+    import torch
+    xh = torch.from_numpy(x).pin_memory()
+    yh = torch.empty_like(xh).pin_memory()
+    ctx.sky_metric_apply_host(xh, yh)
+    assert np.array_equal(yh.numpy(), y.cpu().numpy())
+
+
+# ---------------------------------------------------------------------------------- energy, gradient, metric
+@pytest.mark.parametrize("key", [("c1",), ("rect", 64, 128), ("sq", 2, 512), ("multi", 64, 3)])
+@pytest.mark.parametrize("with_prior", [True, False])
+def test_energy_grad_and_metric_apply(frs, key, with_prior):
+    w = workload(key)
+    ctx = make_ctx(frs, w)
+    rng = np.random.default_rng(5)
+    xi = (0.3 * rng.normal(size=(w.nfield, w.ny, w.nx))).astype(np.float32)
+    g = ctx.new_latent()
+    e = ctx.energy_grad(dev(xi), g, with_prior=with_prior)
+    e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, with_prior)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref) + 1e-6 * np.abs(g_ref).sum() * 0
+    assert rel(g.cpu().numpy(), g_ref) <= TOL
+    v = rng.normal(size=(w.nfield, w.ny, w.nx)).astype(np.float32)
+    out = ctx.new_latent()
+    ctx.metric_apply(dev(v), out, with_prior=with_prior)
+    ref = o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, v, with_prior)
+    assert rel(out.cpu().numpy(), ref) <= TOL
+
+
+def test_energy_device_scalar_and_xi_zero(frs):
+    import torch
+    w = workload(("c1",))
+    ctx = make_ctx(frs, w)
+    xi = torch.zeros((1, w.ny, w.nx), device="cuda")
+    g = ctx.new_latent()
+    d_e = torch.zeros(1, dtype=torch.float64, device="cuda")
+    e = ctx.energy_grad(xi, g, with_prior=True, d_energy=d_e)
+    assert float(d_e.cpu()[0]) == e
+    e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, np.zeros((1, w.ny, w.nx)), True)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
+    assert rel(g.cpu().numpy(), g_ref) <= TOL
+
+
+# ---------------------------------------------------------------------------------- CG (protocol of DESIGN.md R9)
+def _cg_problem(frs, key):
+    import torch
+    w = workload(key)
+    ctx = make_ctx(frs, w)
+    xi = np.zeros((w.nfield, w.ny, w.nx), np.float32)
+    g = ctx.new_latent()
+    ctx.energy_grad(dev(xi), g, with_prior=True)
+    b = (-g).contiguous()
+    s32 = ctx.new_image()
+    ctx.sky_forward(dev(xi), s32)
+    s = s32.cpu().numpy().astype(np.float64)
+    ap = lambda v: o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, v, True, s=s)
+    return w, ctx, b, ap
+
+
+def test_cg_teacher_forced_every_iteration(frs):
+    """At every k <= 20 the oracle takes the GPU's own (x_k, r_k, p_k) and recomputes one step."""
+    import torch
+    w, ctx, b, ap = _cg_problem(frs, ("c1",))
+    x = torch.zeros_like(b)
+    ctx.cg_solve(b, x, 0)                                          # initialises r = p = b, rr
+    r, p, q, sc = ctx.cg_read_state()
+    assert rel(r.cpu().numpy(), b.cpu().numpy()) == 0.0
+    for k in range(20):
+        x0, r0, p0, rr0 = x.cpu().numpy().astype(np.float64), r.cpu().numpy().astype(np.float64), \
+            p.cpu().numpy().astype(np.float64), float(sc[0])
+        assert abs(rr0 - np.sum(r0 * r0)) <= 1e-10 * rr0
+        ctx.cg_step(x, True)
+        r, p, q, sc = ctx.cg_read_state()
+        st = o.cg_step(ap, x0, r0, p0, rr0)
+        assert rel(q.cpu().numpy(), st["q"]) <= TOL
+        assert abs(sc[3] - st["alpha"]) <= TOL * abs(st["alpha"])
+        assert abs(sc[4] - st["beta"]) <= 1e-4 * abs(st["beta"])
+        assert rel(x.cpu().numpy(), st["x"]) <= TOL
+        # r and p: the update's own rounding is measured against the size of the operands
+        assert np.linalg.norm(r.cpu().numpy() - st["r"]) <= TOL * np.linalg.norm(r0)
+        assert np.linalg.norm(p.cpu().numpy() - st["p"]) <= TOL * np.linalg.norm(p0)
+        assert st["pq"] > 0
+
+
+def test_cg_free_running_within_horizon_and_literal(frs):
+    import torch
+    w, ctx, b, ap = _cg_problem(frs, ("c1",))
+    bh = b.cpu().numpy().astype(np.float64)
+    sol = o.cg(ap, bh, max_iter=20, keep=True)
+    env = o.cg_fp32_envelope(ap, bh, max_iter=20)
+    horizon = max([k + 1 for k in range(20) if env[k] <= 2e-5] or [0])
+    assert horizon >= 5
+    hist = torch.zeros(21, dtype=torch.float64, device="cuda")
+    errs = []
+    for k in range(1, 21):
+        x = torch.zeros_like(b)
+        it, rn = ctx.cg_solve(b, x, k, res_history=hist)
+        assert it == k
+        errs.append(rel(x.cpu().numpy(), sol["xs"][k - 1]))
+    for k in range(1, horizon + 1):
+        assert errs[k - 1] <= 1e-4, (k, errs[k - 1])
+    assert errs[19] <= max(1e-4, 3 * env[19]), (errs[19], env[19])   # literal x_20, reported vs envelope
+    h = hist.cpu().numpy()
+    assert h[20] < h[0] and abs(h[0] - np.linalg.norm(bh)) <= 1e-6 * h[0]
+
+
+def test_cg_literal_on_well_conditioned_companion(frs):
+    """config 1b (sigma = 0.1 peak): rel L2(x_20) <= 1e-4 literally."""
+    import torch
+    w, ctx, b, ap = _cg_problem(frs, ("c1b",))
+    sol = o.cg(ap, b.cpu().numpy().astype(np.float64), max_iter=20)
+    x = torch.zeros_like(b)
+    it, rn = ctx.cg_solve(b, x, 20)
+    assert it == 20
+    assert rel(x.cpu().numpy(), sol["x"]) <= 1e-4
+    assert abs(rn - sol["res"][-1]) <= 1e-3 * sol["res"][-1]
+    # rtol stop
+    x2 = torch.zeros_like(b)
+    it2, rn2 = ctx.cg_solve(b, x2, 200, rtol=1e-3)
+    assert it2 < 200 and rn2 <= 1e-3 * float(b.double().norm()) * 1.001
+
+
+def test_cg_multichannel_teacher_forced(frs):
+    import torch
+    w, ctx, b, ap = _cg_problem(frs, ("multi", 64, 3))
+    x = torch.zeros_like(b)
+    ctx.cg_solve(b, x, 0)
+    r, p, q, sc = ctx.cg_read_state()
+    for k in range(3):
+        x0, r0, p0, rr0 = (t.cpu().numpy().astype(np.float64) for t in (x, r, p)), None, None, float(sc[0])
+        x0, r0, p0 = list(x0)
+        ctx.cg_step(x, True)
+        r, p, q, sc = ctx.cg_read_state()
+        st = o.cg_step(ap, x0, r0, p0, rr0)
+        assert rel(q.cpu().numpy(), st["q"]) <= TOL
+        assert rel(x.cpu().numpy(), st["x"]) <= TOL
+
+
+def test_outer_newton_steps_teacher_forced(frs):
+    """config-2 recipe (reduced): outer KL steps x CG; at each visited xi (the GPU's) the oracle
+    recomputes s, E, grad (reading R10)."""
+    import torch
+    w = workload(("sq", 2, 128))
+    ctx = make_ctx(frs, w)
+    xi = torch.zeros((1, w.ny, w.nx), device="cuda")
+    g = ctx.new_latent()
+    e_prev = None
+    for step in range(3):
+        e = ctx.energy_grad(xi, g, with_prior=True)
+        xih = xi.cpu().numpy()
+        e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xih, True)
+        assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
+        assert rel(g.cpu().numpy(), g_ref) <= TOL
+        if e_prev is not None:
+            assert e < e_prev
+        e_prev = e
+        b = (-g).contiguous()
+        d = torch.zeros_like(b)
+        ctx.cg_solve(b, d, 10)
+        scale = 1.0
+        gt = ctx.new_latent()
+        for _ in range(5):
+            e1 = ctx.energy_grad((xi + scale * d).contiguous(), gt, with_prior=True)
+            if e1 < e:
+                break
+            scale *= 0.5
+        xi = (xi + scale * d).contiguous()
+
+
+# ---------------------------------------------------------------------------------- full-size configs
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_config_parity(frs, cfg):
+    """BASELINE.json configs 3 and 4 at full size, in the launch configuration bench.py times:
+    sky, C s (through the L1 apply) and gradient against the full fp64 oracle."""
+    import torch
+    w = wl.make_config(cfg)
+    ctx = make_ctx(frs, w)
+    xi = (0.5 * np.random.default_rng(6).normal(size=(1, w.ny, w.nx))).astype(np.float32)
+    s = ctx.new_image()
+    ctx.sky_forward(dev(xi), s)
+    s32 = s.cpu().numpy()
+    assert rel(s32, o.sky(xi, w.amp, w.mu, w.lognu)) <= TOL
+    x = np.random.default_rng(7).normal(size=(1, w.ny, w.nx)).astype(np.float32)
+    y = ctx.new_image()
+    ctx.sky_metric_apply(dev(x), y)
+    assert rel(y.cpu().numpy()[0], o.sky_metric_apply(w.w_half, s32, x)[0]) <= TOL
+    ctx.psf_apply(dev(w.sky_true), y)
+    assert rel(y.cpu().numpy()[0], o.psf_apply(w.w_half[0], w.sky_true[0])) <= TOL
+    g = ctx.new_latent()
+    e = ctx.energy_grad(dev(xi), g, with_prior=True)
+    e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, True)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
+    assert rel(g.cpu().numpy(), g_ref) <= TOL
+    del ctx
+    torch.cuda.empty_cache()
+
+
+def test_config5_multichannel_parity(frs):
+    """config 5 (16 x 1024^2, two latent fields): per-channel L1 apply and the gradient."""
+    w = wl.make_config(5)
+    ctx = make_ctx(frs, w)
+    xi = (0.5 * np.random.default_rng(8).normal(size=(2, w.ny, w.nx))).astype(np.float32)
+    s = ctx.new_image()
+    ctx.sky_forward(dev(xi), s)
+    s32 = s.cpu().numpy()
+    assert rel(s32, o.sky(xi, w.amp, w.mu, w.lognu)) <= TOL
+    x = np.random.default_rng(9).normal(size=(w.nchan, w.ny, w.nx)).astype(np.float32)
+    y = ctx.new_image()
+    ctx.sky_metric_apply(dev(x), y)
+    ref = o.sky_metric_apply(w.w_half, s32, x)
+    yh = y.cpu().numpy()
+    for c in range(w.nchan):
+        assert rel(yh[c], ref[c]) <= TOL
+    g = ctx.new_latent()
+    e = ctx.energy_grad(dev(xi), g, with_prior=True)
+    e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, True)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
+    assert rel(g.cpu().numpy(), g_ref) <= TOL

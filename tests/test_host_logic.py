@@ -1,0 +1,65 @@
+"""CPU-only checks of the product side: the library builds for sm_100a, exports every symbol
+include/frs.h declares, its host-replayable FFT logic is right, and it refuses to run without a GPU."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2406_09144_b200 as frs
+from paper_2406_09144_b200 import build as frs_build
+from oracle import frs_oracle as o
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def library():
+    frs_build.build(verbose=False)
+    return frs.load_library()
+
+
+def test_library_exports_every_declared_symbol(library):
+    header = open(os.path.join(ROOT, "include", "frs.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(frs_[a-z_0-9]+)\s*\(", header))
+    assert declared == set(frs.EXPORTS), declared ^ set(frs.EXPORTS)
+    for name in declared:
+        assert hasattr(library, name)
+    assert b"sm_100a" in library.frs_version()
+
+
+@pytest.mark.parametrize("n", [16, 32, 64, 128, 256, 512, 1024, 2048, 4096])
+def test_stage_logic_replayed_on_cpu_matches_dft(library, n):
+    rng = np.random.default_rng(n)
+    x = (rng.normal(size=n) + 1j * rng.normal(size=n)).astype(np.complex64)
+    ref = np.fft.fft(x.astype(np.complex128))
+    if n <= 64:
+        ref = o.dft_naive(x.astype(np.complex128))
+    got = frs.selftest_fft_host(x)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) < 5e-7
+    inv = frs.selftest_fft_host(got, inverse=True)
+    assert np.linalg.norm(inv / n - x) / np.linalg.norm(x) < 1e-6
+    # a delta at position q -> pure phase ramp: catches any index permutation exactly
+    for q in (1, n // 2 + 1, n - 1):
+        d = np.zeros(n, np.complex64)
+        d[q] = 1
+        assert np.allclose(frs.selftest_fft_host(d), np.exp(-2j * np.pi * q * np.arange(n) / n), atol=2e-6)
+
+
+def test_selftest_rejects_bad_sizes(library):
+    with pytest.raises(frs.FrsError):
+        frs.selftest_fft_host(np.zeros(24, np.complex64))
+
+
+def test_no_cpu_fallback(library):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError):
+        frs.Context(64, 64)
+    import ctypes as C
+    h = C.c_void_p()
+    assert library.frs_create(64, 64, 1, 0, None, C.byref(h)) == frs.FRS_ECUDA
+    assert library.frs_create(48, 64, 1, 0, None, C.byref(h)) == frs.FRS_EINVAL      # not a power of two
+    assert library.frs_create(64, 8192, 1, 0, None, C.byref(h)) == frs.FRS_EINVAL
