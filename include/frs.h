@@ -93,9 +93,10 @@ int frs_metric_apply(frs_ctx* ctx, const float* v, int with_prior, float* out);
  * d_res_history (DEVICE double [max_iter+1], may be NULL): ||r_k||.  Synchronises at the end. */
 int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior,
                  int* h_iters, double* h_resnorm, double* d_res_history);
-/* CG state of the last frs_cg_solve / frs_cg_step (device pointers owned by the ctx,
- * [nfield][ny][nx] each; d_scal: double[8] = rr, pq, rr_new, alpha, beta, breakdown, bb, -). */
-int frs_cg_state(frs_ctx* ctx, float** r, float** p, float** q, double** d_scal);
+/* Copy out the CG state of the last frs_cg_solve / frs_cg_step: r, p, q (DEVICE pointers,
+ * [nfield][ny][nx] each, any may be NULL) and the scalar block scal_host (HOST double[8], may be NULL:
+ * rr, pq, rr_new, alpha, beta, breakdown, bb, -).  Synchronises. */
+int frs_cg_read_state(frs_ctx* ctx, float* r, float* p, float* q, double* scal_host);
 /* One CG iteration on caller-visible state (teacher-forced parity, R9): given x, and the ctx's
  * r, p and rr (loaded with frs_cg_load), computes q = M p, alpha, x, r, beta, p. */
 int frs_cg_load(frs_ctx* ctx, const float* r, const float* p, double rr_host);

@@ -31,7 +31,7 @@ EXPORTS = {
     "frs_energy_grad": (_i, [_vp, _vp, _i, _vp, C.POINTER(_d), _vp]),
     "frs_metric_apply": (_i, [_vp, _vp, _i, _vp]),
     "frs_cg_solve": (_i, [_vp, _vp, _vp, _i, _f, _i, C.POINTER(_i), C.POINTER(_d), _vp]),
-    "frs_cg_state": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp)]),
+    "frs_cg_read_state": (_i, [_vp, _vp, _vp, _vp, C.POINTER(_d)]),
     "frs_cg_load": (_i, [_vp, _vp, _vp, _d]),
     "frs_cg_step": (_i, [_vp, _vp, _i]),
     "frs_sky_metric_apply_host": (_i, [_vp, _vp, _vp]),
@@ -214,23 +214,10 @@ class Context:
     def cg_read_state(self):
         """Copies of the ctx-owned r, p, q (torch) and the scalar block (numpy float64[8]:
         rr, pq, rr_new, alpha, beta, breakdown, bb, -) after a cg_step / cg_solve."""
-        r, p, q, s = _vp(), _vp(), _vp(), _vp()
-        self._ck(lib().frs_cg_state(self._h, C.byref(r), C.byref(p), C.byref(q), C.byref(s)))
-        n = self.nfield * self.npix
-        self.stream.synchronize()
-        rt = self.torch.cuda.cudart()
-        outs = []
-        for ptr in (r, p, q):
-            t = self.new_latent()
-            rc = rt.cudaMemcpy(t.data_ptr(), ptr.value, n * 4, 3)
-            if int(rc) != 0:
-                raise FrsError(FRS_ECUDA, f"cudaMemcpy {rc}")
-            outs.append(t)
-        sc = self.torch.zeros(8, dtype=self.torch.float64, device=self.device)
-        rc = rt.cudaMemcpy(sc.data_ptr(), s.value, 64, 3)
-        if int(rc) != 0:
-            raise FrsError(FRS_ECUDA, f"cudaMemcpy {rc}")
-        return outs[0], outs[1], outs[2], sc.cpu().numpy()
+        r, p, q = self.new_latent(), self.new_latent(), self.new_latent()
+        sc = (_d * 8)()
+        self._ck(lib().frs_cg_read_state(self._h, r.data_ptr(), p.data_ptr(), q.data_ptr(), sc))
+        return r, p, q, np.array(list(sc), dtype=np.float64)
 
     # ---- host-buffer entry points (torch CPU tensors, ideally pinned)
     def sky_metric_apply_host(self, x_host, y_host):

@@ -494,14 +494,17 @@ int frs_metric_apply(frs_ctx* ctx, const float* v, int with_prior, float* out) {
     return metric_apply_impl(ctx, v, with_prior, out);
 }
 
-int frs_cg_state(frs_ctx* ctx, float** r, float** p, float** q, double** d_scal) {
+int frs_cg_read_state(frs_ctx* ctx, float* r, float* p, float* q, double* scal_host) {
     if (!ctx) return FRS_EINVAL;
     CK(cudaSetDevice(ctx->device));
+    if (!ctx->have_amp) return fail(ctx, FRS_ESTATE, "amplitude spectrum not set");
     RET(cg_alloc(ctx));
-    if (r) *r = ctx->cg_r;
-    if (p) *p = ctx->cg_p;
-    if (q) *q = ctx->cg_q;
-    if (d_scal) *d_scal = ctx->scal;
+    const size_t bytes = (size_t)ctx->nfield * ctx->npix * sizeof(float);
+    if (r) CK(cudaMemcpyAsync(r, ctx->cg_r, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (p) CK(cudaMemcpyAsync(p, ctx->cg_p, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (q) CK(cudaMemcpyAsync(q, ctx->cg_q, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (scal_host) CK(cudaMemcpyAsync(scal_host, ctx->scal, kNScal * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
     return FRS_OK;
 }
 
