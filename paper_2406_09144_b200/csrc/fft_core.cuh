@@ -125,26 +125,59 @@ FRS_HD constexpr int plan_radix(int n, int s) {
 FRS_HD constexpr int plan_ns(int n, int s) {   // product of the radices before stage s
     return s == 0 ? 1 : plan_ns(n, s - 1) * plan_radix(n, s - 1);
 }
-// twiddle-table offset (in units of P entries) of stage s, and total rows
-FRS_HD constexpr int plan_tw_rows(int n, int s) { return s == 0 ? 0 : kE - kE / plan_radix(n, s); }
-FRS_HD constexpr int plan_tw_off(int n, int s) { return s <= 1 ? 0 : plan_tw_off(n, s - 1) + plan_tw_rows(n, s - 1); }
-FRS_HD constexpr int plan_tw_total(int n) { return plan_tw_off(n, plan_stages(n) - 1) + plan_tw_rows(n, plan_stages(n) - 1); }
+// ---- packed twiddle tables (float4 = two consecutive twiddles) -----------------------------------
+// Stage s > 0, butterfly b, output r >= 1 needs w_r = exp(-2 pi i j r / (NS R)), j = (p + b P) mod NS.
+//   NS <= 16: direct table        D[q][j]          = (w_{2q+1}, w_{2q+2}),  q < R/2
+//   NS  > 16: factorised, j = 16 a + c:  w_r = A[q][a] * C[q][c]
+//             A[q][a] = exp(-2 pi i 16 a r / (NS R)),  C[q][c] = exp(-2 pi i c r / (NS R))
+// so the whole table is a few KB for any N and lives in shared memory.
+FRS_HD constexpr bool plan_tw_fact(int n, int s) { return plan_ns(n, s) > 16; }
+FRS_HD constexpr int plan_tw_wa(int n, int s) { return plan_tw_fact(n, s) ? plan_ns(n, s) / 16 : plan_ns(n, s); }
+FRS_HD constexpr int plan_tw_size(int n, int s) {      // float4 slots of stage s
+    return s == 0 ? 0 : (plan_radix(n, s) / 2) * (plan_tw_wa(n, s) + (plan_tw_fact(n, s) ? 16 : 0));
+}
+FRS_HD constexpr int plan_tw_off(int n, int s) { return s <= 1 ? 0 : plan_tw_off(n, s - 1) + plan_tw_size(n, s - 1); }
+FRS_HD constexpr int plan_tw_total(int n) {            // >= 1 so that allocations are non-empty
+    return plan_tw_off(n, plan_stages(n) - 1) + plan_tw_size(n, plan_stages(n) - 1) + 1;
+}
 
 FRS_HD constexpr int xpad(int pos) { return pos + (pos >> 4); }
-// float2 slots of one exchange buffer (holds positions 0..N inclusive: the row passes park X[N] too)
+// slots of one exchange buffer (holds positions 0..N inclusive: the row passes park X[N] too)
 FRS_HD constexpr int xbuf_len(int n) { return n + (n >> 4) + 8; }
 
+FRS_HD float2 lo(float4 a) { return make_float2(a.x, a.y); }
+FRS_HD float2 hi(float4 a) { return make_float2(a.z, a.w); }
+FRS_HD float4 pack(float2 a, float2 b) { return make_float4(a.x, a.y, b.x, b.y); }
+
 // ---- one stage: twiddle the inputs, butterfly, leave result r of butterfly b in v[b + r*NB] ----
-// NT transforms are advanced together so that each twiddle is fetched once.
+// NT transforms are advanced together so that each twiddle is fetched once.  tw: packed tables.
 template <int N, int S, bool INV, int NT>
-FRS_HD void stage_compute(float2 (&v)[NT][kE], int p, const float2* __restrict__ tw) {
-    constexpr int R = plan_radix(N, S), NB = kE / R, P = N / kE;
+FRS_HD void stage_compute(float2 (&v)[NT][kE], int p, const float4* __restrict__ tw) {
+    constexpr int R = plan_radix(N, S), NB = kE / R, HP = R / 2, P = N / kE, NS = plan_ns(N, S);
+    constexpr int WA = plan_tw_wa(N, S);
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
         float2 w[R];
         if (S > 0) {
+            const int j = (p + b * P) & (NS - 1);
+            const float4* ta = tw + plan_tw_off(N, S);
+            if (plan_tw_fact(N, S)) {
+                const float4* tc = ta + HP * WA;
+                const int ia = j >> 4, ic = j & 15;
 #pragma unroll
-            for (int r = 1; r < R; ++r) w[r] = tw[(plan_tw_off(N, S) + b * (R - 1) + (r - 1)) * P + p];
+                for (int q = 0; q < HP; ++q) {
+                    const float4 wa = ta[q * WA + ia], wc = tc[q * 16 + ic];
+                    w[2 * q + 1] = cmul(lo(wa), lo(wc));
+                    if (2 * q + 2 < R) w[2 * q + 2] = cmul(hi(wa), hi(wc));
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < HP; ++q) {
+                    const float4 ww = ta[q * WA + j];
+                    w[2 * q + 1] = lo(ww);
+                    if (2 * q + 2 < R) w[2 * q + 2] = hi(ww);
+                }
+            }
         }
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
@@ -161,54 +194,79 @@ FRS_HD void stage_compute(float2 (&v)[NT][kE], int p, const float2* __restrict__
         }
     }
 }
-// scatter the stage's outputs to their Stockham positions in the exchange buffer
+// Stockham position of output r of butterfly b of stage S
+template <int N, int S>
+FRS_HD int stage_pos(int p, int b, int r) {
+    constexpr int R = plan_radix(N, S), P = N / kE, NS = plan_ns(N, S);
+    const int j = p + b * P;
+    return (j / NS) * NS * R + (j % NS) + r * NS;
+}
+// single transform through a float2 buffer (host replay, odd cases)
 template <int N, int S>
 FRS_HD void stage_scatter(const float2 (&v)[kE], int p, float2* buf) {
-    constexpr int R = plan_radix(N, S), NB = kE / R, P = N / kE, NS = plan_ns(N, S);
+    constexpr int R = plan_radix(N, S), NB = kE / R;
 #pragma unroll
-    for (int b = 0; b < NB; ++b) {
-        const int j = p + b * P;
-        const int base = (j / NS) * NS * R + (j % NS);
+    for (int b = 0; b < NB; ++b)
 #pragma unroll
-        for (int r = 0; r < R; ++r) buf[xpad(base + r * NS)] = v[b + r * NB];
-    }
+        for (int r = 0; r < R; ++r) buf[xpad(stage_pos<N, S>(p, b, r))] = v[b + r * NB];
 }
-// read the canonical distribution back
 template <int N>
 FRS_HD void canon_gather(float2 (&v)[kE], int p, const float2* buf) {
     constexpr int P = N / kE;
 #pragma unroll
     for (int e = 0; e < kE; ++e) v[e] = buf[xpad(p + e * P)];
 }
+// transform pair through ONE float4 buffer: slot = (a.re, a.im, b.re, b.im) -> 128-bit accesses
+template <int N, int S>
+FRS_HD void stage_scatter2(const float2 (&v)[2][kE], int p, float4* buf) {
+    constexpr int R = plan_radix(N, S), NB = kE / R;
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int r = 0; r < R; ++r) buf[xpad(stage_pos<N, S>(p, b, r))] = pack(v[0][b + r * NB], v[1][b + r * NB]);
+}
 template <int N>
-FRS_HD void canon_scatter(const float2 (&v)[kE], int p, float2* buf) {
+FRS_HD void canon_gather2(float2 (&v)[2][kE], int p, const float4* buf) {
     constexpr int P = N / kE;
 #pragma unroll
-    for (int e = 0; e < kE; ++e) buf[xpad(p + e * P)] = v[e];
+    for (int e = 0; e < kE; ++e) {
+        const float4 x = buf[xpad(p + e * P)];
+        v[0][e] = lo(x);
+        v[1][e] = hi(x);
+    }
+}
+template <int N>
+FRS_HD void canon_scatter2(const float2 (&v)[2][kE], int p, float4* buf) {
+    constexpr int P = N / kE;
+#pragma unroll
+    for (int e = 0; e < kE; ++e) buf[xpad(p + e * P)] = pack(v[0][e], v[1][e]);
 }
 
 #ifdef __CUDACC__
-// ---- the whole transform for NT simultaneous transforms sharing one twiddle fetch -------------
-// All threads of the CTA must call this (it uses __syncthreads()).  bufs: NT exchange buffers of
-// xbuf_len(N) float2 each, private to the group.
-template <int N, bool INV, int NT, int S>
-__device__ __forceinline__ void group_fft_from(float2 (&v)[NT][kE], int p, float2* bufs, const float2* __restrict__ tw) {
+// ---- the whole transform of a PAIR of sequences sharing twiddles ---------------------------------
+// All threads of the CTA must call this (it uses __syncthreads()).  buf: one exchange buffer of
+// xbuf_len(N) float4, private to the group.  tw: packed twiddle table (shared memory).
+template <int N, bool INV, int S>
+__device__ __forceinline__ void pair_fft_from(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
     if constexpr (S < plan_stages(N)) {
-        stage_compute<N, S, INV, NT>(v, p, tw);
+        stage_compute<N, S, INV, 2>(v, p, tw);
         if constexpr (S + 1 < plan_stages(N)) {
-#pragma unroll
-            for (int t = 0; t < NT; ++t) stage_scatter<N, S>(v[t], p, bufs + t * xbuf_len(N));
+            stage_scatter2<N, S>(v, p, buf);
             __syncthreads();
-#pragma unroll
-            for (int t = 0; t < NT; ++t) canon_gather<N>(v[t], p, bufs + t * xbuf_len(N));
+            canon_gather2<N>(v, p, buf);
             __syncthreads();
         }
-        group_fft_from<N, INV, NT, S + 1>(v, p, bufs, tw);
+        pair_fft_from<N, INV, S + 1>(v, p, buf, tw);
     }
 }
-template <int N, bool INV, int NT>
-__device__ __forceinline__ void group_fft(float2 (&v)[NT][kE], int p, float2* bufs, const float2* __restrict__ tw) {
-    group_fft_from<N, INV, NT, 0>(v, p, bufs, tw);
+template <int N, bool INV>
+__device__ __forceinline__ void pair_fft(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
+    pair_fft_from<N, INV, 0>(v, p, buf, tw);
+}
+// cooperative copy of the packed twiddle table into shared memory (all threads; caller syncs)
+template <int N>
+__device__ __forceinline__ void load_twiddles(float4* dst, const float4* __restrict__ src) {
+    for (int i = threadIdx.x; i < plan_tw_total(N); i += blockDim.x) dst[i] = src[i];
 }
 #endif
 

@@ -27,7 +27,8 @@ struct frs_ctx {
     cudaStream_t stream = nullptr;
     size_t npix = 0;
     int ntile = 0, ntile_h = 0;
-    std::map<int, float2*> tw, twist;
+    std::map<int, float4*> tw;
+    std::map<int, float2*> twist;
     float *wt = nullptr, *dirty = nullptr, *amp = nullptr, *s = nullptr;
     float *d_mu = nullptr, *d_lognu = nullptr;
     float2 *T = nullptr, *Th = nullptr;
@@ -91,11 +92,13 @@ int dev_alloc(frs_ctx* ctx, T** p, size_t count) {
 
 int ensure_tables(frs_ctx* ctx, int n) {
     if (ctx->tw.count(n)) return FRS_OK;
-    std::vector<float2> tw = build_twiddles(n), ts = build_twist(n);
-    float2 *dtw = nullptr, *dts = nullptr;
-    CK(cudaMalloc(reinterpret_cast<void**>(&dtw), tw.size() * sizeof(float2)));
+    std::vector<float4> tw = build_twiddles(n);
+    std::vector<float2> ts = build_twist(n);
+    float4* dtw = nullptr;
+    float2* dts = nullptr;
+    CK(cudaMalloc(reinterpret_cast<void**>(&dtw), tw.size() * sizeof(float4)));
     CK(cudaMalloc(reinterpret_cast<void**>(&dts), ts.size() * sizeof(float2)));
-    CK(cudaMemcpy(dtw, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(dtw, tw.data(), tw.size() * sizeof(float4), cudaMemcpyHostToDevice));
     CK(cudaMemcpy(dts, ts.data(), ts.size() * sizeof(float2), cudaMemcpyHostToDevice));
     ctx->tw[n] = dtw;
     ctx->twist[n] = dts;
@@ -463,7 +466,7 @@ int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_ene
     RET(conv_cols(ctx));
     int gx = 0;
     RET(conv_rows_inv(ctx, ctx->img, kEnergy, &gx));          // img_c = s_c (C s_c - j_c), partial sums
-    const int np = gx * ctx->nchan;
+    const int np = gx;      // one (sum s.c, sum j.s) pair per persistent CTA
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, np, 2, 0, ctx->scal + 8);
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, np, 2, 1, ctx->scal + 9);
     ctx->launches += 2;

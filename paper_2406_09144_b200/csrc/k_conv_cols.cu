@@ -1,11 +1,21 @@
+#include <cstdlib>
 #include "launch.h"
 namespace frs {
 template <int NF>
-static int run(cudaStream_t st, const ConvColsArgs& a, int nb) {
+static int run(cudaStream_t st, const ConvColsArgs& a0, int nb) {
     using GEO = Geo<NF, 2>;
-    static bool attr = false;
-    if (!attr) { cudaError_t e = set_smem(conv_cols_kernel<NF>, GEO::SMEM); if (e != cudaSuccess) return (int)e; attr = true; }
-    dim3 grid((a.ntile + GEO::G - 1) / GEO::G, nb);
+    static int ctas = 0;
+    if (!ctas) {
+        cudaError_t e = set_smem(conv_cols_kernel<NF>, GEO::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        ctas = resident_ctas(conv_cols_kernel<NF>, GEO::THREADS, GEO::SMEM);
+        if (!ctas) return (int)cudaErrorUnknown;
+    }
+    ConvColsArgs a = a0;
+    { const char* d = getenv("FRS_DBG"); a.dbg = d ? atoi(d) : 0; }
+    a.items_per_batch = (a.ntile + GEO::G - 1) / GEO::G;
+    a.nitems = a.items_per_batch * nb;
+    const int grid = a.nitems < ctas ? a.nitems : ctas;
     conv_cols_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
     return (int)cudaGetLastError();
 }

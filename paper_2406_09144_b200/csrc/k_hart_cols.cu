@@ -1,12 +1,20 @@
 #include "launch.h"
 namespace frs {
 template <int NF>
-static int run(cudaStream_t st, const HartColsArgs& a, int nb) {
+static int run(cudaStream_t st, const HartColsArgs& a0, int nb) {
     using GEO = Geo<NF, 1>;
-    static bool attr = false;
-    if (!attr) { cudaError_t e = set_smem(hart_cols_kernel<NF>, GEO::SMEM); if (e != cudaSuccess) return (int)e; attr = true; }
+    static int ctas = 0;
+    if (!ctas) {
+        cudaError_t e = set_smem(hart_cols_kernel<NF>, GEO::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        ctas = resident_ctas(hart_cols_kernel<NF>, GEO::THREADS, GEO::SMEM);
+        if (!ctas) return (int)cudaErrorUnknown;
+    }
+    HartColsArgs a = a0;
     const int ntile = a.nx / 4 + 1;
-    dim3 grid((ntile + GEO::G - 1) / GEO::G, nb);
+    a.items_per_batch = (ntile + GEO::G - 1) / GEO::G;
+    a.nitems = a.items_per_batch * nb;
+    const int grid = a.nitems < ctas ? a.nitems : ctas;
     hart_cols_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
     return (int)cudaGetLastError();
 }

@@ -1,12 +1,21 @@
+#include <cstdlib>
 #include "launch.h"
 namespace frs {
 template <int NF, bool PAD>
-static int run(cudaStream_t st, const RowsFwdArgs& a, int nb) {
+static int run(cudaStream_t st, const RowsFwdArgs& a0, int nb) {
     using GEO = Geo<NF, 1>;
-    static bool attr = false;
-    if (!attr) { cudaError_t e = set_smem(rows_fwd_kernel<NF, PAD>, GEO::SMEM); if (e != cudaSuccess) return (int)e; attr = true; }
-    const int pairs = a.ny / 2;
-    dim3 grid((pairs + GEO::G - 1) / GEO::G, nb);
+    static int ctas = 0;
+    if (!ctas) {
+        cudaError_t e = set_smem(rows_fwd_kernel<NF, PAD>, GEO::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        ctas = resident_ctas(rows_fwd_kernel<NF, PAD>, GEO::THREADS, GEO::SMEM);
+        if (!ctas) return (int)cudaErrorUnknown;
+    }
+    RowsFwdArgs a = a0;
+    { const char* d = getenv("FRS_DBG"); a.dbg = d ? atoi(d) : 0; }
+    a.items_per_batch = (a.ny / 2 + GEO::G - 1) / GEO::G;
+    a.nitems = a.items_per_batch * nb;
+    const int grid = a.nitems < ctas ? a.nitems : ctas;
     rows_fwd_kernel<NF, PAD><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
     return (int)cudaGetLastError();
 }

@@ -1,25 +1,28 @@
+#include <cstdlib>
 #include "launch.h"
 namespace frs {
+// grid_x: number of CTAs launched (= number of (sum s.c, sum j.s) partial pairs in kEnergy mode)
 template <int NF>
-static int run(cudaStream_t st, const RowsInvArgs& a, int nb, int* grid_x) {
+static int run(cudaStream_t st, const RowsInvArgs& a0, int nb, int* grid_x) {
     using GEO = Geo<NF, 1>;
-    static bool attr = false;
-    if (!attr) { cudaError_t e = set_smem(rows_inv_kernel<NF>, GEO::SMEM); if (e != cudaSuccess) return (int)e; attr = true; }
-    const int pairs = a.ny / 2;
-    dim3 grid((pairs + GEO::G - 1) / GEO::G, nb);
-    if (grid_x) *grid_x = grid.x;
+    static int ctas = 0;
+    if (!ctas) {
+        cudaError_t e = set_smem(rows_inv_kernel<NF>, GEO::SMEM);
+        if (e != cudaSuccess) return (int)e;
+        ctas = resident_ctas(rows_inv_kernel<NF>, GEO::THREADS, GEO::SMEM);
+        if (!ctas) return (int)cudaErrorUnknown;
+    }
+    RowsInvArgs a = a0;
+    { const char* d = getenv("FRS_DBG"); a.dbg = d ? atoi(d) : 0; }
+    a.items_per_batch = (a.ny / 2 + GEO::G - 1) / GEO::G;
+    a.nitems = a.items_per_batch * nb;
+    const int grid = a.nitems < ctas ? a.nitems : ctas;
+    if (grid_x) *grid_x = grid;
     rows_inv_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
     return (int)cudaGetLastError();
 }
 int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* grid_x) {
 #define CALL(N) return run<N>(st, a, nb, grid_x)
-    FRS_DISPATCH_NF(nf, CALL)
-#undef CALL
-    return 0;
-}
-template <int NF> static int gx(int ny) { return (ny / 2 + Geo<NF, 1>::G - 1) / Geo<NF, 1>::G; }
-int rows_inv_grid_x(int nf, int ny) {
-#define CALL(N) return gx<N>(ny)
     FRS_DISPATCH_NF(nf, CALL)
 #undef CALL
     return 0;

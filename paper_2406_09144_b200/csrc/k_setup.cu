@@ -6,13 +6,16 @@ namespace frs {
 // Column pass of the full (not zero-padded) 2NF-point DFT of the row-transformed PSF by one
 // decimation-in-frequency step: even bins = FFT_NF(x[n] + x[n+NF]), odd = FFT_NF((x[n] - x[n+NF]) twist^n).
 template <int NF>
-__global__ void __launch_bounds__(Geo<NF, 2>::THREADS, (Geo<NF, 2>::THREADS >= 512 ? 1 : 2))
+__global__ void __launch_bounds__(Geo<NF, 2>::THREADS, Geo<NF, 2>::MINB)
 psf_cols_kernel(PsfColsArgs a) {
     using GEO = Geo<NF, 2>;
     constexpr int P = GEO::P;
-    extern __shared__ float2 smem[];
+    extern __shared__ float4 smem4[];
+    float4* tws = smem4;
     const int g = threadIdx.x / (2 * P), role = (threadIdx.x / P) & 1, p = threadIdx.x % P;
-    float2* bufs = smem + (size_t)g * 4 * xbuf_len(NF) + role * 2 * xbuf_len(NF);
+    float4* buf = smem4 + GEO::TW + ((size_t)g * 2 + role) * xbuf_len(NF);
+    load_twiddles<NF>(tws, a.tw);
+    __syncthreads();
     const int m = blockIdx.x * GEO::G + g;
     const int b = blockIdx.y;
     const bool live = m < a.ntile;
@@ -35,7 +38,7 @@ psf_cols_kernel(PsfColsArgs a) {
             }
         }
     }
-    group_fft<NF, false, 2>(v, p, bufs, a.tw);
+    pair_fft<NF, false>(v, p, buf, tws);
     float max_im = 0.f, min_re = 0.f, max_re = 0.f;
     if (live) {
         float2* w = reinterpret_cast<float2*>(a.wt + b * a.w_bstride) + ((size_t)m * 2 + role) * NF;

@@ -13,7 +13,6 @@ inline bool valid_nf(int nf) { return nf >= 16 && nf <= 4096 && (nf & (nf - 1)) 
 int launch_rows_fwd(cudaStream_t st, int nf, bool pad, const RowsFwdArgs& a, int nb);
 int launch_conv_cols(cudaStream_t st, int nf, const ConvColsArgs& a, int nb);
 int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* grid_x);
-int rows_inv_grid_x(int nf, int ny);
 int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb);
 
 struct PsfColsArgs {
@@ -23,7 +22,7 @@ struct PsfColsArgs {
     int ntile;
     float scale;          // 1 / (My Mx)
     size_t t_bstride, w_bstride;
-    const float2* tw;
+    const float4* tw;
     const float2* twist;
 };
 int launch_psf_cols(cudaStream_t st, int nf, const PsfColsArgs& a, int nb, int* grid_x);
@@ -45,6 +44,16 @@ int launch_psf_cols(cudaStream_t st, int nf, const PsfColsArgs& a, int nb, int* 
 template <typename K>
 inline cudaError_t set_smem(K kernel, int bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+// resident CTAs of a persistent kernel = SMs x occupancy (0 on error)
+template <typename K>
+inline int resident_ctas(K kernel, int threads, int smem) {
+    int dev = 0, sms = 0, occ = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem) != cudaSuccess) return 0;
+    return sms * (occ > 0 ? occ : 1);
 }
 
 }  // namespace frs

@@ -6,20 +6,31 @@
 
 namespace frs {
 
-// per-thread stage twiddles: tw[(off_s + b*(R-1) + r-1)*P + p] = exp(-2 pi i ((p + b P) mod NS) r / (NS R))
-inline std::vector<float2> build_twiddles(int n) {
-    const int P = n / kE;
-    std::vector<float2> tw((size_t)plan_tw_total(n) * P + 1);
+// packed stage twiddles, layout of fft_core.cuh plan_tw_* (direct or factorised per stage)
+inline std::vector<float4> build_twiddles(int n) {
+    std::vector<float4> tw((size_t)plan_tw_total(n), make_float4(1.f, 0.f, 1.f, 0.f));
     const double two_pi = 6.283185307179586476925286766559;
+    auto ex = [&](long long num, long long den) {
+        const double ang = -two_pi * (double)num / (double)den;
+        return make_float2((float)std::cos(ang), (float)std::sin(ang));
+    };
     for (int s = 1; s < plan_stages(n); ++s) {
-        const int R = plan_radix(n, s), NB = kE / R, NS = plan_ns(n, s), off = plan_tw_off(n, s);
-        for (int b = 0; b < NB; ++b)
-            for (int r = 1; r < R; ++r)
-                for (int p = 0; p < P; ++p) {
-                    const int j = p + b * P;
-                    const double ang = -two_pi * (double)((long long)(j % NS) * r) / (double)((long long)NS * R);
-                    tw[(size_t)(off + b * (R - 1) + (r - 1)) * P + p] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+        const int R = plan_radix(n, s), NS = plan_ns(n, s), off = plan_tw_off(n, s), HP = R / 2, WA = plan_tw_wa(n, s);
+        const bool fact = plan_tw_fact(n, s);
+        const long long den = (long long)NS * R;
+        for (int q = 0; q < HP; ++q) {
+            const int r1 = 2 * q + 1, r2 = 2 * q + 2;
+            for (int a = 0; a < WA; ++a) {
+                const long long j = fact ? 16LL * a : a;
+                const float2 w1 = ex(j * r1, den), w2 = r2 < R ? ex(j * r2, den) : make_float2(1.f, 0.f);
+                tw[(size_t)off + q * WA + a] = make_float4(w1.x, w1.y, w2.x, w2.y);
+            }
+            if (fact)
+                for (int c = 0; c < 16; ++c) {
+                    const float2 w1 = ex((long long)c * r1, den), w2 = r2 < R ? ex((long long)c * r2, den) : make_float2(1.f, 0.f);
+                    tw[(size_t)off + HP * WA + q * 16 + c] = make_float4(w1.x, w1.y, w2.x, w2.y);
                 }
+        }
     }
     return tw;
 }
