@@ -125,20 +125,31 @@ FRS_HD constexpr int plan_radix(int n, int s) {
 FRS_HD constexpr int plan_ns(int n, int s) {   // product of the radices before stage s
     return s == 0 ? 1 : plan_ns(n, s - 1) * plan_radix(n, s - 1);
 }
-// ---- packed twiddle tables (float4 = two consecutive twiddles) -----------------------------------
+// ---- twiddle tables (shared memory, a few KB for any N) -----------------------------------------
 // Stage s > 0, butterfly b, output r >= 1 needs w_r = exp(-2 pi i j r / (NS R)), j = (p + b P) mod NS.
-//   NS <= 16: direct table        D[q][j]          = (w_{2q+1}, w_{2q+2}),  q < R/2
-//   NS  > 16: factorised, j = 16 a + c:  w_r = A[q][a] * C[q][c]
-//             A[q][a] = exp(-2 pi i 16 a r / (NS R)),  C[q][c] = exp(-2 pi i c r / (NS R))
-// so the whole table is a few KB for any N and lives in shared memory.
+//   NS <= 16: direct table of float4 D[q][j] = (w_{2q+1}, w_{2q+2}), q < R/2.
+//   NS  > 16: only w_1 is tabulated, factorised over j = 16 a + c:  w_1 = A[a] C[c] (float2 each,
+//             A[a] = exp(-2 pi i 16 a / (NS R)), C[c] = exp(-2 pi i c / (NS R))); w_2..w_{R-1} follow by a
+//             product tree of depth <= 4 (squares and one multiply), which costs the same arithmetic
+//             as applying a factorised table and far fewer shared-memory reads.
 FRS_HD constexpr bool plan_tw_fact(int n, int s) { return plan_ns(n, s) > 16; }
 FRS_HD constexpr int plan_tw_wa(int n, int s) { return plan_tw_fact(n, s) ? plan_ns(n, s) / 16 : plan_ns(n, s); }
 FRS_HD constexpr int plan_tw_size(int n, int s) {      // float4 slots of stage s
-    return s == 0 ? 0 : (plan_radix(n, s) / 2) * (plan_tw_wa(n, s) + (plan_tw_fact(n, s) ? 16 : 0));
+    return s == 0 ? 0 : (plan_tw_fact(n, s) ? (plan_tw_wa(n, s) + 16) / 2 : (plan_radix(n, s) / 2) * plan_tw_wa(n, s));
 }
 FRS_HD constexpr int plan_tw_off(int n, int s) { return s <= 1 ? 0 : plan_tw_off(n, s - 1) + plan_tw_size(n, s - 1); }
 FRS_HD constexpr int plan_tw_total(int n) {            // >= 1 so that allocations are non-empty
     return plan_tw_off(n, plan_stages(n) - 1) + plan_tw_size(n, plan_stages(n) - 1) + 1;
+}
+FRS_HD float2 csq(float2 a) { return make_float2(fmaf(a.x, a.x, -(a.y * a.y)), 2.0f * a.x * a.y); }
+// w[r] = w[1]^r for r = 2..R-1
+template <int R> FRS_HD void twiddle_powers(float2 (&w)[R]) {
+    if (R > 2) { w[2] = csq(w[1]); w[3] = cmul(w[2], w[1]); }
+    if (R > 4) { w[4] = csq(w[2]); w[5] = cmul(w[4], w[1]); w[6] = csq(w[3]); w[7] = cmul(w[4], w[3]); }
+    if (R > 8) {
+        w[8] = csq(w[4]);  w[9] = cmul(w[8], w[1]);  w[10] = csq(w[5]); w[11] = cmul(w[8], w[3]);
+        w[12] = csq(w[6]); w[13] = cmul(w[8], w[5]); w[14] = csq(w[7]); w[15] = cmul(w[8], w[7]);
+    }
 }
 
 FRS_HD constexpr int xpad(int pos) { return pos + (pos >> 4); }
@@ -162,14 +173,9 @@ FRS_HD void stage_compute(float2 (&v)[NT][kE], int p, const float4* __restrict__
             const int j = (p + b * P) & (NS - 1);
             const float4* ta = tw + plan_tw_off(N, S);
             if (plan_tw_fact(N, S)) {
-                const float4* tc = ta + HP * WA;
-                const int ia = j >> 4, ic = j & 15;
-#pragma unroll
-                for (int q = 0; q < HP; ++q) {
-                    const float4 wa = ta[q * WA + ia], wc = tc[q * 16 + ic];
-                    w[2 * q + 1] = cmul(lo(wa), lo(wc));
-                    if (2 * q + 2 < R) w[2 * q + 2] = cmul(hi(wa), hi(wc));
-                }
+                const float2* fa = reinterpret_cast<const float2*>(ta);
+                w[1] = cmul(fa[j >> 4], fa[WA + (j & 15)]);
+                twiddle_powers<R>(w);
             } else {
 #pragma unroll
                 for (int q = 0; q < HP; ++q) {
@@ -262,6 +268,54 @@ __device__ __forceinline__ void pair_fft_from(float2 (&v)[2][kE], int p, float4*
 template <int N, bool INV>
 __device__ __forceinline__ void pair_fft(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
     pair_fft_from<N, INV, 0>(v, p, buf, tw);
+}
+// The same transform in two halves, so that a caller can reuse `buf` (it is free after the head)
+// while the last stage, which runs entirely in registers, is still to be computed.
+template <int N, bool INV, int S>
+__device__ __forceinline__ void pair_fft_head_from(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
+    if constexpr (S + 1 < plan_stages(N)) {
+        stage_compute<N, S, INV, 2>(v, p, tw);
+        stage_scatter2<N, S>(v, p, buf);
+        __syncthreads();
+        canon_gather2<N>(v, p, buf);
+        __syncthreads();
+        pair_fft_head_from<N, INV, S + 1>(v, p, buf, tw);
+    }
+}
+template <int N, bool INV>
+__device__ __forceinline__ void pair_fft_head(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
+    pair_fft_head_from<N, INV, 0>(v, p, buf, tw);
+}
+template <int N, bool INV>
+__device__ __forceinline__ void pair_fft_tail(float2 (&v)[2][kE], int p, const float4* __restrict__ tw) {
+    stage_compute<N, plan_stages(N) - 1, INV, 2>(v, p, tw);
+}
+
+// ---- asynchronous copies ---------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src_gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+// mbarrier + bulk (TMA) copy of a contiguous block global -> shared
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
 }
 // cooperative copy of the packed twiddle table into shared memory (all threads; caller syncs)
 template <int N>

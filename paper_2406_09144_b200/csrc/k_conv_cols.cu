@@ -1,9 +1,8 @@
-#include <cstdlib>
 #include "launch.h"
 namespace frs {
 template <int NF>
 static int run(cudaStream_t st, const ConvColsArgs& a0, int nb) {
-    using GEO = Geo<NF, 2>;
+    using GEO = Geo<NF, 1>;
     static int ctas = 0;
     if (!ctas) {
         cudaError_t e = set_smem(conv_cols_kernel<NF>, GEO::SMEM);
@@ -12,8 +11,7 @@ static int run(cudaStream_t st, const ConvColsArgs& a0, int nb) {
         if (!ctas) return (int)cudaErrorUnknown;
     }
     ConvColsArgs a = a0;
-    { const char* d = getenv("FRS_DBG"); a.dbg = d ? atoi(d) : 0; }
-    a.items_per_batch = (a.ntile + GEO::G - 1) / GEO::G;
+    a.items_per_batch = (2 * a.ntile + GEO::G - 1) / GEO::G;
     a.nitems = a.items_per_batch * nb;
     const int grid = a.nitems < ctas ? a.nitems : ctas;
     conv_cols_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);

@@ -1,4 +1,3 @@
-#include <cstdlib>
 #include "launch.h"
 namespace frs {
 template <int NF, bool PAD>
@@ -12,7 +11,6 @@ static int run(cudaStream_t st, const RowsFwdArgs& a0, int nb) {
         if (!ctas) return (int)cudaErrorUnknown;
     }
     RowsFwdArgs a = a0;
-    { const char* d = getenv("FRS_DBG"); a.dbg = d ? atoi(d) : 0; }
     a.items_per_batch = (a.ny / 2 + GEO::G - 1) / GEO::G;
     a.nitems = a.items_per_batch * nb;
     const int grid = a.nitems < ctas ? a.nitems : ctas;

@@ -1,4 +1,3 @@
-#include <cstdlib>
 #include "launch.h"
 namespace frs {
 // grid_x: number of CTAs launched (= number of (sum s.c, sum j.s) partial pairs in kEnergy mode)
@@ -13,7 +12,6 @@ static int run(cudaStream_t st, const RowsInvArgs& a0, int nb, int* grid_x) {
         if (!ctas) return (int)cudaErrorUnknown;
     }
     RowsInvArgs a = a0;
-    { const char* d = getenv("FRS_DBG"); a.dbg = d ? atoi(d) : 0; }
     a.items_per_batch = (a.ny / 2 + GEO::G - 1) / GEO::G;
     a.nitems = a.items_per_batch * nb;
     const int grid = a.nitems < ctas ? a.nitems : ctas;

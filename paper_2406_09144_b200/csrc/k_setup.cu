@@ -41,14 +41,15 @@ psf_cols_kernel(PsfColsArgs a) {
     pair_fft<NF, false>(v, p, buf, tws);
     float max_im = 0.f, min_re = 0.f, max_re = 0.f;
     if (live) {
-        float2* w = reinterpret_cast<float2*>(a.wt + b * a.w_bstride) + ((size_t)m * 2 + role) * NF;
+        float* w = a.wt + b * a.w_bstride + (size_t)m * 2 * NF * 2 + role;      // [c][q][parity = role]
 #pragma unroll
         for (int e = 0; e < kE; ++e) {
             const float re0 = v[0][e].x * a.scale, re1 = v[1][e].x * a.scale;
             max_im = fmaxf(max_im, fmaxf(fabsf(v[0][e].y), fabsf(v[1][e].y)) * a.scale);
             min_re = fminf(min_re, fminf(re0, re1));
             max_re = fmaxf(max_re, fmaxf(re0, re1));
-            w[p + e * P] = make_float2(0.5f * fmaxf(re0, 0.f), 0.5f * fmaxf(re1, 0.f));
+            w[(size_t)(p + e * P) * 2] = 0.5f * fmaxf(re0, 0.f);
+            w[(size_t)(NF + p + e * P) * 2] = 0.5f * fmaxf(re1, 0.f);
         }
     }
     __shared__ float red[3][32];
@@ -87,7 +88,7 @@ int launch_psf_cols(cudaStream_t st, int nf, const PsfColsArgs& a, int nb, int* 
     return 0;
 }
 
-// w_half [nb][2ny][nx+1]  ->  wt [nb][ntile][2][ny][2] = 0.5 * W[2q+par][2m+c]  (0 beyond kx = nx)
+// w_half [nb][2ny][nx+1]  ->  wt [nb][ntile][c][q][par] = 0.5 * W[2q+par][2m+c]  (0 beyond kx = nx)
 __global__ void weights_layout_kernel(const float* __restrict__ w_half, float* __restrict__ wt, int ny, int nx,
                                       int* __restrict__ neg_flag) {
     const int ntile = nx / 2 + 1;
@@ -95,9 +96,9 @@ __global__ void weights_layout_kernel(const float* __restrict__ w_half, float* _
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= per) return;
     const int b = blockIdx.y;
-    const int c = i & 1;
+    const int par = i & 1;
     const int q = (i >> 1) % ny;
-    const int par = ((i >> 1) / ny) & 1;
+    const int c = ((i >> 1) / ny) & 1;
     const int m = (int)((i >> 1) / ny / 2);
     const int kx = 2 * m + c, ky = 2 * q + par;
     float v = 0.f;

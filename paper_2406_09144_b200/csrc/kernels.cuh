@@ -6,7 +6,7 @@
 //                                                       kx = 2m, 2m+1 of the row-transformed
 //                                                       array, ntile = NF/2 + 1 (kx = 0..NF; the
 //                                                       odd slot of the last tile is zero)
-//   weights Wt real  [nb][ntile][2][ny][2]             parity (even/odd ky), q, column-in-tile
+//   weights Wt real  [nb][ntile][2][ny][2]             column-in-tile, q, parity (even/odd ky)
 //
 // Passes (all persistent: a CTA walks work items blockIdx.x, blockIdx.x + gridDim.x, ...; the stage
 // twiddles live in shared memory, loaded once per CTA):
@@ -23,15 +23,19 @@
 
 namespace frs {
 
-template <int NF, int ROLES>
+// CTA geometry.  ROLES: thread groups of P cooperating on one work item (conv_cols: even/odd bins).
+// STAGE: extra float4 slots per group for an asynchronously filled staging buffer.
+template <int NF, int ROLES, int STAGE = 0>
 struct Geo {
     static constexpr int P = NF / kE;                                  // threads per transform pair
     static constexpr int GT = P * ROLES;                               // threads per group
-    static constexpr int WANT = NF >= 1024 ? 512 : (NF >= 256 ? 256 : 64);
+    static constexpr int WANT = NF >= 1024 ? (ROLES == 2 ? 512 : 256) : (NF >= 256 ? 256 : 64);
     static constexpr int THREADS = GT >= WANT ? GT : WANT;
     static constexpr int G = THREADS / GT;                             // groups per CTA
-    static constexpr int TW = plan_tw_total(NF);                       // float4 slots of the twiddle table
-    static constexpr int SMEM = (TW + G * ROLES * xbuf_len(NF)) * (int)sizeof(float4);
+    static constexpr int TW = plan_tw_total(NF);                       // float4 slots of the twiddle tables
+    static constexpr int GROUP_SLOTS = ROLES * xbuf_len(NF) + STAGE;   // float4 slots per group
+    static constexpr int BAR_SLOTS = (G + 1) / 2;                      // one 8-byte mbarrier per group
+    static constexpr int SMEM = (TW + G * GROUP_SLOTS + BAR_SLOTS) * (int)sizeof(float4);
     static constexpr int MINB = THREADS >= 512 ? 1 : (THREADS >= 256 ? 2 : 4);
 };
 
@@ -62,7 +66,6 @@ struct RowsFwdArgs {
     const float* mul;     // optional [nb][ny][nxr] multiplier (s or A); nullptr = none
     float2* out;          // [nb][ntile][ny][2]
     int ny;               // rows
-    int dbg;
     int items_per_batch, nitems;
     size_t in_bstride, mul_bstride, out_bstride;   // elements (float / float / float2)
     float scale;
@@ -70,7 +73,9 @@ struct RowsFwdArgs {
     const float2* twist;  // exp(-2 pi i k/(2 NF)), k = 0..NF
 };
 
-// One group (P threads) transforms rows y0, y0+1 together.
+// One group (P threads) transforms rows y0, y0+1 together.  Software pipeline: the loads of the next
+// item are issued into registers as soon as the transform has left them, so they are in flight while
+// this item's spectrum is unpacked from shared memory and stored.
 template <int NF, bool PAD>
 __global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
 rows_fwd_kernel(RowsFwdArgs a) {
@@ -81,67 +86,94 @@ rows_fwd_kernel(RowsFwdArgs a) {
     extern __shared__ float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
-    float4* buf = smem4 + GEO::TW + (size_t)g * xbuf_len(NF);
+    float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
+
+    float2 xin[2][NE], min_[2][NE];
+    auto issue_loads = [&](int item) {
+        const int b = item / a.items_per_batch;
+        const int rp = (item - b * a.items_per_batch) * GEO::G + g;
+        if (item < a.nitems && 2 * rp < a.ny) {
+            const float* r0 = a.in + b * a.in_bstride + (size_t)(2 * rp) * NXR;
+#pragma unroll
+            for (int e = 0; e < NE; ++e) {
+                xin[0][e] = ldg2(r0 + 2 * (p + e * P));
+                xin[1][e] = ldg2(r0 + NXR + 2 * (p + e * P));
+            }
+            if (a.mul) {
+                const float* m0 = a.mul + b * a.mul_bstride + (size_t)(2 * rp) * NXR;
+#pragma unroll
+                for (int e = 0; e < NE; ++e) {
+                    min_[0][e] = ldg2(m0 + 2 * (p + e * P));
+                    min_[1][e] = ldg2(m0 + NXR + 2 * (p + e * P));
+                }
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < NE; ++e) { xin[0][e] = xin[1][e] = make_float2(0.f, 0.f); }
+        }
+    };
+    if (PAD) issue_loads(blockIdx.x);
 
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const int b = item / a.items_per_batch;
         const int rp = (item - b * a.items_per_batch) * GEO::G + g;       // row pair
+        if (!PAD) issue_loads(item);              // unpadded rows fill every register slot: no room to prefetch
         const bool live = 2 * rp < a.ny;
         const int y0 = 2 * rp;
 
         float2 v[2][kE];
 #pragma unroll
-        for (int e = 0; e < kE; ++e) { v[0][e] = make_float2(0.f, 0.f); v[1][e] = make_float2(0.f, 0.f); }
-        if (live) {
-            const float* r0 = a.in + b * a.in_bstride + (size_t)y0 * NXR;
+        for (int e = 0; e < kE; ++e) {
+            if (e < NE) {
 #pragma unroll
-            for (int e = 0; e < NE; ++e) {
-                const int n = p + e * P;
-                v[0][e] = ldg2(r0 + 2 * n);
-                v[1][e] = ldg2(r0 + NXR + 2 * n);
-            }
-            if (a.mul) {
-                const float* m0 = a.mul + b * a.mul_bstride + (size_t)y0 * NXR;
-#pragma unroll
-                for (int e = 0; e < NE; ++e) {
-                    const int n = p + e * P;
-                    const float2 ma = ldg2(m0 + 2 * n), mb = ldg2(m0 + NXR + 2 * n);
-                    v[0][e].x *= ma.x; v[0][e].y *= ma.y;
-                    v[1][e].x *= mb.x; v[1][e].y *= mb.y;
-                }
+                for (int t = 0; t < 2; ++t)
+                    v[t][e] = (a.mul && live) ? make_float2(xin[t][e].x * min_[t][e].x, xin[t][e].y * min_[t][e].y) : xin[t][e];
+            } else {
+                v[0][e] = make_float2(0.f, 0.f);
+                v[1][e] = make_float2(0.f, 0.f);
             }
         }
-        if (!(a.dbg & 2)) pair_fft<NF, false>(v, p, buf, tws);
+        pair_fft<NF, false>(v, p, buf, tws);
         canon_scatter2<NF>(v, p, buf);
         __syncthreads();
+        if (PAD) issue_loads(item + gridDim.x);
         if (live) {
-            // X[k] * scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = 0..NF
-            float4* ob = reinterpret_cast<float4*>(a.out + b * a.out_bstride);
-#pragma unroll
-            for (int i = 0; i <= kE / 2; ++i) {
-                const int m = p + i * P;
-                if (i == kE / 2 && p != 0) break;      // tail tile NF/2 (column NF + a zero slot): thread 0 only
-                float2 res[2][2];
-#pragma unroll
-                for (int c = 0; c < 2; ++c) {
-                    const int k = 2 * m + c;
+            // X[k] * scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = 0..NF.
+            // Four lanes (column c, row r) produce the 32-byte slot of one tile: lane = 4 j + 2 r + c.
+            const float2* zb = reinterpret_cast<const float2*>(buf);       // Z_r[k] at zb[2 xpad(k) + r]
+            float2* ob = a.out + b * a.out_bstride + (size_t)y0 * 2;
+            const int c = p & 1, r = (p >> 1) & 1;
+            auto emit = [&](int m) {
+                const int k = 2 * m + c;
+                float2 x = make_float2(0.f, 0.f);
+                if (k <= NF) {
                     const int ik = k & (NF - 1), im = (NF - k) & (NF - 1);
-                    const float2 w = (k <= NF) ? __ldg(a.twist + k) : make_float2(0.f, 0.f);
-                    const float4 zk = buf[xpad(ik)], zn = buf[xpad(im)];
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-                        const float2 za = t ? hi(zk) : lo(zk), zm = cconj(t ? hi(zn) : lo(zn));
-                        const float2 s = cadd(za, zm), d = cmul(csub(za, zm), w);
-                        float2 x = make_float2((s.x + d.y) * a.scale, (s.y - d.x) * a.scale);
-                        if (k > NF) x = make_float2(0.f, 0.f);
-                        res[t][c] = x;
-                    }
+                    const float2 w = __ldg(a.twist + k);
+                    const float2 za = zb[2 * xpad(ik) + r], zm = cconj(zb[2 * xpad(im) + r]);
+                    const float2 s = cadd(za, zm), d = cmul(csub(za, zm), w);
+                    x = make_float2((s.x + d.y) * a.scale, (s.y - d.x) * a.scale);
                 }
-                float4* o = (a.dbg & 1) ? ob + ((size_t)rp * (NF / 2 + 1) + m) * 2 : ob + (size_t)m * a.ny + y0;
-                stg4(o, pack(res[0][0], res[0][1]));
-                stg4(o + 1, pack(res[1][0], res[1][1]));
+                stg2(ob + (size_t)m * a.ny * 2 + r * 2 + c, x);
+            };
+            if (P >= 4) {
+#pragma unroll
+                for (int i = 0; i < 2 * kE; ++i) emit((p >> 2) + i * (P / 4));
+                if (p < 4) emit(NF / 2);
+            } else {                              // tiny transforms: fewer than 4 threads per row pair
+                for (int q = p; q < 4 * (NF / 2 + 1); q += P) {
+                    const int cc = q & 1, rr = (q >> 1) & 1, m = q >> 2, k = 2 * m + cc;
+                    float2 x = make_float2(0.f, 0.f);
+                    if (k <= NF) {
+                        const int ik = k & (NF - 1), im = (NF - k) & (NF - 1);
+                        const float2 w = __ldg(a.twist + k);
+                        const float2 za = zb[2 * xpad(ik) + rr], zm = cconj(zb[2 * xpad(im) + rr]);
+                        const float2 s = cadd(za, zm), d = cmul(csub(za, zm), w);
+                        x = make_float2((s.x + d.y) * a.scale, (s.y - d.x) * a.scale);
+                    }
+                    stg2(ob + (size_t)m * a.ny * 2 + rr * 2 + cc, x);
+                }
             }
         }
         __syncthreads();

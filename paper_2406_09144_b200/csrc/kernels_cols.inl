@@ -3,100 +3,74 @@
 // ------------------------------------------------------------------------------------------------
 struct ConvColsArgs {
     float2* t;            // [nb][ntile][NF][2] in place
-    const float* wt;      // [nb][ntile][2][NF][2]
-    int ntile, dbg;
-    int items_per_batch;  // ceil(ntile / G)
+    const float* wt;      // [nb][ntile][2 (column in tile)][NF (q)][2 (even, odd bin)]
+    int ntile;
+    int items_per_batch;  // ceil(2 ntile / G)
     int nitems;           // items_per_batch * nb
     size_t t_bstride, w_bstride;
     const float4* tw;
     const float2* twist;  // exp(-2 pi i n/(2 NF))
 };
 
-// Group = 2 roles x P threads; role 0 owns the even output bins of the length-2NF transform of the
-// zero-extended column, role 1 the odd bins (input pre-multiplied by twist^n).  After . W and the
-// inverse transforms:  y[n] = IFFT_NF(E')[n] + conj(twist^n) IFFT_NF(O')[n].
+// One group (P threads) convolves ONE column: the pair of transforms a thread carries are the even
+// and the odd output bins of the length-2NF transform of the zero-extended column,
+//   even bins = FFT_NF(x),  odd bins = FFT_NF(x twist^n);   after . W and the inverse transforms
+//   y[n] = IFFT_NF(E')[n] + conj(twist^n) IFFT_NF(O')[n]
+// so input, twiddles and the final combination are all thread-local.  Work item = (tile, column);
+// the two columns of a tile go to neighbouring CTAs, which share the tile's sectors through L2.
+// Several independent CTAs per SM keep the shared-memory exchange of one overlapped with the
+// arithmetic of another.
 template <int NF>
-__global__ void __launch_bounds__(Geo<NF, 2>::THREADS, Geo<NF, 2>::MINB)
+__global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
 conv_cols_kernel(ConvColsArgs a) {
-    using GEO = Geo<NF, 2>;
+    using GEO = Geo<NF, 1>;
     constexpr int P = GEO::P;
     extern __shared__ float4 smem4[];
     float4* tws = smem4;
-    const int g = threadIdx.x / (2 * P), role = (threadIdx.x / P) & 1, p = threadIdx.x % P;
-    float4* gb = smem4 + GEO::TW + (size_t)g * 2 * xbuf_len(NF);
-    float4* buf = gb + role * xbuf_len(NF);
-    float4* cb = gb + xbuf_len(NF);              // combine buffer = role 1's exchange buffer, [e][p]
+    const int g = threadIdx.x / P, p = threadIdx.x % P;
+    float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
 
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const int b = item / a.items_per_batch;
-        const int m = (item - b * a.items_per_batch) * GEO::G + g;
-        const bool live = m < a.ntile;
-        float4* tile = reinterpret_cast<float4*>(a.t + b * a.t_bstride) + (size_t)m * NF;
-        const float2* w = reinterpret_cast<const float2*>(a.wt + b * a.w_bstride) + ((size_t)m * 2 + role) * NF;
+        const int mc = (item - b * a.items_per_batch) * GEO::G + g;      // 2 m + c
+        const bool live = mc < 2 * a.ntile;
+        float2* col = a.t + b * a.t_bstride + (size_t)(mc >> 1) * NF * 2 + (mc & 1);      // stride 2 float2 per row
+        const float* w = a.wt + b * a.w_bstride + (size_t)mc * NF * 2;
 
         float2 v[2][kE];
         if (live) {
-#pragma unroll
-            for (int e = 0; e < kE; ++e) {
-                const float4 x = ldg4(tile + p + e * P);
-                v[0][e] = lo(x);
-                v[1][e] = hi(x);
-            }
-            // L2 prefetch: this item's weights (needed after the forward transform), the next item's tile
+            // warm L2 with this column's weights (read after the forward transform) and the next item's column
             if ((p & 15) == 0) {
 #pragma unroll
-                for (int e = 0; e < kE; ++e) prefetch_l2(w + p + e * P);
+                for (int e = 0; e < kE; ++e) prefetch_l2(w + 2 * (p + e * P));
             }
-            const int nitem = item + gridDim.x;
-            if (nitem < a.nitems && (p & 7) == 0 && role == 0) {
-                const int nb_ = nitem / a.items_per_batch;
-                const int nm = (nitem - nb_ * a.items_per_batch) * GEO::G + g;
-                if (nm < a.ntile) {
-                    const float4* nt = reinterpret_cast<const float4*>(a.t + nb_ * a.t_bstride) + (size_t)nm * NF;
 #pragma unroll
-                    for (int e = 0; e < kE; ++e) prefetch_l2(nt + p + e * P);
-                }
-            }
-            if (role) {
+            for (int e = 0; e < kE; ++e) v[0][e] = ldg2(reinterpret_cast<const float*>(col + 2 * (p + e * P)));
 #pragma unroll
-                for (int e = 0; e < kE; ++e) {
-                    const float2 tw = __ldg(a.twist + p + e * P);
-                    v[0][e] = cmul(v[0][e], tw);
-                    v[1][e] = cmul(v[1][e], tw);
-                }
-            }
+            for (int e = 0; e < kE; ++e) v[1][e] = cmul(v[0][e], __ldg(a.twist + p + e * P));
         } else {
 #pragma unroll
             for (int e = 0; e < kE; ++e) { v[0][e] = make_float2(0.f, 0.f); v[1][e] = make_float2(0.f, 0.f); }
         }
-        if (!(a.dbg & 2)) pair_fft<NF, false>(v, p, buf, tws);
-        if (live && !(a.dbg & 8)) {
+        pair_fft<NF, false>(v, p, buf, tws);
+        if (live) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 ww = ldg2(reinterpret_cast<const float*>(w + p + e * P));
+                const float2 ww = ldg2(w + 2 * (p + e * P));
                 v[0][e] = cscale(v[0][e], ww.x);
                 v[1][e] = cscale(v[1][e], ww.y);
             }
         }
-        if (!(a.dbg & 2)) pair_fft<NF, true>(v, p, buf, tws);
-        if (role) {
+        pair_fft<NF, true>(v, p, buf, tws);
+        if (live) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 tw = __ldg(a.twist + p + e * P);
-                cb[e * P + p] = pack(cmulc(v[0][e], tw), cmulc(v[1][e], tw));
+                const float2 o = cmulc(v[1][e], __ldg(a.twist + p + e * P));
+                stg2(col + 2 * (p + e * P), make_float2(v[0][e].x + o.x, v[0][e].y + o.y));
             }
         }
-        __syncthreads();
-        if (!role && live) {
-#pragma unroll
-            for (int e = 0; e < kE; ++e) {
-                const float4 o = cb[e * P + p];
-                stg4(tile + p + e * P, make_float4(v[0][e].x + o.x, v[0][e].y + o.y, v[1][e].x + o.z, v[1][e].y + o.w));
-            }
-        }
-        __syncthreads();
     }
 }
 

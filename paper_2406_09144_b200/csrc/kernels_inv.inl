@@ -8,13 +8,17 @@ struct RowsInvArgs {
     const float* s;       // [nb][ny][NF]  (kMulS, kEnergy)
     const float* j;       // [nb][ny][NF]  (kEnergy)
     double* partials;     // [gridDim.x][2]  (kEnergy): sum s*c, sum j*s
-    int ny, mode, dbg;
+    int ny, mode;
     int items_per_batch, nitems;
     size_t t_bstride, img_bstride;
     const float4* tw;
     const float2* twist;
 };
 
+// Pipeline: the half-spectrum rows of the NEXT item are gathered by 16-byte cp.async copies straight
+// into the exchange buffer as soon as the transform has left it (before its last, register-only
+// stage), so the gather is in flight during that stage and the epilogue.  Landing layout:
+// slot r*(NF/2+1) + m = (Y_r[2m], Y_r[2m+1]) for row r of the pair.
 template <int NF>
 __global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
 rows_inv_kernel(RowsInvArgs a) {
@@ -24,10 +28,35 @@ rows_inv_kernel(RowsInvArgs a) {
     extern __shared__ float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
-    float4* buf = smem4 + GEO::TW + (size_t)g * xbuf_len(NF);
+    float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
+    const float2* land = reinterpret_cast<const float2*>(buf);      // Y_r[k] at land[r*2*NTILE + k]
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
     double acc_sc = 0.0, acc_js = 0.0;
+
+    auto gather = [&](int item) {
+        const int b = item / a.items_per_batch;
+        const int rp = (item - b * a.items_per_batch) * GEO::G + g;
+        if (item < a.nitems && 2 * rp < a.ny) {
+            const float4* tb = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + 2 * rp;
+            // lanes (2j, 2j+1) fetch rows (0, 1) of the same tile: one 32-byte sector per lane pair
+            const int r = p & 1;
+#pragma unroll
+            for (int i = 0; i < kE; ++i) {
+                const int m = (p >> 1) + i * (P / 2);
+                cp_async16(buf + r * NTILE + m, tb + (size_t)m * a.ny + r);
+            }
+            if (p < 2) cp_async16(buf + r * NTILE + NTILE - 1, tb + (size_t)(NTILE - 1) * a.ny + r);
+            // warm L2 with the rows of s (and j) the epilogue of that item will read: P lines of 128 B
+            if (a.mode != kPlain) {
+                const size_t row = b * a.img_bstride + (size_t)(2 * rp) * NF;
+                prefetch_l2(a.s + row + 32 * p);
+                if (a.mode == kEnergy) prefetch_l2(a.j + row + 32 * p);
+            }
+        }
+        cp_async_commit();
+    };
+    gather(blockIdx.x);
 
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const int b = item / a.items_per_batch;
@@ -35,27 +64,7 @@ rows_inv_kernel(RowsInvArgs a) {
         const bool live = 2 * rp < a.ny;
         const int y0 = 2 * rp;
 
-        if (live) {
-            const float4* tb = reinterpret_cast<const float4*>(a.t + b * a.t_bstride);
-            float4 r0[kE / 2], r1[kE / 2];
-#pragma unroll
-            for (int i = 0; i < kE / 2; ++i) {
-                const float4* q = (a.dbg & 1) ? tb + ((size_t)rp * (NF / 2) + p + i * P) * 2 : tb + (size_t)(p + i * P) * a.ny + y0;
-                r0[i] = ldg4(q);
-                r1[i] = ldg4(q + 1);
-            }
-#pragma unroll
-            for (int i = 0; i < kE / 2; ++i) {
-                const int k = 2 * (p + i * P);
-                buf[xpad(k)] = make_float4(r0[i].x, r0[i].y, r1[i].x, r1[i].y);
-                buf[xpad(k + 1)] = make_float4(r0[i].z, r0[i].w, r1[i].z, r1[i].w);
-            }
-            if (p == 0) {                               // tail tile: column NF
-                const float4* q = tb + (size_t)(NTILE - 1) * a.ny + y0;
-                const float4 t0 = ldg4(q), t1 = ldg4(q + 1);
-                buf[xpad(NF)] = make_float4(t0.x, t0.y, t1.x, t1.y);
-            }
-        }
+        cp_async_wait_all();
         __syncthreads();
         // Z'[k] = (Y[k] + conj Y[NF-k]) + i conj(twist[k]) (Y[k] - conj Y[NF-k]),  k = 0..NF-1
         float2 v[2][kE];
@@ -63,17 +72,18 @@ rows_inv_kernel(RowsInvArgs a) {
         for (int e = 0; e < kE; ++e) {
             const int k = p + e * P;
             const float2 w = __ldg(a.twist + k);
-            float4 yk = make_float4(0.f, 0.f, 0.f, 0.f), yn = yk;
-            if (live) { yk = buf[xpad(k)]; yn = buf[xpad(NF - k)]; }
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
-                const float2 ya = t ? hi(yk) : lo(yk), ym = cconj(t ? hi(yn) : lo(yn));
+                float2 ya = make_float2(0.f, 0.f), ym = ya;
+                if (live) { ya = land[t * 2 * NTILE + k]; ym = cconj(land[t * 2 * NTILE + NF - k]); }
                 const float2 s = cadd(ya, ym), d = cmulc(csub(ya, ym), w);
                 v[t][e] = make_float2(s.x - d.y, s.y + d.x);
             }
         }
         __syncthreads();
-        if (!(a.dbg & 2)) pair_fft<NF, true>(v, p, buf, tws);
+        pair_fft_head<NF, true>(v, p, buf, tws);
+        gather(item + gridDim.x);                 // buf is free from here to the top of the loop
+        pair_fft_tail<NF, true>(v, p, tws);
 
         if (live) {
 #pragma unroll
@@ -83,8 +93,7 @@ rows_inv_kernel(RowsInvArgs a) {
                 for (int e = 0; e < kE / 2; ++e) {
                     const int n = p + e * P;
                     float2 c = v[t][e];
-                    if (a.dbg & 4) {
-                    } else if (a.mode == kMulS) {
+                    if (a.mode == kMulS) {
                         const float2 s = ldg2(a.s + row + 2 * n);
                         c.x *= s.x; c.y *= s.y;
                     } else if (a.mode == kEnergy) {
@@ -97,8 +106,8 @@ rows_inv_kernel(RowsInvArgs a) {
                 }
             }
         }
-        __syncthreads();
     }
+    cp_async_wait_all();
     if (a.mode == kEnergy) {
         // fixed-order block reduction: warp shuffle tree, then warp 0 over the per-warp sums
         __shared__ double red[2][32];

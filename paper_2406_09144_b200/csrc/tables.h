@@ -16,19 +16,17 @@ inline std::vector<float4> build_twiddles(int n) {
     };
     for (int s = 1; s < plan_stages(n); ++s) {
         const int R = plan_radix(n, s), NS = plan_ns(n, s), off = plan_tw_off(n, s), HP = R / 2, WA = plan_tw_wa(n, s);
-        const bool fact = plan_tw_fact(n, s);
         const long long den = (long long)NS * R;
-        for (int q = 0; q < HP; ++q) {
-            const int r1 = 2 * q + 1, r2 = 2 * q + 2;
-            for (int a = 0; a < WA; ++a) {
-                const long long j = fact ? 16LL * a : a;
-                const float2 w1 = ex(j * r1, den), w2 = r2 < R ? ex(j * r2, den) : make_float2(1.f, 0.f);
-                tw[(size_t)off + q * WA + a] = make_float4(w1.x, w1.y, w2.x, w2.y);
-            }
-            if (fact)
-                for (int c = 0; c < 16; ++c) {
-                    const float2 w1 = ex((long long)c * r1, den), w2 = r2 < R ? ex((long long)c * r2, den) : make_float2(1.f, 0.f);
-                    tw[(size_t)off + HP * WA + q * 16 + c] = make_float4(w1.x, w1.y, w2.x, w2.y);
+        if (plan_tw_fact(n, s)) {
+            float2* f = reinterpret_cast<float2*>(tw.data() + off);
+            for (int a = 0; a < WA; ++a) f[a] = ex(16LL * a, den);
+            for (int c = 0; c < 16; ++c) f[WA + c] = ex(c, den);
+        } else {
+            for (int q = 0; q < HP; ++q)
+                for (int j = 0; j < WA; ++j) {
+                    const int r1 = 2 * q + 1, r2 = 2 * q + 2;
+                    const float2 w1 = ex((long long)j * r1, den), w2 = r2 < R ? ex((long long)j * r2, den) : make_float2(1.f, 0.f);
+                    tw[(size_t)off + q * WA + j] = make_float4(w1.x, w1.y, w2.x, w2.y);
                 }
         }
     }
