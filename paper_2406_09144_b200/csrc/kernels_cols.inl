@@ -47,7 +47,7 @@ conv_cols_kernel(ConvColsArgs a) {
                 for (int e = 0; e < kE; ++e) prefetch_l2(w + 2 * (p + e * P));
             }
 #pragma unroll
-            for (int e = 0; e < kE; ++e) v[0][e] = ldg2(reinterpret_cast<const float*>(col + 2 * (p + e * P)));
+            for (int e = 0; e < kE; ++e) v[0][e] = ld2_inplace(col + 2 * (p + e * P));
 #pragma unroll
             for (int e = 0; e < kE; ++e) v[1][e] = cmul(v[0][e], __ldg(a.twist + p + e * P));
         } else {

@@ -86,23 +86,34 @@ rows_inv_kernel(RowsInvArgs a) {
         pair_fft_tail<NF, true>(v, p, tws);
 
         if (live) {
+            const size_t row0 = b * a.img_bstride + (size_t)y0 * NF;
+            float2 sv[2][kE / 2], jv[2][kE / 2];
+            if (a.mode != kPlain) {
+#pragma unroll
+                for (int t = 0; t < 2; ++t)
+#pragma unroll
+                    for (int e = 0; e < kE / 2; ++e) sv[t][e] = ldg2(a.s + row0 + (size_t)t * NF + 2 * (p + e * P));
+            }
+            if (a.mode == kEnergy) {
+#pragma unroll
+                for (int t = 0; t < 2; ++t)
+#pragma unroll
+                    for (int e = 0; e < kE / 2; ++e) jv[t][e] = ldg2(a.j + row0 + (size_t)t * NF + 2 * (p + e * P));
+            }
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
-                const size_t row = b * a.img_bstride + (size_t)(y0 + t) * NF;
 #pragma unroll
                 for (int e = 0; e < kE / 2; ++e) {
-                    const int n = p + e * P;
                     float2 c = v[t][e];
                     if (a.mode == kMulS) {
-                        const float2 s = ldg2(a.s + row + 2 * n);
-                        c.x *= s.x; c.y *= s.y;
+                        c.x *= sv[t][e].x; c.y *= sv[t][e].y;
                     } else if (a.mode == kEnergy) {
-                        const float2 s = ldg2(a.s + row + 2 * n), j = ldg2(a.j + row + 2 * n);
+                        const float2 s = sv[t][e], j = jv[t][e];
                         acc_sc += (double)s.x * (double)c.x + (double)s.y * (double)c.y;
                         acc_js += (double)j.x * (double)s.x + (double)j.y * (double)s.y;
                         c.x = s.x * (c.x - j.x); c.y = s.y * (c.y - j.y);
                     }
-                    stg2(a.out + row + 2 * n, c);
+                    stg2(a.out + row0 + (size_t)t * NF + 2 * (p + e * P), c);
                 }
             }
         }
