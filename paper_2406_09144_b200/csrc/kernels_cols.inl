@@ -18,8 +18,9 @@ struct ConvColsArgs {
 //   y[n] = IFFT_NF(E')[n] + conj(twist^n) IFFT_NF(O')[n]
 // so input, twiddles and the final combination are all thread-local.  Work item = (tile, column);
 // the two columns of a tile go to neighbouring CTAs, which share the tile's sectors through L2.
-// Several independent CTAs per SM keep the shared-memory exchange of one overlapped with the
-// arithmetic of another.
+// Independent CTAs on one SM keep the shared-memory exchange of one overlapped with the arithmetic
+// of another (staging the column and the weights through cp.async was measured slower: the added
+// shared-memory traffic costs more than the latency it hides).
 template <int NF>
 __global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
 conv_cols_kernel(ConvColsArgs a) {
@@ -41,7 +42,7 @@ conv_cols_kernel(ConvColsArgs a) {
 
         float2 v[2][kE];
         if (live) {
-            // warm L2 with this column's weights (read after the forward transform) and the next item's column
+            // warm L2 with this column's weights (read after the forward transform)
             if ((p & 15) == 0) {
 #pragma unroll
                 for (int e = 0; e < kE; ++e) prefetch_l2(w + 2 * (p + e * P));
