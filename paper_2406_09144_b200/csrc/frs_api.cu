@@ -29,7 +29,10 @@ struct frs_ctx {
     int ntile = 0, ntile_h = 0;
     std::map<int, float4*> tw;
     std::map<int, float2*> twist;
-    float *wt = nullptr, *dirty = nullptr, *amp = nullptr, *s = nullptr;
+    // two orientations of the sky-space arrays: natural [ny][nx] (public sky-space calls) and
+    // transposed [nx][ny] (latent-space path: each 2-pass Hartley transform transposes for free)
+    float *wt = nullptr, *wtT = nullptr, *dirty = nullptr, *dirtyT = nullptr, *amp = nullptr, *s = nullptr, *sT = nullptr;
+    bool s_ok = false, sT_ok = false;
     float *d_mu = nullptr, *d_lognu = nullptr;
     float2 *T = nullptr, *Th = nullptr;
     float *lin = nullptr, *img = nullptr, *acc = nullptr;
@@ -105,14 +108,17 @@ int ensure_tables(frs_ctx* ctx, int n) {
     return FRS_OK;
 }
 
+size_t max2(size_t a, size_t b) { return a > b ? a : b; }
+
 int ensure_scratch(frs_ctx* ctx) {
-    const size_t np = ctx->npix;
-    RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * ctx->ntile * ctx->ny * 2));
-    RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * ctx->ntile_h * ctx->ny * 2));
+    const size_t np = ctx->npix, ny = ctx->ny, nx = ctx->nx;
+    RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
+    RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * max2((nx / 4 + 1) * ny, (ny / 4 + 1) * nx) * 2));
     RET(dev_alloc(ctx, &ctx->lin, 2 * np));
     RET(dev_alloc(ctx, &ctx->acc, 2 * np));
     RET(dev_alloc(ctx, &ctx->img, (size_t)ctx->nchan * np));
     RET(dev_alloc(ctx, &ctx->s, (size_t)ctx->nchan * np));
+    RET(dev_alloc(ctx, &ctx->sT, (size_t)ctx->nchan * np));
     return FRS_OK;
 }
 
@@ -132,61 +138,87 @@ int dot(frs_ctx* ctx, const float* a, const float* b, size_t n, double* d_out) {
 }
 
 // ---- the three passes of C (Eq. 14) -----------------------------------------------------------
-int conv_rows_fwd(frs_ctx* ctx, const float* in, const float* mul) {
+// Orientation of a sky-space image: [rows][len].  Natural: rows = ny, len = nx.  Transposed: rows = nx,
+// len = ny, with the weight table built for the transposed PSF spectrum.
+struct Orient { int rows, len, ntile; const float* wt; };
+Orient orient(const frs_ctx* ctx, bool transposed) {
+    return transposed ? Orient{ctx->nx, ctx->ny, ctx->ny / 2 + 1, ctx->wtT} : Orient{ctx->ny, ctx->nx, ctx->nx / 2 + 1, ctx->wt};
+}
+
+int conv_rows_fwd(frs_ctx* ctx, const Orient& o, const float* in, const float* mul) {
     Prof pr(ctx, kPassRowsFwd);
     RowsFwdArgs a{};
-    a.in = in; a.mul = mul; a.out = ctx->T; a.ny = ctx->ny;
-    a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)ctx->ntile * ctx->ny * 2;
+    a.in = in; a.mul = mul; a.out = ctx->T; a.ny = o.rows;
+    a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)o.ntile * o.rows * 2;
     a.scale = 1.0f;   // yields 2 X[k]; the 1/2 is folded into wt
-    a.tw = ctx->tw[ctx->nx]; a.twist = ctx->twist[ctx->nx];
-    CKL(launch_rows_fwd(ctx->stream, ctx->nx, true, a, ctx->nchan));
+    a.tw = ctx->tw[o.len]; a.twist = ctx->twist[o.len];
+    CKL(launch_rows_fwd(ctx->stream, o.len, true, a, ctx->nchan));
     ctx->launches++;
     return FRS_OK;
 }
-int conv_cols(frs_ctx* ctx) {
+int conv_cols(frs_ctx* ctx, const Orient& o) {
     Prof pr(ctx, kPassConvCols);
     ConvColsArgs a{};
-    a.t = ctx->T; a.wt = ctx->wt; a.ntile = ctx->ntile;
-    a.t_bstride = (size_t)ctx->ntile * ctx->ny * 2; a.w_bstride = (size_t)ctx->ntile * 2 * ctx->ny * 2;
-    a.tw = ctx->tw[ctx->ny]; a.twist = ctx->twist[ctx->ny];
-    CKL(launch_conv_cols(ctx->stream, ctx->ny, a, ctx->nchan));
+    a.t = ctx->T; a.wt = o.wt; a.ntile = o.ntile;
+    a.t_bstride = (size_t)o.ntile * o.rows * 2; a.w_bstride = (size_t)o.ntile * 2 * o.rows * 2;
+    a.tw = ctx->tw[o.rows]; a.twist = ctx->twist[o.rows];
+    CKL(launch_conv_cols(ctx->stream, o.rows, a, ctx->nchan));
     ctx->launches++;
     return FRS_OK;
 }
-int conv_rows_inv(frs_ctx* ctx, float* out, int mode, int* grid_x) {
+int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const float* s, const float* j, int* grid_x) {
     Prof pr(ctx, kPassRowsInv);
     RowsInvArgs a{};
-    a.t = ctx->T; a.out = out; a.s = ctx->s; a.j = ctx->dirty; a.partials = ctx->partials;
-    a.ny = ctx->ny; a.mode = mode;
-    a.t_bstride = (size_t)ctx->ntile * ctx->ny * 2; a.img_bstride = ctx->npix;
-    a.tw = ctx->tw[ctx->nx]; a.twist = ctx->twist[ctx->nx];
-    CKL(launch_rows_inv(ctx->stream, ctx->nx, a, ctx->nchan, grid_x));
+    a.t = ctx->T; a.out = out; a.s = s; a.j = j; a.partials = ctx->partials;
+    a.ny = o.rows; a.mode = mode;
+    a.t_bstride = (size_t)o.ntile * o.rows * 2; a.img_bstride = ctx->npix;
+    a.tw = ctx->tw[o.len]; a.twist = ctx->twist[o.len];
+    CKL(launch_rows_inv(ctx->stream, o.len, a, ctx->nchan, grid_x));
     ctx->launches++;
     return FRS_OK;
 }
 
-// out[b] = (mul .) H[ premul . in[b] ] (+ offset[b]) (+ add)     -- 2-D Hartley transform, two passes
-int hartley(frs_ctx* ctx, const float* in, const float* premul, float* out, const float* mul, const float* add,
-            const float* offset_dev, int nb) {
+// TRANSPOSING 2-D Hartley transform, two passes:  in [nb][n1][n2]  ->  out [nb][n2][n1],
+//   out[x][y] = (mul[x][y] .) ( H[premul . in][y][x] + offset[b] ) (+ add[x][y]).
+// The row pass leaves column tiles, and the column pass of column x produces H[.][x] for all y, which is
+// one contiguous run of the transposed output -- so the transform transposes for free, and the
+// latent-space path keeps its sky-space arrays transposed instead of paying for scattered stores.
+int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul, float* out, const float* mul,
+              const float* add, const float* offset_dev, int nb) {
+    const int ntile_h = n2 / 4 + 1;
     {
         Prof pr(ctx, kPassHartRows);
         RowsFwdArgs a{};
-        a.in = in; a.mul = premul; a.out = ctx->Th; a.ny = ctx->ny;
-        a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)ctx->ntile_h * ctx->ny * 2;
+        a.in = in; a.mul = premul; a.out = ctx->Th; a.ny = n1;
+        a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)ntile_h * n1 * 2;
         a.scale = 0.5f;
-        a.tw = ctx->tw[ctx->nx / 2]; a.twist = ctx->twist[ctx->nx / 2];
-        CKL(launch_rows_fwd(ctx->stream, ctx->nx / 2, false, a, nb));
+        a.tw = ctx->tw[n2 / 2]; a.twist = ctx->twist[n2 / 2];
+        CKL(launch_rows_fwd(ctx->stream, n2 / 2, false, a, nb));
         ctx->launches++;
     }
     {
         Prof pr(ctx, kPassHartCols);
         HartColsArgs a{};
-        a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = ctx->nx;
-        a.t_bstride = (size_t)ctx->ntile_h * ctx->ny * 2; a.img_bstride = ctx->npix;
-        a.tw = ctx->tw[ctx->ny];
-        CKL(launch_hart_cols(ctx->stream, ctx->ny, a, nb));
+        a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = n2;
+        a.t_bstride = (size_t)ntile_h * n1 * 2; a.img_bstride = ctx->npix;
+        a.tw = ctx->tw[n1];
+        CKL(launch_hart_cols(ctx->stream, n1, a, nb));
         ctx->launches++;
     }
+    return FRS_OK;
+}
+
+int transpose(frs_ctx* ctx, const float* in, float* out, int rows, int cols, int nb) {
+    CKL(launch_transpose(ctx->stream, in, out, rows, cols, nb));
+    ctx->launches++;
+    return FRS_OK;
+}
+int need_s_natural(frs_ctx* ctx) {
+    if (!ctx->s_ok) { RET(transpose(ctx, ctx->sT, ctx->s, ctx->nx, ctx->ny, ctx->nchan)); ctx->s_ok = true; }
+    return FRS_OK;
+}
+int need_s_transposed(frs_ctx* ctx) {
+    if (!ctx->sT_ok) { RET(transpose(ctx, ctx->s, ctx->sT, ctx->ny, ctx->nx, ctx->nchan)); ctx->sT_ok = true; }
     return FRS_OK;
 }
 
@@ -201,38 +233,42 @@ int check_hot(frs_ctx* ctx, bool need_s, bool need_model) {
 }
 
 int sky_forward_impl(frs_ctx* ctx, const float* xi) {
-    // tau_f = mu_f + H[A_f xi_f];  s_c = exp(tau_0 + lognu_c tau_1)      (R6)
-    RET(hartley(ctx, xi, ctx->amp, ctx->lin, nullptr, nullptr, ctx->d_mu, ctx->nfield));
-    sky_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->d_lognu, ctx->s, ctx->npix, ctx->nfield, ctx->nchan);
+    // tau_f = mu_f + H[A_f xi_f];  s_c = exp(tau_0 + lognu_c tau_1)      (R6)   -- sky-space arrays transposed
+    RET(hartley_t(ctx, xi, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, ctx->d_mu, ctx->nfield));
+    sky_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->d_lognu, ctx->sT, ctx->npix, ctx->nfield, ctx->nchan);
     ctx->launches++;
     CK(cudaGetLastError());
     ctx->have_s = true;
+    ctx->sT_ok = true;
+    ctx->s_ok = false;
     return FRS_OK;
 }
 
 int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out) {
-    // lin_f = H[A_f v_f]
-    RET(hartley(ctx, v, ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
+    const Orient o = orient(ctx, true);
+    RET(need_s_transposed(ctx));
+    // lin_f = H[A_f v_f]   (transposed)
+    RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
     const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
     if (simple) {
-        RET(conv_rows_fwd(ctx, ctx->lin, ctx->s));                 // s . lin fused into the row pass
+        RET(conv_rows_fwd(ctx, o, ctx->lin, ctx->sT));             // s . lin fused into the row pass
     } else {
-        jvp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->s, ctx->d_lognu, ctx->img,
+        jvp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->sT, ctx->d_lognu, ctx->img,
                                                                                ctx->npix, ctx->nfield, ctx->nchan);
         ctx->launches++;
-        RET(conv_rows_fwd(ctx, ctx->img, nullptr));
+        RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
     }
-    RET(conv_cols(ctx));
+    RET(conv_cols(ctx, o));
     if (simple) {
-        RET(conv_rows_inv(ctx, ctx->acc, kMulS, nullptr));         // acc = s . C(...)
+        RET(conv_rows_inv(ctx, o, ctx->acc, kMulS, ctx->sT, nullptr, nullptr));      // acc = s . C(...)
     } else {
-        RET(conv_rows_inv(ctx, ctx->img, kMulS, nullptr));
+        RET(conv_rows_inv(ctx, o, ctx->img, kMulS, ctx->sT, nullptr, nullptr));
         vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
                                                                                ctx->nfield, ctx->nchan);
         ctx->launches++;
     }
-    // out_f = A_f . H[acc_f] (+ v_f)
-    RET(hartley(ctx, ctx->acc, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield));
+    // out_f = A_f . H[acc_f] (+ v_f)   (transposes back to the latent layout)
+    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield));
     CK(cudaGetLastError());
     return FRS_OK;
 }
@@ -290,6 +326,7 @@ int frs_create(int ny, int nx, int nchan, int device, void* stream, frs_ctx** ou
         RET(ensure_tables(ctx, nx));
         RET(ensure_tables(ctx, ny));
         RET(ensure_tables(ctx, nx / 2));
+        RET(ensure_tables(ctx, ny / 2));
         RET(dev_alloc(ctx, &ctx->partials, (size_t)1 << 16));
         RET(dev_alloc(ctx, &ctx->scal, 16));
         RET(dev_alloc(ctx, &ctx->flag, 4));
@@ -312,11 +349,18 @@ void frs_destroy(frs_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     for (auto& kv : ctx->tw) cudaFree(kv.second);
     for (auto& kv : ctx->twist) cudaFree(kv.second);
-    void* ptrs[] = {ctx->wt, ctx->dirty, ctx->amp, ctx->s, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->Th, ctx->lin, ctx->img,
+    void* ptrs[] = {ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->Th, ctx->lin, ctx->img,
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     delete ctx;
+}
+
+static int build_transposed_weights(frs_ctx* ctx) {
+    RET(dev_alloc(ctx, &ctx->wtT, (size_t)ctx->nchan * (ctx->ny / 2 + 1) * 2 * ctx->nx * 2));
+    CKL(launch_weights_transpose(ctx->stream, ctx->wt, ctx->wtT, ctx->ny, ctx->nx, ctx->nchan));
+    ctx->launches++;
+    return FRS_OK;
 }
 
 int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
@@ -326,6 +370,7 @@ int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
     CK(cudaMemsetAsync(ctx->flag, 0, sizeof(int), ctx->stream));
     CKL(launch_weights_layout(ctx->stream, w_half, ctx->wt, ctx->ny, ctx->nx, ctx->nchan, ctx->flag));
     ctx->launches++;
+    RET(build_transposed_weights(ctx));
     int neg = 0;
     CK(cudaMemcpyAsync(&neg, ctx->flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
@@ -362,6 +407,7 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
         c.tw = ctx->tw[ctx->ny]; c.twist = ctx->twist[ctx->ny];
         CKL(launch_psf_cols(ctx->stream, ctx->ny, c, ctx->nchan, nullptr));
         ctx->launches += 2;
+        RET(build_transposed_weights(ctx));
         hs.resize((size_t)ctx->nchan * gx * 3);
         CK(cudaMemcpyAsync(hs.data(), stats, hs.size() * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
         CK(cudaStreamSynchronize(ctx->stream));
@@ -388,7 +434,9 @@ int frs_set_dirty(frs_ctx* ctx, const float* j) {
     if (!ctx || !j || !aligned16(j)) return fail(ctx, FRS_EINVAL, "frs_set_dirty: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(dev_alloc(ctx, &ctx->dirty, (size_t)ctx->nchan * ctx->npix));
+    RET(dev_alloc(ctx, &ctx->dirtyT, (size_t)ctx->nchan * ctx->npix));
     CK(cudaMemcpyAsync(ctx->dirty, j, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    RET(transpose(ctx, ctx->dirty, ctx->dirtyT, ctx->ny, ctx->nx, ctx->nchan));
     ctx->have_dirty = true;
     return FRS_OK;
 }
@@ -404,7 +452,7 @@ int frs_set_amplitude(frs_ctx* ctx, int nfield, const float* amp, const float* m
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->nfield = nfield;
     ctx->have_amp = true;
-    ctx->have_s = false;
+    ctx->have_s = ctx->s_ok = ctx->sT_ok = false;
     return FRS_OK;
 }
 
@@ -413,7 +461,7 @@ int frs_set_channel_lognu(frs_ctx* ctx, const float* lognu_host) {
     CK(cudaSetDevice(ctx->device));
     CK(cudaMemcpyAsync(ctx->d_lognu, lognu_host, ctx->nchan * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
-    ctx->have_s = false;
+    ctx->have_s = ctx->s_ok = ctx->sT_ok = false;
     return FRS_OK;
 }
 
@@ -422,7 +470,8 @@ int frs_set_sky(frs_ctx* ctx, const float* sky) {
     CK(cudaSetDevice(ctx->device));
     RET(ensure_scratch(ctx));
     CK(cudaMemcpyAsync(ctx->s, sky, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
-    ctx->have_s = true;
+    ctx->have_s = ctx->s_ok = true;
+    ctx->sT_ok = false;
     return FRS_OK;
 }
 
@@ -432,7 +481,10 @@ int frs_sky_forward(frs_ctx* ctx, const float* xi, float* sky) {
     CK(cudaSetDevice(ctx->device));
     RET(ensure_scratch(ctx));
     RET(sky_forward_impl(ctx, xi));
-    if (sky) CK(cudaMemcpyAsync(sky, ctx->s, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    if (sky) {
+        RET(need_s_natural(ctx));
+        CK(cudaMemcpyAsync(sky, ctx->s, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    }
     return FRS_OK;
 }
 
@@ -440,9 +492,10 @@ int frs_psf_apply(frs_ctx* ctx, const float* x, float* y) {
     if (!ctx || !x || !y || !aligned16(x) || !aligned16(y)) return fail(ctx, FRS_EINVAL, "frs_psf_apply: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(check_hot(ctx, false, false));
-    RET(conv_rows_fwd(ctx, x, nullptr));
-    RET(conv_cols(ctx));
-    RET(conv_rows_inv(ctx, y, kPlain, nullptr));
+    const Orient o = orient(ctx, false);
+    RET(conv_rows_fwd(ctx, o, x, nullptr));
+    RET(conv_cols(ctx, o));
+    RET(conv_rows_inv(ctx, o, y, kPlain, nullptr, nullptr, nullptr));
     return FRS_OK;
 }
 
@@ -450,9 +503,11 @@ int frs_sky_metric_apply(frs_ctx* ctx, const float* x, float* y) {
     if (!ctx || !x || !y || !aligned16(x) || !aligned16(y)) return fail(ctx, FRS_EINVAL, "frs_sky_metric_apply: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(check_hot(ctx, true, false));
-    RET(conv_rows_fwd(ctx, x, ctx->s));
-    RET(conv_cols(ctx));
-    RET(conv_rows_inv(ctx, y, kMulS, nullptr));
+    const Orient o = orient(ctx, false);
+    RET(need_s_natural(ctx));
+    RET(conv_rows_fwd(ctx, o, x, ctx->s));
+    RET(conv_cols(ctx, o));
+    RET(conv_rows_inv(ctx, o, y, kMulS, ctx->s, nullptr, nullptr));
     return FRS_OK;
 }
 
@@ -462,10 +517,11 @@ int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_ene
     RET(check_hot(ctx, false, true));
     if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
     RET(sky_forward_impl(ctx, xi));
-    RET(conv_rows_fwd(ctx, ctx->s, nullptr));
-    RET(conv_cols(ctx));
+    const Orient o = orient(ctx, true);                       // sky-space arrays transposed on this path
+    RET(conv_rows_fwd(ctx, o, ctx->sT, nullptr));
+    RET(conv_cols(ctx, o));
     int gx = 0;
-    RET(conv_rows_inv(ctx, ctx->img, kEnergy, &gx));          // img_c = s_c (C s_c - j_c), partial sums
+    RET(conv_rows_inv(ctx, o, ctx->img, kEnergy, ctx->sT, ctx->dirtyT, &gx));   // img_c = s_c (C s_c - j_c), partial sums
     const int np = gx;      // one (sum s.c, sum j.s) pair per persistent CTA
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, np, 2, 0, ctx->scal + 8);
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, np, 2, 1, ctx->scal + 9);
@@ -480,7 +536,7 @@ int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_ene
         ctx->launches++;
         accp = ctx->acc;
     }
-    RET(hartley(ctx, accp, nullptr, grad, ctx->amp, with_prior ? xi : nullptr, nullptr, ctx->nfield));
+    RET(hartley_t(ctx, accp, ctx->nx, ctx->ny, nullptr, grad, ctx->amp, with_prior ? xi : nullptr, nullptr, ctx->nfield));
     CK(cudaGetLastError());
     if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     if (h_energy) {
@@ -582,9 +638,11 @@ static int host_apply(frs_ctx* ctx, const float* xh, float* yh, bool with_s) {
     RET(dev_alloc(ctx, &ctx->hx, n));
     RET(dev_alloc(ctx, &ctx->hy, n));
     CK(cudaMemcpyAsync(ctx->hx, xh, n * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
-    RET(conv_rows_fwd(ctx, ctx->hx, with_s ? ctx->s : nullptr));
-    RET(conv_cols(ctx));
-    RET(conv_rows_inv(ctx, ctx->hy, with_s ? kMulS : kPlain, nullptr));
+    const Orient o = orient(ctx, false);
+    if (with_s) RET(need_s_natural(ctx));
+    RET(conv_rows_fwd(ctx, o, ctx->hx, with_s ? ctx->s : nullptr));
+    RET(conv_cols(ctx, o));
+    RET(conv_rows_inv(ctx, o, ctx->hy, with_s ? kMulS : kPlain, ctx->s, nullptr, nullptr));
     CK(cudaMemcpyAsync(yh, ctx->hy, n * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return FRS_OK;

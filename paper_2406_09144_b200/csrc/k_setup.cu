@@ -115,4 +115,58 @@ int launch_weights_layout(cudaStream_t st, const float* w_half, float* wt, int n
     return (int)cudaGetLastError();
 }
 
+// Weight table of the transposed orientation (image [nx][ny]): rows are transformed along y (tiles over
+// ky = 2m+c, 0..ny), columns along x (padded bins kx = 2q+par, q < nx):
+//   wtT[m][c][q][par] = 0.5 W[ky][kx],  W[ky][kx] = W[(-ky) mod 2ny][2nx - kx] for kx > nx  (Hermitian, R4)
+__device__ __forceinline__ float wt_lookup(const float* wt, int ny, int ky, int kx) {   // kx <= nx
+    return wt[(((size_t)(kx >> 1) * 2 + (kx & 1)) * ny + (ky >> 1)) * 2 + (ky & 1)];
+}
+__global__ void weights_transpose_kernel(const float* __restrict__ wt, float* __restrict__ wtT, int ny, int nx) {
+    const int ntT = ny / 2 + 1;
+    const size_t perT = (size_t)ntT * 2 * nx * 2, per = (size_t)(nx / 2 + 1) * 2 * ny * 2;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= perT) return;
+    const int b = blockIdx.y;
+    const int par = i & 1;
+    const int q = (i >> 1) % nx;
+    const int c = ((i >> 1) / nx) & 1;
+    const int m = (int)((i >> 1) / nx / 2);
+    const int ky = 2 * m + c, kx = 2 * q + par;
+    float v = 0.f;
+    if (ky <= ny) {
+        const float* w = wt + (size_t)b * per;
+        v = kx <= nx ? wt_lookup(w, ny, ky, kx) : wt_lookup(w, ny, (2 * ny - ky) % (2 * ny), 2 * nx - kx);
+    }
+    wtT[(size_t)b * perT + i] = v;
+}
+int launch_weights_transpose(cudaStream_t st, const float* wt, float* wtT, int ny, int nx, int nb) {
+    const size_t perT = (size_t)(ny / 2 + 1) * 2 * nx * 2;
+    dim3 grid((unsigned)((perT + 255) / 256), nb);
+    weights_transpose_kernel<<<grid, 256, 0, st>>>(wt, wtT, ny, nx);
+    return (int)cudaGetLastError();
+}
+
+__global__ void transpose_kernel(const float* __restrict__ in, float* __restrict__ out, int rows, int cols) {
+    __shared__ float tile[32][33];
+    const size_t base = (size_t)blockIdx.z * rows * cols;
+    const int x = blockIdx.x * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int y = blockIdx.y * 32 + threadIdx.y + j;
+        if (x < cols && y < rows) tile[threadIdx.y + j][threadIdx.x] = in[base + (size_t)y * cols + x];
+    }
+    __syncthreads();
+    const int ox = blockIdx.y * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int oy = blockIdx.x * 32 + threadIdx.y + j;
+        if (ox < rows && oy < cols) out[base + (size_t)oy * rows + ox] = tile[threadIdx.x][threadIdx.y + j];
+    }
+}
+int launch_transpose(cudaStream_t st, const float* in, float* out, int rows, int cols, int nb) {
+    dim3 grid((cols + 31) / 32, (rows + 31) / 32, nb), block(32, 8);
+    transpose_kernel<<<grid, block, 0, st>>>(in, out, rows, cols);
+    return (int)cudaGetLastError();
+}
+
 }  // namespace frs

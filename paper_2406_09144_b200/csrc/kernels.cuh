@@ -55,6 +55,11 @@ __device__ __forceinline__ float4 ldg4(const void* p) {
         : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
     return r;
 }
+__device__ __forceinline__ float ldg1(const float* p) {
+    float r;
+    asm("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r) : "l"(p));
+    return r;
+}
 // coherent variant for data the same kernel later overwrites in place (conv_cols tiles)
 __device__ __forceinline__ float2 ld2_inplace(const float2* p) {
     float2 r;

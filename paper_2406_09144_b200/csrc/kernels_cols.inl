@@ -77,18 +77,19 @@ conv_cols_kernel(ConvColsArgs a) {
 
 // ------------------------------------------------------------------------------------------------
 struct HartColsArgs {
-    const float2* t;      // [nb][ntile][NF][2], columns x = 0..nx/2 of the row-transformed field
-    float* out;           // [nb][NF][nx]
-    const float* mul;     // optional [nb][NF][nx]: out = mul * H + add
-    const float* add;     // optional [nb][NF][nx]
-    const float* offset;  // optional device [nb]: out = H + offset[b]   (mu)
+    const float2* t;      // [nb][ntile][NF][2], columns x = 0..nx/2 of the row-transformed field (NF rows)
+    float* out;           // [nb][nx][NF]  TRANSPOSED: out[x][y] = H[y][x]
+    const float* mul;     // optional [nb][nx][NF]: out = mul * (H + offset) + add
+    const float* add;     // optional [nb][nx][NF]
+    const float* offset;  // optional device [nb]   (mu)
     int nx;
     int items_per_batch, nitems;
     size_t t_bstride, img_bstride;
     const float4* tw;
 };
 
-// F[y][x] = column FFT; H[y][x] = Re F - Im F and H[(-y) mod ny][nx - x] = Re F + Im F  (reading R6)
+// F[y][x] = column FFT; H[y][x] = Re F - Im F and H[(-y) mod NF][nx - x] = Re F + Im F  (reading R6).
+// Column x of H is one contiguous run of the transposed output, so all stores are coalesced.
 template <int NF>
 __global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
 hart_cols_kernel(HartColsArgs a) {
@@ -97,7 +98,7 @@ hart_cols_kernel(HartColsArgs a) {
     extern __shared__ float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
-    float4* buf = smem4 + GEO::TW + (size_t)g * xbuf_len(NF);
+    float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
     const int ntile = a.nx / 4 + 1;
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
@@ -126,24 +127,24 @@ hart_cols_kernel(HartColsArgs a) {
             const float off = a.offset ? __ldg(a.offset + b) : 0.f;
             const int half = a.nx / 2;
 #pragma unroll
-            for (int e = 0; e < kE; ++e) {
-                const int y = p + e * P, ym = (NF - y) & (NF - 1);
+            for (int c = 0; c < 2; ++c) {
+                const int x = 2 * m + c;
+                if (x > half) continue;
+                const bool mirror = x > 0 && x < half;
+                const size_t col0 = base + (size_t)x * NF, col1 = base + (size_t)(a.nx - x) * NF;
 #pragma unroll
-                for (int c = 0; c < 2; ++c) {
-                    const int x = 2 * m + c;
-                    if (x > half) continue;
+                for (int e = 0; e < kE; ++e) {
+                    const int y = p + e * P, ym = (NF - y) & (NF - 1);
                     const float2 f = v[c][e];
-                    size_t i0 = base + (size_t)y * a.nx + x;
                     float h0 = f.x - f.y + off;
-                    if (a.mul) h0 *= __ldg(a.mul + i0);
-                    if (a.add) h0 += __ldg(a.add + i0);
-                    a.out[i0] = h0;
-                    if (x > 0 && x < half) {
-                        size_t i1 = base + (size_t)ym * a.nx + (a.nx - x);
+                    if (a.mul) h0 *= ldg1(a.mul + col0 + y);
+                    if (a.add) h0 += ldg1(a.add + col0 + y);
+                    a.out[col0 + y] = h0;
+                    if (mirror) {
                         float h1 = f.x + f.y + off;
-                        if (a.mul) h1 *= __ldg(a.mul + i1);
-                        if (a.add) h1 += __ldg(a.add + i1);
-                        a.out[i1] = h1;
+                        if (a.mul) h1 *= ldg1(a.mul + col1 + ym);
+                        if (a.add) h1 += ldg1(a.add + col1 + ym);
+                        a.out[col1 + ym] = h1;
                     }
                 }
             }
