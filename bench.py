@@ -60,7 +60,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -168,6 +168,8 @@ def run_cuda(args):
     xs = [dev(rng.normal(size=(w.nchan, w.ny, w.nx))) for _ in range(2)]
     y = ctx.new_image()
 
+    l_after_warmup = 0
+
     def barrier():
         if world > 1:
             dist.barrier()
@@ -177,6 +179,8 @@ def run_cuda(args):
         for i in range(warmup):
             fn(i)
         barrier()
+        nonlocal l_after_warmup
+        l_after_warmup = ctx.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         for i in range(steps):
@@ -195,9 +199,8 @@ def run_cuda(args):
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    l0 = ctx.launch_count()
     ms = timed(step, args.steps, args.warmup)
-    launches = ctx.launch_count() - l0 - 3 * args.warmup
+    launches = ctx.launch_count() - l_after_warmup
     clocks = sampler.stop() if rank == 0 else None
     ms_step = ms / args.steps
     value = world * args.steps / (ms * 1e-3)
