@@ -49,68 +49,131 @@ FRS_HD float2 cmul(float2 a, float2 w) {
 FRS_HD float2 cmulc(float2 a, float2 w) {
     return make_float2(fmaf(a.y, w.y, a.x * w.x), fmaf(a.y, w.x, -(a.x * w.y)));
 }
-template <bool INV> FRS_HD float2 cmul_dir(float2 a, float2 w) { return INV ? cmulc(a, w) : cmul(a, w); }
-// a * (-i) forward, a * (+i) inverse
-template <bool INV> FRS_HD float2 mul_mi(float2 a) {
-    return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+// ---- packed pairs ---------------------------------------------------------------------------------
+// A thread advances TWO transforms that share every twiddle.  Their samples travel as one C2: the real
+// parts of both in one float2, the imaginary parts in another (lane .x = transform 0, .y = transform 1).
+// On sm_100a every add / multiply / fma on such a float2 is ONE packed instruction (FADD2 / FMUL2 /
+// FFMA2: two fp32 results per issue slot, a scalar twiddle broadcast to both lanes for free), which
+// halves the issue slots of the butterflies; the host build (selftest.cu) runs the same code with
+// plain float arithmetic.
+struct C2 { float2 re, im; };
+
+FRS_HD float2 f2bc(float s) { return make_float2(s, s); }
+FRS_HD float2 f2neg(float2 a) { return make_float2(-a.x, -a.y); }
+FRS_HD float2 f2add(float2 a, float2 b) {
+#ifdef __CUDA_ARCH__
+    return __fadd2_rn(a, b);
+#else
+    return make_float2(a.x + b.x, a.y + b.y);
+#endif
 }
-// a * w8^k (forward w8 = exp(-2 pi i/8)); inverse uses the conjugate
-template <int K, bool INV> FRS_HD float2 mul_w8(float2 a) {
+FRS_HD float2 f2sub(float2 a, float2 b) { return f2add(a, f2neg(b)); }
+FRS_HD float2 f2mul(float2 a, float2 b) {
+#ifdef __CUDA_ARCH__
+    return __fmul2_rn(a, b);
+#else
+    return make_float2(a.x * b.x, a.y * b.y);
+#endif
+}
+// a * b + c
+FRS_HD float2 f2fma(float2 a, float2 b, float2 c) {
+#ifdef __CUDA_ARCH__
+    return __ffma2_rn(a, b, c);
+#else
+    return make_float2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y));
+#endif
+}
+FRS_HD C2 c2zero() { C2 r; r.re = make_float2(0.f, 0.f); r.im = r.re; return r; }
+FRS_HD C2 c2make(float2 a, float2 b) { C2 r; r.re = make_float2(a.x, b.x); r.im = make_float2(a.y, b.y); return r; }
+FRS_HD float2 c2get(const C2& a, int t) { return t ? make_float2(a.re.y, a.im.y) : make_float2(a.re.x, a.im.x); }
+FRS_HD C2 c2add(C2 a, C2 b) { C2 r; r.re = f2add(a.re, b.re); r.im = f2add(a.im, b.im); return r; }
+FRS_HD C2 c2sub(C2 a, C2 b) { C2 r; r.re = f2sub(a.re, b.re); r.im = f2sub(a.im, b.im); return r; }
+// both transforms times the same scalar complex w (forward) or conj(w) (inverse)
+template <bool INV> FRS_HD C2 c2mul_dir(C2 a, float2 w) {
+    C2 r;
+    if (INV) {
+        r.re = f2fma(a.im, f2bc(w.y), f2mul(a.re, f2bc(w.x)));
+        r.im = f2fma(a.re, f2bc(-w.y), f2mul(a.im, f2bc(w.x)));
+    } else {
+        r.re = f2fma(a.im, f2bc(-w.y), f2mul(a.re, f2bc(w.x)));
+        r.im = f2fma(a.re, f2bc(w.y), f2mul(a.im, f2bc(w.x)));
+    }
+    return r;
+}
+// a + s*(-i d) forward, a + s*(+i d) inverse, s = +1 (PLUS) or -1: the multiplication by -+i is only a
+// choice of components and signs
+template <bool INV, bool PLUS> FRS_HD C2 c2add_mi(C2 a, C2 d) {
+    C2 r;
+    if (INV != PLUS) { r.re = f2add(a.re, d.im); r.im = f2sub(a.im, d.re); }   // a + (d.im, -d.re)
+    else             { r.re = f2sub(a.re, d.im); r.im = f2add(a.im, d.re); }   // a + (-d.im, d.re)
+    return r;
+}
+// a * w8^K (forward w8 = exp(-2 pi i/8)); inverse uses the conjugate
+template <int K, bool INV> FRS_HD C2 c2mul_w8(C2 a) {
+    C2 r;
     if (K == 0) return a;
-    if (K == 2) return mul_mi<INV>(a);
-    if (K == 1) return INV ? make_float2((a.x - a.y) * kSqrtHalf, (a.x + a.y) * kSqrtHalf)
-                           : make_float2((a.x + a.y) * kSqrtHalf, (a.y - a.x) * kSqrtHalf);
-    /* K == 3 */ return INV ? make_float2((-a.x - a.y) * kSqrtHalf, (a.x - a.y) * kSqrtHalf)
-                           : make_float2((a.y - a.x) * kSqrtHalf, (-a.x - a.y) * kSqrtHalf);
+    if (K == 2) {
+        if (INV) { r.re = f2neg(a.im); r.im = a.re; } else { r.re = a.im; r.im = f2neg(a.re); }
+        return r;
+    }
+    const float2 h = f2bc(kSqrtHalf), mh = f2bc(-kSqrtHalf);
+    if (K == 1) {
+        if (INV) { r.re = f2mul(f2sub(a.re, a.im), h); r.im = f2mul(f2add(a.re, a.im), h); }
+        else     { r.re = f2mul(f2add(a.re, a.im), h); r.im = f2mul(f2sub(a.im, a.re), h); }
+    } else { /* K == 3 */
+        if (INV) { r.re = f2mul(f2add(a.re, a.im), mh); r.im = f2mul(f2sub(a.re, a.im), h); }
+        else     { r.re = f2mul(f2sub(a.im, a.re), h);  r.im = f2mul(f2add(a.re, a.im), mh); }
+    }
+    return r;
 }
 // a * w16^K, K in {0,1,2,3,4,6,9}
-template <int K, bool INV> FRS_HD float2 mul_w16(float2 a) {
+template <int K, bool INV> FRS_HD C2 c2mul_w16(C2 a) {
     if (K == 0) return a;
-    if (K == 2) return mul_w8<1, INV>(a);
-    if (K == 4) return mul_mi<INV>(a);
-    if (K == 6) return mul_w8<3, INV>(a);
-    float2 w = (K == 1) ? make_float2(kC1, -kS1) : (K == 3) ? make_float2(kS1, -kC1) : make_float2(-kC1, kS1) /*K==9*/;
-    return cmul_dir<INV>(a, w);
+    if (K == 2) return c2mul_w8<1, INV>(a);
+    if (K == 4) return c2mul_w8<2, INV>(a);
+    if (K == 6) return c2mul_w8<3, INV>(a);
+    const float2 w = (K == 1) ? make_float2(kC1, -kS1) : (K == 3) ? make_float2(kS1, -kC1) : make_float2(-kC1, kS1) /*K==9*/;
+    return c2mul_dir<INV>(a, w);
 }
 
-// ---- small DFTs, natural order in and out, in place ------------------------------------------
-template <bool INV> FRS_HD void dft2(float2& a, float2& b) {
-    float2 t = a;
-    a = cadd(t, b);
-    b = csub(t, b);
+// ---- small DFTs on packed pairs, natural order in and out, in place ----------------------------------
+template <bool INV> FRS_HD void dft2(C2& a, C2& b) {
+    const C2 t = a;
+    a = c2add(t, b);
+    b = c2sub(t, b);
 }
-template <bool INV> FRS_HD void dft4(float2& a0, float2& a1, float2& a2, float2& a3) {
-    float2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = mul_mi<INV>(csub(a1, a3));
-    a0 = cadd(t0, t2);
-    a2 = csub(t0, t2);
-    a1 = cadd(t1, t3);
-    a3 = csub(t1, t3);
+template <bool INV> FRS_HD void dft4(C2& a0, C2& a1, C2& a2, C2& a3) {
+    const C2 t0 = c2add(a0, a2), t1 = c2sub(a0, a2), t2 = c2add(a1, a3), d = c2sub(a1, a3);
+    a0 = c2add(t0, t2);
+    a2 = c2sub(t0, t2);
+    a1 = c2add_mi<INV, true>(t1, d);
+    a3 = c2add_mi<INV, false>(t1, d);
 }
-template <bool INV> FRS_HD void dft8(float2 (&t)[8]) {
+template <bool INV> FRS_HD void dft8(C2 (&t)[8]) {
     dft4<INV>(t[0], t[2], t[4], t[6]);   // E[k] in t[0],t[2],t[4],t[6]
     dft4<INV>(t[1], t[3], t[5], t[7]);   // O[k] in t[1],t[3],t[5],t[7]
-    float2 o0 = t[1], o1 = mul_w8<1, INV>(t[3]), o2 = mul_w8<2, INV>(t[5]), o3 = mul_w8<3, INV>(t[7]);
-    float2 e0 = t[0], e1 = t[2], e2 = t[4], e3 = t[6];
-    t[0] = cadd(e0, o0); t[4] = csub(e0, o0);
-    t[1] = cadd(e1, o1); t[5] = csub(e1, o1);
-    t[2] = cadd(e2, o2); t[6] = csub(e2, o2);
-    t[3] = cadd(e3, o3); t[7] = csub(e3, o3);
+    const C2 o0 = t[1], o1 = c2mul_w8<1, INV>(t[3]), o3 = c2mul_w8<3, INV>(t[7]), d2 = t[5];
+    const C2 e0 = t[0], e1 = t[2], e2 = t[4], e3 = t[6];
+    t[0] = c2add(e0, o0); t[4] = c2sub(e0, o0);
+    t[1] = c2add(e1, o1); t[5] = c2sub(e1, o1);
+    t[2] = c2add_mi<INV, true>(e2, d2); t[6] = c2add_mi<INV, false>(e2, d2);
+    t[3] = c2add(e3, o3); t[7] = c2sub(e3, o3);
 }
-template <bool INV> FRS_HD void dft16(float2 (&t)[16]) {
+template <bool INV> FRS_HD void dft16(C2 (&t)[16]) {
     // n = 4 n1 + n0, k = k0 + 4 k1:  X[k] = sum_n0 w4^{n0 k1} w16^{n0 k0} sum_n1 w4^{n1 k0} a[4 n1 + n0]
     dft4<INV>(t[0], t[4], t[8], t[12]);      // n0 = 0: B[0][k0] at t[4 k0 + 0]
     dft4<INV>(t[1], t[5], t[9], t[13]);
     dft4<INV>(t[2], t[6], t[10], t[14]);
     dft4<INV>(t[3], t[7], t[11], t[15]);
-    t[5] = mul_w16<1, INV>(t[5]);  t[6] = mul_w16<2, INV>(t[6]);   t[7] = mul_w16<3, INV>(t[7]);
-    t[9] = mul_w16<2, INV>(t[9]);  t[10] = mul_w16<4, INV>(t[10]); t[11] = mul_w16<6, INV>(t[11]);
-    t[13] = mul_w16<3, INV>(t[13]); t[14] = mul_w16<6, INV>(t[14]); t[15] = mul_w16<9, INV>(t[15]);
+    t[5] = c2mul_w16<1, INV>(t[5]);   t[6] = c2mul_w16<2, INV>(t[6]);   t[7] = c2mul_w16<3, INV>(t[7]);
+    t[9] = c2mul_w16<2, INV>(t[9]);   t[10] = c2mul_w16<4, INV>(t[10]); t[11] = c2mul_w16<6, INV>(t[11]);
+    t[13] = c2mul_w16<3, INV>(t[13]); t[14] = c2mul_w16<6, INV>(t[14]); t[15] = c2mul_w16<9, INV>(t[15]);
     dft4<INV>(t[0], t[1], t[2], t[3]);       // k0 = 0: X[0 + 4 k1] at t[k1]
     dft4<INV>(t[4], t[5], t[6], t[7]);       // k0 = 1: X[1 + 4 k1] at t[4 + k1]
     dft4<INV>(t[8], t[9], t[10], t[11]);
     dft4<INV>(t[12], t[13], t[14], t[15]);
     // transpose 4x4: X[k0 + 4 k1] currently at t[4 k0 + k1]
-    float2 s;
+    C2 s;
     s = t[1]; t[1] = t[4]; t[4] = s;
     s = t[2]; t[2] = t[8]; t[8] = s;
     s = t[3]; t[3] = t[12]; t[12] = s;
@@ -119,10 +182,10 @@ template <bool INV> FRS_HD void dft16(float2 (&t)[16]) {
     s = t[11]; t[11] = t[14]; t[14] = s;
 }
 template <int R, bool INV> struct Dft;
-template <bool INV> struct Dft<2, INV> { static FRS_HD void run(float2 (&t)[2]) { dft2<INV>(t[0], t[1]); } };
-template <bool INV> struct Dft<4, INV> { static FRS_HD void run(float2 (&t)[4]) { dft4<INV>(t[0], t[1], t[2], t[3]); } };
-template <bool INV> struct Dft<8, INV> { static FRS_HD void run(float2 (&t)[8]) { dft8<INV>(t); } };
-template <bool INV> struct Dft<16, INV> { static FRS_HD void run(float2 (&t)[16]) { dft16<INV>(t); } };
+template <bool INV> struct Dft<2, INV> { static FRS_HD void run(C2 (&t)[2]) { dft2<INV>(t[0], t[1]); } };
+template <bool INV> struct Dft<4, INV> { static FRS_HD void run(C2 (&t)[4]) { dft4<INV>(t[0], t[1], t[2], t[3]); } };
+template <bool INV> struct Dft<8, INV> { static FRS_HD void run(C2 (&t)[8]) { dft8<INV>(t); } };
+template <bool INV> struct Dft<16, INV> { static FRS_HD void run(C2 (&t)[16]) { dft16<INV>(t); } };
 
 // ---- plan: radices per transform length ------------------------------------------------------
 // 16:[16] 32:[16,2] 64:[8,8] 128:[16,8] 256:[16,16] 512:[8,8,8] 1024:[16,8,8] 2048:[16,16,8] 4096:[16,16,16]
@@ -172,14 +235,14 @@ FRS_HD constexpr int xpad(int pos) { return pos + (pos >> 4); }
 // slots of one exchange buffer (holds positions 0..N inclusive: the row passes park X[N] too)
 FRS_HD constexpr int xbuf_len(int n) { return n + (n >> 4) + 8; }
 
-FRS_HD float2 lo(float4 a) { return make_float2(a.x, a.y); }
-FRS_HD float2 hi(float4 a) { return make_float2(a.z, a.w); }
-FRS_HD float4 pack(float2 a, float2 b) { return make_float4(a.x, a.y, b.x, b.y); }
+// exchange slot of one position: (re of transform 0, re of 1, im of 0, im of 1) -> 128-bit accesses
+FRS_HD float4 pack(const C2& a) { return make_float4(a.re.x, a.re.y, a.im.x, a.im.y); }
+FRS_HD C2 unpack(float4 s) { C2 r; r.re = make_float2(s.x, s.y); r.im = make_float2(s.z, s.w); return r; }
 
 // ---- one stage: twiddle the inputs, butterfly, leave result r of butterfly b in v[b + r*NB] ----
-// NT transforms are advanced together so that each twiddle is fetched once.  tw: packed tables.
-template <int N, int S, bool INV, int NT>
-FRS_HD void stage_compute(float2 (&v)[NT][kE], int p, const float4* __restrict__ tw) {
+// Both transforms of the pair are advanced by the same packed instructions.  tw: packed tables.
+template <int N, int S, bool INV>
+FRS_HD void stage_compute(C2 (&v)[kE], int p, const float4* __restrict__ tw) {
     constexpr int R = plan_radix(N, S), NB = kE / R, HP = R / 2, P = N / kE, NS = plan_ns(N, S);
     constexpr int WA = plan_tw_wa(N, S);
 #pragma unroll
@@ -196,24 +259,21 @@ FRS_HD void stage_compute(float2 (&v)[NT][kE], int p, const float4* __restrict__
 #pragma unroll
                 for (int q = 0; q < HP; ++q) {
                     const float4 ww = ta[q * WA + j];
-                    w[2 * q + 1] = lo(ww);
-                    if (2 * q + 2 < R) w[2 * q + 2] = hi(ww);
+                    w[2 * q + 1] = make_float2(ww.x, ww.y);
+                    if (2 * q + 2 < R) w[2 * q + 2] = make_float2(ww.z, ww.w);
                 }
             }
         }
+        C2 x[R];
 #pragma unroll
-        for (int t = 0; t < NT; ++t) {
-            float2 x[R];
+        for (int r = 0; r < R; ++r) x[r] = v[b + r * NB];
+        if (S > 0) {
 #pragma unroll
-            for (int r = 0; r < R; ++r) x[r] = v[t][b + r * NB];
-            if (S > 0) {
-#pragma unroll
-                for (int r = 1; r < R; ++r) x[r] = cmul_dir<INV>(x[r], w[r]);
-            }
-            Dft<R, INV>::run(x);
-#pragma unroll
-            for (int r = 0; r < R; ++r) v[t][b + r * NB] = x[r];
+            for (int r = 1; r < R; ++r) x[r] = c2mul_dir<INV>(x[r], w[r]);
         }
+        Dft<R, INV>::run(x);
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[b + r * NB] = x[r];
     }
 }
 // Stockham position of output r of butterfly b of stage S
@@ -223,45 +283,25 @@ FRS_HD int stage_pos(int p, int b, int r) {
     const int j = p + b * P;
     return (j / NS) * NS * R + (j % NS) + r * NS;
 }
-// single transform through a float2 buffer (host replay, odd cases)
 template <int N, int S>
-FRS_HD void stage_scatter(const float2 (&v)[kE], int p, float2* buf) {
+FRS_HD void stage_scatter2(const C2 (&v)[kE], int p, float4* buf) {
     constexpr int R = plan_radix(N, S), NB = kE / R;
 #pragma unroll
     for (int b = 0; b < NB; ++b)
 #pragma unroll
-        for (int r = 0; r < R; ++r) buf[xpad(stage_pos<N, S>(p, b, r))] = v[b + r * NB];
+        for (int r = 0; r < R; ++r) buf[xpad(stage_pos<N, S>(p, b, r))] = pack(v[b + r * NB]);
 }
 template <int N>
-FRS_HD void canon_gather(float2 (&v)[kE], int p, const float2* buf) {
+FRS_HD void canon_gather2(C2 (&v)[kE], int p, const float4* buf) {
     constexpr int P = N / kE;
 #pragma unroll
-    for (int e = 0; e < kE; ++e) v[e] = buf[xpad(p + e * P)];
-}
-// transform pair through ONE float4 buffer: slot = (a.re, a.im, b.re, b.im) -> 128-bit accesses
-template <int N, int S>
-FRS_HD void stage_scatter2(const float2 (&v)[2][kE], int p, float4* buf) {
-    constexpr int R = plan_radix(N, S), NB = kE / R;
-#pragma unroll
-    for (int b = 0; b < NB; ++b)
-#pragma unroll
-        for (int r = 0; r < R; ++r) buf[xpad(stage_pos<N, S>(p, b, r))] = pack(v[0][b + r * NB], v[1][b + r * NB]);
+    for (int e = 0; e < kE; ++e) v[e] = unpack(buf[xpad(p + e * P)]);
 }
 template <int N>
-FRS_HD void canon_gather2(float2 (&v)[2][kE], int p, const float4* buf) {
+FRS_HD void canon_scatter2(const C2 (&v)[kE], int p, float4* buf) {
     constexpr int P = N / kE;
 #pragma unroll
-    for (int e = 0; e < kE; ++e) {
-        const float4 x = buf[xpad(p + e * P)];
-        v[0][e] = lo(x);
-        v[1][e] = hi(x);
-    }
-}
-template <int N>
-FRS_HD void canon_scatter2(const float2 (&v)[2][kE], int p, float4* buf) {
-    constexpr int P = N / kE;
-#pragma unroll
-    for (int e = 0; e < kE; ++e) buf[xpad(p + e * P)] = pack(v[0][e], v[1][e]);
+    for (int e = 0; e < kE; ++e) buf[xpad(p + e * P)] = pack(v[e]);
 }
 
 #ifdef __CUDACC__
@@ -269,9 +309,9 @@ FRS_HD void canon_scatter2(const float2 (&v)[2][kE], int p, float4* buf) {
 // All threads of the CTA must call this (it uses __syncthreads()).  buf: one exchange buffer of
 // xbuf_len(N) float4, private to the group.  tw: packed twiddle table (shared memory).
 template <int N, bool INV, int S>
-__device__ __forceinline__ void pair_fft_from(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
+__device__ __forceinline__ void pair_fft_from(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
     if constexpr (S < plan_stages(N)) {
-        stage_compute<N, S, INV, 2>(v, p, tw);
+        stage_compute<N, S, INV>(v, p, tw);
         if constexpr (S + 1 < plan_stages(N)) {
             stage_scatter2<N, S>(v, p, buf);
             __syncthreads();
@@ -282,15 +322,15 @@ __device__ __forceinline__ void pair_fft_from(float2 (&v)[2][kE], int p, float4*
     }
 }
 template <int N, bool INV>
-__device__ __forceinline__ void pair_fft(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
+__device__ __forceinline__ void pair_fft(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
     pair_fft_from<N, INV, 0>(v, p, buf, tw);
 }
 // The same transform in two halves, so that a caller can reuse `buf` (it is free after the head)
 // while the last stage, which runs entirely in registers, is still to be computed.
 template <int N, bool INV, int S>
-__device__ __forceinline__ void pair_fft_head_from(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
+__device__ __forceinline__ void pair_fft_head_from(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
     if constexpr (S + 1 < plan_stages(N)) {
-        stage_compute<N, S, INV, 2>(v, p, tw);
+        stage_compute<N, S, INV>(v, p, tw);
         stage_scatter2<N, S>(v, p, buf);
         __syncthreads();
         canon_gather2<N>(v, p, buf);
@@ -299,12 +339,12 @@ __device__ __forceinline__ void pair_fft_head_from(float2 (&v)[2][kE], int p, fl
     }
 }
 template <int N, bool INV>
-__device__ __forceinline__ void pair_fft_head(float2 (&v)[2][kE], int p, float4* buf, const float4* __restrict__ tw) {
+__device__ __forceinline__ void pair_fft_head(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
     pair_fft_head_from<N, INV, 0>(v, p, buf, tw);
 }
 template <int N, bool INV>
-__device__ __forceinline__ void pair_fft_tail(float2 (&v)[2][kE], int p, const float4* __restrict__ tw) {
-    stage_compute<N, plan_stages(N) - 1, INV, 2>(v, p, tw);
+__device__ __forceinline__ void pair_fft_tail(C2 (&v)[kE], int p, const float4* __restrict__ tw) {
+    stage_compute<N, plan_stages(N) - 1, INV>(v, p, tw);
 }
 
 // ---- asynchronous copies ---------------------------------------------------------------------------

@@ -19,9 +19,9 @@ psf_cols_kernel(PsfColsArgs a) {
     const int m = blockIdx.x * GEO::G + g;
     const int b = blockIdx.y;
     const bool live = m < a.ntile;
-    float2 v[2][kE];
+    C2 v[kE];
 #pragma unroll
-    for (int e = 0; e < kE; ++e) { v[0][e] = make_float2(0.f, 0.f); v[1][e] = make_float2(0.f, 0.f); }
+    for (int e = 0; e < kE; ++e) v[e] = c2zero();
     if (live) {
         const float4* tile = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + (size_t)m * 2 * NF;
 #pragma unroll
@@ -29,12 +29,10 @@ psf_cols_kernel(PsfColsArgs a) {
             const int n = p + e * P;
             const float4 x0 = ldg4(tile + n), x1 = ldg4(tile + n + NF);
             if (!role) {
-                v[0][e] = make_float2(x0.x + x1.x, x0.y + x1.y);
-                v[1][e] = make_float2(x0.z + x1.z, x0.w + x1.w);
+                v[e] = c2make(make_float2(x0.x + x1.x, x0.y + x1.y), make_float2(x0.z + x1.z, x0.w + x1.w));
             } else {
                 const float2 w = __ldg(a.twist + n);
-                v[0][e] = cmul(make_float2(x0.x - x1.x, x0.y - x1.y), w);
-                v[1][e] = cmul(make_float2(x0.z - x1.z, x0.w - x1.w), w);
+                v[e] = c2make(cmul(make_float2(x0.x - x1.x, x0.y - x1.y), w), cmul(make_float2(x0.z - x1.z, x0.w - x1.w), w));
             }
         }
     }
@@ -44,8 +42,8 @@ psf_cols_kernel(PsfColsArgs a) {
         float* w = a.wt + b * a.w_bstride + (size_t)m * 2 * NF * 2 + role;      // [c][q][parity = role]
 #pragma unroll
         for (int e = 0; e < kE; ++e) {
-            const float re0 = v[0][e].x * a.scale, re1 = v[1][e].x * a.scale;
-            max_im = fmaxf(max_im, fmaxf(fabsf(v[0][e].y), fabsf(v[1][e].y)) * a.scale);
+            const float re0 = v[e].re.x * a.scale, re1 = v[e].re.y * a.scale;
+            max_im = fmaxf(max_im, fmaxf(fabsf(v[e].im.x), fabsf(v[e].im.y)) * a.scale);
             min_re = fminf(min_re, fminf(re0, re1));
             max_re = fmaxf(max_re, fmaxf(re0, re1));
             w[(size_t)(p + e * P) * 2] = 0.5f * fmaxf(re0, 0.f);

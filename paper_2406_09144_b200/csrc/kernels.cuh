@@ -137,16 +137,17 @@ rows_fwd_kernel(RowsFwdArgs a) {
         const bool live = 2 * rp < a.ny;
         const int y0 = 2 * rp;
 
-        float2 v[2][kE];
+        C2 v[kE];
 #pragma unroll
         for (int e = 0; e < kE; ++e) {
             if (e < NE) {
+                float2 x[2];
 #pragma unroll
                 for (int t = 0; t < 2; ++t)
-                    v[t][e] = (a.mul && live) ? make_float2(xin[t][e].x * min_[t][e].x, xin[t][e].y * min_[t][e].y) : xin[t][e];
+                    x[t] = (a.mul && live) ? make_float2(xin[t][e].x * min_[t][e].x, xin[t][e].y * min_[t][e].y) : xin[t][e];
+                v[e] = c2make(x[0], x[1]);
             } else {
-                v[0][e] = make_float2(0.f, 0.f);
-                v[1][e] = make_float2(0.f, 0.f);
+                v[e] = c2zero();
             }
         }
         pair_fft<NF, false>(v, p, buf, tws);
@@ -156,7 +157,7 @@ rows_fwd_kernel(RowsFwdArgs a) {
         if (live) {
             // X[k] * scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = 0..NF.
             // Four lanes (column c, row r) produce the 32-byte slot of one tile: lane = 4 j + 2 r + c.
-            const float2* zb = reinterpret_cast<const float2*>(buf);       // Z_r[k] at zb[2 xpad(k) + r]
+            const float* zb = reinterpret_cast<const float*>(buf);         // Z_r[k] = (zb[4 xpad(k) + r], zb[4 xpad(k) + 2 + r])
             float2* ob = a.out + b * a.out_bstride + (size_t)y0 * 2;
             const int c = p & 1, r = (p >> 1) & 1;
             auto emit = [&](int m) {
@@ -165,7 +166,8 @@ rows_fwd_kernel(RowsFwdArgs a) {
                 if (k <= NF) {
                     const int ik = k & (NF - 1), im = (NF - k) & (NF - 1);
                     const float2 w = __ldg(a.twist + k);
-                    const float2 za = zb[2 * xpad(ik) + r], zm = cconj(zb[2 * xpad(im) + r]);
+                    const float2 za = make_float2(zb[4 * xpad(ik) + r], zb[4 * xpad(ik) + 2 + r]);
+                    const float2 zm = make_float2(zb[4 * xpad(im) + r], -zb[4 * xpad(im) + 2 + r]);
                     const float2 s = cadd(za, zm), d = cmul(csub(za, zm), w);
                     x = make_float2((s.x + d.y) * a.scale, (s.y - d.x) * a.scale);
                 }
@@ -182,7 +184,8 @@ rows_fwd_kernel(RowsFwdArgs a) {
                     if (k <= NF) {
                         const int ik = k & (NF - 1), im = (NF - k) & (NF - 1);
                         const float2 w = __ldg(a.twist + k);
-                        const float2 za = zb[2 * xpad(ik) + rr], zm = cconj(zb[2 * xpad(im) + rr]);
+                        const float2 za = make_float2(zb[4 * xpad(ik) + rr], zb[4 * xpad(ik) + 2 + rr]);
+                        const float2 zm = make_float2(zb[4 * xpad(im) + rr], -zb[4 * xpad(im) + 2 + rr]);
                         const float2 s = cadd(za, zm), d = cmul(csub(za, zm), w);
                         x = make_float2((s.x + d.y) * a.scale, (s.y - d.x) * a.scale);
                     }

@@ -40,36 +40,37 @@ conv_cols_kernel(ConvColsArgs a) {
         float2* col = a.t + b * a.t_bstride + (size_t)(mc >> 1) * NF * 2 + (mc & 1);      // stride 2 float2 per row
         const float* w = a.wt + b * a.w_bstride + (size_t)mc * NF * 2;
 
-        float2 v[2][kE];
+        C2 v[kE];
         if (live) {
             // warm L2 with this column's weights (read after the forward transform)
             if ((p & 15) == 0) {
 #pragma unroll
                 for (int e = 0; e < kE; ++e) prefetch_l2(w + 2 * (p + e * P));
             }
+            float2 x[kE];
 #pragma unroll
-            for (int e = 0; e < kE; ++e) v[0][e] = ld2_inplace(col + 2 * (p + e * P));
+            for (int e = 0; e < kE; ++e) x[e] = ld2_inplace(col + 2 * (p + e * P));
 #pragma unroll
-            for (int e = 0; e < kE; ++e) v[1][e] = cmul(v[0][e], __ldg(a.twist + p + e * P));
+            for (int e = 0; e < kE; ++e) v[e] = c2make(x[e], cmul(x[e], __ldg(a.twist + p + e * P)));
         } else {
 #pragma unroll
-            for (int e = 0; e < kE; ++e) { v[0][e] = make_float2(0.f, 0.f); v[1][e] = make_float2(0.f, 0.f); }
+            for (int e = 0; e < kE; ++e) v[e] = c2zero();
         }
         pair_fft<NF, false>(v, p, buf, tws);
         if (live) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 ww = ldg2(w + 2 * (p + e * P));
-                v[0][e] = cscale(v[0][e], ww.x);
-                v[1][e] = cscale(v[1][e], ww.y);
+                const float2 ww = ldg2(w + 2 * (p + e * P));      // (even-bin weight, odd-bin weight)
+                v[e].re = f2mul(v[e].re, ww);
+                v[e].im = f2mul(v[e].im, ww);
             }
         }
         pair_fft<NF, true>(v, p, buf, tws);
         if (live) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 o = cmulc(v[1][e], __ldg(a.twist + p + e * P));
-                stg2(col + 2 * (p + e * P), make_float2(v[0][e].x + o.x, v[0][e].y + o.y));
+                const float2 o = cmulc(c2get(v[e], 1), __ldg(a.twist + p + e * P));
+                stg2(col + 2 * (p + e * P), make_float2(v[e].re.x + o.x, v[e].im.x + o.y));
             }
         }
     }
@@ -108,18 +109,17 @@ hart_cols_kernel(HartColsArgs a) {
         const int m = (item - b * a.items_per_batch) * GEO::G + g;
         const bool live = m < ntile;
 
-        float2 v[2][kE];
+        C2 v[kE];
         if (live) {
             const float4* tile = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + (size_t)m * NF;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const float4 x = ldg4(tile + p + e * P);
-                v[0][e] = lo(x);
-                v[1][e] = hi(x);
+                v[e] = c2make(make_float2(x.x, x.y), make_float2(x.z, x.w));
             }
         } else {
 #pragma unroll
-            for (int e = 0; e < kE; ++e) { v[0][e] = make_float2(0.f, 0.f); v[1][e] = make_float2(0.f, 0.f); }
+            for (int e = 0; e < kE; ++e) v[e] = c2zero();
         }
         pair_fft<NF, false>(v, p, buf, tws);
         if (live) {
@@ -135,7 +135,7 @@ hart_cols_kernel(HartColsArgs a) {
 #pragma unroll
                 for (int e = 0; e < kE; ++e) {
                     const int y = p + e * P, ym = (NF - y) & (NF - 1);
-                    const float2 f = v[c][e];
+                    const float2 f = c2get(v[e], c);
                     float h0 = f.x - f.y + off;
                     if (a.mul) h0 *= ldg1(a.mul + col0 + y);
                     if (a.add) h0 += ldg1(a.add + col0 + y);

@@ -67,18 +67,20 @@ rows_inv_kernel(RowsInvArgs a) {
         cp_async_wait_all();
         __syncthreads();
         // Z'[k] = (Y[k] + conj Y[NF-k]) + i conj(twist[k]) (Y[k] - conj Y[NF-k]),  k = 0..NF-1
-        float2 v[2][kE];
+        C2 v[kE];
 #pragma unroll
         for (int e = 0; e < kE; ++e) {
             const int k = p + e * P;
             const float2 w = __ldg(a.twist + k);
+            float2 z[2];
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 float2 ya = make_float2(0.f, 0.f), ym = ya;
                 if (live) { ya = land[t * 2 * NTILE + k]; ym = cconj(land[t * 2 * NTILE + NF - k]); }
                 const float2 s = cadd(ya, ym), d = cmulc(csub(ya, ym), w);
-                v[t][e] = make_float2(s.x - d.y, s.y + d.x);
+                z[t] = make_float2(s.x - d.y, s.y + d.x);
             }
+            v[e] = c2make(z[0], z[1]);
         }
         __syncthreads();
         pair_fft_head<NF, true>(v, p, buf, tws);
@@ -104,7 +106,7 @@ rows_inv_kernel(RowsInvArgs a) {
             for (int t = 0; t < 2; ++t) {
 #pragma unroll
                 for (int e = 0; e < kE / 2; ++e) {
-                    float2 c = v[t][e];
+                    float2 c = c2get(v[e], t);
                     if (a.mode == kMulS) {
                         c.x *= sv[t][e].x; c.y *= sv[t][e].y;
                     } else if (a.mode == kEnergy) {

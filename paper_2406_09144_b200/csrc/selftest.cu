@@ -7,14 +7,14 @@
 #include "tables.h"
 
 namespace frs {
-struct Regs { float2 v[2][kE]; };
+struct Regs { C2 v[kE]; };
 
 // pair (a, b = 2a) through the float4 exchange path the kernels use
 template <int N, bool INV, int S>
 static void emu_from(std::vector<Regs>& regs, std::vector<float4>& buf, const float4* tw) {
     constexpr int P = N / kE;
     if constexpr (S < plan_stages(N)) {
-        for (int p = 0; p < P; ++p) stage_compute<N, S, INV, 2>(regs[p].v, p, tw);
+        for (int p = 0; p < P; ++p) stage_compute<N, S, INV>(regs[p].v, p, tw);
         if constexpr (S + 1 < plan_stages(N)) {
             for (int p = 0; p < P; ++p) stage_scatter2<N, S>(regs[p].v, p, buf.data());
             for (int p = 0; p < P; ++p) canon_gather2<N>(regs[p].v, p, buf.data());
@@ -30,16 +30,15 @@ static int emu(int inverse, const float2* in, float2* out) {
     std::vector<float4> buf(xbuf_len(N));
     for (int p = 0; p < P; ++p)
         for (int e = 0; e < kE; ++e) {
-            regs[p].v[0][e] = in[p + e * P];
-            regs[p].v[1][e] = cscale(in[p + e * P], 2.0f);
+            regs[p].v[e] = c2make(in[p + e * P], cscale(in[p + e * P], 2.0f));
         }
     if (inverse) emu_from<N, true, 0>(regs, buf, tw.data());
     else emu_from<N, false, 0>(regs, buf, tw.data());
     int bad = 0;
     for (int p = 0; p < P; ++p)
         for (int e = 0; e < kE; ++e) {
-            out[p + e * P] = regs[p].v[0][e];
-            const float2 a = regs[p].v[0][e], b = regs[p].v[1][e];
+            const float2 a = c2get(regs[p].v[e], 0), b = c2get(regs[p].v[e], 1);
+            out[p + e * P] = a;
             if (b.x != 2.0f * a.x || b.y != 2.0f * a.y) bad = 1;     // scaling by 2 is exact in fp32
         }
     return bad ? FRS_ESTATE : 0;
