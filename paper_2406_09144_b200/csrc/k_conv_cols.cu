@@ -2,7 +2,7 @@
 namespace frs {
 template <int NF>
 static int run(cudaStream_t st, const ConvColsArgs& a0, int nb) {
-    using GEO = Geo<NF, 1>;
+    using GEO = ColsGeo<NF>;
     static int ctas = 0;
     if (!ctas) {
         cudaError_t e = set_smem(conv_cols_kernel<NF>, GEO::SMEM);

@@ -18,53 +18,98 @@ struct ConvColsArgs {
 //   y[n] = IFFT_NF(E')[n] + conj(twist^n) IFFT_NF(O')[n]
 // so input, twiddles and the final combination are all thread-local.  Work item = (tile, column);
 // the two columns of a tile go to neighbouring CTAs, which share the tile's sectors through L2.
-// Independent CTAs on one SM keep the shared-memory exchange of one overlapped with the arithmetic
-// of another (staging the column and the weights through cp.async was measured slower: the added
-// shared-memory traffic costs more than the latency it hides).
+//
+// Global reads never stall the arithmetic: one 8 NF-byte staging buffer per group is time-shared by
+//   the column of the NEXT item  (cp.async, every thread copies exactly the 16 samples it will use, so
+//                                 no barrier is needed; issued once the weights have been consumed,
+//                                 in flight during the inverse transforms), and
+//   the weights of THIS item     (one bulk TMA copy of the contiguous 8 NF-byte weight column, issued
+//                                 after the first exchange barrier of the forward transform -- every
+//                                 thread has picked up its samples by then -- and awaited on an
+//                                 mbarrier after the forward transform).
+template <int NF> struct ColsGeo : Geo<NF, 1, NF / 2> {};
+
 template <int NF>
-__global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
+__global__ void __launch_bounds__(ColsGeo<NF>::THREADS, ColsGeo<NF>::MINB)
 conv_cols_kernel(ConvColsArgs a) {
-    using GEO = Geo<NF, 1>;
+    using GEO = ColsGeo<NF>;
     constexpr int P = GEO::P;
     extern __shared__ float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
+    float2* stage = reinterpret_cast<float2*>(buf + xbuf_len(NF));                     // [NF] float2
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem4 + GEO::TW + (size_t)GEO::G * GEO::GROUP_SLOTS) + g;
     load_twiddles<NF>(tws, a.tw);
-    __syncthreads();
+    if (p == 0) mbar_init(bar, 1);
 
-    for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
+    auto column = [&](int item, bool& live, float2*& col, const float*& w) {
         const int b = item / a.items_per_batch;
         const int mc = (item - b * a.items_per_batch) * GEO::G + g;      // 2 m + c
-        const bool live = mc < 2 * a.ntile;
-        float2* col = a.t + b * a.t_bstride + (size_t)(mc >> 1) * NF * 2 + (mc & 1);      // stride 2 float2 per row
-        const float* w = a.wt + b * a.w_bstride + (size_t)mc * NF * 2;
+        live = item < a.nitems && mc < 2 * a.ntile;
+        col = a.t + b * a.t_bstride + (size_t)(mc >> 1) * NF * 2 + (mc & 1);      // stride 2 float2 per row
+        w = a.wt + b * a.w_bstride + (size_t)mc * NF * 2;
+    };
+    auto stage_column = [&](int item) {
+        bool live; float2* col; const float* w;
+        column(item, live, col, w);
+        if (live) {
+#pragma unroll
+            for (int e = 0; e < kE; ++e) cp_async8(stage + p + e * P, col + 2 * (p + e * P));
+        }
+        cp_async_commit();
+    };
+    stage_column(blockIdx.x);
+    __syncthreads();
+    unsigned parity = 0;
+
+    for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
+        bool live; float2* col; const float* w;
+        column(item, live, col, w);
 
         C2 v[kE];
+        cp_async_wait_all();
         if (live) {
-            // warm L2 with this column's weights (read after the forward transform)
-            if ((p & 15) == 0) {
 #pragma unroll
-                for (int e = 0; e < kE; ++e) prefetch_l2(w + 2 * (p + e * P));
+            for (int e = 0; e < kE; ++e) {
+                const float2 x = stage[p + e * P];
+                v[e] = c2make(x, cmul(x, __ldg(a.twist + p + e * P)));
             }
-            float2 x[kE];
-#pragma unroll
-            for (int e = 0; e < kE; ++e) x[e] = ld2_inplace(col + 2 * (p + e * P));
-#pragma unroll
-            for (int e = 0; e < kE; ++e) v[e] = c2make(x[e], cmul(x[e], __ldg(a.twist + p + e * P)));
         } else {
 #pragma unroll
             for (int e = 0; e < kE; ++e) v[e] = c2zero();
         }
-        pair_fft<NF, false>(v, p, buf, tws);
+        // forward transforms; the weights start to arrive behind the first barrier
+        stage_compute<NF, 0, false>(v, p, tws);
+        if constexpr (plan_stages(NF) > 1) {
+            stage_scatter2<NF, 0>(v, p, buf);
+            __syncthreads();
+        } else {
+            __syncthreads();
+        }
+        if (p == 0 && live) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, NF * 8);
+            bulk_g2s(stage, w, NF * 8, bar);
+        }
+        __syncwarp();   // the issuing lane must not be left behind a warp that spins on the mbarrier
+        if constexpr (plan_stages(NF) > 1) {
+            canon_gather2<NF>(v, p, buf);
+            __syncthreads();
+            pair_fft_from<NF, false, 1>(v, p, buf, tws);
+        }
         if (live) {
+            mbar_wait(bar, parity);
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 ww = ldg2(w + 2 * (p + e * P));      // (even-bin weight, odd-bin weight)
+                const float2 ww = stage[p + e * P];               // (even-bin weight, odd-bin weight)
                 v[e].re = f2mul(v[e].re, ww);
                 v[e].im = f2mul(v[e].im, ww);
             }
+            parity ^= 1u;
         }
+        // the staging slots a thread has just read are its own: refill them with the next column
+        stage_column(item + gridDim.x);
         pair_fft<NF, true>(v, p, buf, tws);
         if (live) {
 #pragma unroll
@@ -74,6 +119,7 @@ conv_cols_kernel(ConvColsArgs a) {
             }
         }
     }
+    cp_async_wait_all();
 }
 
 // ------------------------------------------------------------------------------------------------
