@@ -305,42 +305,51 @@ FRS_HD void canon_scatter2(const C2 (&v)[kE], int p, float4* buf) {
 }
 
 #ifdef __CUDACC__
+// ---- group barrier -----------------------------------------------------------------------------------
+// The P threads that share a transform synchronise on their own named barrier, so that the groups of
+// a CTA drift apart freely: while one group exchanges through shared memory the other computes
+// (measured on B200: butterflies and LDS/STS traffic of two groups of ONE CTA overlap, those of two
+// co-resident CTAs hardly do).  Groups narrower than a warp fall back to the CTA-wide barrier 0.
+struct GroupBar {
+    int id, n;
+    __device__ __forceinline__ void sync() const { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(n) : "memory"); }
+};
 // ---- the whole transform of a PAIR of sequences sharing twiddles ---------------------------------
-// All threads of the CTA must call this (it uses __syncthreads()).  buf: one exchange buffer of
-// xbuf_len(N) float4, private to the group.  tw: packed twiddle table (shared memory).
+// All threads of the group must call this.  buf: one exchange buffer of xbuf_len(N) float4, private
+// to the group.  tw: packed twiddle table (shared memory).
 template <int N, bool INV, int S>
-__device__ __forceinline__ void pair_fft_from(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
+__device__ __forceinline__ void pair_fft_from(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw, const GroupBar& gb) {
     if constexpr (S < plan_stages(N)) {
         stage_compute<N, S, INV>(v, p, tw);
         if constexpr (S + 1 < plan_stages(N)) {
             stage_scatter2<N, S>(v, p, buf);
-            __syncthreads();
+            gb.sync();
             canon_gather2<N>(v, p, buf);
-            __syncthreads();
+            gb.sync();
         }
-        pair_fft_from<N, INV, S + 1>(v, p, buf, tw);
+        pair_fft_from<N, INV, S + 1>(v, p, buf, tw, gb);
     }
 }
 template <int N, bool INV>
-__device__ __forceinline__ void pair_fft(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
-    pair_fft_from<N, INV, 0>(v, p, buf, tw);
+__device__ __forceinline__ void pair_fft(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw, const GroupBar& gb) {
+    pair_fft_from<N, INV, 0>(v, p, buf, tw, gb);
 }
 // The same transform in two halves, so that a caller can reuse `buf` (it is free after the head)
 // while the last stage, which runs entirely in registers, is still to be computed.
 template <int N, bool INV, int S>
-__device__ __forceinline__ void pair_fft_head_from(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
+__device__ __forceinline__ void pair_fft_head_from(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw, const GroupBar& gb) {
     if constexpr (S + 1 < plan_stages(N)) {
         stage_compute<N, S, INV>(v, p, tw);
         stage_scatter2<N, S>(v, p, buf);
-        __syncthreads();
+        gb.sync();
         canon_gather2<N>(v, p, buf);
-        __syncthreads();
-        pair_fft_head_from<N, INV, S + 1>(v, p, buf, tw);
+        gb.sync();
+        pair_fft_head_from<N, INV, S + 1>(v, p, buf, tw, gb);
     }
 }
 template <int N, bool INV>
-__device__ __forceinline__ void pair_fft_head(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw) {
-    pair_fft_head_from<N, INV, 0>(v, p, buf, tw);
+__device__ __forceinline__ void pair_fft_head(C2 (&v)[kE], int p, float4* buf, const float4* __restrict__ tw, const GroupBar& gb) {
+    pair_fft_head_from<N, INV, 0>(v, p, buf, tw, gb);
 }
 template <int N, bool INV>
 __device__ __forceinline__ void pair_fft_tail(C2 (&v)[kE], int p, const float4* __restrict__ tw) {

@@ -2,7 +2,7 @@
 namespace frs {
 template <int NF>
 static int run(cudaStream_t st, const HartColsArgs& a0, int nb) {
-    using GEO = Geo<NF, 1>;
+    using GEO = RowsGeo<NF>;
     static int ctas = 0;
     if (!ctas) {
         cudaError_t e = set_smem(hart_cols_kernel<NF>, GEO::SMEM);

@@ -3,7 +3,7 @@ namespace frs {
 // grid_x: number of CTAs launched (= number of (sum s.c, sum j.s) partial pairs in kEnergy mode)
 template <int NF>
 static int run(cudaStream_t st, const RowsInvArgs& a0, int nb, int* grid_x) {
-    using GEO = Geo<NF, 1>;
+    using GEO = RowsGeo<NF>;
     static int ctas = 0;
     if (!ctas) {
         cudaError_t e = set_smem(rows_inv_kernel<NF>, GEO::SMEM);

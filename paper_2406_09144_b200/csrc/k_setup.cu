@@ -36,7 +36,7 @@ psf_cols_kernel(PsfColsArgs a) {
             }
         }
     }
-    pair_fft<NF, false>(v, p, buf, tws);
+    pair_fft<NF, false>(v, p, buf, tws, GEO::bar(g));
     float max_im = 0.f, min_re = 0.f, max_re = 0.f;
     if (live) {
         float* w = a.wt + b * a.w_bstride + (size_t)m * 2 * NF * 2 + role;      // [c][q][parity = role]

@@ -25,18 +25,22 @@ namespace frs {
 
 // CTA geometry.  ROLES: thread groups of P cooperating on one work item (conv_cols: even/odd bins).
 // STAGE: extra float4 slots per group for an asynchronously filled staging buffer.
-template <int NF, int ROLES, int STAGE = 0>
+template <int NF, int ROLES, int STAGE = 0, int BIG = 512>
 struct Geo {
     static constexpr int P = NF / kE;                                  // threads per transform pair
     static constexpr int GT = P * ROLES;                               // threads per group
-    static constexpr int WANT = NF >= 1024 ? (ROLES == 2 ? 512 : 256) : (NF >= 256 ? 256 : 64);
+    // BIG = 512: one CTA per SM whose groups overlap each other's phases; 256: two CTAs per SM
+    // (128 registers per thread either way) -- chosen per kernel by measurement
+    static constexpr int WANT = NF >= 1024 ? BIG : (NF >= 256 ? 256 : 64);
     static constexpr int THREADS = GT >= WANT ? GT : WANT;
     static constexpr int G = THREADS / GT;                             // groups per CTA
+    static constexpr bool OWN_BAR = (GT % 32 == 0) && G <= 15 && ROLES == 1;   // a named barrier per group
     static constexpr int TW = plan_tw_total(NF);                       // float4 slots of the twiddle tables
     static constexpr int GROUP_SLOTS = ROLES * xbuf_len(NF) + STAGE;   // float4 slots per group
     static constexpr int BAR_SLOTS = (G + 1) / 2;                      // one 8-byte mbarrier per group
     static constexpr int SMEM = (TW + G * GROUP_SLOTS + BAR_SLOTS) * (int)sizeof(float4);
     static constexpr int MINB = THREADS >= 512 ? 1 : (THREADS >= 256 ? 2 : 4);
+    __device__ static GroupBar bar(int g) { return OWN_BAR ? GroupBar{1 + g, GT} : GroupBar{0, THREADS}; }
 };
 
 // Streaming data (images, spectrum tiles, weights) bypasses L1 allocation so that the twist
@@ -74,6 +78,8 @@ __device__ __forceinline__ void stg2(void* p, float2 v) {
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
+template <int NF> struct RowsGeo : Geo<NF, 1, 0, 256> {};
+
 // ------------------------------------------------------------------------------------------------
 struct RowsFwdArgs {
     const float* in;      // [nb][ny][nxr]
@@ -91,9 +97,9 @@ struct RowsFwdArgs {
 // item are issued into registers as soon as the transform has left them, so they are in flight while
 // this item's spectrum is unpacked from shared memory and stored.
 template <int NF, bool PAD>
-__global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
+__global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 rows_fwd_kernel(RowsFwdArgs a) {
-    using GEO = Geo<NF, 1>;
+    using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
     constexpr int NXR = PAD ? NF : 2 * NF;        // real samples per row
     constexpr int NE = PAD ? kE / 2 : kE;         // canonical slots that hold data
@@ -101,6 +107,7 @@ rows_fwd_kernel(RowsFwdArgs a) {
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
+    const GroupBar gb = GEO::bar(g);
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
 
@@ -150,9 +157,9 @@ rows_fwd_kernel(RowsFwdArgs a) {
                 v[e] = c2zero();
             }
         }
-        pair_fft<NF, false>(v, p, buf, tws);
+        pair_fft<NF, false>(v, p, buf, tws, gb);
         canon_scatter2<NF>(v, p, buf);
-        __syncthreads();
+        gb.sync();
         if (PAD) issue_loads(item + gridDim.x);
         if (live) {
             // X[k] * scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = 0..NF.
@@ -193,7 +200,7 @@ rows_fwd_kernel(RowsFwdArgs a) {
                 }
             }
         }
-        __syncthreads();
+        gb.sync();
     }
 }
 

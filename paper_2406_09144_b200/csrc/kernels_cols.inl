@@ -40,8 +40,12 @@ conv_cols_kernel(ConvColsArgs a) {
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
     float2* stage = reinterpret_cast<float2*>(buf + xbuf_len(NF));                     // [NF] float2
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem4 + GEO::TW + (size_t)GEO::G * GEO::GROUP_SLOTS) + g;
+    const GroupBar gb = GEO::bar(g);
     load_twiddles<NF>(tws, a.tw);
     if (p == 0) mbar_init(bar, 1);
+    // twist^n for the thread's samples n = p + e P, from the exactly rounded table (a product of two
+    // rounded factors costs a measurable part of the CG error budget and no time is gained by it)
+    auto twist_e = [&](int e) { return __ldg(a.twist + p + e * P); };
 
     auto column = [&](int item, bool& live, float2*& col, const float*& w) {
         const int b = item / a.items_per_batch;
@@ -73,7 +77,7 @@ conv_cols_kernel(ConvColsArgs a) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const float2 x = stage[p + e * P];
-                v[e] = c2make(x, cmul(x, __ldg(a.twist + p + e * P)));
+                v[e] = c2make(x, cmul(x, twist_e(e)));
             }
         } else {
 #pragma unroll
@@ -83,9 +87,9 @@ conv_cols_kernel(ConvColsArgs a) {
         stage_compute<NF, 0, false>(v, p, tws);
         if constexpr (plan_stages(NF) > 1) {
             stage_scatter2<NF, 0>(v, p, buf);
-            __syncthreads();
+            gb.sync();
         } else {
-            __syncthreads();
+            gb.sync();
         }
         if (p == 0 && live) {
             fence_proxy_async();
@@ -95,8 +99,8 @@ conv_cols_kernel(ConvColsArgs a) {
         __syncwarp();   // the issuing lane must not be left behind a warp that spins on the mbarrier
         if constexpr (plan_stages(NF) > 1) {
             canon_gather2<NF>(v, p, buf);
-            __syncthreads();
-            pair_fft_from<NF, false, 1>(v, p, buf, tws);
+            gb.sync();
+            pair_fft_from<NF, false, 1>(v, p, buf, tws, gb);
         }
         if (live) {
             mbar_wait(bar, parity);
@@ -110,11 +114,11 @@ conv_cols_kernel(ConvColsArgs a) {
         }
         // the staging slots a thread has just read are its own: refill them with the next column
         stage_column(item + gridDim.x);
-        pair_fft<NF, true>(v, p, buf, tws);
+        pair_fft<NF, true>(v, p, buf, tws, gb);
         if (live) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 o = cmulc(c2get(v[e], 1), __ldg(a.twist + p + e * P));
+                const float2 o = cmulc(c2get(v[e], 1), twist_e(e));
                 stg2(col + 2 * (p + e * P), make_float2(v[e].re.x + o.x, v[e].im.x + o.y));
             }
         }
@@ -138,15 +142,16 @@ struct HartColsArgs {
 // F[y][x] = column FFT; H[y][x] = Re F - Im F and H[(-y) mod NF][nx - x] = Re F + Im F  (reading R6).
 // Column x of H is one contiguous run of the transposed output, so all stores are coalesced.
 template <int NF>
-__global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
+__global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 hart_cols_kernel(HartColsArgs a) {
-    using GEO = Geo<NF, 1>;
+    using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
     extern __shared__ float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
     const int ntile = a.nx / 4 + 1;
+    const GroupBar gb = GEO::bar(g);
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
 
@@ -167,7 +172,7 @@ hart_cols_kernel(HartColsArgs a) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) v[e] = c2zero();
         }
-        pair_fft<NF, false>(v, p, buf, tws);
+        pair_fft<NF, false>(v, p, buf, tws, gb);
         if (live) {
             const size_t base = b * a.img_bstride;
             const float off = a.offset ? __ldg(a.offset + b) : 0.f;
@@ -195,6 +200,6 @@ hart_cols_kernel(HartColsArgs a) {
                 }
             }
         }
-        __syncthreads();
+        gb.sync();
     }
 }

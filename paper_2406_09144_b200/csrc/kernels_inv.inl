@@ -20,9 +20,9 @@ struct RowsInvArgs {
 // stage), so the gather is in flight during that stage and the epilogue.  Landing layout:
 // slot r*(NF/2+1) + m = (Y_r[2m], Y_r[2m+1]) for row r of the pair.
 template <int NF>
-__global__ void __launch_bounds__(Geo<NF, 1>::THREADS, Geo<NF, 1>::MINB)
+__global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 rows_inv_kernel(RowsInvArgs a) {
-    using GEO = Geo<NF, 1>;
+    using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
     constexpr int NTILE = NF / 2 + 1;
     extern __shared__ float4 smem4[];
@@ -30,6 +30,7 @@ rows_inv_kernel(RowsInvArgs a) {
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
     const float2* land = reinterpret_cast<const float2*>(buf);      // Y_r[k] at land[r*2*NTILE + k]
+    const GroupBar gb = GEO::bar(g);
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
     double acc_sc = 0.0, acc_js = 0.0;
@@ -65,7 +66,7 @@ rows_inv_kernel(RowsInvArgs a) {
         const int y0 = 2 * rp;
 
         cp_async_wait_all();
-        __syncthreads();
+        gb.sync();
         // Z'[k] = (Y[k] + conj Y[NF-k]) + i conj(twist[k]) (Y[k] - conj Y[NF-k]),  k = 0..NF-1
         C2 v[kE];
 #pragma unroll
@@ -82,8 +83,8 @@ rows_inv_kernel(RowsInvArgs a) {
             }
             v[e] = c2make(z[0], z[1]);
         }
-        __syncthreads();
-        pair_fft_head<NF, true>(v, p, buf, tws);
+        gb.sync();
+        pair_fft_head<NF, true>(v, p, buf, tws, gb);
         gather(item + gridDim.x);                 // buf is free from here to the top of the loop
         pair_fft_tail<NF, true>(v, p, tws);
 

@@ -270,7 +270,9 @@ def test_cg_free_running_within_horizon_and_literal(frs):
     w, ctx, b, ap = _cg_problem(frs, ("c1",))
     bh = b.cpu().numpy().astype(np.float64)
     sol = o.cg(ap, bh, max_iter=20, keep=True)
-    env = o.cg_fp32_envelope(ap, bh, max_iter=20)
+    # the envelope is a random quantity (one seeded noise draw per apply): take the upper envelope of
+    # four draws, so that the horizon does not hinge on one lucky realisation (R9)
+    env = np.max([o.cg_fp32_envelope(ap, bh, max_iter=20, seed=sd) for sd in (1234, 1235, 1236, 1237)], axis=0)
     horizon = max([k + 1 for k in range(20) if env[k] <= 2e-5] or [0])
     assert horizon >= 5
     hist = torch.zeros(21, dtype=torch.float64, device="cuda")
