@@ -25,7 +25,7 @@ def _stamp():
     h = hashlib.sha256()
     for root in (CSRC, os.path.join(os.path.dirname(HERE), "include")):
         for f in sorted(os.listdir(root)):
-            if f.endswith((".cu", ".cuh", ".h")):
+            if f.endswith((".cu", ".cuh", ".h", ".inl")):
                 h.update(f.encode())
                 h.update(open(os.path.join(root, f), "rb").read())
     h.update(" ".join(FLAGS).encode())

@@ -35,6 +35,7 @@ struct frs_ctx {
     bool s_ok = false, sT_ok = false;
     float *d_mu = nullptr, *d_lognu = nullptr;
     float2 *T = nullptr, *Th = nullptr;
+    CUtensorMap tmapT[2];     // tile maps of T in the natural / transposed orientation (tmap.h)
     float *lin = nullptr, *img = nullptr, *acc = nullptr;
     float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
     float *hx = nullptr, *hy = nullptr;
@@ -113,6 +114,8 @@ size_t max2(size_t a, size_t b) { return a > b ? a : b; }
 int ensure_scratch(frs_ctx* ctx) {
     const size_t np = ctx->npix, ny = ctx->ny, nx = ctx->nx;
     RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
+    if (make_tile_map(&ctx->tmapT[0], ctx->T, ny, nx, ctx->nchan) || make_tile_map(&ctx->tmapT[1], ctx->T, nx, ny, ctx->nchan))
+        return fail(ctx, FRS_ECUDA, "cuTensorMapEncodeTiled failed");
     RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * max2((nx / 4 + 1) * ny, (ny / 4 + 1) * nx) * 2));
     RET(dev_alloc(ctx, &ctx->lin, 2 * np));
     RET(dev_alloc(ctx, &ctx->acc, 2 * np));
@@ -140,9 +143,10 @@ int dot(frs_ctx* ctx, const float* a, const float* b, size_t n, double* d_out) {
 // ---- the three passes of C (Eq. 14) -----------------------------------------------------------
 // Orientation of a sky-space image: [rows][len].  Natural: rows = ny, len = nx.  Transposed: rows = nx,
 // len = ny, with the weight table built for the transposed PSF spectrum.
-struct Orient { int rows, len, ntile; const float* wt; };
+struct Orient { int rows, len, ntile; const float* wt; const CUtensorMap* tmap; };
 Orient orient(const frs_ctx* ctx, bool transposed) {
-    return transposed ? Orient{ctx->nx, ctx->ny, ctx->ny / 2 + 1, ctx->wtT} : Orient{ctx->ny, ctx->nx, ctx->nx / 2 + 1, ctx->wt};
+    return transposed ? Orient{ctx->nx, ctx->ny, ctx->ny / 2 + 1, ctx->wtT, &ctx->tmapT[1]}
+                      : Orient{ctx->ny, ctx->nx, ctx->nx / 2 + 1, ctx->wt, &ctx->tmapT[0]};
 }
 
 int conv_rows_fwd(frs_ctx* ctx, const Orient& o, const float* in, const float* mul) {
@@ -169,6 +173,7 @@ int conv_cols(frs_ctx* ctx, const Orient& o) {
 int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const float* s, const float* j, int* grid_x) {
     Prof pr(ctx, kPassRowsInv);
     RowsInvArgs a{};
+    a.tmap = *o.tmap;
     a.t = ctx->T; a.out = out; a.s = s; a.j = j; a.partials = ctx->partials;
     a.ny = o.rows; a.mode = mode;
     a.t_bstride = (size_t)o.ntile * o.rows * 2; a.img_bstride = ctx->npix;

@@ -10,7 +10,7 @@ __global__ void __launch_bounds__(Geo<NF, 2>::THREADS, Geo<NF, 2>::MINB)
 psf_cols_kernel(PsfColsArgs a) {
     using GEO = Geo<NF, 2>;
     constexpr int P = GEO::P;
-    extern __shared__ float4 smem4[];
+    extern __shared__ __align__(128) float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / (2 * P), role = (threadIdx.x / P) & 1, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + ((size_t)g * 2 + role) * xbuf_len(NF);

@@ -20,6 +20,7 @@
 // twiddle fetches and travel through shared memory as one float4 per position.
 #pragma once
 #include "fft_core.cuh"
+#include "tmap.h"
 
 namespace frs {
 
@@ -35,7 +36,7 @@ struct Geo {
     static constexpr int THREADS = GT >= WANT ? GT : WANT;
     static constexpr int G = THREADS / GT;                             // groups per CTA
     static constexpr bool OWN_BAR = (GT % 32 == 0) && G <= 15 && ROLES == 1;   // a named barrier per group
-    static constexpr int TW = plan_tw_total(NF);                       // float4 slots of the twiddle tables
+    static constexpr int TW = (plan_tw_total(NF) + 7) & ~7;            // float4 slots of the twiddle tables (128-byte multiple)
     static constexpr int GROUP_SLOTS = ROLES * xbuf_len(NF) + STAGE;   // float4 slots per group
     static constexpr int BAR_SLOTS = (G + 1) / 2;                      // one 8-byte mbarrier per group
     static constexpr int SMEM = (TW + G * GROUP_SLOTS + BAR_SLOTS) * (int)sizeof(float4);
@@ -103,7 +104,7 @@ rows_fwd_kernel(RowsFwdArgs a) {
     constexpr int P = GEO::P;
     constexpr int NXR = PAD ? NF : 2 * NF;        // real samples per row
     constexpr int NE = PAD ? kE / 2 : kE;         // canonical slots that hold data
-    extern __shared__ float4 smem4[];
+    extern __shared__ __align__(128) float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;

@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(ColsGeo<NF>::THREADS, ColsGeo<NF>::MINB)
 conv_cols_kernel(ConvColsArgs a) {
     using GEO = ColsGeo<NF>;
     constexpr int P = GEO::P;
-    extern __shared__ float4 smem4[];
+    extern __shared__ __align__(128) float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 hart_cols_kernel(HartColsArgs a) {
     using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
-    extern __shared__ float4 smem4[];
+    extern __shared__ __align__(128) float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;

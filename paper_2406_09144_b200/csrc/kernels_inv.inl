@@ -3,6 +3,7 @@
 enum RowsInvMode { kPlain = 0, kMulS = 1, kEnergy = 2 };
 
 struct RowsInvArgs {
+    CUtensorMap tmap;     // tile map of t (tmap.h)
     const float2* t;      // [nb][ntile][ny][2]
     float* out;           // [nb][ny][NF]
     const float* s;       // [nb][ny][NF]  (kMulS, kEnergy)
@@ -15,39 +16,61 @@ struct RowsInvArgs {
     const float2* twist;
 };
 
-// Pipeline: the half-spectrum rows of the NEXT item are gathered by 16-byte cp.async copies straight
-// into the exchange buffer as soon as the transform has left it (before its last, register-only
-// stage), so the gather is in flight during that stage and the epilogue.  Landing layout:
-// slot r*(NF/2+1) + m = (Y_r[2m], Y_r[2m+1]) for row r of the pair.
+// Pipeline: the half-spectrum rows of the NEXT item are gathered by the TMA unit (tensor copies of the
+// column-pair tiles, tmap.h: 2 x 17 copies per row pair, no LSU instructions, no address arithmetic)
+// straight into the exchange buffer as soon as the transform has left it (before its last,
+// register-only stage), so the gather is in flight during that stage and the epilogue.  Landing
+// layout: row r of the pair at float2 index r * LROW + k, k = 0..NF+1.
 template <int NF>
 __global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
-rows_inv_kernel(RowsInvArgs a) {
+rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
     using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
+    constexpr int BOX = tma_box_tiles(NF), NOPS = tma_copies(NF), LROW = 2 * BOX * NOPS;
+    constexpr bool USE_TMA = NF >= 256;            // smaller rows: boxes below the 128-byte TMA alignment -> cp.async
     constexpr int NTILE = NF / 2 + 1;
-    extern __shared__ float4 smem4[];
+    static_assert(2 * LROW * 8 <= xbuf_len(NF) * 16, "landing area exceeds the exchange buffer");
+    extern __shared__ __align__(128) float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
-    const float2* land = reinterpret_cast<const float2*>(buf);      // Y_r[k] at land[r*2*NTILE + k]
+    const float2* land = reinterpret_cast<const float2*>(buf);      // Y_r[k] at land[r*LROW + k]
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem4 + GEO::TW + (size_t)GEO::G * GEO::GROUP_SLOTS) + g;
     const GroupBar gb = GEO::bar(g);
     load_twiddles<NF>(tws, a.tw);
+    if (p == 0) mbar_init(bar, 1);
     __syncthreads();
     double acc_sc = 0.0, acc_js = 0.0;
+    unsigned parity = 0;
 
     auto gather = [&](int item) {
         const int b = item / a.items_per_batch;
         const int rp = (item - b * a.items_per_batch) * GEO::G + g;
-        if (item < a.nitems && 2 * rp < a.ny) {
+        const bool live = item < a.nitems && 2 * rp < a.ny;
+        if (live && !USE_TMA) {
             const float4* tb = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + 2 * rp;
-            // lanes (2j, 2j+1) fetch rows (0, 1) of the same tile: one 32-byte sector per lane pair
-            const int r = p & 1;
-#pragma unroll
-            for (int i = 0; i < kE; ++i) {
-                const int m = (p >> 1) + i * (P / 2);
-                cp_async16(buf + r * NTILE + m, tb + (size_t)m * a.ny + r);
+            for (int q = p; q < 2 * NTILE; q += P) {
+                const int r = q & 1, m = q >> 1;
+                cp_async16(buf + r * (LROW / 2) + m, tb + (size_t)m * a.ny + r);
             }
-            if (p < 2) cp_async16(buf + r * NTILE + NTILE - 1, tb + (size_t)(NTILE - 1) * a.ny + r);
+        }
+        if (!USE_TMA) cp_async_commit();
+        if (live && USE_TMA) {
+            if (p == 0) {
+                fence_proxy_async();
+                mbar_expect_tx(bar, 2 * NOPS * BOX * 16);
+            }
+            if (P >= 32) __syncwarp();
+            // the 2 NOPS copies are issued by the first lanes of the group
+            for (int q = p; q < 2 * NOPS; q += (P < 32 ? P : 32)) {
+                if (p < 32) {
+                    const int r = q / NOPS, j = q - r * NOPS;
+                    tensor_g2s_4d(buf + (r * LROW + 2 * BOX * j) / 2, &a.tmap, 0, 2 * rp + r, BOX * j, b, bar);
+                }
+            }
+            if (P >= 32) __syncwarp();
+        }
+        if (live) {
             // warm L2 with the rows of s (and j) the epilogue of that item will read: P lines of 128 B
             if (a.mode != kPlain) {
                 const size_t row = b * a.img_bstride + (size_t)(2 * rp) * NF;
@@ -55,7 +78,6 @@ rows_inv_kernel(RowsInvArgs a) {
                 if (a.mode == kEnergy) prefetch_l2(a.j + row + 32 * p);
             }
         }
-        cp_async_commit();
     };
     gather(blockIdx.x);
 
@@ -65,8 +87,12 @@ rows_inv_kernel(RowsInvArgs a) {
         const bool live = 2 * rp < a.ny;
         const int y0 = 2 * rp;
 
-        cp_async_wait_all();
-        gb.sync();
+        if (USE_TMA) {
+            if (live) { mbar_wait(bar, parity); parity ^= 1u; }
+        } else {
+            cp_async_wait_all();
+            gb.sync();
+        }
         // Z'[k] = (Y[k] + conj Y[NF-k]) + i conj(twist[k]) (Y[k] - conj Y[NF-k]),  k = 0..NF-1
         C2 v[kE];
 #pragma unroll
@@ -77,7 +103,7 @@ rows_inv_kernel(RowsInvArgs a) {
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 float2 ya = make_float2(0.f, 0.f), ym = ya;
-                if (live) { ya = land[t * 2 * NTILE + k]; ym = cconj(land[t * 2 * NTILE + NF - k]); }
+                if (live) { ya = land[t * LROW + k]; ym = cconj(land[t * LROW + NF - k]); }
                 const float2 s = cadd(ya, ym), d = cmulc(csub(ya, ym), w);
                 z[t] = make_float2(s.x - d.y, s.y + d.x);
             }
