@@ -233,7 +233,7 @@ template <int R> FRS_HD void twiddle_powers(float2 (&w)[R]) {
 
 FRS_HD constexpr int xpad(int pos) { return pos + (pos >> 4); }
 // slots of one exchange buffer (holds positions 0..N inclusive: the row passes park X[N] too)
-FRS_HD constexpr int xbuf_len(int n) { return n + (n >> 4) + 8; }
+FRS_HD constexpr int xbuf_len(int n) { return (n + (n >> 4) + 8 + 7) & ~7; }   // multiple of 128 bytes (TMA boxes)
 
 // exchange slot of one position: (re of transform 0, re of 1, im of 0, im of 1) -> 128-bit accesses
 FRS_HD float4 pack(const C2& a) { return make_float4(a.re.x, a.re.y, a.im.x, a.im.y); }
@@ -378,10 +378,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  :: "r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-// 4-D tensor (TMA) copy global -> shared of one box of the map, completion counted on an mbarrier
+// tensor (TMA) copies global -> shared of one box of a map, completion counted on an mbarrier
 __device__ __forceinline__ void tensor_g2s_4d(void* dst_smem, const void* tmap, int c0, int c1, int c2, int c3, unsigned long long* bar) {
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                  :: "r"(smem_u32(dst_smem)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tensor_g2s_5d(void* dst_smem, const void* tmap, int c0, int c1, int c2, int c3, int c4, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+                 :: "r"(smem_u32(dst_smem)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {

@@ -35,7 +35,8 @@ struct frs_ctx {
     bool s_ok = false, sT_ok = false;
     float *d_mu = nullptr, *d_lognu = nullptr;
     float2 *T = nullptr, *Th = nullptr;
-    CUtensorMap tmapT[2];     // tile maps of T in the natural / transposed orientation (tmap.h)
+    struct MapKey { const void* p; int rows, nf, nb; CUtensorMap row, col; };
+    std::vector<MapKey> maps;  // spectrum tensor maps (tmap.h), built on first use
     float *lin = nullptr, *img = nullptr, *acc = nullptr;
     float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
     float *hx = nullptr, *hy = nullptr;
@@ -114,8 +115,6 @@ size_t max2(size_t a, size_t b) { return a > b ? a : b; }
 int ensure_scratch(frs_ctx* ctx) {
     const size_t np = ctx->npix, ny = ctx->ny, nx = ctx->nx;
     RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
-    if (make_tile_map(&ctx->tmapT[0], ctx->T, ny, nx, ctx->nchan) || make_tile_map(&ctx->tmapT[1], ctx->T, nx, ny, ctx->nchan))
-        return fail(ctx, FRS_ECUDA, "cuTensorMapEncodeTiled failed");
     RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * max2((nx / 4 + 1) * ny, (ny / 4 + 1) * nx) * 2));
     RET(dev_alloc(ctx, &ctx->lin, 2 * np));
     RET(dev_alloc(ctx, &ctx->acc, 2 * np));
@@ -143,17 +142,31 @@ int dot(frs_ctx* ctx, const float* a, const float* b, size_t n, double* d_out) {
 // ---- the three passes of C (Eq. 14) -----------------------------------------------------------
 // Orientation of a sky-space image: [rows][len].  Natural: rows = ny, len = nx.  Transposed: rows = nx,
 // len = ny, with the weight table built for the transposed PSF spectrum.
-struct Orient { int rows, len, ntile; const float* wt; const CUtensorMap* tmap; };
+struct Orient { int rows, len, ntile; const float* wt; };
 Orient orient(const frs_ctx* ctx, bool transposed) {
-    return transposed ? Orient{ctx->nx, ctx->ny, ctx->ny / 2 + 1, ctx->wtT, &ctx->tmapT[1]}
-                      : Orient{ctx->ny, ctx->nx, ctx->nx / 2 + 1, ctx->wt, &ctx->tmapT[0]};
+    return transposed ? Orient{ctx->nx, ctx->ny, ctx->ny / 2 + 1, ctx->wtT} : Orient{ctx->ny, ctx->nx, ctx->nx / 2 + 1, ctx->wt};
+}
+// tensor maps of a spectrum buffer in the block layout (tmap.h), cached per shape
+int spectrum_maps(frs_ctx* ctx, const float2* T, int rows, int nf, int nb, CUtensorMap* row, CUtensorMap* col) {
+    for (const auto& k : ctx->maps)
+        if (k.p == T && k.rows == rows && k.nf == nf && k.nb == nb) {
+            if (row) *row = k.row;
+            if (col) *col = k.col;
+            return FRS_OK;
+        }
+    frs_ctx::MapKey k{T, rows, nf, nb, {}, {}};
+    if (make_spectrum_maps(&k.row, &k.col, T, rows, nf, nb)) return fail(ctx, FRS_ECUDA, "cuTensorMapEncodeTiled failed");
+    ctx->maps.push_back(k);
+    if (row) *row = k.row;
+    if (col) *col = k.col;
+    return FRS_OK;
 }
 
 int conv_rows_fwd(frs_ctx* ctx, const Orient& o, const float* in, const float* mul) {
     Prof pr(ctx, kPassRowsFwd);
     RowsFwdArgs a{};
     a.in = in; a.mul = mul; a.out = ctx->T; a.ny = o.rows;
-    a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)o.ntile * o.rows * 2;
+    a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix;
     a.scale = 1.0f;   // yields 2 X[k]; the 1/2 is folded into wt
     a.tw = ctx->tw[o.len]; a.twist = ctx->twist[o.len];
     CKL(launch_rows_fwd(ctx->stream, o.len, true, a, ctx->nchan));
@@ -163,8 +176,9 @@ int conv_rows_fwd(frs_ctx* ctx, const Orient& o, const float* in, const float* m
 int conv_cols(frs_ctx* ctx, const Orient& o) {
     Prof pr(ctx, kPassConvCols);
     ConvColsArgs a{};
-    a.t = ctx->T; a.wt = o.wt; a.ntile = o.ntile;
-    a.t_bstride = (size_t)o.ntile * o.rows * 2; a.w_bstride = (size_t)o.ntile * 2 * o.rows * 2;
+    a.t = ctx->T; a.wt = o.wt; a.ncols = o.len + 1; a.ntile = o.ntile;
+    RET(spectrum_maps(ctx, ctx->T, o.rows, o.len, ctx->nchan, nullptr, &a.tmap));
+    a.w_bstride = (size_t)o.ntile * 2 * o.rows * 2;
     a.tw = ctx->tw[o.rows]; a.twist = ctx->twist[o.rows];
     CKL(launch_conv_cols(ctx->stream, o.rows, a, ctx->nchan));
     ctx->launches++;
@@ -173,10 +187,10 @@ int conv_cols(frs_ctx* ctx, const Orient& o) {
 int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const float* s, const float* j, int* grid_x) {
     Prof pr(ctx, kPassRowsInv);
     RowsInvArgs a{};
-    a.tmap = *o.tmap;
     a.t = ctx->T; a.out = out; a.s = s; a.j = j; a.partials = ctx->partials;
     a.ny = o.rows; a.mode = mode;
-    a.t_bstride = (size_t)o.ntile * o.rows * 2; a.img_bstride = ctx->npix;
+    RET(spectrum_maps(ctx, ctx->T, o.rows, o.len, ctx->nchan, &a.tmap, nullptr));
+    a.img_bstride = ctx->npix;
     a.tw = ctx->tw[o.len]; a.twist = ctx->twist[o.len];
     CKL(launch_rows_inv(ctx->stream, o.len, a, ctx->nchan, grid_x));
     ctx->launches++;
@@ -195,7 +209,7 @@ int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul
         Prof pr(ctx, kPassHartRows);
         RowsFwdArgs a{};
         a.in = in; a.mul = premul; a.out = ctx->Th; a.ny = n1;
-        a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix; a.out_bstride = (size_t)ntile_h * n1 * 2;
+        a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix;
         a.scale = 0.5f;
         a.tw = ctx->tw[n2 / 2]; a.twist = ctx->twist[n2 / 2];
         CKL(launch_rows_fwd(ctx->stream, n2 / 2, false, a, nb));
@@ -205,7 +219,7 @@ int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul
         Prof pr(ctx, kPassHartCols);
         HartColsArgs a{};
         a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = n2;
-        a.t_bstride = (size_t)ntile_h * n1 * 2; a.img_bstride = ctx->npix;
+        a.img_bstride = ctx->npix;
         a.tw = ctx->tw[n1];
         CKL(launch_hart_cols(ctx->stream, n1, a, nb));
         ctx->launches++;
@@ -400,7 +414,7 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
     auto body = [&]() -> int {
         RowsFwdArgs a{};
         a.in = psf; a.mul = nullptr; a.out = tmp; a.ny = my;
-        a.in_bstride = (size_t)my * mx; a.mul_bstride = 0; a.out_bstride = tstride;
+        a.in_bstride = (size_t)my * mx; a.mul_bstride = 0;
         a.scale = 0.5f; a.tw = ctx->tw[ctx->nx]; a.twist = ctx->twist[ctx->nx];
         CKL(launch_rows_fwd(ctx->stream, ctx->nx, false, a, ctx->nchan));
         PsfColsArgs c{};
@@ -408,7 +422,7 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
         CKL(launch_psf_cols(ctx->stream, ctx->ny, c, ctx->nchan, &gx));   // grid size only
         CK(cudaMalloc(reinterpret_cast<void**>(&stats), (size_t)ctx->nchan * gx * 3 * sizeof(float)));
         c.t = tmp; c.wt = ctx->wt; c.stats = stats; c.scale = 1.0f / ((float)my * (float)mx);
-        c.t_bstride = tstride; c.w_bstride = (size_t)ctx->ntile * 2 * ctx->ny * 2;
+        c.ncols = ctx->nx + 1; c.w_bstride = (size_t)ctx->ntile * 2 * ctx->ny * 2;
         c.tw = ctx->tw[ctx->ny]; c.twist = ctx->twist[ctx->ny];
         CKL(launch_psf_cols(ctx->stream, ctx->ny, c, ctx->nchan, nullptr));
         ctx->launches += 2;

@@ -11,7 +11,7 @@ static int run(cudaStream_t st, const ConvColsArgs& a0, int nb) {
         if (!ctas) return (int)cudaErrorUnknown;
     }
     ConvColsArgs a = a0;
-    a.items_per_batch = (2 * a.ntile + GEO::G - 1) / GEO::G;
+    a.items_per_batch = (a.ncols + GEO::G - 1) / GEO::G;
     a.nitems = a.items_per_batch * nb;
     const int grid = a.nitems < ctas ? a.nitems : ctas;
     conv_cols_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);

@@ -23,16 +23,21 @@ psf_cols_kernel(PsfColsArgs a) {
 #pragma unroll
     for (int e = 0; e < kE; ++e) v[e] = c2zero();
     if (live) {
-        const float4* tile = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + (size_t)m * 2 * NF;
+        // tile m = columns 2m, 2m+1, 2 NF rows: sample y at block y >> 1, position (c, y & 1)
+        const float2* c0 = a.t + ((size_t)(b * a.ntile + m) * NF) * 4;
+        const bool two = 2 * m + 1 < a.ncols;
+        auto at = [&](int c, int y) { return ldg2(reinterpret_cast<const float*>(c0 + (y >> 1) * 4 + c * 2 + (y & 1))); };
 #pragma unroll
         for (int e = 0; e < kE; ++e) {
             const int n = p + e * P;
-            const float4 x0 = ldg4(tile + n), x1 = ldg4(tile + n + NF);
+            const float2 z = make_float2(0.f, 0.f);
+            const float2 a0 = at(0, n), a1 = at(0, n + NF);
+            const float2 b0 = two ? at(1, n) : z, b1 = two ? at(1, n + NF) : z;
             if (!role) {
-                v[e] = c2make(make_float2(x0.x + x1.x, x0.y + x1.y), make_float2(x0.z + x1.z, x0.w + x1.w));
+                v[e] = c2make(make_float2(a0.x + a1.x, a0.y + a1.y), make_float2(b0.x + b1.x, b0.y + b1.y));
             } else {
                 const float2 w = __ldg(a.twist + n);
-                v[e] = c2make(cmul(make_float2(x0.x - x1.x, x0.y - x1.y), w), cmul(make_float2(x0.z - x1.z, x0.w - x1.w), w));
+                v[e] = c2make(cmul(make_float2(a0.x - a1.x, a0.y - a1.y), w), cmul(make_float2(b0.x - b1.x, b0.y - b1.y), w));
             }
         }
     }

@@ -85,10 +85,10 @@ template <int NF> struct RowsGeo : Geo<NF, 1, 0, 256> {};
 struct RowsFwdArgs {
     const float* in;      // [nb][ny][nxr]
     const float* mul;     // optional [nb][ny][nxr] multiplier (s or A); nullptr = none
-    float2* out;          // [nb][ntile][ny][2]
+    float2* out;          // [nb][NF/2+1][ny/2][2][2]: 32-byte blocks (bins 2m, 2m+1) x (rows 2r, 2r+1), tmap.h
     int ny;               // rows
     int items_per_batch, nitems;
-    size_t in_bstride, mul_bstride, out_bstride;   // elements (float / float / float2)
+    size_t in_bstride, mul_bstride;   // elements (float)
     float scale;
     const float4* tw;     // packed stage twiddles for NF (global; copied to shared memory)
     const float2* twist;  // exp(-2 pi i k/(2 NF)), k = 0..NF
@@ -96,7 +96,11 @@ struct RowsFwdArgs {
 
 // One group (P threads) transforms rows y0, y0+1 together.  Software pipeline: the loads of the next
 // item are issued into registers as soon as the transform has left them, so they are in flight while
-// this item's spectrum is unpacked from shared memory and stored.
+// this item's spectrum is unpacked and stored.
+// Unpacking X[k] from the half-length transform Z needs Z[k] (still in the thread's registers) and
+// Z[NF-k] (another thread's): Z is parked in the exchange buffer once and every thread reads its 16
+// mirror slots.  A thread then holds X[k] of both rows (16 bytes); neighbouring lanes hold
+// neighbouring bins, so each lane pair stores one whole 32-byte sector of the block layout.
 template <int NF, bool PAD>
 __global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 rows_fwd_kernel(RowsFwdArgs a) {
@@ -159,49 +163,39 @@ rows_fwd_kernel(RowsFwdArgs a) {
             }
         }
         pair_fft<NF, false>(v, p, buf, tws, gb);
-        canon_scatter2<NF>(v, p, buf);
+        canon_scatter2<NF>(v, p, buf);            // park Z: slot xpad(k) = Z_0[k], Z_1[k]
         gb.sync();
         if (PAD) issue_loads(item + gridDim.x);
-        if (live) {
-            // X[k] * scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = 0..NF.
-            // Four lanes (column c, row r) produce the 32-byte slot of one tile: lane = 4 j + 2 r + c.
-            const float* zb = reinterpret_cast<const float*>(buf);         // Z_r[k] = (zb[4 xpad(k) + r], zb[4 xpad(k) + 2 + r])
-            float2* ob = a.out + b * a.out_bstride + (size_t)y0 * 2;
-            const int c = p & 1, r = (p >> 1) & 1;
-            auto emit = [&](int m) {
-                const int k = 2 * m + c;
-                float2 x = make_float2(0.f, 0.f);
-                if (k <= NF) {
-                    const int ik = k & (NF - 1), im = (NF - k) & (NF - 1);
-                    const float2 w = __ldg(a.twist + k);
-                    const float2 za = make_float2(zb[4 * xpad(ik) + r], zb[4 * xpad(ik) + 2 + r]);
-                    const float2 zm = make_float2(zb[4 * xpad(im) + r], -zb[4 * xpad(im) + 2 + r]);
-                    const float2 s = cadd(za, zm), d = cmul(csub(za, zm), w);
-                    x = make_float2((s.x + d.y) * a.scale, (s.y - d.x) * a.scale);
-                }
-                stg2(ob + (size_t)m * a.ny * 2 + r * 2 + c, x);
-            };
-            if (P >= 4) {
+        // X[k] scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = p + e P (and k = NF from Z[0])
+        C2 xn = c2zero();
 #pragma unroll
-                for (int i = 0; i < 2 * kE; ++i) emit((p >> 2) + i * (P / 4));
-                if (p < 4) emit(NF / 2);
-            } else {                              // tiny transforms: fewer than 4 threads per row pair
-                for (int q = p; q < 4 * (NF / 2 + 1); q += P) {
-                    const int cc = q & 1, rr = (q >> 1) & 1, m = q >> 2, k = 2 * m + cc;
-                    float2 x = make_float2(0.f, 0.f);
-                    if (k <= NF) {
-                        const int ik = k & (NF - 1), im = (NF - k) & (NF - 1);
-                        const float2 w = __ldg(a.twist + k);
-                        const float2 za = make_float2(zb[4 * xpad(ik) + rr], zb[4 * xpad(ik) + 2 + rr]);
-                        const float2 zm = make_float2(zb[4 * xpad(im) + rr], -zb[4 * xpad(im) + 2 + rr]);
-                        const float2 s = cadd(za, zm), d = cmul(csub(za, zm), w);
-                        x = make_float2((s.x + d.y) * a.scale, (s.y - d.x) * a.scale);
-                    }
-                    stg2(ob + (size_t)m * a.ny * 2 + rr * 2 + cc, x);
-                }
+        for (int e = 0; e < kE; ++e) {
+            const int k = p + e * P;
+            const C2 zm = unpack(buf[xpad((NF - k) & (NF - 1))]);
+            const float2 w = __ldg(a.twist + k);
+            C2 s, d0;
+            s.re = f2add(v[e].re, zm.re);  s.im = f2sub(v[e].im, zm.im);
+            d0.re = f2sub(v[e].re, zm.re); d0.im = f2add(v[e].im, zm.im);
+            const C2 d = c2mul_dir<false>(d0, w);
+            if (e == 0 && p == 0) {               // k = 0: twist[NF] = -1 gives X[NF] from the same Z[0]
+                xn.re = f2mul(f2sub(s.re, d.im), f2bc(a.scale));
+                xn.im = f2mul(f2add(s.im, d.re), f2bc(a.scale));
             }
+            v[e].re = f2mul(f2add(s.re, d.im), f2bc(a.scale));
+            v[e].im = f2mul(f2sub(s.im, d.re), f2bc(a.scale));
         }
-        gb.sync();
+        gb.sync();                                // every mirror slot has been read: the buffer is free again
+        if (live) {
+            // (X_0[k], X_1[k]) -> block (k >> 1, y0 / 2), half k & 1
+            auto slot = [](const C2& x) { return make_float4(x.re.x, x.im.x, x.re.y, x.im.y); };
+            float4* ob = reinterpret_cast<float4*>(a.out) + ((size_t)b * (NF / 2 + 1) * (a.ny / 2) + rp) * 2;
+#pragma unroll
+            for (int e = 0; e < kE; ++e) {
+                const int k = p + e * P;
+                stg4(ob + (size_t)(k >> 1) * a.ny + (k & 1), slot(v[e]));
+            }
+            if (p == 0) stg4(ob + (size_t)(NF / 2) * a.ny, slot(xn));
+        }
     }
 }
 

@@ -2,12 +2,14 @@
 
 // ------------------------------------------------------------------------------------------------
 struct ConvColsArgs {
-    float2* t;            // [nb][ntile][NF][2] in place
+    CUtensorMap tmap;     // column map of t (tmap.h)
+    float2* t;            // [nb][ntile][NF/2][2][2] block layout (tmap.h), in place
     const float* wt;      // [nb][ntile][2 (column in tile)][NF (q)][2 (even, odd bin)]
-    int ntile;
-    int items_per_batch;  // ceil(2 ntile / G)
+    int ncols;            // columns that exist per batch (row length + 1)
+    int ntile;            // tiles per batch
+    int items_per_batch;  // ceil(ncols / G)
     int nitems;           // items_per_batch * nb
-    size_t t_bstride, w_bstride;
+    size_t w_bstride;
     const float4* tw;
     const float2* twist;  // exp(-2 pi i n/(2 NF))
 };
@@ -16,22 +18,21 @@ struct ConvColsArgs {
 // and the odd output bins of the length-2NF transform of the zero-extended column,
 //   even bins = FFT_NF(x),  odd bins = FFT_NF(x twist^n);   after . W and the inverse transforms
 //   y[n] = IFFT_NF(E')[n] + conj(twist^n) IFFT_NF(O')[n]
-// so input, twiddles and the final combination are all thread-local.  Work item = (tile, column);
-// the two columns of a tile go to neighbouring CTAs, which share the tile's sectors through L2.
+// so input, twiddles and the final combination are all thread-local.
 //
-// Global reads never stall the arithmetic: one 8 NF-byte staging buffer per group is time-shared by
-//   the column of the NEXT item  (cp.async, every thread copies exactly the 16 samples it will use, so
-//                                 no barrier is needed; issued once the weights have been consumed,
-//                                 in flight during the inverse transforms), and
-//   the weights of THIS item     (one bulk TMA copy of the contiguous 8 NF-byte weight column, issued
-//                                 after the first exchange barrier of the forward transform -- every
-//                                 thread has picked up its samples by then -- and awaited on an
-//                                 mbarrier after the forward transform).
+// Global reads never stall the arithmetic and cost no LSU instructions: one 8 NF-byte staging buffer
+// per group is filled by the TMA unit (the weights by one bulk copy, the column -- 16-byte pieces at a
+// 32-byte stride in the block layout -- by tensor copies that land it contiguously), alternately with
+//   the weights of THIS item     (issued after the first exchange barrier of the forward transform --
+//                                 every thread has picked up its samples by then -- and awaited
+//                                 after the forward transform), and
+//   the column of the NEXT item  (issued after the first exchange barrier of the inverse transform --
+//                                 the weights have been consumed -- in flight during the rest of it).
 template <int NF> struct ColsGeo : Geo<NF, 1, NF / 2> {};
 
 template <int NF>
 __global__ void __launch_bounds__(ColsGeo<NF>::THREADS, ColsGeo<NF>::MINB)
-conv_cols_kernel(ConvColsArgs a) {
+conv_cols_kernel(const __grid_constant__ ConvColsArgs a) {
     using GEO = ColsGeo<NF>;
     constexpr int P = GEO::P;
     extern __shared__ __align__(128) float4 smem4[];
@@ -47,33 +48,45 @@ conv_cols_kernel(ConvColsArgs a) {
     // rounded factors costs a measurable part of the CG error budget and no time is gained by it)
     auto twist_e = [&](int e) { return __ldg(a.twist + p + e * P); };
 
-    auto column = [&](int item, bool& live, float2*& col, const float*& w) {
-        const int b = item / a.items_per_batch;
-        const int mc = (item - b * a.items_per_batch) * GEO::G + g;      // 2 m + c
-        live = item < a.nitems && mc < 2 * a.ntile;
-        col = a.t + b * a.t_bstride + (size_t)(mc >> 1) * NF * 2 + (mc & 1);      // stride 2 float2 per row
-        w = a.wt + b * a.w_bstride + (size_t)mc * NF * 2;
+    constexpr int BOXR = tma_box_pairs(NF), NCOPY = tma_col_copies(NF);
+    auto column = [&](int item, bool& live, int& b, int& kx, const float*& w) {
+        b = item / a.items_per_batch;
+        kx = (item - b * a.items_per_batch) * GEO::G + g;
+        live = item < a.nitems && kx < a.ncols;
+        w = a.wt + b * a.w_bstride + (size_t)kx * NF * 2;
     };
-    auto stage_column = [&](int item) {
-        bool live; float2* col; const float* w;
-        column(item, live, col, w);
-        if (live) {
-#pragma unroll
-            for (int e = 0; e < kE; ++e) cp_async8(stage + p + e * P, col + 2 * (p + e * P));
+    auto fetch_weights = [&](const void* src, bool live) {       // one bulk copy of 8 NF bytes into the staging buffer
+        if (p == 0 && live) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, NF * 8);
+            bulk_g2s(stage, src, NF * 8, bar);
         }
-        cp_async_commit();
+        __syncwarp();   // the issuing lane must not be left behind a warp that spins on the mbarrier
     };
-    stage_column(blockIdx.x);
-    __syncthreads();
+    auto fetch_column = [&](int b, int kx, bool live) {          // column kx lands as NF contiguous samples
+        if (p == 0 && live) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, NF * 8);
+            for (int j = 0; j < NCOPY; ++j) tensor_g2s_5d(stage + 2 * BOXR * j, &a.tmap, 0, kx & 1, BOXR * j, kx >> 1, b, bar);
+        }
+        __syncwarp();
+    };
     unsigned parity = 0;
+    __syncthreads();
+    {
+        bool live; int b, kx; const float* w;
+        column(blockIdx.x, live, b, kx, w);
+        fetch_column(b, kx, live);
+    }
 
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
-        bool live; float2* col; const float* w;
-        column(item, live, col, w);
+        bool live; int b, kx; const float* w;
+        column(item, live, b, kx, w);
 
         C2 v[kE];
-        cp_async_wait_all();
         if (live) {
+            mbar_wait(bar, parity);
+            parity ^= 1u;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const float2 x = stage[p + e * P];
@@ -85,18 +98,9 @@ conv_cols_kernel(ConvColsArgs a) {
         }
         // forward transforms; the weights start to arrive behind the first barrier
         stage_compute<NF, 0, false>(v, p, tws);
-        if constexpr (plan_stages(NF) > 1) {
-            stage_scatter2<NF, 0>(v, p, buf);
-            gb.sync();
-        } else {
-            gb.sync();
-        }
-        if (p == 0 && live) {
-            fence_proxy_async();
-            mbar_expect_tx(bar, NF * 8);
-            bulk_g2s(stage, w, NF * 8, bar);
-        }
-        __syncwarp();   // the issuing lane must not be left behind a warp that spins on the mbarrier
+        if constexpr (plan_stages(NF) > 1) stage_scatter2<NF, 0>(v, p, buf);
+        gb.sync();
+        fetch_weights(w, live);
         if constexpr (plan_stages(NF) > 1) {
             canon_gather2<NF>(v, p, buf);
             gb.sync();
@@ -104,38 +108,50 @@ conv_cols_kernel(ConvColsArgs a) {
         }
         if (live) {
             mbar_wait(bar, parity);
+            parity ^= 1u;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const float2 ww = stage[p + e * P];               // (even-bin weight, odd-bin weight)
                 v[e].re = f2mul(v[e].re, ww);
                 v[e].im = f2mul(v[e].im, ww);
             }
-            parity ^= 1u;
         }
-        // the staging slots a thread has just read are its own: refill them with the next column
-        stage_column(item + gridDim.x);
-        pair_fft<NF, true>(v, p, buf, tws, gb);
+        // inverse transforms; the next column starts to arrive behind the first barrier
+        stage_compute<NF, 0, true>(v, p, tws);
+        if constexpr (plan_stages(NF) > 1) stage_scatter2<NF, 0>(v, p, buf);
+        gb.sync();
+        {
+            bool nlive; int nb_, nkx; const float* nw;
+            column(item + gridDim.x, nlive, nb_, nkx, nw);
+            fetch_column(nb_, nkx, nlive);
+        }
+        if constexpr (plan_stages(NF) > 1) {
+            canon_gather2<NF>(v, p, buf);
+            gb.sync();
+            pair_fft_from<NF, true, 1>(v, p, buf, tws, gb);
+        }
         if (live) {
+            // sample y of column kx: block (kx >> 1, y >> 1), position (kx & 1, y & 1)
+            float2* col = a.t + ((size_t)(b * a.ntile + (kx >> 1)) * (NF / 2)) * 4 + (kx & 1) * 2 + (p & 1);
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const float2 o = cmulc(c2get(v[e], 1), twist_e(e));
-                stg2(col + 2 * (p + e * P), make_float2(v[e].re.x + o.x, v[e].im.x + o.y));
+                stg2(col + (size_t)((p + e * P) >> 1) * 4, make_float2(v[e].re.x + o.x, v[e].im.x + o.y));
             }
         }
     }
-    cp_async_wait_all();
 }
 
 // ------------------------------------------------------------------------------------------------
 struct HartColsArgs {
-    const float2* t;      // [nb][ntile][NF][2], columns x = 0..nx/2 of the row-transformed field (NF rows)
+    const float2* t;      // [nb][ntile][NF/2][2][2] block layout: columns x = 0..nx/2 of the row-transformed field (NF rows)
     float* out;           // [nb][nx][NF]  TRANSPOSED: out[x][y] = H[y][x]
     const float* mul;     // optional [nb][nx][NF]: out = mul * (H + offset) + add
     const float* add;     // optional [nb][nx][NF]
     const float* offset;  // optional device [nb]   (mu)
     int nx;
     int items_per_batch, nitems;
-    size_t t_bstride, img_bstride;
+    size_t img_bstride;
     const float4* tw;
 };
 
@@ -162,11 +178,16 @@ hart_cols_kernel(HartColsArgs a) {
 
         C2 v[kE];
         if (live) {
-            const float4* tile = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + (size_t)m * NF;
+            // tile m = columns 2m, 2m+1: sample y at block y >> 1, position (c, y & 1)
+            const float* c0 = reinterpret_cast<const float*>(a.t + ((size_t)(b * ntile + m) * (NF / 2)) * 4);
+            const bool two = 2 * m + 1 <= a.nx / 2;            // the last pair may hold one column only
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float4 x = ldg4(tile + p + e * P);
-                v[e] = c2make(make_float2(x.x, x.y), make_float2(x.z, x.w));
+                const int y = p + e * P;
+                const float* q = c0 + 2 * ((y >> 1) * 4 + (y & 1));
+                const float2 x0 = ldg2(q);
+                const float2 x1 = two ? ldg2(q + 4) : make_float2(0.f, 0.f);
+                v[e] = c2make(x0, x1);
             }
         } else {
 #pragma unroll

@@ -3,38 +3,36 @@
 enum RowsInvMode { kPlain = 0, kMulS = 1, kEnergy = 2 };
 
 struct RowsInvArgs {
-    CUtensorMap tmap;     // tile map of t (tmap.h)
-    const float2* t;      // [nb][ntile][ny][2]
+    CUtensorMap tmap;     // row map of t (tmap.h)
+    const float2* t;      // [nb][NF/2+1][ny/2][2][2] block layout (tmap.h)
     float* out;           // [nb][ny][NF]
     const float* s;       // [nb][ny][NF]  (kMulS, kEnergy)
     const float* j;       // [nb][ny][NF]  (kEnergy)
     double* partials;     // [gridDim.x][2]  (kEnergy): sum s*c, sum j*s
     int ny, mode;
     int items_per_batch, nitems;
-    size_t t_bstride, img_bstride;
+    size_t img_bstride;
     const float4* tw;
     const float2* twist;
 };
 
-// Pipeline: the half-spectrum rows of the NEXT item are gathered by the TMA unit (tensor copies of the
-// column-pair tiles, tmap.h: 2 x 17 copies per row pair, no LSU instructions, no address arithmetic)
-// straight into the exchange buffer as soon as the transform has left it (before its last,
-// register-only stage), so the gather is in flight during that stage and the epilogue.  Landing
-// layout: row r of the pair at float2 index r * LROW + k, k = 0..NF+1.
+// Pipeline: the half spectrum of the NEXT row pair is gathered by the TMA unit (17 tensor copies of
+// 32-byte blocks, tmap.h: no LSU instructions, no address arithmetic) straight into the
+// exchange buffer as soon as the transform has left it (before its last, register-only stage), so
+// the gather is in flight during that stage and the epilogue.  Landing layout: dense 16-byte slots,
+// slot k = (Y_0[k], Y_1[k]) of the two rows, k = 0..NF.
 template <int NF>
 __global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
     using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
-    constexpr int BOX = tma_box_tiles(NF), NOPS = tma_copies(NF), LROW = 2 * BOX * NOPS;
-    constexpr bool USE_TMA = NF >= 256;            // smaller rows: boxes below the 128-byte TMA alignment -> cp.async
-    constexpr int NTILE = NF / 2 + 1;
-    static_assert(2 * LROW * 8 <= xbuf_len(NF) * 16, "landing area exceeds the exchange buffer");
+    constexpr bool USE_TMA = tma_rows_ok(NF);      // smaller rows: boxes below the 128-byte TMA alignment -> cp.async
+    constexpr int BOX = tma_box_tiles(NF), NOPS = tma_row_copies(NF);
+    static_assert(2 * BOX * NOPS <= xbuf_len(NF), "landing area exceeds the exchange buffer");
     extern __shared__ __align__(128) float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
-    const float2* land = reinterpret_cast<const float2*>(buf);      // Y_r[k] at land[r*LROW + k]
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem4 + GEO::TW + (size_t)GEO::G * GEO::GROUP_SLOTS) + g;
     const GroupBar gb = GEO::bar(g);
     load_twiddles<NF>(tws, a.tw);
@@ -48,28 +46,16 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         const int rp = (item - b * a.items_per_batch) * GEO::G + g;
         const bool live = item < a.nitems && 2 * rp < a.ny;
         if (live && !USE_TMA) {
-            const float4* tb = reinterpret_cast<const float4*>(a.t + b * a.t_bstride) + 2 * rp;
-            for (int q = p; q < 2 * NTILE; q += P) {
-                const int r = q & 1, m = q >> 1;
-                cp_async16(buf + r * (LROW / 2) + m, tb + (size_t)m * a.ny + r);
-            }
+            const float4* tb = reinterpret_cast<const float4*>(a.t) + ((size_t)b * (NF / 2 + 1) * (a.ny / 2) + rp) * 2;
+            for (int k = p; k <= NF; k += P) cp_async16(buf + k, tb + (size_t)(k >> 1) * a.ny + (k & 1));
         }
         if (!USE_TMA) cp_async_commit();
-        if (live && USE_TMA) {
-            if (p == 0) {
-                fence_proxy_async();
-                mbar_expect_tx(bar, 2 * NOPS * BOX * 16);
-            }
-            if (P >= 32) __syncwarp();
-            // the 2 NOPS copies are issued by the first lanes of the group
-            for (int q = p; q < 2 * NOPS; q += (P < 32 ? P : 32)) {
-                if (p < 32) {
-                    const int r = q / NOPS, j = q - r * NOPS;
-                    tensor_g2s_4d(buf + (r * LROW + 2 * BOX * j) / 2, &a.tmap, 0, 2 * rp + r, BOX * j, b, bar);
-                }
-            }
-            if (P >= 32) __syncwarp();
+        if (live && USE_TMA && p == 0) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, NOPS * BOX * 32);
+            for (int j = 0; j < NOPS; ++j) tensor_g2s_4d(buf + 2 * BOX * j, &a.tmap, 0, rp, BOX * j, b, bar);
         }
+        if (P >= 32) __syncwarp();
         if (live) {
             // warm L2 with the rows of s (and j) the epilogue of that item will read: P lines of 128 B
             if (a.mode != kPlain) {
@@ -99,15 +85,19 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         for (int e = 0; e < kE; ++e) {
             const int k = p + e * P;
             const float2 w = __ldg(a.twist + k);
-            float2 z[2];
-#pragma unroll
-            for (int t = 0; t < 2; ++t) {
-                float2 ya = make_float2(0.f, 0.f), ym = ya;
-                if (live) { ya = land[t * LROW + k]; ym = cconj(land[t * LROW + NF - k]); }
-                const float2 s = cadd(ya, ym), d = cmulc(csub(ya, ym), w);
-                z[t] = make_float2(s.x - d.y, s.y + d.x);
+            if (live) {
+                const float4 qa = buf[k], qm = buf[NF - k];
+                const C2 ya = c2make(make_float2(qa.x, qa.y), make_float2(qa.z, qa.w));
+                const C2 ym = c2make(make_float2(qm.x, qm.y), make_float2(qm.z, qm.w));
+                C2 s, d0;
+                s.re = f2add(ya.re, ym.re);  s.im = f2sub(ya.im, ym.im);
+                d0.re = f2sub(ya.re, ym.re); d0.im = f2add(ya.im, ym.im);
+                const C2 d = c2mul_dir<true>(d0, w);
+                v[e].re = f2sub(s.re, d.im);
+                v[e].im = f2add(s.im, d.re);
+            } else {
+                v[e] = c2zero();
             }
-            v[e] = c2make(z[0], z[1]);
         }
         gb.sync();
         pair_fft_head<NF, true>(v, p, buf, tws, gb);

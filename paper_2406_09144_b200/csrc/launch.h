@@ -16,12 +16,13 @@ int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* 
 int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb);
 
 struct PsfColsArgs {
-    const float2* t;      // [nb][ntile][2 NF][2]  row-transformed PSF, all 2 NF rows
+    const float2* t;      // [nb][ntile][NF][2][2]  row-transformed PSF, all 2 NF rows, block layout (tmap.h)
+    int ncols;            // columns that exist (nx + 1)
     float* wt;            // [nb][ntile][2][NF][2]
     float* stats;         // [nb][gridDim.x][3]: max |Im W|, min Re W, max Re W   (unscaled by fold)
     int ntile;
     float scale;          // 1 / (My Mx)
-    size_t t_bstride, w_bstride;
+    size_t w_bstride;
     const float4* tw;
     const float2* twist;
 };
