@@ -140,12 +140,24 @@ rows_fwd_kernel(RowsFwdArgs a) {
             for (int e = 0; e < NE; ++e) { xin[0][e] = xin[1][e] = make_float2(0.f, 0.f); }
         }
     };
-    if (PAD) issue_loads(blockIdx.x);
+    // warm L2 with the rows of the item after this one (a register prefetch would not fit beside the
+    // unpacking phase: the compiler spills it, and the spill stores wait for the loads)
+    auto prefetch_rows = [&](int item) {
+        const int b = item / a.items_per_batch;
+        const int rp = (item - b * a.items_per_batch) * GEO::G + g;
+        if (item < a.nitems && 2 * rp < a.ny) {
+            for (int i = p * 32; i < 2 * NXR; i += P * 32) {
+                prefetch_l2(a.in + b * a.in_bstride + (size_t)(2 * rp) * NXR + i);
+                if (a.mul) prefetch_l2(a.mul + b * a.mul_bstride + (size_t)(2 * rp) * NXR + i);
+            }
+        }
+    };
 
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const int b = item / a.items_per_batch;
         const int rp = (item - b * a.items_per_batch) * GEO::G + g;       // row pair
-        if (!PAD) issue_loads(item);              // unpadded rows fill every register slot: no room to prefetch
+        issue_loads(item);
+        prefetch_rows(item + gridDim.x);
         const bool live = 2 * rp < a.ny;
         const int y0 = 2 * rp;
 
@@ -165,7 +177,6 @@ rows_fwd_kernel(RowsFwdArgs a) {
         pair_fft<NF, false>(v, p, buf, tws, gb);
         canon_scatter2<NF>(v, p, buf);            // park Z: slot xpad(k) = Z_0[k], Z_1[k]
         gb.sync();
-        if (PAD) issue_loads(item + gridDim.x);
         // X[k] scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = p + e P (and k = NF from Z[0])
         C2 xn = c2zero();
 #pragma unroll
