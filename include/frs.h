@@ -101,6 +101,14 @@ int frs_cg_read_state(frs_ctx* ctx, float* r, float* p, float* q, double* scal_h
  * r, p and rr (loaded with frs_cg_load), computes q = M p, alpha, x, r, beta, p. */
 int frs_cg_load(frs_ctx* ctx, const float* r, const float* p, double rr_host);
 int frs_cg_step(frs_ctx* ctx, float* x, int with_prior);
+/* The same iteration split around the one exchange step of a channel-sharded run (each
+ * rank holds a subset of the channels, latent vectors are replicated).  frs_cg_step_begin computes
+ * the likelihood part q = J^T C J p of THIS context's channels (no prior term) into ctx-owned storage
+ * and returns its DEVICE pointer in *d_q ([nfield][ny][nx]); the caller sums q over the ranks in place
+ * (ncclAllReduce on the ctx's stream); frs_cg_step_end adds the prior term (q += p if with_prior) and
+ * finishes the iteration exactly as frs_cg_step (alpha, x, r, beta, p).  Errors as frs_cg_step. */
+int frs_cg_step_begin(frs_ctx* ctx, float** d_q);
+int frs_cg_step_end(frs_ctx* ctx, float* x, int with_prior);
 
 /* ---- host-buffer entry points (end-to-end measurements: copies are part of the call) -------- */
 

@@ -34,6 +34,8 @@ EXPORTS = {
     "frs_cg_read_state": (_i, [_vp, _vp, _vp, _vp, C.POINTER(_d)]),
     "frs_cg_load": (_i, [_vp, _vp, _vp, _d]),
     "frs_cg_step": (_i, [_vp, _vp, _i]),
+    "frs_cg_step_begin": (_i, [_vp, C.POINTER(_vp)]),
+    "frs_cg_step_end": (_i, [_vp, _vp, _i]),
     "frs_sky_metric_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_psf_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_launch_count": (C.c_longlong, [_vp]),
@@ -92,6 +94,18 @@ def _ptr(t, dtype=None, numel=None, name="tensor"):
     if numel is not None and t.numel() != numel:
         raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
     return t.data_ptr()
+
+
+class _DevicePtr:
+    """Minimal __cuda_array_interface__ carrier so that torch can view library-owned device memory."""
+
+    def __init__(self, ptr, shape):
+        self.__cuda_array_interface__ = {"data": (int(ptr), False), "shape": tuple(shape), "typestr": "<f4", "version": 2}
+
+
+def _device_view(ptr, shape, device):
+    import torch
+    return torch.as_tensor(_DevicePtr(ptr, shape), device=device)
 
 
 class Context:
@@ -210,6 +224,16 @@ class Context:
 
     def cg_step(self, x, with_prior=True):
         self._ck(lib().frs_cg_step(self._h, _ptr(x, self.f32, self.nfield * self.npix, "x"), int(with_prior)))
+
+    def cg_step_begin(self):
+        """Likelihood part q = J^T C J p of this context's channels; returns q as a tensor VIEW of the
+        ctx-owned device buffer (to be summed over ranks in place), see frs_cg_step_begin."""
+        q = _vp()
+        self._ck(lib().frs_cg_step_begin(self._h, C.byref(q)))
+        return _device_view(q.value, (self.nfield, self.ny, self.nx), self.device)
+
+    def cg_step_end(self, x, with_prior=True):
+        self._ck(lib().frs_cg_step_end(self._h, _ptr(x, self.f32, self.nfield * self.npix, "x"), int(with_prior)))
 
     def cg_read_state(self):
         """Copies of the ctx-owned r, p, q (torch) and the scalar block (numpy float64[8]:

@@ -177,6 +177,18 @@ __global__ void __launch_bounds__(kEwThreads) cg_update_p_kernel(float* __restri
     }
 }
 
+// q += p (prior term of the metric, added after the cross-rank sum of the likelihood part)
+__global__ void __launch_bounds__(kEwThreads) add_inplace_kernel(float* __restrict__ q, const float* __restrict__ p, size_t n) {
+    const size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (i + 3 < n) {
+        float4 a = *reinterpret_cast<float4*>(q + i);
+        const float4 b = *reinterpret_cast<const float4*>(p + i);
+        a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+        *reinterpret_cast<float4*>(q + i) = a;
+    } else {
+        for (size_t j = i; j < n; ++j) q[j] += p[j];
+    }
+}
 __global__ void cg_shift_kernel(double* __restrict__ scal, double* __restrict__ hist, int k) {
     scal[kRR] = scal[kRRNew];
     if (hist) hist[k] = sqrt(scal[kRRNew]);

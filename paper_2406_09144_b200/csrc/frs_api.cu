@@ -301,11 +301,10 @@ int cg_alloc(frs_ctx* ctx) {
     return FRS_OK;
 }
 
-// one iteration from (x, r, p, scal[kRR]); leaves scal[kRR] = new <r,r>
-int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k) {
+// second half of an iteration: from q = M p to the updated (x, r, p, scal)
+int cg_iter_finish(frs_ctx* ctx, float* x, double* d_hist, int k) {
     const size_t n = (size_t)ctx->nfield * ctx->npix;
     const int nb = red_blocks(n);
-    RET(metric_apply_impl(ctx, ctx->cg_p, with_prior, ctx->cg_q));
     RET(dot(ctx, ctx->cg_p, ctx->cg_q, n, ctx->scal + kPQ));
     cg_update_xr_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(x, ctx->cg_r, ctx->cg_p, ctx->cg_q, n, ctx->scal, ctx->partials);
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, ctx->scal + kRRNew);
@@ -314,6 +313,11 @@ int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k) {
     ctx->launches += 4;
     CK(cudaGetLastError());
     return FRS_OK;
+}
+// one iteration from (x, r, p, scal[kRR]); leaves scal[kRR] = new <r,r>
+int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k) {
+    RET(metric_apply_impl(ctx, ctx->cg_p, with_prior, ctx->cg_q));
+    return cg_iter_finish(ctx, x, d_hist, k);
 }
 
 }  // namespace
@@ -607,6 +611,29 @@ int frs_cg_step(frs_ctx* ctx, float* x, int with_prior) {
     RET(check_hot(ctx, true, true));
     RET(cg_alloc(ctx));
     return cg_iter(ctx, x, with_prior, nullptr, 0);
+}
+
+int frs_cg_step_begin(frs_ctx* ctx, float** d_q) {
+    if (!ctx || !d_q) return fail(ctx, FRS_EINVAL, "frs_cg_step_begin: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, true));
+    RET(cg_alloc(ctx));
+    RET(metric_apply_impl(ctx, ctx->cg_p, 0, ctx->cg_q));
+    *d_q = ctx->cg_q;
+    return FRS_OK;
+}
+
+int frs_cg_step_end(frs_ctx* ctx, float* x, int with_prior) {
+    if (!ctx || !x || !aligned16(x)) return fail(ctx, FRS_EINVAL, "frs_cg_step_end: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, true));
+    RET(cg_alloc(ctx));
+    const size_t n = (size_t)ctx->nfield * ctx->npix;
+    if (with_prior) {
+        add_inplace_kernel<<<(unsigned)((n / 4 + kEwThreads - 1) / kEwThreads + 1), kEwThreads, 0, ctx->stream>>>(ctx->cg_q, ctx->cg_p, n);
+        ctx->launches++;
+    }
+    return cg_iter_finish(ctx, x, nullptr, 0);
 }
 
 int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,

@@ -289,6 +289,23 @@ def test_cg_free_running_within_horizon_and_literal(frs):
     assert h[20] < h[0] and abs(h[0] - np.linalg.norm(bh)) <= 1e-6 * h[0]
 
 
+def test_cg_split_step_equals_fused_step(frs):
+    """frs_cg_step_begin / frs_cg_step_end (the channel-sharded iteration, world size 1: nothing to
+    sum) reproduces frs_cg_step bit for bit."""
+    import torch
+    w, ctx, b, ap = _cg_problem(frs, ("c1",))
+    xa, xb = torch.zeros_like(b), torch.zeros_like(b)
+    ctx.cg_solve(b, xa, 0)
+    for _ in range(4):
+        ctx.cg_step(xa, True)
+    ctx.cg_solve(b, xb, 0)
+    for _ in range(4):
+        q = ctx.cg_step_begin()
+        assert q.shape == b.shape and q.data_ptr() % 16 == 0
+        ctx.cg_step_end(xb, True)
+    assert torch.equal(xa, xb)
+
+
 def test_cg_literal_on_well_conditioned_companion(frs):
     """config 1b (sigma = 0.1 peak): rel L2(x_20) <= 1e-4 literally."""
     import torch
