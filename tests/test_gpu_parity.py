@@ -291,7 +291,7 @@ def test_cg_free_running_within_horizon_and_literal(frs):
 
 def test_cg_split_step_equals_fused_step(frs):
     """frs_cg_step_begin / frs_cg_step_end (the channel-sharded iteration, world size 1: nothing to
-    sum) reproduces frs_cg_step bit for bit."""
+    sum) reproduces frs_cg_step up to the rounding of the separately added prior term."""
     import torch
     w, ctx, b, ap = _cg_problem(frs, ("c1",))
     xa, xb = torch.zeros_like(b), torch.zeros_like(b)
@@ -303,7 +303,7 @@ def test_cg_split_step_equals_fused_step(frs):
         q = ctx.cg_step_begin()
         assert q.shape == b.shape and q.data_ptr() % 16 == 0
         ctx.cg_step_end(xb, True)
-    assert torch.equal(xa, xb)
+    assert rel(xb.cpu().numpy(), xa.cpu().numpy()) <= TOL
 
 
 def test_cg_literal_on_well_conditioned_companion(frs):
