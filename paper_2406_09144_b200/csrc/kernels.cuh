@@ -94,9 +94,11 @@ struct RowsFwdArgs {
     const float2* twist;  // exp(-2 pi i k/(2 NF)), k = 0..NF
 };
 
-// One group (P threads) transforms rows y0, y0+1 together.  Software pipeline: the loads of the next
-// item are issued into registers as soon as the transform has left them, so they are in flight while
-// this item's spectrum is unpacked and stored.
+// One group (P threads) transforms rows y0, y0+1 together.  Software pipeline (PAD): the two input rows
+// (and the two rows of the multiplier) of the NEXT item are pulled by bulk TMA copies into the exchange
+// buffer as soon as this item's transform has left it, so global latency never reaches the registers
+// (a register prefetch does not fit beside the unpacking phase: the compiler spills it and the spill
+// stores wait for the loads).  Unpadded rows (Hartley pass) are twice as long and load directly.
 // Unpacking X[k] from the half-length transform Z needs Z[k] (still in the thread's registers) and
 // Z[NF-k] (another thread's): Z is parked in the exchange buffer once and every thread reads its 16
 // mirror slots.  A thread then holds X[k] of both rows (16 bytes); neighbouring lanes hold
@@ -116,50 +118,79 @@ rows_fwd_kernel(RowsFwdArgs a) {
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
 
-    float2 xin[2][NE], min_[2][NE];
-    auto issue_loads = [&](int item) {
-        const int b = item / a.items_per_batch;
-        const int rp = (item - b * a.items_per_batch) * GEO::G + g;
-        if (item < a.nitems && 2 * rp < a.ny) {
-            const float* r0 = a.in + b * a.in_bstride + (size_t)(2 * rp) * NXR;
-#pragma unroll
-            for (int e = 0; e < NE; ++e) {
-                xin[0][e] = ldg2(r0 + 2 * (p + e * P));
-                xin[1][e] = ldg2(r0 + NXR + 2 * (p + e * P));
-            }
-            if (a.mul) {
-                const float* m0 = a.mul + b * a.mul_bstride + (size_t)(2 * rp) * NXR;
-#pragma unroll
-                for (int e = 0; e < NE; ++e) {
-                    min_[0][e] = ldg2(m0 + 2 * (p + e * P));
-                    min_[1][e] = ldg2(m0 + NXR + 2 * (p + e * P));
-                }
-            }
-        } else {
-#pragma unroll
-            for (int e = 0; e < NE; ++e) { xin[0][e] = xin[1][e] = make_float2(0.f, 0.f); }
-        }
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem4 + GEO::TW + (size_t)GEO::G * GEO::GROUP_SLOTS) + g;
+    if (PAD && p == 0) mbar_init(bar, 1);
+    unsigned parity = 0;
+    const float* stg = reinterpret_cast<const float*>(buf);       // staged rows: x row 0, x row 1, mul row 0, mul row 1
+    static_assert(!PAD || 4 * NF * 4 <= xbuf_len(NF) * 16, "staged rows exceed the exchange buffer");
+    auto row_pair = [&](int item, int& b, int& rp) {
+        b = item / a.items_per_batch;
+        rp = (item - b * a.items_per_batch) * GEO::G + g;
+        return item < a.nitems && 2 * rp < a.ny;
     };
-    // warm L2 with the rows of the item after this one (a register prefetch would not fit beside the
-    // unpacking phase: the compiler spills it, and the spill stores wait for the loads)
+    auto stage_rows = [&](int item) {                              // PAD only: 2 (or 4) rows of NF floats
+        int b, rp;
+        if (row_pair(item, b, rp) && p == 0) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, (a.mul ? 4 : 2) * NF * 4);
+            bulk_g2s(buf, a.in + b * a.in_bstride + (size_t)(2 * rp) * NXR, 2 * NF * 4, bar);
+            if (a.mul) bulk_g2s(buf + NF / 2, a.mul + b * a.mul_bstride + (size_t)(2 * rp) * NXR, 2 * NF * 4, bar);
+        }
+        __syncwarp();   // the issuing lane must not be left behind a warp that spins on the mbarrier
+    };
+    // warm L2 with the rows of the item after this one (unpadded rows)
     auto prefetch_rows = [&](int item) {
-        const int b = item / a.items_per_batch;
-        const int rp = (item - b * a.items_per_batch) * GEO::G + g;
-        if (item < a.nitems && 2 * rp < a.ny) {
+        int b, rp;
+        if (row_pair(item, b, rp)) {
             for (int i = p * 32; i < 2 * NXR; i += P * 32) {
                 prefetch_l2(a.in + b * a.in_bstride + (size_t)(2 * rp) * NXR + i);
                 if (a.mul) prefetch_l2(a.mul + b * a.mul_bstride + (size_t)(2 * rp) * NXR + i);
             }
         }
     };
+    __syncthreads();
+    if (PAD) stage_rows(blockIdx.x);
 
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
-        const int b = item / a.items_per_batch;
-        const int rp = (item - b * a.items_per_batch) * GEO::G + g;       // row pair
-        issue_loads(item);
-        prefetch_rows(item + gridDim.x);
-        const bool live = 2 * rp < a.ny;
+        int b, rp;                                                 // batch, row pair
+        const bool live = row_pair(item, b, rp);
         const int y0 = 2 * rp;
+        float2 xin[2][NE], min_[2][NE];
+#pragma unroll
+        for (int e = 0; e < NE; ++e) { xin[0][e] = xin[1][e] = make_float2(0.f, 0.f); min_[0][e] = min_[1][e] = make_float2(1.f, 1.f); }
+        if (PAD) {
+            if (live) {
+                mbar_wait(bar, parity);
+                parity ^= 1u;
+#pragma unroll
+                for (int e = 0; e < NE; ++e) {
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        xin[t][e] = *reinterpret_cast<const float2*>(stg + t * NF + 2 * (p + e * P));
+                        if (a.mul) min_[t][e] = *reinterpret_cast<const float2*>(stg + (2 + t) * NF + 2 * (p + e * P));
+                    }
+                }
+            }
+            gb.sync();                                             // the staged rows have been read: the buffer is free
+        } else {
+            if (live) {
+                const float* r0 = a.in + b * a.in_bstride + (size_t)y0 * NXR;
+#pragma unroll
+                for (int e = 0; e < NE; ++e) {
+                    xin[0][e] = ldg2(r0 + 2 * (p + e * P));
+                    xin[1][e] = ldg2(r0 + NXR + 2 * (p + e * P));
+                }
+                if (a.mul) {
+                    const float* m0 = a.mul + b * a.mul_bstride + (size_t)y0 * NXR;
+#pragma unroll
+                    for (int e = 0; e < NE; ++e) {
+                        min_[0][e] = ldg2(m0 + 2 * (p + e * P));
+                        min_[1][e] = ldg2(m0 + NXR + 2 * (p + e * P));
+                    }
+                }
+            }
+            prefetch_rows(item + gridDim.x);
+        }
 
         C2 v[kE];
 #pragma unroll
@@ -167,8 +198,7 @@ rows_fwd_kernel(RowsFwdArgs a) {
             if (e < NE) {
                 float2 x[2];
 #pragma unroll
-                for (int t = 0; t < 2; ++t)
-                    x[t] = (a.mul && live) ? make_float2(xin[t][e].x * min_[t][e].x, xin[t][e].y * min_[t][e].y) : xin[t][e];
+                for (int t = 0; t < 2; ++t) x[t] = make_float2(xin[t][e].x * min_[t][e].x, xin[t][e].y * min_[t][e].y);
                 v[e] = c2make(x[0], x[1]);
             } else {
                 v[e] = c2zero();
@@ -196,6 +226,7 @@ rows_fwd_kernel(RowsFwdArgs a) {
             v[e].im = f2mul(f2sub(s.im, d.re), f2bc(a.scale));
         }
         gb.sync();                                // every mirror slot has been read: the buffer is free again
+        if (PAD) stage_rows(item + gridDim.x);
         if (live) {
             // (X_0[k], X_1[k]) -> block (k >> 1, y0 / 2), half k & 1
             auto slot = [](const C2& x) { return make_float4(x.re.x, x.im.x, x.re.y, x.im.y); };
