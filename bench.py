@@ -223,6 +223,15 @@ def run_cuda(args):
                 "unit": "GB/s", "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": b_f2, "ms_per_launch": f2_ms,
                 "pass_ms": {k: v[0] / max(1, v[1]) for k, v in prof.items() if v[1]}}
+    # the co-binding roof of the same kernel: FP32 pipe slots.  One slot = one fp32
+    # add / mul / fma per lane (a packed FFMA2 counts two); conv_cols executes 2759 slots per thread and column
+    # (SASS count at NF = 4096: 1220 packed + 319 scalar), 256 threads per column; peak = SMs x 128 lanes x clock.
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    fp_peak = sms * 128 * (clocks["sm_mhz"] if clocks and clocks.get("sm_mhz") else 1965.0) * 1e6 / 1e12
+    fp_ach = 2759.0 * 256 * (w.nx + 1) * w.nchan * (w.ny / 4096.0) / (f2_ms * 1e-3) / 1e12 if w.ny == 4096 else None
+    roofline_fp32 = {"bound": "alu", "kernel": "conv_cols_kernel", "achieved": fp_ach, "peak": fp_peak, "unit": "T fp32 lane-ops/s",
+                     "frac": (fp_ach / fp_peak) if fp_ach else None,
+                     "peak_source": "148 SMs x 128 fp32 lanes x SM clock sampled during the run (B200_PROFILING.md unit counts)"}
     ach_step = b_l1 / (ms_step * 1e-3) / 1e9
     roofline_step = {"what": "whole L1 apply (3 kernels), minimal 3-pass byte model", "bytes": b_l1, "achieved": ach_step,
                      "unit": "GB/s", "frac_of_measured_peak": ach_step / peak, "frac_of_nominal_8TBs": ach_step / 8000.0}
@@ -299,7 +308,7 @@ def run_cuda(args):
                        "l2": "no flush: a step streams 0.94 GB (inputs 2 x 67 MB rotated, 134 MB spectrum, 134 MB weights) "
                              ">> 126 MB L2",
                        "parallelism": f"replicas x{world} (single-channel path does not shard)"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_step": roofline_step,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_step": roofline_step, "roofline_fp32": roofline_fp32,
             "cpu_baseline": cpu, "extra": extra}
     print(json.dumps(line), flush=True)
     if world > 1:
