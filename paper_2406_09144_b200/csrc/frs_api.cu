@@ -203,7 +203,7 @@ int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const flo
 // one contiguous run of the transposed output -- so the transform transposes for free, and the
 // latent-space path keeps its sky-space arrays transposed instead of paying for scattered stores.
 int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul, float* out, const float* mul,
-              const float* add, const float* offset_dev, int nb) {
+              const float* add, const float* offset_dev, int nb, double* d_dot = nullptr) {
     const int ntile_h = n2 / 4 + 1;
     {
         Prof pr(ctx, kPassHartRows);
@@ -221,8 +221,14 @@ int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul
         a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = n2;
         a.img_bstride = ctx->npix;
         a.tw = ctx->tw[n1];
-        CKL(launch_hart_cols(ctx->stream, n1, a, nb));
+        a.dot_partials = (d_dot && add) ? ctx->partials : nullptr;   // <add, out> fused into the epilogue (fp64)
+        int gx = 0;
+        CKL(launch_hart_cols(ctx->stream, n1, a, nb, &gx));
         ctx->launches++;
+        if (a.dot_partials) {
+            reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, gx, 1, 0, d_dot);
+            ctx->launches++;
+        }
     }
     return FRS_OK;
 }
@@ -263,7 +269,8 @@ int sky_forward_impl(frs_ctx* ctx, const float* xi) {
     return FRS_OK;
 }
 
-int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out) {
+// d_vmv (device, optional, needs with_prior): <v, M v>, accumulated in the last pass instead of a separate dot
+int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, double* d_vmv = nullptr) {
     const Orient o = orient(ctx, true);
     RET(need_s_transposed(ctx));
     // lin_f = H[A_f v_f]   (transposed)
@@ -287,7 +294,8 @@ int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out) 
         ctx->launches++;
     }
     // out_f = A_f . H[acc_f] (+ v_f)   (transposes back to the latent layout)
-    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield));
+    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield,
+                  with_prior ? d_vmv : nullptr));
     CK(cudaGetLastError());
     return FRS_OK;
 }
@@ -302,10 +310,10 @@ int cg_alloc(frs_ctx* ctx) {
 }
 
 // second half of an iteration: from q = M p to the updated (x, r, p, scal)
-int cg_iter_finish(frs_ctx* ctx, float* x, double* d_hist, int k) {
+int cg_iter_finish(frs_ctx* ctx, float* x, double* d_hist, int k, bool have_pq = false) {
     const size_t n = (size_t)ctx->nfield * ctx->npix;
     const int nb = red_blocks(n);
-    RET(dot(ctx, ctx->cg_p, ctx->cg_q, n, ctx->scal + kPQ));
+    if (!have_pq) RET(dot(ctx, ctx->cg_p, ctx->cg_q, n, ctx->scal + kPQ));
     cg_update_xr_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(x, ctx->cg_r, ctx->cg_p, ctx->cg_q, n, ctx->scal, ctx->partials);
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, ctx->scal + kRRNew);
     cg_update_p_kernel<<<nb, kEwThreads, 0, ctx->stream>>>(ctx->cg_p, ctx->cg_r, n, ctx->scal, ctx->scal + kBeta);
@@ -316,8 +324,9 @@ int cg_iter_finish(frs_ctx* ctx, float* x, double* d_hist, int k) {
 }
 // one iteration from (x, r, p, scal[kRR]); leaves scal[kRR] = new <r,r>
 int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k) {
-    RET(metric_apply_impl(ctx, ctx->cg_p, with_prior, ctx->cg_q));
-    return cg_iter_finish(ctx, x, d_hist, k);
+    // with the prior term the last Hartley pass has p and q = M p side by side: <p, q> comes out of its epilogue
+    RET(metric_apply_impl(ctx, ctx->cg_p, with_prior, ctx->cg_q, with_prior ? ctx->scal + kPQ : nullptr));
+    return cg_iter_finish(ctx, x, d_hist, k, with_prior != 0);
 }
 
 }  // namespace

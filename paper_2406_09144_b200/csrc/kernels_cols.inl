@@ -149,6 +149,7 @@ struct HartColsArgs {
     const float* mul;     // optional [nb][nx][NF]: out = mul * (H + offset) + add
     const float* add;     // optional [nb][nx][NF]
     const float* offset;  // optional device [nb]   (mu)
+    double* dot_partials; // optional [gridDim.x]: sum over the CTA's outputs of out * add (fp64) -- <v, M v> of a CG step
     int nx;
     int items_per_batch, nitems;
     size_t img_bstride;
@@ -168,6 +169,7 @@ hart_cols_kernel(HartColsArgs a) {
     float4* buf = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
     const int ntile = a.nx / 4 + 1;
     const GroupBar gb = GEO::bar(g);
+    double dacc = 0.0;
     load_twiddles<NF>(tws, a.tw);
     __syncthreads();
 
@@ -210,17 +212,41 @@ hart_cols_kernel(HartColsArgs a) {
                     const float2 f = c2get(v[e], c);
                     float h0 = f.x - f.y + off;
                     if (a.mul) h0 *= ldg1(a.mul + col0 + y);
-                    if (a.add) h0 += ldg1(a.add + col0 + y);
+                    if (a.add) {
+                        const float ad = ldg1(a.add + col0 + y);
+                        h0 += ad;
+                        if (a.dot_partials) dacc += (double)h0 * (double)ad;
+                    }
                     a.out[col0 + y] = h0;
                     if (mirror) {
                         float h1 = f.x + f.y + off;
                         if (a.mul) h1 *= ldg1(a.mul + col1 + ym);
-                        if (a.add) h1 += ldg1(a.add + col1 + ym);
+                        if (a.add) {
+                            const float ad = ldg1(a.add + col1 + ym);
+                            h1 += ad;
+                            if (a.dot_partials) dacc += (double)h1 * (double)ad;
+                        }
                         a.out[col1 + ym] = h1;
                     }
                 }
             }
         }
         gb.sync();
+    }
+    if (a.dot_partials) {
+        // fixed-order block reduction: warp shuffle tree, then warp 0 over the per-warp sums
+        __shared__ double dred[32];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) dacc += __shfl_down_sync(0xffffffffu, dacc, o);
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+        if (l == 0) dred[w] = dacc;
+        __syncthreads();
+        if (w == 0) {
+            const int nw = blockDim.x >> 5;
+            double x = l < nw ? dred[l] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+            if (l == 0) a.dot_partials[blockIdx.x] = x;
+        }
     }
 }

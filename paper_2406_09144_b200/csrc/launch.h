@@ -13,7 +13,7 @@ inline bool valid_nf(int nf) { return nf >= 16 && nf <= 4096 && (nf & (nf - 1)) 
 int launch_rows_fwd(cudaStream_t st, int nf, bool pad, const RowsFwdArgs& a, int nb);
 int launch_conv_cols(cudaStream_t st, int nf, const ConvColsArgs& a, int nb);
 int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* grid_x);
-int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb);
+int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb, int* grid_x = nullptr);
 
 struct PsfColsArgs {
     const float2* t;      // [nb][ntile][NF][2][2]  row-transformed PSF, all 2 NF rows, block layout (tmap.h)
