@@ -34,8 +34,8 @@ struct frs_ctx {
     float *wt = nullptr, *wtT = nullptr, *dirty = nullptr, *dirtyT = nullptr, *amp = nullptr, *s = nullptr, *sT = nullptr;
     bool s_ok = false, sT_ok = false;
     float *d_mu = nullptr, *d_lognu = nullptr;
-    float2 *T = nullptr, *Th = nullptr;
-    struct MapKey { const void* p; int rows, nf, nb; CUtensorMap row, col; };
+    float2 *T = nullptr, *T2 = nullptr, *Th = nullptr;   // T: block layout (rows_fwd -> conv_cols); T2: columns (conv_cols -> rows_inv)
+    struct MapKey { const void* p; int rows, nf, nb; CUtensorMap row, col; };   // col: of T; row: columns map of T2
     std::vector<MapKey> maps;  // spectrum tensor maps (tmap.h), built on first use
     float *lin = nullptr, *img = nullptr, *acc = nullptr;
     float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
@@ -115,6 +115,7 @@ size_t max2(size_t a, size_t b) { return a > b ? a : b; }
 int ensure_scratch(frs_ctx* ctx) {
     const size_t np = ctx->npix, ny = ctx->ny, nx = ctx->nx;
     RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
+    RET(dev_alloc(ctx, &ctx->T2, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
     RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * max2((nx / 4 + 1) * ny, (ny / 4 + 1) * nx) * 2));
     RET(dev_alloc(ctx, &ctx->lin, 2 * np));
     RET(dev_alloc(ctx, &ctx->acc, 2 * np));
@@ -155,7 +156,9 @@ int spectrum_maps(frs_ctx* ctx, const float2* T, int rows, int nf, int nb, CUten
             return FRS_OK;
         }
     frs_ctx::MapKey k{T, rows, nf, nb, {}, {}};
-    if (make_spectrum_maps(&k.row, &k.col, T, rows, nf, nb)) return fail(ctx, FRS_ECUDA, "cuTensorMapEncodeTiled failed");
+    CUtensorMap unused;
+    if (make_spectrum_maps(&unused, &k.col, T, rows, nf, nb) || make_columns_map(&k.row, ctx->T2, rows, nf, nf + 2, nb))
+        return fail(ctx, FRS_ECUDA, "cuTensorMapEncodeTiled failed");
     ctx->maps.push_back(k);
     if (row) *row = k.row;
     if (col) *col = k.col;
@@ -176,7 +179,7 @@ int conv_rows_fwd(frs_ctx* ctx, const Orient& o, const float* in, const float* m
 int conv_cols(frs_ctx* ctx, const Orient& o) {
     Prof pr(ctx, kPassConvCols);
     ConvColsArgs a{};
-    a.t = ctx->T; a.wt = o.wt; a.ncols = o.len + 1; a.ntile = o.ntile;
+    a.t = ctx->T; a.out = ctx->T2; a.wt = o.wt; a.ncols = o.len + 1; a.ntile = o.ntile;
     RET(spectrum_maps(ctx, ctx->T, o.rows, o.len, ctx->nchan, nullptr, &a.tmap));
     a.w_bstride = (size_t)o.ntile * 2 * o.rows * 2;
     a.tw = ctx->tw[o.rows]; a.twist = ctx->twist[o.rows];
@@ -187,8 +190,8 @@ int conv_cols(frs_ctx* ctx, const Orient& o) {
 int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const float* s, const float* j, int* grid_x) {
     Prof pr(ctx, kPassRowsInv);
     RowsInvArgs a{};
-    a.t = ctx->T; a.out = out; a.s = s; a.j = j; a.partials = ctx->partials;
-    a.ny = o.rows; a.mode = mode;
+    a.t = ctx->T2; a.out = out; a.s = s; a.j = j; a.partials = ctx->partials;
+    a.ny = o.rows; a.mode = mode; a.cols = 2 * o.ntile;
     RET(spectrum_maps(ctx, ctx->T, o.rows, o.len, ctx->nchan, &a.tmap, nullptr));
     a.img_bstride = ctx->npix;
     a.tw = ctx->tw[o.len]; a.twist = ctx->twist[o.len];
@@ -381,7 +384,7 @@ void frs_destroy(frs_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     for (auto& kv : ctx->tw) cudaFree(kv.second);
     for (auto& kv : ctx->twist) cudaFree(kv.second);
-    void* ptrs[] = {ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->Th, ctx->lin, ctx->img,
+    void* ptrs[] = {ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }

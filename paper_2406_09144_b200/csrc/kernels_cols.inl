@@ -3,7 +3,8 @@
 // ------------------------------------------------------------------------------------------------
 struct ConvColsArgs {
     CUtensorMap tmap;     // column map of t (tmap.h)
-    float2* t;            // [nb][ntile][NF/2][2][2] block layout (tmap.h), in place
+    const float2* t;      // [nb][ntile][NF/2][2][2] block layout (tmap.h): input
+    float2* out;          // [nb][2 ntile][NF]: output, column kx contiguous (whole-sector, coalesced stores)
     const float* wt;      // [nb][ntile][2 (column in tile)][NF (q)][2 (even, odd bin)]
     int ncols;            // columns that exist per batch (row length + 1)
     int ntile;            // tiles per batch
@@ -131,12 +132,11 @@ conv_cols_kernel(const __grid_constant__ ConvColsArgs a) {
             pair_fft_from<NF, true, 1>(v, p, buf, tws, gb);
         }
         if (live) {
-            // sample y of column kx: block (kx >> 1, y >> 1), position (kx & 1, y & 1)
-            float2* col = a.t + ((size_t)(b * a.ntile + (kx >> 1)) * (NF / 2)) * 4 + (kx & 1) * 2 + (p & 1);
+            float2* col = a.out + ((size_t)b * 2 * a.ntile + kx) * NF + p;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const float2 o = cmulc(c2get(v[e], 1), twist_e(e));
-                stg2(col + (size_t)((p + e * P) >> 1) * 4, make_float2(v[e].re.x + o.x, v[e].im.x + o.y));
+                stg2(col + e * P, make_float2(v[e].re.x + o.x, v[e].im.x + o.y));
             }
         }
     }

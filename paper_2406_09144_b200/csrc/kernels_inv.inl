@@ -3,8 +3,9 @@
 enum RowsInvMode { kPlain = 0, kMulS = 1, kEnergy = 2 };
 
 struct RowsInvArgs {
-    CUtensorMap tmap;     // row map of t (tmap.h)
-    const float2* t;      // [nb][NF/2+1][ny/2][2][2] block layout (tmap.h)
+    CUtensorMap tmap;     // columns map of t (tmap.h)
+    const float2* t;      // [nb][cols][ny]: column kx contiguous (written by conv_cols)
+    int cols;             // allocated columns per batch
     float* out;           // [nb][ny][NF]
     const float* s;       // [nb][ny][NF]  (kMulS, kEnergy)
     const float* j;       // [nb][ny][NF]  (kEnergy)
@@ -17,7 +18,7 @@ struct RowsInvArgs {
 };
 
 // Pipeline: the half spectrum of the NEXT row pair is gathered by the TMA unit (17 tensor copies of
-// 32-byte blocks, tmap.h: no LSU instructions, no address arithmetic) straight into the
+// 16-byte pieces of the column-contiguous array conv_cols wrote, tmap.h: no LSU instructions) straight into the
 // exchange buffer as soon as the transform has left it (before its last, register-only stage), so
 // the gather is in flight during that stage and the epilogue.  Landing layout: dense 16-byte slots,
 // slot k = (Y_0[k], Y_1[k]) of the two rows, k = 0..NF.
@@ -27,8 +28,8 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
     using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
     constexpr bool USE_TMA = tma_rows_ok(NF);      // smaller rows: boxes below the 128-byte TMA alignment -> cp.async
-    constexpr int BOX = tma_box_tiles(NF), NOPS = tma_row_copies(NF);
-    static_assert(2 * BOX * NOPS <= xbuf_len(NF), "landing area exceeds the exchange buffer");
+    constexpr int BOX = tma_box_bins(NF), NOPS = tma_bin_copies(NF);
+    static_assert(BOX * NOPS <= xbuf_len(NF), "landing area exceeds the exchange buffer");
     extern __shared__ __align__(128) float4 smem4[];
     float4* tws = smem4;
     const int g = threadIdx.x / P, p = threadIdx.x % P;
@@ -46,14 +47,14 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         const int rp = (item - b * a.items_per_batch) * GEO::G + g;
         const bool live = item < a.nitems && 2 * rp < a.ny;
         if (live && !USE_TMA) {
-            const float4* tb = reinterpret_cast<const float4*>(a.t) + ((size_t)b * (NF / 2 + 1) * (a.ny / 2) + rp) * 2;
-            for (int k = p; k <= NF; k += P) cp_async16(buf + k, tb + (size_t)(k >> 1) * a.ny + (k & 1));
+            const float4* tb = reinterpret_cast<const float4*>(a.t + ((size_t)b * a.cols) * a.ny) + rp;
+            for (int k = p; k <= NF; k += P) cp_async16(buf + k, tb + (size_t)k * (a.ny / 2));
         }
         if (!USE_TMA) cp_async_commit();
         if (live && USE_TMA && p == 0) {
             fence_proxy_async();
-            mbar_expect_tx(bar, NOPS * BOX * 32);
-            for (int j = 0; j < NOPS; ++j) tensor_g2s_4d(buf + 2 * BOX * j, &a.tmap, 0, rp, BOX * j, b, bar);
+            mbar_expect_tx(bar, NOPS * BOX * 16);
+            for (int j = 0; j < NOPS; ++j) tensor_g2s_3d(buf + BOX * j, &a.tmap, 4 * rp, BOX * j, b, bar);
         }
         if (P >= 32) __syncwarp();
         if (live) {

@@ -7,7 +7,8 @@
 //             box {8, 1, B, 1} = bins [2 m0, 2 m0 + 2B) of one row pair -> 16-byte slots (Y_0[k], Y_1[k])
 //   col map  (5-D floats): d0 = 4 floats of a piece, d1 = c (16 B), d2 = y/2 (32 B), d3 = m, d4 = b;
 //             box {4, 1, R, 1, 1} = rows [2 r0, 2 r0 + 2R) of one column -> contiguous complex samples
-// Blocks beyond the last tile read as zero.  The driver entry point is fetched through the runtime,
+// Blocks beyond the last tile read as zero.  The column pass writes its result to a second array in plain
+// column-contiguous order (whole sectors, coalesced), which the inverse row pass gathers through a third map.  The driver entry point is fetched through the runtime,
 // so the library does not link against libcuda.
 #pragma once
 #include <cuda.h>
@@ -23,6 +24,11 @@ __host__ __device__ constexpr bool tma_rows_ok(int nf) { return nf >= 128; }
 // col map: copies of up to 256 row pairs (rows >= 32: boxes of >= 256 bytes)
 __host__ __device__ constexpr int tma_box_pairs(int rows) { return rows / 2 < 256 ? rows / 2 : 256; }
 __host__ __device__ constexpr int tma_col_copies(int rows) { return (rows / 2) / tma_box_pairs(rows); }
+
+// column-contiguous spectrum T2[b][kx][y] (what conv_cols writes): 3-D floats d0 = 2 y + {re, im}, d1 = kx (8 rows B),
+// d2 = b; box {4, B, 1} = bins [kx0, kx0 + B) of one row pair, 16 bytes per bin; 17 copies of B = nf/16 bins
+__host__ __device__ constexpr int tma_box_bins(int nf) { return nf >= 16 ? nf / 16 : 1; }
+__host__ __device__ constexpr int tma_bin_copies(int nf) { return (nf + 1 + tma_box_bins(nf) - 1) / tma_box_bins(nf); }
 
 typedef CUresult (*TmapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -60,6 +66,19 @@ inline int make_spectrum_maps(CUtensorMap* row_map, CUtensorMap* col_map, const 
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
     }
     return 0;
+}
+
+// T2: [nb][cols][rows] complex64, bins kx = 0..nf exist
+inline int make_columns_map(CUtensorMap* map, const float2* T2, int rows, int nf, int cols, int nb) {
+    TmapEncodeFn encode = tmap_encoder();
+    if (!encode) return (int)cudaErrorUnknown;
+    const cuuint64_t dims[3] = {(cuuint64_t)rows * 2, (cuuint64_t)nf + 1, (cuuint64_t)nb};
+    const cuuint64_t strides[2] = {(cuuint64_t)rows * 8, (cuuint64_t)rows * 8 * cols};
+    const cuuint32_t box[3] = {4, (cuuint32_t)tma_box_bins(nf), 1};
+    const cuuint32_t one[3] = {1, 1, 1};
+    return encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float2*>(T2), dims, strides, box, one,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
 }
 
 }  // namespace frs
