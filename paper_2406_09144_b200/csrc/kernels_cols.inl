@@ -68,8 +68,9 @@ conv_cols_kernel(const __grid_constant__ ConvColsArgs a) {
         if (p == 0 && live) {
             fence_proxy_async();
             mbar_expect_tx(bar, NF * 8);
-            for (int j = 0; j < NCOPY; ++j) tensor_g2s_5d(stage + 2 * BOXR * j, &a.tmap, 0, kx & 1, BOXR * j, kx >> 1, b, bar);
         }
+        __syncwarp();
+        if (p < NCOPY && live) tensor_g2s_5d(stage + 2 * BOXR * p, &a.tmap, 0, kx & 1, BOXR * p, kx >> 1, b, bar);   // one copy per lane
         __syncwarp();
     };
     unsigned parity = 0;

@@ -54,8 +54,10 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         if (live && USE_TMA && p == 0) {
             fence_proxy_async();
             mbar_expect_tx(bar, NOPS * BOX * 16);
-            for (int j = 0; j < NOPS; ++j) tensor_g2s_3d(buf + BOX * j, &a.tmap, 4 * rp, BOX * j, b, bar);
         }
+        if (P >= 32) __syncwarp();
+        if (live && USE_TMA && p < 32)                                // the copies are spread over the first lanes
+            for (int j = p; j < NOPS; j += (P < 32 ? P : 32)) tensor_g2s_3d(buf + BOX * j, &a.tmap, 4 * rp, BOX * j, b, bar);
         if (P >= 32) __syncwarp();
         if (live) {
             // warm L2 with the rows of s (and j) the epilogue of that item will read: P lines of 128 B
