@@ -133,6 +133,11 @@ int frs_profile_read(frs_ctx* ctx, double ms[5], long long launches[5]);
 /* Replays the register/shared-memory FFT stage logic thread by thread on the CPU for an n-point
  * transform (n a power of two in [16, 4096]); in/out: interleaved complex float [n]. */
 int frs_selftest_fft_host(int n, int inverse, const float* in, float* out);
+/* Geometry of the TMA tensor copies that feed the row and column passes (csrc/tmap.h), for rows of nf
+ * bins and columns of `rows` samples (powers of two, nf >= 16, rows >= 32; else FRS_EINVAL).  out (HOST
+ * int[6]): bins per row-gather copy, copies per row pair, row pairs per column copy, copies per column,
+ * 16-byte slots of the exchange buffer the row gather lands in, 1 if rows of nf bins use TMA. */
+int frs_selftest_tma_geometry(int nf, int rows, int* out);
 
 #ifdef __cplusplus
 }

@@ -42,6 +42,7 @@ EXPORTS = {
     "frs_profile_enable": (_i, [_vp, _i]),
     "frs_profile_read": (_i, [_vp, C.POINTER(_d), C.POINTER(C.c_longlong)]),
     "frs_selftest_fft_host": (_i, [_i, _i, _vp, _vp]),
+    "frs_selftest_tma_geometry": (_i, [_i, _i, C.POINTER(_i)]),
 }
 
 _lib = None
@@ -94,6 +95,15 @@ def _ptr(t, dtype=None, numel=None, name="tensor"):
     if numel is not None and t.numel() != numel:
         raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
     return t.data_ptr()
+
+
+def selftest_tma_geometry(nf, rows):
+    """(box_bins, bin_copies, box_pairs, col_copies, xbuf_slots, rows_use_tma) of csrc/tmap.h."""
+    out = (_i * 6)()
+    rc = lib().frs_selftest_tma_geometry(int(nf), int(rows), out)
+    if rc != 0:
+        raise FrsError(rc, "selftest_tma_geometry")
+    return tuple(int(v) for v in out)
 
 
 class _DevicePtr:

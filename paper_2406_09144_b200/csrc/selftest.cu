@@ -5,6 +5,7 @@
 #include "../../include/frs.h"
 #include "fft_core.cuh"
 #include "tables.h"
+#include "tmap.h"
 
 namespace frs {
 struct Regs { C2 v[kE]; };
@@ -61,4 +62,17 @@ extern "C" int frs_selftest_fft_host(int n, int inverse, const float* in, float*
         case 4096: return frs::emu<4096>(inverse, i2, o2);
         default: return FRS_EINVAL;
     }
+}
+
+// Geometry of the TMA tensor copies (tmap.h) for rows of nf bins and columns of `rows` samples:
+// out = {box_bins, bin_copies, box_pairs, col_copies, xbuf_len(nf) [16-byte slots], tma usable for rows (0/1)}
+extern "C" int frs_selftest_tma_geometry(int nf, int rows, int* out) {
+    if (!out || nf < 16 || rows < 32 || (nf & (nf - 1)) || (rows & (rows - 1))) return FRS_EINVAL;
+    out[0] = frs::tma_box_bins(nf);
+    out[1] = frs::tma_bin_copies(nf);
+    out[2] = frs::tma_box_pairs(rows);
+    out[3] = frs::tma_col_copies(rows);
+    out[4] = frs::xbuf_len(nf);
+    out[5] = frs::tma_rows_ok(nf) ? 1 : 0;
+    return 0;
 }

@@ -47,6 +47,25 @@ def test_stage_logic_replayed_on_cpu_matches_dft(library, n):
         assert np.allclose(frs.selftest_fft_host(d), np.exp(-2j * np.pi * q * np.arange(n) / n), atol=2e-6)
 
 
+@pytest.mark.parametrize("nf", [16, 32, 64, 128, 256, 512, 1024, 2048, 4096])
+def test_tma_copy_geometry_covers_and_fits(library, nf):
+    """The tensor copies that feed the passes (csrc/tmap.h): the row gather must cover all nf + 1 bins of a
+    row pair, land inside the exchange buffer, and use 128-byte aligned boxes whenever TMA is used; the
+    column copies must tile a column of `rows` samples exactly."""
+    for rows in (32, 256, 4096):
+        box_bins, bin_copies, box_pairs, col_copies, xbuf, use_tma = frs.selftest_tma_geometry(nf, rows)
+        assert box_bins * bin_copies >= nf + 1                      # every bin kx = 0..nf is fetched
+        assert box_bins * (bin_copies - 1) < nf + 1                 # ... by no more copies than needed
+        assert box_bins * bin_copies <= xbuf                        # 16-byte slots: lands inside the buffer
+        assert xbuf % 8 == 0 and xbuf >= nf + nf // 16              # 128-byte multiple, padded positions fit
+        if use_tma:
+            assert (box_bins * 16) % 128 == 0                       # consecutive boxes stay 128-byte aligned
+        assert box_pairs * col_copies == rows // 2 and box_pairs <= 256
+        assert (box_pairs * 16) % 128 == 0
+    with pytest.raises(frs.FrsError):
+        frs.selftest_tma_geometry(24, 64)
+
+
 def test_selftest_rejects_bad_sizes(library):
     with pytest.raises(frs.FrsError):
         frs.selftest_fft_host(np.zeros(24, np.complex64))
