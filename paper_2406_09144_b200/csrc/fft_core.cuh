@@ -402,10 +402,12 @@ __device__ __forceinline__ void tensor_g2s_5d(void* dst_smem, const void* tmap, 
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-    unsigned ok;
+    unsigned ok, spins = 0;
     do {
         asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
                      : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        // a copy that never completes (bad map, lost issue) must fail loudly, not hang the device
+        if (!ok && ++spins > (1u << 26)) __trap();
     } while (!ok);
 }
 // cooperative copy of the packed twiddle table into shared memory (all threads; caller syncs)
