@@ -1,14 +1,14 @@
 #include "launch.h"
 namespace frs {
 // grid_x: number of CTAs launched (= number of (sum s.c, sum j.s) partial pairs in kEnergy mode)
-template <int NF>
+template <int NF, int MODE>
 static int run(cudaStream_t st, const RowsInvArgs& a0, int nb, int* grid_x) {
     using GEO = RowsGeo<NF>;
     static int ctas = 0;
     if (!ctas) {
-        cudaError_t e = set_smem(rows_inv_kernel<NF>, GEO::SMEM);
+        cudaError_t e = set_smem(rows_inv_kernel<NF, MODE>, GEO::SMEM);
         if (e != cudaSuccess) return (int)e;
-        ctas = resident_ctas(rows_inv_kernel<NF>, GEO::THREADS, GEO::SMEM);
+        ctas = resident_ctas(rows_inv_kernel<NF, MODE>, GEO::THREADS, GEO::SMEM);
         if (!ctas) return (int)cudaErrorUnknown;
     }
     RowsInvArgs a = a0;
@@ -16,11 +16,14 @@ static int run(cudaStream_t st, const RowsInvArgs& a0, int nb, int* grid_x) {
     a.nitems = a.items_per_batch * nb;
     const int grid = a.nitems < ctas ? a.nitems : ctas;
     if (grid_x) *grid_x = grid;
-    rows_inv_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
+    rows_inv_kernel<NF, MODE><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
     return (int)cudaGetLastError();
 }
 int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* grid_x) {
-#define CALL(N) return run<N>(st, a, nb, grid_x)
+#define CALL(N)                                                            \
+    return a.mode == kPlain ? run<N, kPlain>(st, a, nb, grid_x)            \
+         : a.mode == kMulS  ? run<N, kMulS>(st, a, nb, grid_x)             \
+                            : run<N, kEnergy>(st, a, nb, grid_x)
     FRS_DISPATCH_NF(nf, CALL)
 #undef CALL
     return 0;

@@ -22,7 +22,9 @@ struct RowsInvArgs {
 // exchange buffer as soon as the transform has left it (before its last, register-only stage), so
 // the gather is in flight during that stage and the epilogue.  Landing layout: dense 16-byte slots,
 // slot k = (Y_0[k], Y_1[k]) of the two rows, k = 0..NF.
-template <int NF>
+// MODE is a template parameter: the energy epilogue needs 32 more registers than the others and would
+// make every variant spill.
+template <int NF, int MODE>
 __global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
     using GEO = RowsGeo<NF>;
@@ -61,10 +63,10 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         if (P >= 32) __syncwarp();
         if (live) {
             // warm L2 with the rows of s (and j) the epilogue of that item will read: P lines of 128 B
-            if (a.mode != kPlain) {
+            if (MODE != kPlain) {
                 const size_t row = b * a.img_bstride + (size_t)(2 * rp) * NF;
                 prefetch_l2(a.s + row + 32 * p);
-                if (a.mode == kEnergy) prefetch_l2(a.j + row + 32 * p);
+                if (MODE == kEnergy) prefetch_l2(a.j + row + 32 * p);
             }
         }
     };
@@ -110,13 +112,13 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         if (live) {
             const size_t row0 = b * a.img_bstride + (size_t)y0 * NF;
             float2 sv[2][kE / 2], jv[2][kE / 2];
-            if (a.mode != kPlain) {
+            if (MODE != kPlain) {
 #pragma unroll
                 for (int t = 0; t < 2; ++t)
 #pragma unroll
                     for (int e = 0; e < kE / 2; ++e) sv[t][e] = ldg2(a.s + row0 + (size_t)t * NF + 2 * (p + e * P));
             }
-            if (a.mode == kEnergy) {
+            if (MODE == kEnergy) {
 #pragma unroll
                 for (int t = 0; t < 2; ++t)
 #pragma unroll
@@ -127,9 +129,9 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
 #pragma unroll
                 for (int e = 0; e < kE / 2; ++e) {
                     float2 c = c2get(v[e], t);
-                    if (a.mode == kMulS) {
+                    if (MODE == kMulS) {
                         c.x *= sv[t][e].x; c.y *= sv[t][e].y;
-                    } else if (a.mode == kEnergy) {
+                    } else if (MODE == kEnergy) {
                         const float2 s = sv[t][e], j = jv[t][e];
                         acc_sc += (double)s.x * (double)c.x + (double)s.y * (double)c.y;
                         acc_js += (double)j.x * (double)s.x + (double)j.y * (double)s.y;
@@ -141,7 +143,7 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         }
     }
     cp_async_wait_all();
-    if (a.mode == kEnergy) {
+    if (MODE == kEnergy) {
         // fixed-order block reduction: warp shuffle tree, then warp 0 over the per-warp sums
         __shared__ double red[2][32];
 #pragma unroll
