@@ -213,17 +213,19 @@ rows_fwd_kernel(RowsFwdArgs a) {
         for (int e = 0; e < kE; ++e) {
             const int k = p + e * P;
             const C2 zm = unpack(buf[xpad((NF - k) & (NF - 1))]);
-            const float2 w = __ldg(a.twist + k);
+            const float2 w0 = __ldg(a.twist + k);
+            const float2 w = make_float2(w0.x * a.scale, w0.y * a.scale);     // the output scale rides on the twist ...
+            const float2 sc = f2bc(a.scale);                                  // ... and on one fma per component
             C2 s, d0;
             s.re = f2add(v[e].re, zm.re);  s.im = f2sub(v[e].im, zm.im);
             d0.re = f2sub(v[e].re, zm.re); d0.im = f2add(v[e].im, zm.im);
             const C2 d = c2mul_dir<false>(d0, w);
             if (e == 0 && p == 0) {               // k = 0: twist[NF] = -1 gives X[NF] from the same Z[0]
-                xn.re = f2mul(f2sub(s.re, d.im), f2bc(a.scale));
-                xn.im = f2mul(f2add(s.im, d.re), f2bc(a.scale));
+                xn.re = f2fma(s.re, sc, f2neg(d.im));
+                xn.im = f2fma(s.im, sc, d.re);
             }
-            v[e].re = f2mul(f2add(s.re, d.im), f2bc(a.scale));
-            v[e].im = f2mul(f2sub(s.im, d.re), f2bc(a.scale));
+            v[e].re = f2fma(s.re, sc, d.im);
+            v[e].im = f2fma(s.im, sc, f2neg(d.re));
         }
         gb.sync();                                // every mirror slot has been read: the buffer is free again
         if (PAD) stage_rows(item + gridDim.x);
