@@ -136,8 +136,9 @@ conv_cols_kernel(const __grid_constant__ ConvColsArgs a) {
             float2* col = a.out + ((size_t)b * 2 * a.ntile + kx) * NF + p;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 o = cmulc(c2get(v[e], 1), twist_e(e));
-                stg2(col + e * P, make_float2(v[e].re.x + o.x, v[e].im.x + o.y));
+                // y = e + conj(twist) o, as two fma chains
+                const float2 t = twist_e(e), o = c2get(v[e], 1);
+                stg2(col + e * P, make_float2(fmaf(o.x, t.x, fmaf(o.y, t.y, v[e].re.x)), fmaf(o.y, t.x, fmaf(-o.x, t.y, v[e].im.x))));
             }
         }
     }
