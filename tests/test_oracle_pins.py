@@ -206,6 +206,58 @@ def test_hartley_closed_forms():
     assert rel(o.hartley2(z), brute) < 1e-12
 
 
+def test_golden_hand_worked_two_field_sky(golden_dir):
+    """Pins sky / log_sky / channel_coeff (R6, c-6): which field carries ln nu_c, where mu enters, and the
+    orientation of the Hartley modes -- against exponents derived by hand in tests/golden/."""
+    rows = [l.split() for l in open(os.path.join(golden_dir, "hand_sky_two_fields.txt")) if not l.startswith("#")]
+    log_s = np.array(rows, float).reshape(3, 2, 4)
+    ny, nx = 2, 4
+    xi = np.zeros((2, ny, nx)); amp = np.zeros((2, ny, nx))
+    xi[0, 0, 1], amp[0, 0, 1] = 1.0, 0.5
+    xi[1, 1, 0], amp[1, 1, 0] = 2.0, 0.25
+    mu, lognu = [0.3, -0.7], [-0.5, 0.0, 0.25]
+    assert np.allclose(o.sky(xi, amp, mu, lognu), np.exp(log_s), rtol=1e-13)
+    assert np.allclose(o.log_sky(xi, amp, mu)[0], log_s[1], atol=1e-13)              # lognu = 0: tau_0 alone
+    assert np.allclose(o.log_sky(xi, amp, mu)[1], np.array([[-0.2] * 4, [-1.2] * 4]), atol=1e-13)
+    # a single field ignores lognu altogether: s = exp(tau)
+    assert np.allclose(o.sky(xi[:1], amp[:1], mu[:1], [0.4]), np.exp(log_s[1])[None], rtol=1e-13)
+    co = o.channel_coeff(2, lognu)
+    assert np.array_equal(co, np.array([[1, -0.5], [1, 0.0], [1, 0.25]]))
+    assert np.array_equal(o.channel_coeff(1, lognu), np.ones((3, 1)))
+
+
+def test_sky_closed_form_single_modes_and_offset():
+    """xi = delta_k  =>  s[x] = exp(mu + A[k] cas(2 pi k.x/N)) on a rectangle, incl. k = 0 and Nyquist modes;
+    mu enters exactly once: field 0 scales every channel by e^c, field 1 channel c by e^(c lognu_c)."""
+    ny, nx = 4, 8
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    rng = np.random.default_rng(61)
+    a = rng.uniform(0.2, 1.0, size=(1, ny, nx))
+    for (ky, kx) in [(0, 0), (2, 0), (0, 4), (2, 4), (1, 3), (3, 7)]:
+        xi = np.zeros((1, ny, nx))
+        xi[0, ky, kx] = -1.5
+        th = 2 * np.pi * (ky * yy / ny + kx * xx / nx)
+        want = np.exp(0.37 - 1.5 * a[0, ky, kx] * (np.cos(th) + np.sin(th)))
+        assert np.allclose(o.sky(xi, a, [0.37], [0.0])[0], want, rtol=1e-12)
+    xi2, a2 = rng.normal(size=(2, ny, nx)), rng.uniform(0.1, 0.5, size=(2, ny, nx))
+    lognu = np.array([-0.3, 0.2, 0.6])
+    s0 = o.sky(xi2, a2, [0.1, -0.7], lognu)
+    c = 0.25
+    assert np.allclose(o.sky(xi2, a2, [0.1 + c, -0.7], lognu), np.exp(c) * s0, rtol=1e-12)
+    assert np.allclose(o.sky(xi2, a2, [0.1, -0.7 + c], lognu), np.exp(c * lognu)[:, None, None] * s0, rtol=1e-12)
+    # two channels with the same lognu see the same sky; distinct lognu do not
+    s_same = o.sky(xi2, a2, [0.1, -0.7], [0.2, 0.2])
+    assert np.array_equal(s_same[0], s_same[1]) and not np.allclose(s0[0], s0[1])
+
+
+def test_cg_fp32_envelope_on_a_scaled_identity():
+    """M = c 1: CG converges in one step to b/c, and the seeded relative perturbation of the operator output
+    (|u| <= 2^-24) moves x_1 by a weighted mean of u -- so the envelope is > 0 and <= 2^-24 there."""
+    b = np.random.default_rng(5).normal(size=(4, 8))
+    env = o.cg_fp32_envelope(lambda v: 3.0 * v, b, max_iter=1)
+    assert env.shape == (1,) and 0.0 < env[0] <= 2.0 ** -24
+
+
 def test_field_variance_is_sum_of_A_squared():
     """Var(lin[x]) = sum_k A[k]^2 at every pixel, exact for even A (R6)."""
     ny, nx = 8, 16
