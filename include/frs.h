@@ -133,6 +133,15 @@ int frs_profile_read(frs_ctx* ctx, double ms[5], long long launches[5]);
 /* Replays the register/shared-memory FFT stage logic thread by thread on the CPU for an n-point
  * transform (n a power of two in [16, 4096]); in/out: interleaved complex float [n]. */
 int frs_selftest_fft_host(int n, int inverse, const float* in, float* out);
+/* The same for the second FFT core (csrc/fft_dif.cuh: forward decimated in frequency, inverse decimated in
+ * time, spectrum in a permuted order), n a power of two in [256, 4096].  Forward: natural order in, the
+ * permuted spectrum sorted to natural order out; inverse: natural frequency order in, natural time order out. */
+int frs_selftest_dif_host(int n, int inverse, const float* in, float* out);
+/* Lane-by-lane analysis of that core's shared-memory exchange over two consecutive columns.  out (HOST int[6]):
+ * worst bank-conflict degree of any 128-bit access (1 = none), number of cross-thread read/write hazards not
+ * ordered by a barrier (block barrier, or warp sync between lanes of one warp), out-of-range slots, slots
+ * used, slots allocated, defects of the register <-> frequency map (0 = bijection). */
+int frs_selftest_dif_exchange(int n, int* out);
 /* Geometry of the TMA tensor copies that feed the row and column passes (csrc/tmap.h), for rows of nf
  * bins and columns of `rows` samples (powers of two, nf >= 16, rows >= 32; else FRS_EINVAL).  out (HOST
  * int[6]): bins per row-gather copy, copies per row pair, row pairs per column copy, copies per column,

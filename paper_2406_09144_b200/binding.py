@@ -43,6 +43,8 @@ EXPORTS = {
     "frs_profile_read": (_i, [_vp, C.POINTER(_d), C.POINTER(C.c_longlong)]),
     "frs_selftest_fft_host": (_i, [_i, _i, _vp, _vp]),
     "frs_selftest_tma_geometry": (_i, [_i, _i, C.POINTER(_i)]),
+    "frs_selftest_dif_host": (_i, [_i, _i, _vp, _vp]),
+    "frs_selftest_dif_exchange": (_i, [_i, C.POINTER(_i)]),
 }
 
 _lib = None
@@ -82,6 +84,26 @@ def selftest_fft_host(x, inverse=False):
     if rc != 0:
         raise FrsError(rc, "selftest")
     return out
+
+
+def selftest_dif_host(x, inverse=False):
+    """CPU replay of the DIF/DIT core of the column convolution (complex64 [n], natural order both sides)."""
+    x = np.ascontiguousarray(x, dtype=np.complex64)
+    out = np.empty_like(x)
+    rc = lib().frs_selftest_dif_host(x.shape[0], int(inverse), x.ctypes.data, out.ctypes.data)
+    if rc != 0:
+        raise FrsError(rc, "selftest_dif_host")
+    return out
+
+
+def selftest_dif_exchange(n):
+    """(worst bank-conflict degree, unordered hazards, out-of-range slots, slots used, slots allocated,
+    frequency-map defects) of the DIF core's exchange pattern."""
+    out = (_i * 6)()
+    rc = lib().frs_selftest_dif_exchange(int(n), out)
+    if rc != 0:
+        raise FrsError(rc, "selftest_dif_exchange")
+    return tuple(int(v) for v in out)
 
 
 def _ptr(t, dtype=None, numel=None, name="tensor"):

@@ -27,7 +27,8 @@ struct frs_ctx {
     cudaStream_t stream = nullptr;
     size_t npix = 0;
     int ntile = 0, ntile_h = 0;
-    std::map<int, float4*> tw;
+    std::map<int, float4*> tw;       // stage twiddles of the sorting core, per transform length
+    std::map<int, float4*> twd;      // twiddles of the DIF/DIT core (column convolution, length >= 256)
     std::map<int, float2*> twist;
     // two orientations of the sky-space arrays: natural [ny][nx] (public sky-space calls) and
     // transposed [nx][ny] (latent-space path: each 2-pass Hartley transform transposes for free)
@@ -107,6 +108,13 @@ int ensure_tables(frs_ctx* ctx, int n) {
     CK(cudaMemcpy(dts, ts.data(), ts.size() * sizeof(float2), cudaMemcpyHostToDevice));
     ctx->tw[n] = dtw;
     ctx->twist[n] = dts;
+    if (conv_cols_uses_dif(n)) {
+        std::vector<float4> td = build_dif_twiddles(n);
+        float4* dtd = nullptr;
+        CK(cudaMalloc(reinterpret_cast<void**>(&dtd), td.size() * sizeof(float4)));
+        CK(cudaMemcpy(dtd, td.data(), td.size() * sizeof(float4), cudaMemcpyHostToDevice));
+        ctx->twd[n] = dtd;
+    }
     return FRS_OK;
 }
 
@@ -182,7 +190,8 @@ int conv_cols(frs_ctx* ctx, const Orient& o) {
     a.t = ctx->T; a.out = ctx->T2; a.wt = o.wt; a.ncols = o.len + 1; a.ntile = o.ntile;
     RET(spectrum_maps(ctx, ctx->T, o.rows, o.len, ctx->nchan, nullptr, &a.tmap));
     a.w_bstride = (size_t)o.ntile * 2 * o.rows * 2;
-    a.tw = ctx->tw[o.rows]; a.twist = ctx->twist[o.rows];
+    a.tw = conv_cols_uses_dif(o.rows) ? ctx->twd[o.rows] : ctx->tw[o.rows];
+    a.twist = ctx->twist[o.rows];
     CKL(launch_conv_cols(ctx->stream, o.rows, a, ctx->nchan));
     ctx->launches++;
     return FRS_OK;
@@ -383,6 +392,7 @@ void frs_destroy(frs_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     for (auto& kv : ctx->tw) cudaFree(kv.second);
+    for (auto& kv : ctx->twd) cudaFree(kv.second);
     for (auto& kv : ctx->twist) cudaFree(kv.second);
     void* ptrs[] = {ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
@@ -395,6 +405,15 @@ static int build_transposed_weights(frs_ctx* ctx) {
     RET(dev_alloc(ctx, &ctx->wtT, (size_t)ctx->nchan * (ctx->ny / 2 + 1) * 2 * ctx->nx * 2));
     CKL(launch_weights_transpose(ctx->stream, ctx->wt, ctx->wtT, ctx->ny, ctx->nx, ctx->nchan));
     ctx->launches++;
+    // both tables exist in natural order now: bring each into the order its column pass consumes
+    if (conv_cols_uses_dif(ctx->ny)) {
+        CKL(launch_weights_permute(ctx->stream, ctx->wt, ctx->ny, 2 * ctx->ntile, ctx->nchan));
+        ctx->launches++;
+    }
+    if (conv_cols_uses_dif(ctx->nx)) {
+        CKL(launch_weights_permute(ctx->stream, ctx->wtT, ctx->nx, 2 * (ctx->ny / 2 + 1), ctx->nchan));
+        ctx->launches++;
+    }
     return FRS_OK;
 }
 

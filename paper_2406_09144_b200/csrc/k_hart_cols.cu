@@ -3,13 +3,9 @@ namespace frs {
 template <int NF>
 static int run(cudaStream_t st, const HartColsArgs& a0, int nb, int* grid_x) {
     using GEO = RowsGeo<NF>;
-    static int ctas = 0;
-    if (!ctas) {
-        cudaError_t e = set_smem(hart_cols_kernel<NF>, GEO::SMEM);
-        if (e != cudaSuccess) return (int)e;
-        ctas = resident_ctas(hart_cols_kernel<NF>, GEO::THREADS, GEO::SMEM);
-        if (!ctas) return (int)cudaErrorUnknown;
-    }
+    static int cache[kMaxDevices] = {};
+    int ctas = 0;
+    if (int e = persistent_ctas(cache, hart_cols_kernel<NF>, GEO::THREADS, GEO::SMEM, &ctas)) return e;
     HartColsArgs a = a0;
     const int ntile = a.nx / 4 + 1;
     a.items_per_batch = (ntile + GEO::G - 1) / GEO::G;

@@ -3,13 +3,9 @@ namespace frs {
 template <int NF, bool PAD>
 static int run(cudaStream_t st, const RowsFwdArgs& a0, int nb) {
     using GEO = RowsGeo<NF>;
-    static int ctas = 0;
-    if (!ctas) {
-        cudaError_t e = set_smem(rows_fwd_kernel<NF, PAD>, GEO::SMEM);
-        if (e != cudaSuccess) return (int)e;
-        ctas = resident_ctas(rows_fwd_kernel<NF, PAD>, GEO::THREADS, GEO::SMEM);
-        if (!ctas) return (int)cudaErrorUnknown;
-    }
+    static int cache[kMaxDevices] = {};
+    int ctas = 0;
+    if (int e = persistent_ctas(cache, rows_fwd_kernel<NF, PAD>, GEO::THREADS, GEO::SMEM, &ctas)) return e;
     RowsFwdArgs a = a0;
     a.items_per_batch = (a.ny / 2 + GEO::G - 1) / GEO::G;
     a.nitems = a.items_per_batch * nb;

@@ -4,13 +4,9 @@ namespace frs {
 template <int NF, int MODE>
 static int run(cudaStream_t st, const RowsInvArgs& a0, int nb, int* grid_x) {
     using GEO = RowsGeo<NF>;
-    static int ctas = 0;
-    if (!ctas) {
-        cudaError_t e = set_smem(rows_inv_kernel<NF, MODE>, GEO::SMEM);
-        if (e != cudaSuccess) return (int)e;
-        ctas = resident_ctas(rows_inv_kernel<NF, MODE>, GEO::THREADS, GEO::SMEM);
-        if (!ctas) return (int)cudaErrorUnknown;
-    }
+    static int cache[kMaxDevices] = {};
+    int ctas = 0;
+    if (int e = persistent_ctas(cache, rows_inv_kernel<NF, MODE>, GEO::THREADS, GEO::SMEM, &ctas)) return e;
     RowsInvArgs a = a0;
     a.items_per_batch = (a.ny / 2 + GEO::G - 1) / GEO::G;
     a.nitems = a.items_per_batch * nb;

@@ -77,8 +77,9 @@ psf_cols_kernel(PsfColsArgs a) {
 template <int NF>
 static int run(cudaStream_t st, const PsfColsArgs& a, int nb, int* grid_x) {
     using GEO = Geo<NF, 2>;
-    static bool attr = false;
-    if (!attr) { cudaError_t e = set_smem(psf_cols_kernel<NF>, GEO::SMEM); if (e != cudaSuccess) return (int)e; attr = true; }
+    static int cache[kMaxDevices] = {};
+    int unused = 0;
+    if (int e = persistent_ctas(cache, psf_cols_kernel<NF>, GEO::THREADS, GEO::SMEM, &unused)) return e;
     dim3 grid((a.ntile + GEO::G - 1) / GEO::G, nb);
     if (grid_x) *grid_x = grid.x;
     if (a.t) psf_cols_kernel<NF><<<grid, GEO::THREADS, GEO::SMEM, st>>>(a);
@@ -147,6 +148,32 @@ int launch_weights_transpose(cudaStream_t st, const float* wt, float* wtT, int n
     dim3 grid((unsigned)((perT + 255) / 256), nb);
     weights_transpose_kernel<<<grid, 256, 0, st>>>(wt, wtT, ny, nx);
     return (int)cudaGetLastError();
+}
+
+// Column pass on the DIF/DIT core (fft_dif.cuh): register e of thread t multiplies frequency freq_index(t, e), and reads
+// its weight pair from slot e P + t of the column -- permute every column of a weight table into that order, in place.
+template <int NF>
+__global__ void weights_permute_kernel(float2* __restrict__ wt, int cols) {
+    extern __shared__ float2 colbuf[];
+    float2* w = wt + ((size_t)blockIdx.y * cols + blockIdx.x) * NF;
+    for (int i = threadIdx.x; i < NF; i += blockDim.x) colbuf[i] = w[i];
+    __syncthreads();
+    for (int i = threadIdx.x; i < NF; i += blockDim.x) w[i] = colbuf[Dif<NF>::freq_index(i % Dif<NF>::P, i / Dif<NF>::P)];
+}
+template <int NF>
+static int run_permute(cudaStream_t st, float* wt, int cols, int nb) {
+    weights_permute_kernel<NF><<<dim3(cols, nb), 256, NF * sizeof(float2), st>>>(reinterpret_cast<float2*>(wt), cols);
+    return (int)cudaGetLastError();
+}
+int launch_weights_permute(cudaStream_t st, float* wt, int nf, int cols, int nb) {
+    switch (nf) {
+        case 256: return run_permute<256>(st, wt, cols, nb);
+        case 512: return run_permute<512>(st, wt, cols, nb);
+        case 1024: return run_permute<1024>(st, wt, cols, nb);
+        case 2048: return run_permute<2048>(st, wt, cols, nb);
+        case 4096: return run_permute<4096>(st, wt, cols, nb);
+        default: return (int)cudaErrorInvalidValue;
+    }
 }
 
 __global__ void transpose_kernel(const float* __restrict__ in, float* __restrict__ out, int rows, int cols) {

@@ -2,11 +2,13 @@
 //
 // Data layouts:
 //   image      real  [nb][ny][nx]                      row-major, x fastest
-//   spectrum T cplx  [nb][ntile][ny][2]                column-pair tiles: tile m holds columns
-//                                                       kx = 2m, 2m+1 of the row-transformed
-//                                                       array, ntile = NF/2 + 1 (kx = 0..NF; the
-//                                                       odd slot of the last tile is zero)
-//   weights Wt real  [nb][ntile][2][ny][2]             column-in-tile, q, parity (even/odd ky)
+//   spectrum T cplx  [nb][ntile][ny/2][2][2]           32-byte blocks (bins kx = 2m, 2m+1) x (rows 2r, 2r+1),
+//                                                       ntile = NF/2 + 1 (kx = 0..NF; the odd slot of the
+//                                                       last tile is zero): rows_fwd -> conv_cols (tmap.h)
+//   spectrum T2 cplx [nb][2 ntile][ny]                 column kx contiguous: conv_cols -> rows_inv
+//   weights Wt real  [nb][2 ntile (kx)][ny][2]         per column, (even-bin, odd-bin) weight pairs in the order the
+//                                                       column pass consumes them (natural q for ny < 256, the
+//                                                       permuted order of fft_dif.cuh otherwise)
 //
 // Passes (all persistent: a CTA walks work items blockIdx.x, blockIdx.x + gridDim.x, ...; the stage
 // twiddles live in shared memory, loaded once per CTA):
@@ -20,6 +22,7 @@
 // twiddle fetches and travel through shared memory as one float4 per position.
 #pragma once
 #include "fft_core.cuh"
+#include "fft_dif.cuh"
 #include "tmap.h"
 
 namespace frs {
@@ -63,12 +66,6 @@ __device__ __forceinline__ float4 ldg4(const void* p) {
 __device__ __forceinline__ float ldg1(const float* p) {
     float r;
     asm("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r) : "l"(p));
-    return r;
-}
-// coherent variant for data the same kernel later overwrites in place (conv_cols tiles)
-__device__ __forceinline__ float2 ld2_inplace(const float2* p) {
-    float2 r;
-    asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
     return r;
 }
 __device__ __forceinline__ void stg4(void* p, float4 v) {
@@ -244,6 +241,7 @@ rows_fwd_kernel(RowsFwdArgs a) {
 }
 
 #include "kernels_cols.inl"
+#include "kernels_cols_dif.inl"
 #include "kernels_inv.inl"
 
 }  // namespace frs

@@ -1,0 +1,137 @@
+// kernels_cols_dif.inl -- column convolution on the DIF/DIT core (included inside namespace frs by kernels.cuh)
+//
+// Same operation and the same staging scheme as conv_cols_kernel (kernels_cols.inl), for NF >= 256, on the
+// FFT core of fft_dif.cuh: the spectrum between the forward and the inverse transform stays in the permuted
+// order of that core (the weights are stored in it, k_setup.cu weights_permute), every exchange overwrites the
+// slots the thread has just read, and one exchange of each transform stays inside C neighbouring lanes.  Per
+// column a group passes TWO blocking barriers (eight in the sorting core) plus one release barrier that only
+// its first warp waits on.
+template <int NF> struct ColsDifGeo {
+    using D = Dif<NF>;
+    static constexpr int P = D::P;
+    static constexpr int WANT = NF >= 1024 ? 512 : 256;
+    static constexpr int THREADS = P >= WANT ? P : WANT;
+    static constexpr int G = THREADS / P;                               // groups (columns in flight) per CTA
+    static constexpr bool OWN_BAR = (P % 32 == 0) && G <= 15;           // named barrier 1 + g per group (exchange)
+    static constexpr bool SPLIT_RELEASE = OWN_BAR && P >= 64 && 2 * G <= 15;   // barrier 1 + G + g: first warp waits, the others only arrive
+    static constexpr int TW = D::TW_TOTAL;                              // float4 slots, multiple of 8
+    static constexpr int STAGE = NF / 2;                                // float4 slots of the staging buffer (NF float2)
+    static constexpr int GROUP_SLOTS = D::XLEN + STAGE;
+    static constexpr int BAR_SLOTS = (G + 1) / 2;
+    static constexpr int SMEM = (TW + G * GROUP_SLOTS + BAR_SLOTS) * (int)sizeof(float4);
+    static constexpr int MINB = THREADS >= 512 ? 1 : 2;
+};
+
+template <int NF>
+__global__ void __launch_bounds__(ColsDifGeo<NF>::THREADS, ColsDifGeo<NF>::MINB)
+conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
+    using GEO = ColsDifGeo<NF>;
+    using D = Dif<NF>;
+    constexpr int P = GEO::P;
+    extern __shared__ __align__(128) float4 smem4[];
+    float4* tws = smem4;
+    const int g = threadIdx.x / P, t = threadIdx.x % P;
+    float4* X = smem4 + GEO::TW + (size_t)g * GEO::GROUP_SLOTS;
+    float2* stage = reinterpret_cast<float2*>(X + D::XLEN);                            // [NF] float2
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem4 + GEO::TW + (size_t)GEO::G * GEO::GROUP_SLOTS) + g;
+    const GroupBar gb = GEO::OWN_BAR ? GroupBar{1 + g, P} : GroupBar{0, GEO::THREADS};
+    dif_load_twiddles<NF>(tws, a.tw);
+    if (t == 0) mbar_init(bar, 1);
+    auto twist_e = [&](int e) { return __ldg(a.twist + t + e * P); };
+
+    constexpr int BOXR = tma_box_pairs(NF), NCOPY = tma_col_copies(NF);
+    auto column = [&](int item, bool& live, int& b, int& kx, const float*& w) {
+        b = item / a.items_per_batch;
+        kx = (item - b * a.items_per_batch) * GEO::G + g;
+        live = item < a.nitems && kx < a.ncols;
+        w = a.wt + b * a.w_bstride + (size_t)kx * NF * 2;
+    };
+    auto fetch_weights = [&](const void* src, bool live) {       // one bulk copy of 8 NF bytes into the staging buffer
+        if (t == 0 && live) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, NF * 8);
+            bulk_g2s(stage, src, NF * 8, bar);
+        }
+        __syncwarp();
+    };
+    auto fetch_column = [&](int b, int kx, bool live) {          // column kx lands as NF contiguous samples
+        if (t == 0 && live) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, NF * 8);
+        }
+        __syncwarp();
+        if (t < NCOPY && live) tensor_g2s_5d(stage + 2 * BOXR * t, &a.tmap, 0, kx & 1, BOXR * t, kx >> 1, b, bar);
+        __syncwarp();
+    };
+    // every thread of the group has consumed the staging buffer: only the issuing warp has to know
+    auto release_stage = [&]() {
+        if constexpr (GEO::SPLIT_RELEASE) {
+            if (t < 32) asm volatile("bar.sync %0, %1;" :: "r"(1 + GEO::G + g), "r"(P) : "memory");
+            else asm volatile("bar.arrive %0, %1;" :: "r"(1 + GEO::G + g), "r"(P) : "memory");
+        } else {
+            gb.sync();
+        }
+    };
+    unsigned parity = 0;
+    __syncthreads();
+    {
+        bool live; int b, kx; const float* w;
+        column(blockIdx.x, live, b, kx, w);
+        fetch_column(b, kx, live);
+    }
+
+    for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
+        bool live; int b, kx; const float* w;
+        column(item, live, b, kx, w);
+
+        C2 v[kE];
+        if (live) {
+            mbar_wait(bar, parity);
+            parity ^= 1u;
+#pragma unroll
+            for (int e = 0; e < kE; ++e) {
+                const float2 x = stage[t + e * P];
+                v[e] = c2make(x, cmul(x, twist_e(e)));                 // even bins: x, odd bins: x twist^n
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < kE; ++e) v[e] = c2zero();
+        }
+        dif_fwd_0<NF>(v, t, X, tws);
+        gb.sync();                                  // X1 written; and every thread has picked up its samples
+        fetch_weights(w, live);
+        dif_fwd_1<NF>(v, t, X, tws);
+        dif_warp_sync();
+        dif_fwd_2<NF>(v, t, X);
+        if (live) {
+            mbar_wait(bar, parity);
+            parity ^= 1u;
+#pragma unroll
+            for (int e = 0; e < kE; ++e) {
+                const float2 ww = stage[t + e * P];                   // (even-bin weight, odd-bin weight) of register e
+                v[e].re = f2mul(v[e].re, ww);
+                v[e].im = f2mul(v[e].im, ww);
+            }
+        }
+        release_stage();                            // the weights have been consumed: the next column may land
+        {
+            bool nlive; int nb_, nkx; const float* nw;
+            column(item + gridDim.x, nlive, nb_, nkx, nw);
+            fetch_column(nb_, nkx, nlive);
+        }
+        dif_inv_0<NF>(v, t, X);
+        dif_warp_sync();
+        dif_inv_1<NF>(v, t, X, tws);
+        gb.sync();
+        dif_inv_2<NF>(v, t, X, tws);
+        if (live) {
+            float2* col = a.out + ((size_t)b * 2 * a.ntile + kx) * NF + t;
+#pragma unroll
+            for (int e = 0; e < kE; ++e) {
+                // y = e + conj(twist) o, as two fma chains
+                const float2 tw_ = twist_e(e), o = c2get(v[e], 1);
+                stg2(col + e * P, make_float2(fmaf(o.x, tw_.x, fmaf(o.y, tw_.y, v[e].re.x)), fmaf(o.y, tw_.x, fmaf(-o.x, tw_.y, v[e].im.x))));
+            }
+        }
+    }
+}

@@ -11,7 +11,9 @@ inline bool valid_nf(int nf) { return nf >= 16 && nf <= 4096 && (nf & (nf - 1)) 
 
 // rows: number of image rows (even).  nf: complex transform length (PAD: nf = nx; else nf = nx/2).
 int launch_rows_fwd(cudaStream_t st, int nf, bool pad, const RowsFwdArgs& a, int nb);
+// nf >= 256 runs the DIF/DIT kernel (a.tw: its tables, a.wt: weights in its permuted order), smaller nf the sorting core
 int launch_conv_cols(cudaStream_t st, int nf, const ConvColsArgs& a, int nb);
+inline bool conv_cols_uses_dif(int nf) { return nf >= 256; }
 int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* grid_x);
 int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb, int* grid_x = nullptr);
 
@@ -45,6 +47,27 @@ int launch_psf_cols(cudaStream_t st, int nf, const PsfColsArgs& a, int nb, int* 
 template <typename K>
 inline cudaError_t set_smem(K kernel, int bytes) {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+// The shared-memory opt-in and the resident-CTA count belong to a (kernel, DEVICE) pair: cached per device,
+// in a table owned by the launcher of each kernel instantiation.
+constexpr int kMaxDevices = 64;
+template <typename K> inline int resident_ctas(K kernel, int threads, int smem);
+template <typename K>
+inline int persistent_ctas(int (&cache)[kMaxDevices], K kernel, int threads, int smem, int* ctas) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
+    if (dev < 0 || dev >= kMaxDevices) return (int)cudaErrorInvalidDevice;
+    if (!cache[dev]) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return (int)e;
+        const int c = resident_ctas(kernel, threads, smem);
+        if (!c) return (int)cudaErrorUnknown;
+        cache[dev] = c;
+    }
+    *ctas = cache[dev];
+    return 0;
 }
 
 // resident CTAs of a persistent kernel = SMs x occupancy (0 on error)

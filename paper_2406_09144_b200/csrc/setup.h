@@ -4,6 +4,8 @@ namespace frs {
 int launch_weights_layout(cudaStream_t st, const float* w_half, float* wt, int ny, int nx, int nb, int* neg_flag);
 // wt [nb][nx/2+1][2][ny][2] (natural orientation) -> wtT [nb][ny/2+1][2][nx][2] (transposed image orientation)
 int launch_weights_transpose(cudaStream_t st, const float* wt, float* wtT, int ny, int nx, int nb);
+// wt [nb][cols][nf][2]: every column into the consumption order of the DIF/DIT column pass (nf >= 256), in place
+int launch_weights_permute(cudaStream_t st, float* wt, int nf, int cols, int nb);
 // out[b][j][i] = in[b][i][j], in [nb][rows][cols]
 int launch_transpose(cudaStream_t st, const float* in, float* out, int rows, int cols, int nb);
 }

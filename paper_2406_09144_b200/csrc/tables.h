@@ -3,6 +3,7 @@
 #include <cmath>
 #include <vector>
 #include "fft_core.cuh"
+#include "fft_dif.cuh"
 
 namespace frs {
 
@@ -31,6 +32,39 @@ inline std::vector<float4> build_twiddles(int n) {
         }
     }
     return tw;
+}
+
+// twiddles of the DIF/DIT core (fft_dif.cuh): direct table of tw2, factorised base of tw1
+template <int N>
+inline std::vector<float4> build_dif_twiddles() {
+    using D = Dif<N>;
+    std::vector<float4> tw((size_t)D::TW_TOTAL, make_float4(1.f, 0.f, 1.f, 0.f));
+    const double two_pi = 6.283185307179586476925286766559;
+    auto ex = [&](long long num, long long den) {
+        const double ang = -two_pi * (double)num / (double)den;
+        return make_float2((float)std::cos(ang), (float)std::sin(ang));
+    };
+    if (D::C > 1)
+        for (int q = 0; q < 8; ++q)
+            for (int n0 = 0; n0 < D::C; ++n0) {
+                const float2 w1 = ex((long long)n0 * (2 * q + 1), 16LL * D::C);
+                const float2 w2 = 2 * q + 2 < kE ? ex((long long)n0 * (2 * q + 2), 16LL * D::C) : make_float2(1.f, 0.f);
+                tw[(size_t)q * D::C + n0] = make_float4(w1.x, w1.y, w2.x, w2.y);
+            }
+    float2* f = reinterpret_cast<float2*>(tw.data() + D::TW_D);
+    for (int a = 0; a < D::C; ++a) f[a] = ex(16LL * a, N);
+    for (int c = 0; c < 16; ++c) f[D::C + c] = ex(c, N);
+    return tw;
+}
+inline std::vector<float4> build_dif_twiddles(int n) {
+    switch (n) {
+        case 256: return build_dif_twiddles<256>();
+        case 512: return build_dif_twiddles<512>();
+        case 1024: return build_dif_twiddles<1024>();
+        case 2048: return build_dif_twiddles<2048>();
+        case 4096: return build_dif_twiddles<4096>();
+        default: return {};
+    }
 }
 
 // twist[k] = exp(-2 pi i k / (2 n)), k = 0..n  (real<->complex packing, and the odd-bin shift of the
