@@ -122,9 +122,9 @@ size_t max2(size_t a, size_t b) { return a > b ? a : b; }
 
 int ensure_scratch(frs_ctx* ctx) {
     const size_t np = ctx->npix, ny = ctx->ny, nx = ctx->nx;
-    RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
+    RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2(spec_batch_stride(ctx->ny, ctx->nx), spec_batch_stride(ctx->nx, ctx->ny))));
     RET(dev_alloc(ctx, &ctx->T2, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
-    RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * max2((nx / 4 + 1) * ny, (ny / 4 + 1) * nx) * 2));
+    RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * max2(spec_batch_stride(ctx->ny, ctx->nx / 2), spec_batch_stride(ctx->nx, ctx->ny / 2))));
     RET(dev_alloc(ctx, &ctx->lin, 2 * np));
     RET(dev_alloc(ctx, &ctx->acc, 2 * np));
     RET(dev_alloc(ctx, &ctx->img, (size_t)ctx->nchan * np));
@@ -164,8 +164,7 @@ int spectrum_maps(frs_ctx* ctx, const float2* T, int rows, int nf, int nb, CUten
             return FRS_OK;
         }
     frs_ctx::MapKey k{T, rows, nf, nb, {}, {}};
-    CUtensorMap unused;
-    if (make_spectrum_maps(&unused, &k.col, T, rows, nf, nb) || make_columns_map(&k.row, ctx->T2, rows, nf, nf + 2, nb))
+    if (make_spectrum_col_map(&k.col, T, rows, nf, nb) || make_columns_map(&k.row, ctx->T2, rows, nf, nf + 2, nb))
         return fail(ctx, FRS_ECUDA, "cuTensorMapEncodeTiled failed");
     ctx->maps.push_back(k);
     if (row) *row = k.row;
@@ -441,7 +440,7 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
     // row pass over all 2 ny rows of length 2 nx (no padding), then one DIF step + ny-point column FFTs
     float2* tmp = nullptr;
     float* stats = nullptr;
-    const size_t tstride = (size_t)ctx->ntile * my * 2;
+    const size_t tstride = spec_batch_stride(my, ctx->nx);
     CK(cudaMalloc(reinterpret_cast<void**>(&tmp), (size_t)ctx->nchan * tstride * sizeof(float2)));
     int rc = FRS_OK;
     std::vector<float> hs;

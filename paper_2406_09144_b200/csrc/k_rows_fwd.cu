@@ -2,7 +2,7 @@
 namespace frs {
 template <int NF, bool PAD>
 static int run(cudaStream_t st, const RowsFwdArgs& a0, int nb) {
-    using GEO = RowsGeo<NF>;
+    using GEO = typename std::conditional<PAD, RowsFwdGeo<NF>, RowsGeo<NF>>::type;
     static int cache[kMaxDevices] = {};
     int ctas = 0;
     if (int e = persistent_ctas(cache, rows_fwd_kernel<NF, PAD>, GEO::THREADS, GEO::SMEM, &ctas)) return e;

@@ -2,9 +2,9 @@
 //
 // Data layouts:
 //   image      real  [nb][ny][nx]                      row-major, x fastest
-//   spectrum T cplx  [nb][ntile][ny/2][2][2]           32-byte blocks (bins kx = 2m, 2m+1) x (rows 2r, 2r+1),
-//                                                       ntile = NF/2 + 1 (kx = 0..NF; the odd slot of the
-//                                                       last tile is zero): rows_fwd -> conv_cols (tmap.h)
+//   spectrum T cplx  [nb][NF/8+1][ny/2][8][2]          128-byte blocks (8 bins kx) x (rows 2r, 2r+1), kx = 0..NF (the
+//                                                       unused slots of the last block are never read):
+//                                                       rows_fwd -> conv_cols (tmap.h)
 //   spectrum T2 cplx [nb][2 ntile][ny]                 column kx contiguous: conv_cols -> rows_inv
 //   weights Wt real  [nb][2 ntile (kx)][ny][2]         per column, (even-bin, odd-bin) weight pairs in the order the
 //                                                       column pass consumes them (natural q for ny < 256, the
@@ -21,6 +21,7 @@
 // Every thread carries a PAIR of transforms (two rows / the two columns of a tile): they share the
 // twiddle fetches and travel through shared memory as one float4 per position.
 #pragma once
+#include <type_traits>
 #include "fft_core.cuh"
 #include "fft_dif.cuh"
 #include "tmap.h"
@@ -77,12 +78,15 @@ __device__ __forceinline__ void stg2(void* p, float2 v) {
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
 template <int NF> struct RowsGeo : Geo<NF, 1, 0, 256> {};
+// padded row pass: plus a staging buffer of 2 rows of NF floats per group (the next item's input lands there while this
+// item's transform owns the exchange buffer)
+template <int NF> struct RowsFwdGeo : Geo<NF, 1, NF / 2, 256> {};
 
 // ------------------------------------------------------------------------------------------------
 struct RowsFwdArgs {
     const float* in;      // [nb][ny][nxr]
     const float* mul;     // optional [nb][ny][nxr] multiplier (s or A); nullptr = none
-    float2* out;          // [nb][NF/2+1][ny/2][2][2]: 32-byte blocks (bins 2m, 2m+1) x (rows 2r, 2r+1), tmap.h
+    float2* out;          // [nb][NF/8+1][ny/2][8][2]: 128-byte blocks (8 bins) x (rows 2r, 2r+1), tmap.h
     int ny;               // rows
     int items_per_batch, nitems;
     size_t in_bstride, mul_bstride;   // elements (float)
@@ -91,11 +95,12 @@ struct RowsFwdArgs {
     const float2* twist;  // exp(-2 pi i k/(2 NF)), k = 0..NF
 };
 
-// One group (P threads) transforms rows y0, y0+1 together.  Software pipeline (PAD): the two input rows
-// (and the two rows of the multiplier) of the NEXT item are pulled by bulk TMA copies into the exchange
-// buffer as soon as this item's transform has left it, so global latency never reaches the registers
-// (a register prefetch does not fit beside the unpacking phase: the compiler spills it and the spill
-// stores wait for the loads).  Unpadded rows (Hartley pass) are twice as long and load directly.
+// One group (P threads) transforms rows y0, y0+1 together.  Software pipeline (PAD): the two input rows of the NEXT item
+// are pulled by one bulk TMA copy into a staging buffer of their own as soon as this item has picked its rows up, so the
+// copy has a whole transform to land (when it landed in the exchange buffer it could only start behind the transform and
+// 16 % of the warp time was spent waiting for it, profiles/r1_l1_apply_ncu.md); the rows of the multiplier are read
+// straight into registers, from L2: a bulk prefetch pulls them in one item ahead.  Unpadded rows (Hartley pass) are
+// twice as long and load directly.
 // Unpacking X[k] from the half-length transform Z needs Z[k] (still in the thread's registers) and
 // Z[NF-k] (another thread's): Z is parked in the exchange buffer once and every thread reads its 16
 // mirror slots.  A thread then holds X[k] of both rows (16 bytes); neighbouring lanes hold
@@ -103,7 +108,7 @@ struct RowsFwdArgs {
 template <int NF, bool PAD>
 __global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
 rows_fwd_kernel(RowsFwdArgs a) {
-    using GEO = RowsGeo<NF>;
+    using GEO = typename std::conditional<PAD, RowsFwdGeo<NF>, RowsGeo<NF>>::type;
     constexpr int P = GEO::P;
     constexpr int NXR = PAD ? NF : 2 * NF;        // real samples per row
     constexpr int NE = PAD ? kE / 2 : kE;         // canonical slots that hold data
@@ -118,20 +123,19 @@ rows_fwd_kernel(RowsFwdArgs a) {
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem4 + GEO::TW + (size_t)GEO::G * GEO::GROUP_SLOTS) + g;
     if (PAD && p == 0) mbar_init(bar, 1);
     unsigned parity = 0;
-    const float* stg = reinterpret_cast<const float*>(buf);       // staged rows: x row 0, x row 1, mul row 0, mul row 1
-    static_assert(!PAD || 4 * NF * 4 <= xbuf_len(NF) * 16, "staged rows exceed the exchange buffer");
+    const float* stg = reinterpret_cast<const float*>(buf + xbuf_len(NF));       // staged rows: x row 0, x row 1
     auto row_pair = [&](int item, int& b, int& rp) {
         b = item / a.items_per_batch;
         rp = (item - b * a.items_per_batch) * GEO::G + g;
         return item < a.nitems && 2 * rp < a.ny;
     };
-    auto stage_rows = [&](int item) {                              // PAD only: 2 (or 4) rows of NF floats
+    auto stage_rows = [&](int item) {                              // PAD only: 2 rows of NF floats; multiplier rows -> L2
         int b, rp;
         if (row_pair(item, b, rp) && p == 0) {
             fence_proxy_async();
-            mbar_expect_tx(bar, (a.mul ? 4 : 2) * NF * 4);
-            bulk_g2s(buf, a.in + b * a.in_bstride + (size_t)(2 * rp) * NXR, 2 * NF * 4, bar);
-            if (a.mul) bulk_g2s(buf + NF / 2, a.mul + b * a.mul_bstride + (size_t)(2 * rp) * NXR, 2 * NF * 4, bar);
+            mbar_expect_tx(bar, 2 * NF * 4);
+            bulk_g2s(const_cast<float*>(stg), a.in + b * a.in_bstride + (size_t)(2 * rp) * NXR, 2 * NF * 4, bar);
+            if (a.mul) bulk_prefetch_l2(a.mul + b * a.mul_bstride + (size_t)(2 * rp) * NXR, 2 * NF * 4);
         }
         __syncwarp();   // the issuing lane must not be left behind a warp that spins on the mbarrier
     };
@@ -155,6 +159,14 @@ rows_fwd_kernel(RowsFwdArgs a) {
         float2 xin[2][NE], min_[2][NE];
 #pragma unroll
         for (int e = 0; e < NE; ++e) { xin[0][e] = xin[1][e] = make_float2(0.f, 0.f); min_[0][e] = min_[1][e] = make_float2(1.f, 1.f); }
+        if (live && a.mul) {
+            const float* m0 = a.mul + b * a.mul_bstride + (size_t)y0 * NXR;
+#pragma unroll
+            for (int e = 0; e < NE; ++e) {
+                min_[0][e] = ldg2(m0 + 2 * (p + e * P));
+                min_[1][e] = ldg2(m0 + NXR + 2 * (p + e * P));
+            }
+        }
         if (PAD) {
             if (live) {
                 mbar_wait(bar, parity);
@@ -162,13 +174,12 @@ rows_fwd_kernel(RowsFwdArgs a) {
 #pragma unroll
                 for (int e = 0; e < NE; ++e) {
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-                        xin[t][e] = *reinterpret_cast<const float2*>(stg + t * NF + 2 * (p + e * P));
-                        if (a.mul) min_[t][e] = *reinterpret_cast<const float2*>(stg + (2 + t) * NF + 2 * (p + e * P));
-                    }
+                    for (int t = 0; t < 2; ++t) xin[t][e] = *reinterpret_cast<const float2*>(stg + t * NF + 2 * (p + e * P));
                 }
             }
-            gb.sync();                                             // the staged rows have been read: the buffer is free
+            // the staged rows have been read (and the mirror slots of the previous item: the exchange buffer is free)
+            gb.sync();
+            stage_rows(item + gridDim.x);
         } else {
             if (live) {
                 const float* r0 = a.in + b * a.in_bstride + (size_t)y0 * NXR;
@@ -176,14 +187,6 @@ rows_fwd_kernel(RowsFwdArgs a) {
                 for (int e = 0; e < NE; ++e) {
                     xin[0][e] = ldg2(r0 + 2 * (p + e * P));
                     xin[1][e] = ldg2(r0 + NXR + 2 * (p + e * P));
-                }
-                if (a.mul) {
-                    const float* m0 = a.mul + b * a.mul_bstride + (size_t)y0 * NXR;
-#pragma unroll
-                    for (int e = 0; e < NE; ++e) {
-                        min_[0][e] = ldg2(m0 + 2 * (p + e * P));
-                        min_[1][e] = ldg2(m0 + NXR + 2 * (p + e * P));
-                    }
                 }
             }
             prefetch_rows(item + gridDim.x);
@@ -224,18 +227,14 @@ rows_fwd_kernel(RowsFwdArgs a) {
             v[e].re = f2fma(s.re, sc, d.im);
             v[e].im = f2fma(s.im, sc, f2neg(d.re));
         }
-        gb.sync();                                // every mirror slot has been read: the buffer is free again
-        if (PAD) stage_rows(item + gridDim.x);
+        if (!PAD) gb.sync();                      // every mirror slot has been read (PAD: the barrier at the top of the next item)
         if (live) {
-            // (X_0[k], X_1[k]) -> block (k >> 1, y0 / 2), half k & 1
+            // (X_0[k], X_1[k]) -> 16-byte slot k % 8 of block (k / 8, y0 / 2): 8 neighbouring lanes fill one 128-byte line
             auto slot = [](const C2& x) { return make_float4(x.re.x, x.im.x, x.re.y, x.im.y); };
-            float4* ob = reinterpret_cast<float4*>(a.out) + ((size_t)b * (NF / 2 + 1) * (a.ny / 2) + rp) * 2;
+            float4* ob = reinterpret_cast<float4*>(a.out + b * spec_batch_stride(a.ny, NF));
 #pragma unroll
-            for (int e = 0; e < kE; ++e) {
-                const int k = p + e * P;
-                stg4(ob + (size_t)(k >> 1) * a.ny + (k & 1), slot(v[e]));
-            }
-            if (p == 0) stg4(ob + (size_t)(NF / 2) * a.ny, slot(xn));
+            for (int e = 0; e < kE; ++e) stg4(ob + spec_index(a.ny, p + e * P, y0) / 2, slot(v[e]));
+            if (p == 0) stg4(ob + spec_index(a.ny, NF, y0) / 2, slot(xn));
         }
     }
 }

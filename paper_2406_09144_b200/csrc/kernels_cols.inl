@@ -3,7 +3,7 @@
 // ------------------------------------------------------------------------------------------------
 struct ConvColsArgs {
     CUtensorMap tmap;     // column map of t (tmap.h)
-    const float2* t;      // [nb][ntile][NF/2][2][2] block layout (tmap.h): input
+    const float2* t;      // [nb][len/8+1][NF/2][8][2] block layout (tmap.h): input
     float2* out;          // [nb][2 ntile][NF]: output, column kx contiguous (whole-sector, coalesced stores)
     const float* wt;      // [nb][ntile][2 (column in tile)][NF (q)][2 (even, odd bin)]
     int ncols;            // columns that exist per batch (row length + 1)
@@ -70,7 +70,7 @@ conv_cols_kernel(const __grid_constant__ ConvColsArgs a) {
             mbar_expect_tx(bar, NF * 8);
         }
         __syncwarp();
-        if (p < NCOPY && live) tensor_g2s_5d(stage + 2 * BOXR * p, &a.tmap, 0, kx & 1, BOXR * p, kx >> 1, b, bar);   // one copy per lane
+        if (p < NCOPY && live) tensor_g2s_5d(stage + 2 * BOXR * p, &a.tmap, 0, kx % kBlockBins, BOXR * p, kx / kBlockBins, b, bar);   // one copy per lane
         __syncwarp();
     };
     unsigned parity = 0;
@@ -146,7 +146,7 @@ conv_cols_kernel(const __grid_constant__ ConvColsArgs a) {
 
 // ------------------------------------------------------------------------------------------------
 struct HartColsArgs {
-    const float2* t;      // [nb][ntile][NF/2][2][2] block layout: columns x = 0..nx/2 of the row-transformed field (NF rows)
+    const float2* t;      // block layout of tmap.h: columns x = 0..nx/2 of the row-transformed field (NF rows)
     float* out;           // [nb][nx][NF]  TRANSPOSED: out[x][y] = H[y][x]
     const float* mul;     // optional [nb][nx][NF]: out = mul * (H + offset) + add
     const float* add;     // optional [nb][nx][NF]
@@ -182,13 +182,13 @@ hart_cols_kernel(HartColsArgs a) {
 
         C2 v[kE];
         if (live) {
-            // tile m = columns 2m, 2m+1: sample y at block y >> 1, position (c, y & 1)
-            const float* c0 = reinterpret_cast<const float*>(a.t + ((size_t)(b * ntile + m) * (NF / 2)) * 4);
+            // columns 2m, 2m+1 (neighbouring 16-byte slots of one block of T)
+            const float* c0 = reinterpret_cast<const float*>(a.t + b * spec_batch_stride(NF, a.nx / 2));
             const bool two = 2 * m + 1 <= a.nx / 2;            // the last pair may hold one column only
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const int y = p + e * P;
-                const float* q = c0 + 2 * ((y >> 1) * 4 + (y & 1));
+                const float* q = c0 + 2 * spec_index(NF, 2 * m, y);
                 const float2 x0 = ldg2(q);
                 const float2 x1 = two ? ldg2(q + 4) : make_float2(0.f, 0.f);
                 v[e] = c2make(x0, x1);

@@ -37,7 +37,13 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
     const GroupBar gb = GEO::OWN_BAR ? GroupBar{1 + g, P} : GroupBar{0, GEO::THREADS};
     dif_load_twiddles<NF>(tws, a.tw);
     if (t == 0) mbar_init(bar, 1);
-    auto twist_e = [&](int e) { return __ldg(a.twist + t + e * P); };
+    // twist^n for the thread's samples n = t + e P, from the exactly rounded table.  Only its first half is read
+    // (twist^(NF-m) = -conj twist^m), so that it stays resident in the few KB of L1 this kernel leaves
+    auto twist_e = [&](int e) {
+        if (e < kE / 2) return __ldg(a.twist + t + e * P);
+        const float2 c = __ldg(a.twist + (NF - e * P) - t);
+        return make_float2(-c.x, c.y);
+    };
 
     constexpr int BOXR = tma_box_pairs(NF), NCOPY = tma_col_copies(NF);
     auto column = [&](int item, bool& live, int& b, int& kx, const float*& w) {
@@ -60,7 +66,7 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
             mbar_expect_tx(bar, NF * 8);
         }
         __syncwarp();
-        if (t < NCOPY && live) tensor_g2s_5d(stage + 2 * BOXR * t, &a.tmap, 0, kx & 1, BOXR * t, kx >> 1, b, bar);
+        if (t < NCOPY && live) tensor_g2s_5d(stage + 2 * BOXR * t, &a.tmap, 0, kx % kBlockBins, BOXR * t, kx / kBlockBins, b, bar);
         __syncwarp();
     };
     // every thread of the group has consumed the staging buffer: only the issuing warp has to know

@@ -18,7 +18,7 @@ int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* 
 int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb, int* grid_x = nullptr);
 
 struct PsfColsArgs {
-    const float2* t;      // [nb][ntile][NF][2][2]  row-transformed PSF, all 2 NF rows, block layout (tmap.h)
+    const float2* t;      // row-transformed PSF, all 2 NF rows, ncols - 1 = nx bins + 1: block layout of tmap.h
     int ncols;            // columns that exist (nx + 1)
     float* wt;            // [nb][ntile][2][NF][2]
     float* stats;         // [nb][gridDim.x][3]: max |Im W|, min Re W, max Re W   (unscaled by fold)

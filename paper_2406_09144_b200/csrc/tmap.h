@@ -1,25 +1,32 @@
-// tmap.h -- TMA tensor maps over the spectrum T.
-// T[b][m][y/2][c][y%2] (complex64): 32-byte blocks of (2 bins kx = 2m + c) x (2 image rows), so that
-//   * a row pass writes / reads whole 32-byte sectors (bins 2m, 2m+1 of its row pair), and
-//   * a column kx is a run of 16-byte pieces (rows 2r, 2r+1) at a stride of 32 bytes,
-// both of which the TMA unit moves as boxes of a strided tensor, landing them DENSELY in shared memory:
-//   row map  (4-D floats): d0 = 8 floats of a block, d1 = y/2 (32 B), d2 = m (16 rows B), d3 = b;
-//             box {8, 1, B, 1} = bins [2 m0, 2 m0 + 2B) of one row pair -> 16-byte slots (Y_0[k], Y_1[k])
-//   col map  (5-D floats): d0 = 4 floats of a piece, d1 = c (16 B), d2 = y/2 (32 B), d3 = m, d4 = b;
-//             box {4, 1, R, 1, 1} = rows [2 r0, 2 r0 + 2R) of one column -> contiguous complex samples
-// Blocks beyond the last tile read as zero.  The column pass writes its result to a second array in plain
-// column-contiguous order (whole sectors, coalesced), which the inverse row pass gathers through a third map.  The driver entry point is fetched through the runtime,
-// so the library does not link against libcuda.
+// tmap.h -- layout of the spectrum T between the row pass and the column pass, and the TMA tensor maps over it and over
+// T2.
+// T[b][m][y/2][c][y%2] (complex64), kx = 8 m + c: 128-byte blocks of (8 bins) x (2 image rows), so that
+//   * a row pass writes whole 128-byte lines: a thread holds (X_0[k], X_1[k]) of its row pair, 8 neighbouring lanes hold
+//     the 8 bins of a block (a warp store touches 4 lines; with 32-byte blocks of 2 bins it touched 16, and those
+//     scattered stores were a third of the row pass's L1 data-pipe load, profiles/r2_notes.md), and
+//   * a column kx is a run of 16-byte pieces (rows 2r, 2r+1) at a stride of 128 bytes inside one contiguous region of
+//     64 rows bytes, which the TMA unit gathers as boxes of a strided tensor, landing them DENSELY in shared memory:
+//   col map  (5-D floats): d0 = 4 floats of a piece, d1 = c (16 B), d2 = y/2 (128 B), d3 = m, d4 = b;
+//             box {4, 1, R, 1, 1} = rows [2 r0, 2 r0 + 2R) of one column -> contiguous complex samples.
+// The 8 columns of a block are convolved by neighbouring CTAs at about the same time, so each line leaves DRAM once.
+// Blocks beyond the last bin read as zero.  The column pass writes its result to a second array T2 in plain
+// column-contiguous order (coalesced), which the inverse row pass gathers through a 3-D map.  The driver entry point is
+// fetched through the runtime, so the library does not link against libcuda.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
 
 namespace frs {
 
-// row map: 17 copies of nf/32 tiles cover the nf/2 + 1 tiles of a row pair and fill an exchange buffer
-// of xbuf_len(nf) slots almost exactly; TMA needs 128-byte aligned boxes in shared memory
-__host__ __device__ constexpr int tma_box_tiles(int nf) { return nf >= 32 ? nf / 32 : 1; }
-__host__ __device__ constexpr int tma_row_copies(int nf) { return (nf / 2 + 1 + tma_box_tiles(nf) - 1) / tma_box_tiles(nf); }
+constexpr int kBlockBins = 8;                                     // bins kx per 128-byte block of T
+__host__ __device__ constexpr int spec_tiles(int nf) { return nf / kBlockBins + 1; }   // bins kx = 0..nf
+// float2 index, inside one batch, of sample (kx, y) of the row-transformed array of `rows` image rows
+__host__ __device__ constexpr size_t spec_index(int rows, int kx, int y) {
+    return ((((size_t)(kx / kBlockBins) * (rows / 2) + (y >> 1)) * kBlockBins + (kx % kBlockBins)) << 1) + (y & 1);
+}
+__host__ __device__ constexpr size_t spec_batch_stride(int rows, int nf) { return (size_t)spec_tiles(nf) * rows * kBlockBins; }
+
+// smaller rows: boxes below the 128-byte TMA alignment -> cp.async
 __host__ __device__ constexpr bool tma_rows_ok(int nf) { return nf >= 128; }
 // col map: copies of up to 256 row pairs (rows >= 32: boxes of >= 256 bytes)
 __host__ __device__ constexpr int tma_box_pairs(int rows) { return rows / 2 < 256 ? rows / 2 : 256; }
@@ -43,29 +50,18 @@ inline TmapEncodeFn tmap_encoder() {
     }
     return encode;
 }
-// T: [nb][ntile][rows/2][2][2] complex64, ntile = nf/2 + 1
-inline int make_spectrum_maps(CUtensorMap* row_map, CUtensorMap* col_map, const float2* T, int rows, int nf, int nb) {
+// column map of T: [nb][spec_tiles(nf)][rows/2][8][2] complex64
+inline int make_spectrum_col_map(CUtensorMap* col_map, const float2* T, int rows, int nf, int nb) {
     TmapEncodeFn encode = tmap_encoder();
     if (!encode) return (int)cudaErrorUnknown;
-    const cuuint64_t ntile = (cuuint64_t)nf / 2 + 1, tile_bytes = (cuuint64_t)rows * 16;
+    const cuuint64_t ntile = (cuuint64_t)spec_tiles(nf), tile_bytes = (cuuint64_t)rows * 8 * kBlockBins;
     const cuuint32_t one[5] = {1, 1, 1, 1, 1};
-    {
-        const cuuint64_t dims[4] = {8, (cuuint64_t)rows / 2, ntile, (cuuint64_t)nb};
-        const cuuint64_t strides[3] = {32, tile_bytes, tile_bytes * ntile};
-        const cuuint32_t box[4] = {8, 1, (cuuint32_t)tma_box_tiles(nf), 1};
-        if (encode(row_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float2*>(T), dims, strides, box, one,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
-    }
-    {
-        const cuuint64_t dims[5] = {4, 2, (cuuint64_t)rows / 2, ntile, (cuuint64_t)nb};
-        const cuuint64_t strides[4] = {16, 32, tile_bytes, tile_bytes * ntile};
-        const cuuint32_t box[5] = {4, 1, (cuuint32_t)tma_box_pairs(rows), 1, 1};
-        if (encode(col_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<float2*>(T), dims, strides, box, one,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
-    }
-    return 0;
+    const cuuint64_t dims[5] = {4, (cuuint64_t)kBlockBins, (cuuint64_t)rows / 2, ntile, (cuuint64_t)nb};
+    const cuuint64_t strides[4] = {16, 16 * kBlockBins, tile_bytes, tile_bytes * ntile};
+    const cuuint32_t box[5] = {4, 1, (cuuint32_t)tma_box_pairs(rows), 1, 1};
+    return encode(col_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<float2*>(T), dims, strides, box, one,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
 }
 
 // T2: [nb][cols][rows] complex64, bins kx = 0..nf exist
