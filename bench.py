@@ -8,13 +8,21 @@ metric apply y = s . C(s . x) ("L1 apply") on BASELINE.json conf
 channel) -- three kernels (row R2C, column FFT.W.iFFT, row C2R).  The same run also times the latent
 metric apply, one energy+gradient and a CG iteration (reported under "extra"), the dominant kernel
 alone for the roofline, the end-to-end call with host buffers, and the fp64 oracle on the host cores.
-Single-channel configs do not shard: --gpus N runs N independent replicas.
+Single-channel configs do not shard: --gpus N runs N independent replicas, one process
+per GPU (started here through torch.distributed.run when the caller has not already done so).  The multi-channel
+config does shard: `--config 5 --shard channels` times the channel-sharded latent metric apply and CG iteration
+(ChannelShard: one NCCL all-reduce per apply), strong scaling.
+
+The timed operator is the N' = R' limit of the paper's Eq. 9 (E = 1/2 s^T C s - j^T s, metric J^T C J, DESIGN.md R1);
+the separate fitted noise kernel of Eq. 15-18 is the `--noise-kernel` variant of the latent calls (three convolutions
+per apply), reported under "extra".
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -195,6 +203,15 @@ def run_cuda(args):
         return ms
 
     step = lambda i: ctx.sky_metric_apply(xs[i & 1], y)  # noqa: E731
+    # ---- the timed operator must be the operator: symmetry <x1, A x0> = <A x1, x0> and positivity <x0, A x0> >= 0 of
+    # A = s . C (s . ) on this very configuration (the oracle comparison at this size lives in tests/, minutes of CPU)
+    y1 = ctx.new_image()
+    ctx.sky_metric_apply(xs[0], y)
+    ctx.sky_metric_apply(xs[1], y1)
+    d01, d10 = float((xs[1].double() * y.double()).sum()), float((y1.double() * xs[0].double()).sum())
+    d00 = float((xs[0].double() * y.double()).sum())
+    assert abs(d01 - d10) <= 1e-4 * max(abs(d01), abs(d10), 1e-300) and d00 > 0.0, ("L1 apply not symmetric PSD", d01, d10, d00)
+    del y1
     # ---- headline: K L1 applies, inputs resident in HBM
     sampler = ClockSampler(local)
     if rank == 0:
@@ -215,22 +232,29 @@ def run_cuda(args):
     peak, peak_src = peaks()
     f2_ms = prof["conv_cols"][0] / max(1, prof["conv_cols"][1])
     ach = b_f2 / (f2_ms * 1e-3) / 1e9
-    traffic = None
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic_conv_cols.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
-    roofline = {"bound": "hbm", "kernel": "conv_cols_kernel (column FFT . W . iFFT)", "achieved": ach, "peak": peak,
-                "unit": "GB/s", "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
+    if os.path.exists(tpath) and args.config == 4:
+        tj = json.load(open(tpath))
+        traffic = tj.get("dram_bytes_per_launch")
+        traffic_src = "from " + tj.get("source", "profiles/") + " -- an ncu capture of this kernel, NOT measured in this run"
+    roofline = {"bound": "hbm", "kernel": "conv_cols_dif_kernel (column FFT . W . iFFT)", "achieved": ach, "peak": peak,
+                "unit": "GB/s", "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": b_f2, "ms_per_launch": f2_ms,
                 "pass_ms": {k: v[0] / max(1, v[1]) for k, v in prof.items() if v[1]}}
-    # the co-binding roof of the same kernel: FP32 pipe slots.  One slot = one fp32
-    # add / mul / fma per lane (a packed FFMA2 counts two); conv_cols executes 2759 slots per thread and column
-    # (SASS count at NF = 4096: 1220 packed + 319 scalar), 256 threads per column; peak = SMs x 128 lanes x clock.
+    # the co-binding roof of the same kernel: FP32 pipe slots.  One slot = one fp32 add / mul /
+    # fma per lane (a packed FADD2 / FMUL2 / FFMA2 counts two).  Slots per thread and column: the SASS instruction mix of
+    # conv_cols_dif_kernel<4096> kept in profiles/sass_mix_conv_cols.json (cuobjdump count, command inside); 256 threads
+    # per column; peak = SMs x 128 lanes x SM clock.
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     fp_peak = sms * 128 * (clocks["sm_mhz"] if clocks and clocks.get("sm_mhz") else 1965.0) * 1e6 / 1e12
-    fp_ach = 2759.0 * 256 * (w.nx + 1) * w.nchan * (w.ny / 4096.0) / (f2_ms * 1e-3) / 1e12 if w.ny == 4096 else None
-    roofline_fp32 = {"bound": "alu", "kernel": "conv_cols_kernel", "achieved": fp_ach, "peak": fp_peak, "unit": "T fp32 lane-ops/s",
-                     "frac": (fp_ach / fp_peak) if fp_ach else None,
+    fp_ach, slots = None, None
+    spath = os.path.join(ROOT, "profiles", "sass_mix_conv_cols.json")
+    if os.path.exists(spath) and w.ny == 4096:
+        slots = float(json.load(open(spath))["fp32_lane_ops_per_thread_per_column"])
+        fp_ach = slots * 256 * (w.nx + 1) * w.nchan / (f2_ms * 1e-3) / 1e12
+    roofline_fp32 = {"bound": "alu", "kernel": "conv_cols_dif_kernel", "achieved": fp_ach, "peak": fp_peak, "unit": "T fp32 lane-ops/s",
+                     "frac": (fp_ach / fp_peak) if fp_ach else None, "lane_ops_per_thread_per_column": slots,
                      "peak_source": "148 SMs x 128 fp32 lanes x SM clock sampled during the run (B200_PROFILING.md unit counts)"}
     ach_step = b_l1 / (ms_step * 1e-3) / 1e9
     roofline_step = {"what": "whole L1 apply (3 kernels), minimal 3-pass byte model", "bytes": b_l1, "achieved": ach_step,
@@ -307,12 +331,106 @@ def run_cuda(args):
                                    "frs_sky_metric_apply y = s.C(s.x)",
                        "l2": "no flush: a step streams 0.94 GB (inputs 2 x 67 MB rotated, 134 MB spectrum, 134 MB weights) "
                              ">> 126 MB L2",
-                       "parallelism": f"replicas x{world} (single-channel path does not shard)"},
+                       "operator": "N' = R' limit of Eq. 9 (E = 1/2 s^T C s - j^T s): one padded PSF convolution per apply",
+                       "parallelism": f"replicas x{world} (single-channel path does not shard), one process per GPU"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_step": roofline_step, "roofline_fp32": roofline_fp32,
             "cpu_baseline": cpu, "extra": extra}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+# ----------------------------------------------------------------------------------------- sharded arm (config 5)
+def run_sharded(args):
+    """--config 5 --shard channels: the 16 channels are partitioned over the ranks (ChannelShard), the latent vectors are
+    replicated, every latent metric apply / CG iteration ends in ONE NCCL all-reduce of a latent-sized vector."""
+    import torch
+    import torch.distributed as dist
+    import paper_2406_09144_b200 as frs
+    from paper_2406_09144_b200.parallel import ChannelShard
+    from gen import workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if not dist.is_initialized():
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", str(_free_port()))
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    frs.load_library()
+    w = wl.make_config(5, seed=0)                        # the SAME problem on every rank; each keeps its channels
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).cuda()  # noqa: E731
+    sh = ChannelShard(w.ny, w.nx, w.nchan, w.lognu)
+    sh.set_psf_weights(dev(w.w_half))
+    sh.set_dirty(dev(w.dirty))
+    sh.set_amplitude(dev(w.amp), w.mu)
+    rng = np.random.default_rng(100)
+    xi = dev(0.5 * rng.normal(size=(w.nfield, w.ny, w.nx)))
+    g = torch.empty_like(xi)
+    sh.energy_grad(xi, g, True)                          # sets the position
+    v, out = dev(rng.normal(size=(w.nfield, w.ny, w.nx))), torch.empty_like(xi)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, warmup):
+        for i in range(warmup):
+            fn(i)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(steps):
+            fn(i)
+        e1.record()
+        barrier()
+        t = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sh.ctx.launch_count()
+    ms = timed(lambda i: sh.metric_apply(v, out, True), args.steps, args.warmup)
+    launches = (sh.ctx.launch_count() - l0) * args.steps // (args.steps + args.warmup)
+    clocks = sampler.stop() if rank == 0 else None
+    b = (-g).contiguous()
+    x = torch.zeros_like(b)
+    iters = 10
+    ms_cg = timed(lambda i: sh.cg_solve(b, x, iters, True), 2, 1) / (2 * iters)
+    if rank == 0:
+        line = {"metric": "16-channel latent metric applies/s at 1024^2 (2048^2 padded), channel-sharded", "value": args.steps / (ms * 1e-3),
+                "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": f"config5: {w.nchan} x {w.ny}x{w.nx}, two latent fields; one step = frs_metric_apply on "
+                                       f"{len(sh.channels)} of {w.nchan} channels per rank + ONE all-reduce (NCCL) of {w.nfield} x {w.ny}x{w.nx} fp32",
+                           "l2": "no flush: a step streams > 1 GB per rank at world 1",
+                           "parallelism": f"channels sharded x{world} (ChannelShard), latent vectors replicated"},
+                "clocks": clocks, "gpu_launches": int(launches), "extra": {"ms_per_cg_iter": ms_cg}}
+        print(json.dumps(line), flush=True)
+    dist.destroy_process_group()
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start N ranks (one process per GPU) through torch.distributed.run,
+    exactly as the driver would, and hand its exit code back.  Rank 0 prints the single JSON line."""
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                         # keep NCCL's communicator log (transport, NVLS) ...
+    env.setdefault("NCCL_DEBUG_FILE", os.path.join(ROOT, "gpurun_out", "nccl_%h_%p.log"))   # ... out of the JSON line
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
 
 
 def main():
@@ -322,11 +440,18 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--shard", default="none", choices=["none", "channels"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
-        run_reference(args)
+        run_reference(args)                              # rank 0 alone runs the oracle; other ranks exit 0
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
+    elif args.shard == "channels":
+        if args.config != 5:
+            sys.exit("--shard channels needs --config 5 (single-channel configs do not shard, DESIGN.md Multi-GPU)")
+        run_sharded(args)
     else:
         run_cuda(args)
 

@@ -40,8 +40,12 @@ class ChannelShard:
         if len(self.channels) == 0:
             raise ValueError(f"rank {self.rank}: no channels to own ({nchan} channels over {self.world} ranks)")
         if make_ctx is None:
+            import torch
             from .binding import Context
-            make_ctx = Context
+            device = torch.cuda.current_device()              # one process per GPU: the rank's own device
+
+            def make_ctx(ny_, nx_, nc_):
+                return Context(ny_, nx_, nc_, device=device)
         self.ctx = make_ctx(ny, nx, len(self.channels))
         self.lognu = [float(lognu[c]) for c in self.channels]
         self.first = self.rank == 0                      # the rank that contributes the prior terms

@@ -371,6 +371,37 @@ def test_outer_newton_steps_teacher_forced(frs):
         xi = (xi + scale * d).contiguous()
 
 
+def _check_l2_apply_and_one_cg_step(frs, ctx, w, xi, s32):
+    """Latent metric apply (with and without the prior term) and ONE teacher-forced CG step at the position xi,
+    in the launch configuration of this size: the oracle repeats the step from the GPU's own (x, r, p, rr)."""
+    import torch
+    s64 = s32.astype(np.float64)
+    ap = lambda v, pr=True: o.metric_apply(w.w_half, w.amp, w.mu, w.lognu, xi, v, pr, s=s64)  # noqa: E731
+    v = np.random.default_rng(11).normal(size=xi.shape).astype(np.float32)
+    out = ctx.new_latent()
+    ctx.metric_apply(dev(v), out, with_prior=True)
+    mv = ap(v)
+    assert rel(out.cpu().numpy(), mv) <= TOL
+    ctx.metric_apply(dev(v), out, with_prior=False)
+    assert rel(out.cpu().numpy(), mv - v.astype(np.float64)) <= TOL
+    b = dev(np.random.default_rng(12).normal(size=xi.shape).astype(np.float32))
+    x = torch.zeros_like(b)
+    ctx.cg_solve(b, x, 0)                                          # r = p = b, rr = <b, b>
+    r, p, q, sc = ctx.cg_read_state()
+    x0, r0, p0, rr0 = (t.cpu().numpy().astype(np.float64) for t in (x, r, p)), None, None, float(sc[0])
+    x0, r0, p0 = list(x0)
+    assert abs(rr0 - np.sum(r0 * r0)) <= 1e-10 * rr0
+    ctx.cg_step(x, True)
+    r, p, q, sc = ctx.cg_read_state()
+    st = o.cg_step(ap, x0, r0, p0, rr0)
+    assert rel(q.cpu().numpy(), st["q"]) <= TOL
+    assert abs(sc[3] - st["alpha"]) <= TOL * abs(st["alpha"])
+    assert rel(x.cpu().numpy(), st["x"]) <= TOL
+    # r+ = r - alpha q: its rounding is measured against the size of the two operands
+    assert np.linalg.norm(r.cpu().numpy() - st["r"]) <= TOL * (np.linalg.norm(r0) + abs(st["alpha"]) * np.linalg.norm(st["q"]))
+    assert abs(sc[4] - st["beta"]) <= 1e-4 * abs(st["beta"])
+
+
 # ---------------------------------------------------------------------------------- full-size configs
 @pytest.mark.parametrize("cfg", [3, 4])
 def test_full_size_config_parity(frs, cfg):
@@ -395,6 +426,7 @@ def test_full_size_config_parity(frs, cfg):
     e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, True)
     assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
     assert rel(g.cpu().numpy(), g_ref) <= TOL
+    _check_l2_apply_and_one_cg_step(frs, ctx, w, xi, s32)
     del ctx
     torch.cuda.empty_cache()
 
@@ -420,3 +452,48 @@ def test_config5_multichannel_parity(frs):
     e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, True)
     assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
     assert rel(g.cpu().numpy(), g_ref) <= TOL
+    _check_l2_apply_and_one_cg_step(frs, ctx, w, xi, s32)
+
+
+def test_config2_as_stated_outer_steps_teacher_forced(frs):
+    """BASELINE.json configs[1] as stated: 512^2, 5 outer KL steps x 50 CG iterations (reading R10: zero-sample
+    Newton-CG with step halving).  Teacher-forced: at every xi the GPU visits, the oracle recomputes s, E and the
+    gradient; the energy must go down from step to step and every solve must run its 50 iterations."""
+    import torch
+    w = wl.make_config(2)
+    assert (w.ny, w.nx) == (512, 512)
+    ctx = make_ctx(frs, w)
+    xi = torch.zeros((1, w.ny, w.nx), device="cuda")
+    g, gt, s = ctx.new_latent(), ctx.new_latent(), ctx.new_image()
+    e_prev = None
+    for step in range(5):
+        e = ctx.energy_grad(xi, g, with_prior=True)
+        xih = xi.cpu().numpy()
+        ctx.sky_forward(xi, s)
+        assert rel(s.cpu().numpy(), o.sky(xih, w.amp, w.mu, w.lognu)) <= TOL
+        e_ref, g_ref = o.energy_grad(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xih, True)
+        assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
+        # Near the optimum the gradient J^T (C s - j) + xi is a cancellation (80-fold at the fifth step: |g| = 1e5 out of
+        # operands of 8e6), so there the error is held to 1e-6 of the operands J^T C s and J^T j; elsewhere to 1e-5 of g.
+        s64 = o.sky(xih, w.amp, w.mu, w.lognu)
+        ops = np.linalg.norm(o.vjp(w.amp, w.lognu, s64, np.stack([o.psf_apply(w.w_half[0], s64[0])]))) \
+            + np.linalg.norm(o.vjp(w.amp, w.lognu, s64, w.dirty.astype(np.float64)))
+        err = np.linalg.norm(g.cpu().numpy().astype(np.float64) - g_ref)
+        assert err <= max(TOL * np.linalg.norm(g_ref), 1e-6 * ops), (step, err, np.linalg.norm(g_ref), ops)
+        if step == 0:
+            assert err <= TOL * np.linalg.norm(g_ref)
+        if e_prev is not None:
+            assert e < e_prev
+        e_prev = e
+        b = (-g).contiguous()
+        d = torch.zeros_like(b)
+        it, rn = ctx.cg_solve(b, d, 50)
+        assert it == 50 and np.isfinite(rn)
+        scale = 1.0
+        for _ in range(5):
+            e1 = ctx.energy_grad((xi + scale * d).contiguous(), gt, with_prior=True)
+            if e1 < e:
+                break
+            scale *= 0.5
+        assert e1 < e
+        xi = (xi + scale * d).contiguous()

@@ -47,6 +47,37 @@ def test_stage_logic_replayed_on_cpu_matches_dft(library, n):
         assert np.allclose(frs.selftest_fft_host(d), np.exp(-2j * np.pi * q * np.arange(n) / n), atol=2e-6)
 
 
+@pytest.mark.parametrize("n", [256, 512, 1024, 2048, 4096])
+def test_dif_core_replayed_on_cpu_matches_dft(library, n):
+    """The DIF/DIT core of the column convolution (csrc/fft_dif.cuh), replayed thread by thread: the permuted spectrum,
+    sorted through its own register <-> frequency map, is the DFT; the inverse brings a sorted spectrum back."""
+    rng = np.random.default_rng(100 + n)
+    x = (rng.normal(size=n) + 1j * rng.normal(size=n)).astype(np.complex64)
+    ref = np.fft.fft(x.astype(np.complex128))
+    got = frs.selftest_dif_host(x)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) < 8e-7
+    inv = frs.selftest_dif_host(got, inverse=True)
+    assert np.linalg.norm(inv / n - x) / np.linalg.norm(x) < 1.5e-6
+    for q in (1, n // 2 + 1, n - 1):
+        d = np.zeros(n, np.complex64)
+        d[q] = 1
+        assert np.allclose(frs.selftest_dif_host(d), np.exp(-2j * np.pi * q * np.arange(n) / n), atol=3e-6)
+        assert np.allclose(frs.selftest_dif_host(d, inverse=True), np.exp(2j * np.pi * q * np.arange(n) / n), atol=3e-6)
+    with pytest.raises(frs.FrsError):
+        frs.selftest_dif_host(np.zeros(128, np.complex64))
+
+
+@pytest.mark.parametrize("n", [256, 512, 1024, 2048, 4096])
+def test_dif_exchange_is_race_free_and_conflict_free(library, n):
+    """What compute-sanitizer's racecheck would look at (the tool is closed on the GPU pool, profiles/r2_sanitizer.md):
+    every shared-memory access of two consecutive columns, lane by lane -- no two threads touch a slot (one of them
+    writing) without a barrier that orders them (a block barrier, or a warp sync between lanes of one warp), no slot
+    out of range, no bank conflict in any 128-bit access, and the register <-> frequency map is a bijection."""
+    conflict, hazards, oob, used, alloc, dup = frs.selftest_dif_exchange(n)
+    assert conflict == 1 and hazards == 0 and oob == 0 and dup == 0
+    assert used == n and used <= alloc
+
+
 @pytest.mark.parametrize("nf", [16, 32, 64, 128, 256, 512, 1024, 2048, 4096])
 def test_tma_copy_geometry_covers_and_fits(library, nf):
     """The tensor copies that feed the passes (csrc/tmap.h): the row gather must cover all nf + 1 bins of a
