@@ -9,9 +9,10 @@ bench.py's cpu_baseline / --impl reference legs.
 Library primitives used as steps: numpy.fft (pinned in tests against the O(n^2) DFT written
 out below and against the O(N^4) direct convolution), numpy.linalg.solve (CG pin only).
 
-Pins: tests/test_oracle_pins.py.  "parity unpinned": the absolute values of E and grad on
-real data -- the paper prints no operator value (last pin row); they are pinned
-only through the identities tested there.
+Pins: tests/test_oracle_pins.py (every function, incl. sky / log_sky / channel_coeff through the
+hand-worked fixture tests/golden/hand_sky_two_fields.txt, and the Eq. 9 / Eq. 15-18 functions).
+"parity unpinned": the absolute values of E and grad on real data -- the paper prints no operator
+value (last pin row); they are pinned only through the identities tested there.
 
 Shapes:  xi, amp  [nfield, ny, nx];  mu [nfield];  lognu [nchan];
          w_half   [nchan, My, nx+1]  (My = 2 ny, Mx = 2 nx; real >= 0 half spectrum of the PSF);
@@ -232,6 +233,61 @@ def metric_apply(w_half, amp, mu, lognu, xi, v, with_prior=True, s=None):
     jv = jvp(amp, mu, lognu, xi, v, s=s)
     cj = np.stack([psf_apply(w_half[c], jv[c]) for c in range(s.shape[0])])
     out = vjp(amp, lognu, s, cj)
+    if with_prior:
+        out = out + np.asarray(v, dtype=F64)
+    return out
+
+
+# =============================================================================
+# The likelihood the paper ran: Eq. 9 with the fitted noise kernel (Eq. 15-18; reading R14)
+# =============================================================================
+def noise_kernel_from_psf(w_half_c, eps):
+    """K = exp(xi_bar) + eps of Eq. 16-17 for one channel, [ny, nx].
+
+    Eq. 17: xi_bar minimises || N'(I_delta) - FFT^-1[(exp xi + eps) FFT(I_delta)] ||^2 with I_delta a point source in
+    the centre of the field and N' = R'+ eps 1 (Eq. 11), R' = the PSF convolution C (Eq. 13).  |FFT(I_delta)| = 1 at
+    every mode, so by Parseval the objective is sum_k |K[k] - K*[k]|^2 with K* = FFT(N' I_delta) conj FFT(I_delta),
+    and the minimiser over REAL K is Re K*; exp xi > 0 makes eps the floor (reading R14: K = max(Re K*, eps))."""
+    w = np.asarray(w_half_c, dtype=F64)
+    ny, nx = w.shape[0] // 2, w.shape[1] - 1
+    delta = np.zeros((ny, nx), dtype=F64)
+    delta[ny // 2, nx // 2] = 1.0
+    n_delta = psf_apply(w, delta) + eps * delta                      # N'(I_delta), Eq. 11 with Eq. 13
+    kstar = np.fft.fft2(n_delta) * np.conj(np.fft.fft2(delta))
+    return np.maximum(kstar.real, eps)
+
+
+def ninv_apply(kern, x):
+    """N'^-1 x = FFT^-1[ K^-1 . FFT x ] on the UNPADDED grid, periodic boundary (Eq. 18)."""
+    return np.real(np.fft.ifft2(np.fft.fft2(np.asarray(x, dtype=F64)) / np.asarray(kern, dtype=F64)))
+
+
+def energy_grad_eq9(w_half, kern, dirty, amp, mu, lognu, xi, with_prior=True):
+    """E = sum_c 1/2 (j_c - C_c s_c)^T N'_c^-1 (j_c - C_c s_c)  (Eq. 9 without the s-independent ln|2 pi N'|),
+    grad = -J^T C N'^-1 (j - C s);  + 1/2 <xi,xi>, + xi with the standard-normal prior."""
+    xi = np.asarray(xi, dtype=F64)
+    s = sky(xi, amp, mu, lognu)
+    e = 0.0
+    back = np.empty_like(s)
+    for c in range(s.shape[0]):
+        r = np.asarray(dirty[c], F64) - psf_apply(w_half[c], s[c])
+        u = ninv_apply(kern[c], r)
+        e += 0.5 * float(np.sum(r * u))
+        back[c] = -psf_apply(w_half[c], u)                           # C is symmetric
+    g = vjp(amp, lognu, s, back)
+    if with_prior:
+        e += 0.5 * float(np.sum(xi ** 2))
+        g = g + xi
+    return e, g
+
+
+def metric_apply_eq9(w_half, kern, amp, mu, lognu, xi, v, with_prior=True, s=None):
+    """M v = J^T C N'^-1 C J v (+ v): Fisher metric of the Gaussian likelihood of Eq. 9 (mean C s, covariance N')."""
+    if s is None:
+        s = sky(xi, amp, mu, lognu)
+    jv = jvp(amp, mu, lognu, xi, v, s=s)
+    t = np.stack([psf_apply(w_half[c], ninv_apply(kern[c], psf_apply(w_half[c], jv[c]))) for c in range(s.shape[0])])
+    out = vjp(amp, lognu, s, t)
     if with_prior:
         out = out + np.asarray(v, dtype=F64)
     return out

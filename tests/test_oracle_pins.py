@@ -393,3 +393,107 @@ def test_newton_cg_step_decreases_energy():
     xi = np.zeros((1, 16, 16))
     xi1, e0, e1 = o.newton_cg_step(w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, cg_iters=30)
     assert e1 < e0
+
+
+# ------------------------------------------------------------------ Eq. 9 with the fitted noise kernel (Eq. 15-18, R14)
+def test_noise_kernel_is_the_minimiser_of_eq17(small):
+    """Eq. 17 by brute force on a tiny grid: a generic minimiser over xi (K = exp xi + eps) lands on the closed form
+    wherever the unconstrained optimum is above the floor, and no perturbation of K lowers the residual."""
+    from scipy.optimize import minimize
+    w = wl.make_config(1, n=4, npts=300)
+    ny = nx = 4
+    eps = 1e-2 * float(np.sum(o.full_spectrum(w.w_half[0])))
+    kern = o.noise_kernel_from_psf(w.w_half[0], eps)
+    assert kern.shape == (ny, nx) and np.all(kern >= eps)
+    delta = np.zeros((ny, nx)); delta[ny // 2, nx // 2] = 1.0
+    target = o.psf_apply(w.w_half[0], delta) + eps * delta           # N'(I_delta)
+
+    def resid(k):
+        return float(np.sum(np.abs(target - np.fft.ifft2(k.reshape(ny, nx) * np.fft.fft2(delta))) ** 2))
+
+    r0 = resid(kern)
+    rng = np.random.default_rng(1)
+    for _ in range(50):                                              # K is a minimum among admissible kernels
+        trial = np.maximum(kern * (1 + 1e-3 * rng.normal(size=kern.shape)), eps)
+        assert resid(trial) >= r0 * (1 - 1e-12)
+    sol = minimize(lambda xi: resid(np.exp(xi) + eps), np.log(np.maximum(kern.ravel() - eps, 1e-3 * eps) + 1e-30),
+                   method="L-BFGS-B", options={"maxiter": 500, "ftol": 1e-15, "gtol": 1e-12})
+    free = kern.ravel() > 1.001 * eps
+    assert np.allclose((np.exp(sol.x) + eps)[free], kern.ravel()[free], rtol=1e-4)
+    assert sol.fun >= r0 * (1 - 1e-9)
+
+
+def test_noise_kernel_closed_forms():
+    ny, nx = 8, 16
+    # W == c: the PSF is a delta of weight c (2ny)(2nx), so N' = (c M + eps) 1 and K is flat
+    c, eps = 0.37, 0.05
+    wc = np.full((2 * ny, nx + 1), c)
+    assert np.allclose(o.noise_kernel_from_psf(wc, eps), c * 4 * ny * nx + eps, rtol=1e-12)
+    # K is real, even (K[-k] = K[k]) and >= eps for a generated PSF; its mean is the PSF peak + eps (sum_k K = N^2 n_delta[0])
+    w = wl.make_config(3, ny=ny, nx=nx, npts=3000)
+    eps = 1e-3 * float(np.sum(o.full_spectrum(w.w_half[0])))
+    k = o.noise_kernel_from_psf(w.w_half[0], eps)
+    kyi, kxi = (-np.arange(ny)) % ny, (-np.arange(nx)) % nx
+    assert np.allclose(k, k[np.ix_(kyi, kxi)], rtol=1e-12) and np.all(k >= eps)
+    unfloored = np.real(np.fft.fft2(np.roll(o.psf_from_weights(w.w_half[0]), (ny // 2, nx // 2), (0, 1))[:ny, :nx]
+                                    ) * np.conj(np.fft.fft2(np.eye(1, ny * nx, (ny // 2) * nx + nx // 2).reshape(ny, nx)))) + eps
+    assert np.allclose(k, np.maximum(unfloored, eps), rtol=1e-10, atol=1e-10 * k.max())      # the PSF stamp route
+
+
+def test_ninv_apply_closed_forms_and_symmetry():
+    ny, nx = 8, 16
+    rng = np.random.default_rng(21)
+    k = np.exp(rng.normal(size=(ny, nx)))
+    kyi, kxi = (-np.arange(ny)) % ny, (-np.arange(nx)) % nx
+    k = 0.5 * (k + k[np.ix_(kyi, kxi)])                              # a real even positive kernel
+    x, y = rng.normal(size=(ny, nx)), rng.normal(size=(ny, nx))
+    d = np.zeros((ny, nx)); d[0, 0] = 1.0
+    assert np.allclose(o.ninv_apply(k, d), np.real(np.fft.ifft2(1.0 / k)), atol=1e-14)      # N'^-1 delta = IFFT(1/K)
+    assert np.allclose(o.ninv_apply(np.full((ny, nx), 2.5), x), x / 2.5, atol=1e-14)        # K == c: N'^-1 = 1/c
+    assert abs(np.sum(o.ninv_apply(k, x) * y) - np.sum(x * o.ninv_apply(k, y))) <= 1e-12 * np.linalg.norm(x) * np.linalg.norm(y) / k.min()
+    assert np.sum(x * o.ninv_apply(k, x)) > 0
+    # inverse of the forward convolution of Eq. 15, and periodic (P:206): a shift commutes with it
+    assert np.allclose(o.ninv_apply(k, np.real(np.fft.ifft2(k * np.fft.fft2(x)))), x, atol=1e-12)
+    assert np.allclose(o.ninv_apply(k, np.roll(x, (3, 5), (0, 1))), np.roll(o.ninv_apply(k, x), (3, 5), (0, 1)), atol=1e-13)
+    # the Hartley form the kernels use: N'^-1 x = H[ K^-1 . H[x] ] / (ny nx) for an even kernel
+    assert np.allclose(o.hartley2(o.hartley2(x) / k) / (ny * nx), o.ninv_apply(k, x), atol=1e-13)
+
+
+@pytest.mark.parametrize("which", ["small", "multi"])
+def test_eq9_gradient_metric_and_limits(which, small, multi):
+    w = small if which == "small" else multi
+    rng = np.random.default_rng(22)
+    eps = 1e-2 * float(np.sum(o.full_spectrum(w.w_half[0])))
+    kern = np.stack([o.noise_kernel_from_psf(w.w_half[c], eps) for c in range(w.nchan)])
+    xi = 0.3 * rng.normal(size=(w.nfield, w.ny, w.nx))
+    e0, g = o.energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi, True)
+    # written out: E = 1/2 sum_c r_c^T N'^-1 r_c + 1/2 xi^2, r = j - C s
+    s = o.sky(xi, w.amp, w.mu, w.lognu)
+    e_def = 0.5 * np.sum(xi ** 2)
+    for c in range(w.nchan):
+        r = w.dirty[c] - o.psf_apply(w.w_half[c], s[c])
+        e_def += 0.5 * np.sum(r * np.real(np.fft.ifft2(np.fft.fft2(r) / kern[c])))
+    assert abs(e0 - e_def) <= 1e-12 * abs(e_def)
+    for _ in range(5):                                               # central differences, 1e-6
+        d = rng.normal(size=xi.shape)
+        h = 1e-5 * np.linalg.norm(xi) / np.linalg.norm(d)
+        ep = o.energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi + h * d, True)[0]
+        em = o.energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi - h * d, True)[0]
+        fd = (ep - em) / (2 * h)
+        assert abs(fd - np.sum(g * d)) <= 1e-6 * max(abs(fd), np.linalg.norm(g) * np.linalg.norm(d) * 1e-3)
+    # metric: composition, symmetry, M >= 1
+    u, v = rng.normal(size=xi.shape), rng.normal(size=xi.shape)
+    mv = o.metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, v, True)
+    jv = o.jvp(w.amp, w.mu, w.lognu, xi, v)
+    comp = o.vjp(w.amp, w.lognu, s, np.stack([o.psf_apply(w.w_half[c], o.ninv_apply(kern[c], o.psf_apply(w.w_half[c], jv[c])))
+                                              for c in range(w.nchan)])) + v
+    assert rel(mv, comp) < 1e-13
+    mu_ = o.metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, u, True)
+    assert abs(np.sum(u * mv) - np.sum(mu_ * v)) <= 1e-10 * abs(np.sum(u * mv))
+    assert np.sum(v * mv) >= np.sum(v * v)
+    # eps -> infinity: N'^-1 -> 1/eps, so eps E_lh -> 1/2 |j - C s|^2 and eps M_lh -> J^T C C J
+    big = 1e12 * float(np.max(kern))
+    kbig = np.stack([o.noise_kernel_from_psf(w.w_half[c], big) for c in range(w.nchan)])
+    e_big = o.energy_grad_eq9(w.w_half, kbig, w.dirty, w.amp, w.mu, w.lognu, xi, False)[0]
+    r2 = sum(np.sum((w.dirty[c] - o.psf_apply(w.w_half[c], s[c])) ** 2) for c in range(w.nchan))
+    assert abs(big * e_big - 0.5 * r2) <= 1e-9 * r2
