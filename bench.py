@@ -14,8 +14,8 @@ config does shard: `--config 5 --shard channels` times the channel-sharded laten
 (ChannelShard: one NCCL all-reduce per apply), strong scaling.
 
 The timed operator is the N' = R' limit of the paper's Eq. 9 (E = 1/2 s^T C s - j^T s, metric J^T C J, DESIGN.md R1);
-the separate fitted noise kernel of Eq. 15-18 is the `--noise-kernel` variant of the latent calls (three convolutions
-per apply), reported under "extra".
+with the separately fitted noise kernel of Eq. 15-18 (frs_set_noise_kernel + frs_set_likelihood(1)) a latent metric apply
+is three convolutions; its time is reported under "extra" (eq9_metric_apply_ms).
 """
 from __future__ import annotations
 
@@ -305,6 +305,12 @@ def run_cuda(args):
             e1.record()
             torch.cuda.synchronize()
             extra["ms_per_cg_iter"] = e0.elapsed_time(e1) / (iters + 1)   # + the initial M x0 apply
+            # the paper's literal likelihood (Eq. 9 with the fitted noise kernel): J^T C N'^-1 C J + 1
+            ctx.set_noise_kernel(1e-2 * float(np.sum(w.w_half[0][:, 0]) + 2 * np.sum(w.w_half[0][:, 1:-1]) + np.sum(w.w_half[0][:, -1])))
+            ctx.set_likelihood(1)
+            m = timed(lambda i: ctx.metric_apply(v, out, True), k2, 3)
+            extra["eq9_metric_apply_ms"] = m / k2
+            ctx.set_likelihood(0)
 
     if world > 1:
         dist.barrier()

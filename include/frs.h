@@ -110,6 +110,28 @@ int frs_cg_step(frs_ctx* ctx, float* x, int with_prior);
 int frs_cg_step_begin(frs_ctx* ctx, float** d_q);
 int frs_cg_step_end(frs_ctx* ctx, float* x, int with_prior);
 
+/* ---- the likelihood the paper ran: Eq. 9 with the separately fitted noise kernel ----------------
+ * P:154 (Eq. 9), P:162 (Eq. 11), P:186-206 (Eq. 15-18); reading R14.
+ *   E_lh = 1/2 (j - C s)^T N'^-1 (j - C s),  N'^-1 x = FFT^-1[ K^-1 . FFT x ]  on the UNPADDED ny x nx grid, periodic
+ *   (Eq. 18), K = exp(xi_bar) + eps real, even and >= eps (Eq. 16);  Fisher metric J^T C N'^-1 C J (+ 1).
+ * The default likelihood of every call above is its N' = R' limit (mode 0). */
+
+/* Fit K to the PSF that is set (Eq. 17, closed form by Parseval: K = max(Re[FFT(N' I_delta) conj FFT(I_delta)], eps),
+ * I_delta a point source at (ny/2, nx/2), N' = C + eps 1).  eps > 0 (same units as the PSF).  Errors: FRS_ESTATE
+ * without a PSF, FRS_EINVAL for eps <= 0.  A later frs_set_psf* discards the kernel and returns to mode 0. */
+int frs_set_noise_kernel(frs_ctx* ctx, float eps);
+/* Or supply K directly: device [nchan][ny][nx], harmonic (DFT) order, strictly positive and even (K[-k] = K[k] to
+ * 1e-5 relative), else FRS_ENOTPSD.  Copied. */
+int frs_set_noise_kernel_array(frs_ctx* ctx, const float* kern);
+/* Copy of the kernel in use, device [nchan][ny][nx]. */
+int frs_get_noise_kernel(frs_ctx* ctx, float* kern);
+/* y = N'^-1 x (sky space, [nchan][ny][nx]); x == y allowed. */
+int frs_ninv_apply(frs_ctx* ctx, const float* x, float* y);
+/* mode 0: E = 1/2 s^T C s - j^T s, metric J^T C J (+1)   (N' = R' limit, R1)
+ * mode 1: Eq. 9 with N'^-1 of Eq. 18, metric J^T C N'^-1 C J (+1); needs a noise kernel (else FRS_ESTATE).
+ * Affects frs_energy_grad, frs_metric_apply, frs_cg_solve / _step / _step_begin. */
+int frs_set_likelihood(frs_ctx* ctx, int mode);
+
 /* ---- host-buffer entry points (end-to-end measurements: copies are part of the call) -------- */
 
 /* y = s . C (s . x) with x, y in HOST memory (pinned or pageable), [nchan][ny][nx].

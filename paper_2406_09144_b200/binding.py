@@ -36,6 +36,11 @@ EXPORTS = {
     "frs_cg_step": (_i, [_vp, _vp, _i]),
     "frs_cg_step_begin": (_i, [_vp, C.POINTER(_vp)]),
     "frs_cg_step_end": (_i, [_vp, _vp, _i]),
+    "frs_set_noise_kernel": (_i, [_vp, _f]),
+    "frs_set_noise_kernel_array": (_i, [_vp, _vp]),
+    "frs_get_noise_kernel": (_i, [_vp, _vp]),
+    "frs_ninv_apply": (_i, [_vp, _vp, _vp]),
+    "frs_set_likelihood": (_i, [_vp, _i]),
     "frs_sky_metric_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_psf_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_launch_count": (C.c_longlong, [_vp]),
@@ -210,6 +215,26 @@ class Context:
 
     def set_sky(self, sky):
         self._ck(lib().frs_set_sky(self._h, _ptr(sky, self.f32, self.nchan * self.npix, "sky")))
+
+    # ---- Eq. 9 with the fitted noise kernel
+    def set_noise_kernel(self, eps=None, kern=None):
+        if kern is not None:
+            self._ck(lib().frs_set_noise_kernel_array(self._h, _ptr(kern, self.f32, self.nchan * self.npix, "kern")))
+        else:
+            self._ck(lib().frs_set_noise_kernel(self._h, float(eps)))
+
+    def get_noise_kernel(self):
+        k = self.new_image()
+        self._ck(lib().frs_get_noise_kernel(self._h, k.data_ptr()))
+        return k
+
+    def ninv_apply(self, x, y):
+        self._ck(lib().frs_ninv_apply(self._h, _ptr(x, self.f32, self.nchan * self.npix, "x"),
+                                      _ptr(y, self.f32, self.nchan * self.npix, "y")))
+        return y
+
+    def set_likelihood(self, mode):
+        self._ck(lib().frs_set_likelihood(self._h, int(mode)))
 
     # ---- hot path
     def sky_forward(self, xi, sky=None):

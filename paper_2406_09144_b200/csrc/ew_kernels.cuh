@@ -111,6 +111,44 @@ __global__ void energy_final_kernel(const double* __restrict__ sc_sc, const doub
     *e = 0.5 * (*sc_sc) - (*sc_js) + (with_prior ? 0.5 * (*sc_xx) : 0.0);
 }
 
+// ---- noise kernel of Eq. 16-17 (reading R14) from the transposed Hartley transform HT[kx][ky] of t = C I_delta, I_delta at
+// (ny/2, nx/2):  Re FFT(t)[k] = (H[k] + H[-k]) / 2, conj FFT(I_delta)[k] = (-1)^(ky+kx), + eps from the eps I_delta term:
+//   K = max((-1)^(ky+kx) (H[k] + H[-k]) / 2 + eps, eps);   kern[ky][kx] = K;  kinv = 1 / (K ny nx) in both orientations
+__global__ void noise_kernel_finish_kernel(const float* __restrict__ ht, float eps, float* __restrict__ kern,
+                                           float* __restrict__ kinv_n, float* __restrict__ kinv_t, int ny, int nx) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, npix = (size_t)ny * nx;
+    if (i >= npix) return;
+    const size_t b = blockIdx.y * npix;
+    const int ky = (int)(i / nx), kx = (int)(i % nx);
+    const int my = (ny - ky) % ny, mx = (nx - kx) % nx;
+    const float h = ht[b + (size_t)kx * ny + ky], hm = ht[b + (size_t)mx * ny + my];
+    const float sgn = ((ky + kx) & 1) ? -1.f : 1.f;
+    const float k = fmaxf(fmaf(sgn * 0.5f, h + hm, eps), eps);
+    kern[b + i] = k;
+    const float inv = 1.0f / (k * (float)ny * (float)nx);
+    kinv_n[b + i] = inv;
+    kinv_t[b + (size_t)kx * ny + ky] = inv;
+}
+// a caller-supplied kernel: flags non-positive / NaN entries and departures from K[-k] = K[k] beyond 1e-5 max-free relative
+__global__ void noise_kernel_from_array_kernel(const float* __restrict__ kern, float* __restrict__ kinv_n,
+                                               float* __restrict__ kinv_t, int ny, int nx, int* __restrict__ bad) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, npix = (size_t)ny * nx;
+    if (i >= npix) return;
+    const size_t b = blockIdx.y * npix;
+    const int ky = (int)(i / nx), kx = (int)(i % nx);
+    const float k = kern[b + i], km = kern[b + (size_t)((ny - ky) % ny) * nx + (nx - kx) % nx];
+    if (!(k > 0.f) || !(fabsf(k - km) <= 1e-5f * fmaxf(k, km))) atomicExch(bad, 1);
+    const float inv = 1.0f / (k * (float)ny * (float)nx);
+    kinv_n[b + i] = inv;
+    kinv_t[b + (size_t)kx * ny + ky] = inv;
+}
+__global__ void set_delta_kernel(float* __restrict__ img, size_t npix, size_t pos) { img[blockIdx.x * npix + pos] = 1.0f; }
+// E = 0.5 <r, N'^-1 r> + 0.5 with_prior <xi, xi>
+__global__ void energy9_final_kernel(const double* __restrict__ ru, const double* __restrict__ xx, int with_prior,
+                                     double* __restrict__ e) {
+    *e = 0.5 * (*ru) + (with_prior ? 0.5 * (*xx) : 0.0);
+}
+
 // ---- CG (reading R9).  scal[0]=rr, [1]=pq, [2]=rr_new, [3]=alpha, [4]=beta, [5]=breakdown flag
 enum { kRR = 0, kPQ = 1, kRRNew = 2, kAlpha = 3, kBeta = 4, kBreak = 5, kBB = 6, kNScal = 8 };
 

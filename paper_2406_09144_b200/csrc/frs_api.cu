@@ -39,6 +39,10 @@ struct frs_ctx {
     struct MapKey { const void* p; int rows, nf, nb; CUtensorMap row, col; };   // col: of T; row: columns map of T2
     std::vector<MapKey> maps;  // spectrum tensor maps (tmap.h), built on first use
     float *lin = nullptr, *img = nullptr, *acc = nullptr;
+    // Eq. 9 with the fitted noise kernel (R14): K, 1/(K ny nx) in both orientations, two more image-sized scratch arrays
+    float *kern = nullptr, *kinvN = nullptr, *kinvT = nullptr, *img2 = nullptr, *img3 = nullptr;
+    bool have_kern = false;
+    int lik_mode = 0;                // 0: N' = R' limit, 1: Eq. 9 with N'^-1 of Eq. 18
     float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
     float *hx = nullptr, *hy = nullptr;
     double *partials = nullptr, *scal = nullptr;   // scal: [0..7] CG, [8] sum s.c, [9] sum j.s, [10] <xi,xi>, [11] E
@@ -124,7 +128,8 @@ int ensure_scratch(frs_ctx* ctx) {
     const size_t np = ctx->npix, ny = ctx->ny, nx = ctx->nx;
     RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2(spec_batch_stride(ctx->ny, ctx->nx), spec_batch_stride(ctx->nx, ctx->ny))));
     RET(dev_alloc(ctx, &ctx->T2, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
-    RET(dev_alloc(ctx, &ctx->Th, (size_t)2 * max2(spec_batch_stride(ctx->ny, ctx->nx / 2), spec_batch_stride(ctx->nx, ctx->ny / 2))));
+    RET(dev_alloc(ctx, &ctx->Th, (size_t)(ctx->nchan > 2 ? ctx->nchan : 2) *
+                                     max2(spec_batch_stride(ctx->ny, ctx->nx / 2), spec_batch_stride(ctx->nx, ctx->ny / 2))));
     RET(dev_alloc(ctx, &ctx->lin, 2 * np));
     RET(dev_alloc(ctx, &ctx->acc, 2 * np));
     RET(dev_alloc(ctx, &ctx->img, (size_t)ctx->nchan * np));
@@ -214,14 +219,14 @@ int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const flo
 // one contiguous run of the transposed output -- so the transform transposes for free, and the
 // latent-space path keeps its sky-space arrays transposed instead of paying for scattered stores.
 int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul, float* out, const float* mul,
-              const float* add, const float* offset_dev, int nb, double* d_dot = nullptr) {
+              const float* add, const float* offset_dev, int nb, double* d_dot = nullptr, float sign = 1.0f) {
     const int ntile_h = n2 / 4 + 1;
     {
         Prof pr(ctx, kPassHartRows);
         RowsFwdArgs a{};
         a.in = in; a.mul = premul; a.out = ctx->Th; a.ny = n1;
         a.in_bstride = ctx->npix; a.mul_bstride = ctx->npix;
-        a.scale = 0.5f;
+        a.scale = 0.5f * sign;   // sign = -1: the transform of -in (offset must be absent)
         a.tw = ctx->tw[n2 / 2]; a.twist = ctx->twist[n2 / 2];
         CKL(launch_rows_fwd(ctx->stream, n2 / 2, false, a, nb));
         ctx->launches++;
@@ -280,8 +285,57 @@ int sky_forward_impl(frs_ctx* ctx, const float* xi) {
     return FRS_OK;
 }
 
+// ---- Eq. 9 with the fitted noise kernel (reading R14) -------------------------------------
+// u = N'^-1 r = H[ K^-1 . H[r] ] / (ny nx) for the real even kernel K (Eq. 18: periodic, unpadded), in the transposed
+// orientation of the latent-space path: r, u [nchan][nx][ny]; the intermediate is in the natural orientation.
+int ninv_transposed(frs_ctx* ctx, const float* r, float* u) {
+    RET(hartley_t(ctx, r, ctx->nx, ctx->ny, nullptr, ctx->img3, ctx->kinvN, nullptr, nullptr, ctx->nchan));
+    RET(hartley_t(ctx, ctx->img3, ctx->ny, ctx->nx, nullptr, u, nullptr, nullptr, nullptr, ctx->nchan));
+    return FRS_OK;
+}
+int ensure_scratch9(frs_ctx* ctx) {
+    RET(dev_alloc(ctx, &ctx->img2, (size_t)ctx->nchan * ctx->npix));
+    RET(dev_alloc(ctx, &ctx->img3, (size_t)ctx->nchan * ctx->npix));
+    return FRS_OK;
+}
+
+// M v = J^T C N'^-1 C J v (+ v): three convolutions per apply (two padded, one periodic)
+int metric_apply9_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, double* d_vmv) {
+    const Orient o = orient(ctx, true);
+    RET(need_s_transposed(ctx));
+    RET(ensure_scratch9(ctx));
+    RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
+    const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
+    if (simple) {
+        RET(conv_rows_fwd(ctx, o, ctx->lin, ctx->sT));
+    } else {
+        jvp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->sT, ctx->d_lognu, ctx->img,
+                                                                               ctx->npix, ctx->nfield, ctx->nchan);
+        ctx->launches++;
+        RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
+    }
+    RET(conv_cols(ctx, o));
+    RET(conv_rows_inv(ctx, o, ctx->img2, kPlain, nullptr, nullptr, nullptr));            // C J v
+    RET(ninv_transposed(ctx, ctx->img2, ctx->img));                                       // N'^-1 C J v
+    RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
+    RET(conv_cols(ctx, o));
+    if (simple) {
+        RET(conv_rows_inv(ctx, o, ctx->acc, kMulS, ctx->sT, nullptr, nullptr));
+    } else {
+        RET(conv_rows_inv(ctx, o, ctx->img, kMulS, ctx->sT, nullptr, nullptr));
+        vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
+                                                                               ctx->nfield, ctx->nchan);
+        ctx->launches++;
+    }
+    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield,
+                  with_prior ? d_vmv : nullptr));
+    CK(cudaGetLastError());
+    return FRS_OK;
+}
+
 // d_vmv (device, optional, needs with_prior): <v, M v>, accumulated in the last pass instead of a separate dot
 int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, double* d_vmv = nullptr) {
+    if (ctx->lik_mode == 1) return metric_apply9_impl(ctx, v, with_prior, out, d_vmv);
     const Orient o = orient(ctx, true);
     RET(need_s_transposed(ctx));
     // lin_f = H[A_f v_f]   (transposed)
@@ -393,7 +447,7 @@ void frs_destroy(frs_ctx* ctx) {
     for (auto& kv : ctx->tw) cudaFree(kv.second);
     for (auto& kv : ctx->twd) cudaFree(kv.second);
     for (auto& kv : ctx->twist) cudaFree(kv.second);
-    void* ptrs[] = {ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
+    void* ptrs[] = {ctx->kern, ctx->kinvN, ctx->kinvT, ctx->img2, ctx->img3, ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -429,6 +483,7 @@ int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
     CK(cudaStreamSynchronize(ctx->stream));
     if (neg) { ctx->have_psf = false; return fail(ctx, FRS_ENOTPSD, "PSF weights contain negative or NaN entries"); }
     ctx->have_psf = true;
+    ctx->have_kern = false; ctx->lik_mode = 0;    // a kernel fitted to the previous PSF no longer applies
     return FRS_OK;
 }
 
@@ -571,6 +626,36 @@ int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_ene
     if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
     RET(sky_forward_impl(ctx, xi));
     const Orient o = orient(ctx, true);                       // sky-space arrays transposed on this path
+    if (ctx->lik_mode == 1) {
+        // E = 1/2 r^T N'^-1 r, r = j - C s;  grad = -J^T C N'^-1 r (+ xi)        (Eq. 9, R14)
+        RET(ensure_scratch9(ctx));
+        RET(conv_rows_fwd(ctx, o, ctx->sT, nullptr));
+        RET(conv_cols(ctx, o));
+        RET(conv_rows_inv(ctx, o, ctx->img2, kResid, nullptr, ctx->dirtyT, nullptr));     // r
+        RET(ninv_transposed(ctx, ctx->img2, ctx->img));                                    // u = N'^-1 r
+        RET(dot(ctx, ctx->img2, ctx->img, (size_t)ctx->nchan * ctx->npix, ctx->scal + 8));
+        if (with_prior) RET(dot(ctx, xi, xi, (size_t)ctx->nfield * ctx->npix, ctx->scal + 10));
+        energy9_final_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal + 8, ctx->scal + 10, with_prior, ctx->scal + 11);
+        ctx->launches++;
+        RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
+        RET(conv_cols(ctx, o));
+        const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
+        RET(conv_rows_inv(ctx, o, simple ? ctx->acc : ctx->img, kMulS, ctx->sT, nullptr, nullptr));   // s . C u
+        if (!simple) {
+            vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
+                                                                                   ctx->nfield, ctx->nchan);
+            ctx->launches++;
+        }
+        RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, grad, ctx->amp, with_prior ? xi : nullptr, nullptr, ctx->nfield,
+                      nullptr, -1.0f));
+        CK(cudaGetLastError());
+        if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+        if (h_energy) {
+            CK(cudaMemcpyAsync(h_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+        }
+        return FRS_OK;
+    }
     RET(conv_rows_fwd(ctx, o, ctx->sT, nullptr));
     RET(conv_cols(ctx, o));
     int gx = 0;
@@ -703,6 +788,82 @@ int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rto
     if (h_iters) *h_iters = it;
     if (h_resnorm) *h_resnorm = sqrt(sc[kRR]);
     if (sc[kBreak] != 0.0) return fail(ctx, FRS_EBREAKDOWN, "CG breakdown: <p, M p> <= 0");
+    return FRS_OK;
+}
+
+// ---- the paper's literal likelihood: noise kernel of Eq. 15-18 ------------------------------------
+static int kernel_arrays(frs_ctx* ctx) {
+    const size_t n = (size_t)ctx->nchan * ctx->npix;
+    RET(dev_alloc(ctx, &ctx->kern, n));
+    RET(dev_alloc(ctx, &ctx->kinvN, n));
+    RET(dev_alloc(ctx, &ctx->kinvT, n));
+    return ensure_scratch9(ctx);
+}
+
+int frs_set_noise_kernel(frs_ctx* ctx, float eps) {
+    if (!ctx || !(eps > 0.f)) return fail(ctx, FRS_EINVAL, "frs_set_noise_kernel: eps must be > 0");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, false, false));
+    RET(kernel_arrays(ctx));
+    const size_t n = (size_t)ctx->nchan * ctx->npix;
+    // t = C I_delta with the point source in the centre of the field (Eq. 17), one per channel
+    CK(cudaMemsetAsync(ctx->img2, 0, n * sizeof(float), ctx->stream));
+    set_delta_kernel<<<ctx->nchan, 1, 0, ctx->stream>>>(ctx->img2, ctx->npix, (size_t)(ctx->ny / 2) * ctx->nx + ctx->nx / 2);
+    ctx->launches++;
+    const Orient o = orient(ctx, false);
+    RET(conv_rows_fwd(ctx, o, ctx->img2, nullptr));
+    RET(conv_cols(ctx, o));
+    RET(conv_rows_inv(ctx, o, ctx->img, kPlain, nullptr, nullptr, nullptr));
+    RET(hartley_t(ctx, ctx->img, ctx->ny, ctx->nx, nullptr, ctx->img3, nullptr, nullptr, nullptr, ctx->nchan));   // [nx][ny]
+    dim3 grid((unsigned)((ctx->npix + 255) / 256), ctx->nchan);
+    noise_kernel_finish_kernel<<<grid, 256, 0, ctx->stream>>>(ctx->img3, eps, ctx->kern, ctx->kinvN, ctx->kinvT, ctx->ny, ctx->nx);
+    ctx->launches++;
+    CK(cudaGetLastError());
+    ctx->have_kern = true;
+    return FRS_OK;
+}
+
+int frs_set_noise_kernel_array(frs_ctx* ctx, const float* kern) {
+    if (!ctx || !kern || !aligned16(kern)) return fail(ctx, FRS_EINVAL, "frs_set_noise_kernel_array: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(ensure_scratch(ctx));
+    RET(kernel_arrays(ctx));
+    const size_t n = (size_t)ctx->nchan * ctx->npix;
+    CK(cudaMemcpyAsync(ctx->kern, kern, n * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaMemsetAsync(ctx->flag, 0, sizeof(int), ctx->stream));
+    dim3 grid((unsigned)((ctx->npix + 255) / 256), ctx->nchan);
+    noise_kernel_from_array_kernel<<<grid, 256, 0, ctx->stream>>>(ctx->kern, ctx->kinvN, ctx->kinvT, ctx->ny, ctx->nx, ctx->flag);
+    ctx->launches++;
+    int bad = 0;
+    CK(cudaMemcpyAsync(&bad, ctx->flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (bad) { ctx->have_kern = false; return fail(ctx, FRS_ENOTPSD, "noise kernel must be > 0 and even (K[-k] = K[k])"); }
+    ctx->have_kern = true;
+    return FRS_OK;
+}
+
+int frs_get_noise_kernel(frs_ctx* ctx, float* kern) {
+    if (!ctx || !kern || !aligned16(kern)) return fail(ctx, FRS_EINVAL, "frs_get_noise_kernel: bad argument");
+    if (!ctx->have_kern) return fail(ctx, FRS_ESTATE, "noise kernel not set (frs_set_noise_kernel)");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemcpyAsync(kern, ctx->kern, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    return FRS_OK;
+}
+
+int frs_ninv_apply(frs_ctx* ctx, const float* x, float* y) {
+    if (!ctx || !x || !y || !aligned16(x) || !aligned16(y)) return fail(ctx, FRS_EINVAL, "frs_ninv_apply: bad argument");
+    if (!ctx->have_kern) return fail(ctx, FRS_ESTATE, "noise kernel not set (frs_set_noise_kernel)");
+    CK(cudaSetDevice(ctx->device));
+    RET(ensure_scratch(ctx));
+    RET(hartley_t(ctx, x, ctx->ny, ctx->nx, nullptr, ctx->img3, ctx->kinvT, nullptr, nullptr, ctx->nchan));   // [nx][ny]
+    RET(hartley_t(ctx, ctx->img3, ctx->nx, ctx->ny, nullptr, y, nullptr, nullptr, nullptr, ctx->nchan));
+    return FRS_OK;
+}
+
+int frs_set_likelihood(frs_ctx* ctx, int mode) {
+    if (!ctx || (mode != 0 && mode != 1)) return fail(ctx, FRS_EINVAL, "frs_set_likelihood: mode must be 0 or 1");
+    if (mode == 1 && !ctx->have_kern) return fail(ctx, FRS_ESTATE, "noise kernel not set (frs_set_noise_kernel)");
+    ctx->lik_mode = mode;
     return FRS_OK;
 }
 

@@ -19,6 +19,7 @@ int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* 
 #define CALL(N)                                                            \
     return a.mode == kPlain ? run<N, kPlain>(st, a, nb, grid_x)            \
          : a.mode == kMulS  ? run<N, kMulS>(st, a, nb, grid_x)             \
+         : a.mode == kResid ? run<N, kResid>(st, a, nb, grid_x)            \
                             : run<N, kEnergy>(st, a, nb, grid_x)
     FRS_DISPATCH_NF(nf, CALL)
 #undef CALL

@@ -1,6 +1,6 @@
 // kernels_inv.inl -- inverse row pass of the convolution (included inside namespace frs by kernels.cuh)
 
-enum RowsInvMode { kPlain = 0, kMulS = 1, kEnergy = 2 };
+enum RowsInvMode { kPlain = 0, kMulS = 1, kEnergy = 2, kResid = 3 };   // kResid: out = j - c (residual of Eq. 9)
 
 struct RowsInvArgs {
     CUtensorMap tmap;     // columns map of t (tmap.h)
@@ -8,7 +8,7 @@ struct RowsInvArgs {
     int cols;             // allocated columns per batch
     float* out;           // [nb][ny][NF]
     const float* s;       // [nb][ny][NF]  (kMulS, kEnergy)
-    const float* j;       // [nb][ny][NF]  (kEnergy)
+    const float* j;       // [nb][ny][NF]  (kEnergy, kResid)
     double* partials;     // [gridDim.x][2]  (kEnergy): sum s*c, sum j*s
     int ny, mode;
     int items_per_batch, nitems;
@@ -65,8 +65,8 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
             // warm L2 with the rows of s (and j) the epilogue of that item will read: P lines of 128 B
             if (MODE != kPlain) {
                 const size_t row = b * a.img_bstride + (size_t)(2 * rp) * NF;
-                prefetch_l2(a.s + row + 32 * p);
-                if (MODE == kEnergy) prefetch_l2(a.j + row + 32 * p);
+                if (MODE != kResid) prefetch_l2(a.s + row + 32 * p);
+                if (MODE == kEnergy || MODE == kResid) prefetch_l2(a.j + row + 32 * p);
             }
         }
     };
@@ -112,13 +112,13 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
         if (live) {
             const size_t row0 = b * a.img_bstride + (size_t)y0 * NF;
             float2 sv[2][kE / 2], jv[2][kE / 2];
-            if (MODE != kPlain) {
+            if (MODE == kMulS || MODE == kEnergy) {
 #pragma unroll
                 for (int t = 0; t < 2; ++t)
 #pragma unroll
                     for (int e = 0; e < kE / 2; ++e) sv[t][e] = ldg2(a.s + row0 + (size_t)t * NF + 2 * (p + e * P));
             }
-            if (MODE == kEnergy) {
+            if (MODE == kEnergy || MODE == kResid) {
 #pragma unroll
                 for (int t = 0; t < 2; ++t)
 #pragma unroll
@@ -136,6 +136,8 @@ rows_inv_kernel(const __grid_constant__ RowsInvArgs a) {
                         acc_sc += (double)s.x * (double)c.x + (double)s.y * (double)c.y;
                         acc_js += (double)j.x * (double)s.x + (double)j.y * (double)s.y;
                         c.x = s.x * (c.x - j.x); c.y = s.y * (c.y - j.y);
+                    } else if (MODE == kResid) {
+                        c.x = jv[t][e].x - c.x; c.y = jv[t][e].y - c.y;
                     }
                     stg2(a.out + row0 + (size_t)t * NF + 2 * (p + e * P), c);
                 }
