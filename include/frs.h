@@ -89,8 +89,12 @@ int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_ene
 int frs_metric_apply(frs_ctx* ctx, const float* v, int with_prior, float* out);
 /* Solve M x = b by textbook CG (R9).  x: in = x0, out = solution.  Runs until max_iter or
  * ||r|| <= rtol ||b|| (rtol = 0: exactly max_iter iterations, fully asynchronous until the end).
+ * The stopping test is evaluated on the DEVICE after every iteration; once it holds, the vector updates of the
+ * iterations still enqueued are no-ops, so x is exactly the iterate at which the test was met.  With rtol > 0 the
+ * host reads the flag every 8 iterations only to stop enqueueing (up to 7 wasted metric applies, no change of x).
  * h_iters (host, may be NULL): iterations done.  h_resnorm (host, may be NULL): final ||r||.
- * d_res_history (DEVICE double [max_iter+1], may be NULL): ||r_k||.  Synchronises at the end. */
+ * d_res_history (DEVICE double [max_iter+1], may be NULL): ||r_k|| (constant after the stopping point).
+ * Synchronises at the end.  FRS_EBREAKDOWN if <p, M p> <= 0 was met (x is the last good iterate). */
 int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior,
                  int* h_iters, double* h_resnorm, double* d_res_history);
 /* Copy out the CG state of the last frs_cg_solve / frs_cg_step: r, p, q (DEVICE pointers,

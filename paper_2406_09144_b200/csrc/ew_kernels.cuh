@@ -149,8 +149,11 @@ __global__ void energy9_final_kernel(const double* __restrict__ ru, const double
     *e = 0.5 * (*ru) + (with_prior ? 0.5 * (*xx) : 0.0);
 }
 
-// ---- CG (reading R9).  scal[0]=rr, [1]=pq, [2]=rr_new, [3]=alpha, [4]=beta, [5]=breakdown flag
-enum { kRR = 0, kPQ = 1, kRRNew = 2, kAlpha = 3, kBeta = 4, kBreak = 5, kBB = 6, kNScal = 8 };
+// ---- CG (reading R9).  scal[0]=rr, [1]=pq, [2]=rr_new, [3]=alpha, [4]=beta, [5]=breakdown flag, [6]=<b,b>, [7]=done flag;
+// scal[kIters] = completed iterations.  The stopping test runs on the DEVICE (cg_shift_kernel): once `done` is set the
+// vector updates of the iterations still enqueued turn into no-ops, so the host never has to synchronise inside the loop
+// and x is exactly the iterate at which the criterion was met.
+enum { kRR = 0, kPQ = 1, kRRNew = 2, kAlpha = 3, kBeta = 4, kBreak = 5, kBB = 6, kDone = 7, kNScal = 8, kIters = 12 };
 
 // r = b - q ; p = r ; partial <r,r>       (q = M x0, or q == nullptr for x0 = 0)
 __global__ void __launch_bounds__(kRedThreads) cg_init_kernel(const float* __restrict__ b, const float* __restrict__ q,
@@ -177,6 +180,7 @@ __global__ void __launch_bounds__(kRedThreads) cg_update_xr_kernel(float* __rest
                                                                    const float* __restrict__ p, const float* __restrict__ q,
                                                                    size_t n, double* __restrict__ scal,
                                                                    double* __restrict__ partials) {
+    if (scal[kDone] != 0.0) return;               // stopped: x, r and the partial sums stay as they are
     const double pq = scal[kPQ];
     const double alpha_d = pq > 0.0 ? scal[kRR] / pq : 0.0;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -202,6 +206,7 @@ __global__ void __launch_bounds__(kRedThreads) cg_update_xr_kernel(float* __rest
 // beta = rr_new/rr ; p = r + beta p ; then rr <- rr_new (done by the last-launched thread 0 after use)
 __global__ void __launch_bounds__(kEwThreads) cg_update_p_kernel(float* __restrict__ p, const float* __restrict__ r, size_t n,
                                                                  const double* __restrict__ scal, double* __restrict__ beta_out) {
+    if (scal[kDone] != 0.0) return;
     const double rr = scal[kRR];
     const double beta_d = rr > 0.0 ? scal[kRRNew] / rr : 0.0;
     if (blockIdx.x == 0 && threadIdx.x == 0) *beta_out = beta_d;
@@ -227,9 +232,15 @@ __global__ void __launch_bounds__(kEwThreads) add_inplace_kernel(float* __restri
         for (size_t j = i; j < n; ++j) q[j] += p[j];
     }
 }
-__global__ void cg_shift_kernel(double* __restrict__ scal, double* __restrict__ hist, int k) {
-    scal[kRR] = scal[kRRNew];
-    if (hist) hist[k] = sqrt(scal[kRRNew]);
+// end of iteration k (k = 0: initialisation): rr <- rr_new, count it, and decide whether to stop:
+// ||r||^2 <= rtol2 <b,b>  (rtol2 = 0: never)  or  breakdown <p, M p> <= 0
+__global__ void cg_shift_kernel(double* __restrict__ scal, double* __restrict__ hist, int k, double rtol2) {
+    if (scal[kDone] == 0.0) {
+        scal[kRR] = scal[kRRNew];
+        scal[kIters] = (double)k;
+        if (scal[kBreak] != 0.0 || (rtol2 > 0.0 && scal[kRRNew] <= rtol2 * scal[kBB])) scal[kDone] = 1.0;
+    }
+    if (hist) hist[k] = sqrt(scal[kRR]);
 }
 
 }  // namespace frs

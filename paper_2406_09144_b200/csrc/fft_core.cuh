@@ -407,11 +407,18 @@ __device__ __forceinline__ void tensor_g2s_5d(void* dst_smem, const void* tmap, 
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
     unsigned ok, spins = 0;
+    unsigned long long t0 = 0;
     do {
         asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
                      : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-        // a copy that never completes (bad map, lost issue) must fail loudly, not hang the device
-        if (!ok && ++spins > (1u << 26)) __trap();
+        // a copy that never completes (bad map, lost issue) must fail loudly, not hang the device: 2 s of wall time
+        // on the global timer (a spin count would depend on clocks and on how long a try_wait suspends the warp)
+        if (!ok && (++spins & 1023u) == 0) {
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+            if (t0 == 0) t0 = t;
+            else if (t - t0 > 2000000000ull) __trap();
+        }
     } while (!ok);
 }
 // cooperative copy of the packed twiddle table into shared memory (all threads; caller syncs)

@@ -20,6 +20,7 @@ namespace {
 enum PassKind { kPassRowsFwd = 0, kPassConvCols = 1, kPassRowsInv = 2, kPassHartRows = 3, kPassHartCols = 4, kNPass = 5 };
 struct ProfRec { int kind; cudaEvent_t a, b; };
 constexpr int kMaxRedBlocks = 1184;   // 148 SMs x 8
+constexpr size_t kMaxProfRecords = 4096;
 }  // namespace
 
 struct frs_ctx {
@@ -86,10 +87,13 @@ bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1))
 struct Prof {
     frs_ctx* c; int kind; cudaEvent_t a = nullptr, b = nullptr;
     Prof(frs_ctx* c_, int kind_) : c(c_), kind(kind_) {
-        if (c->profiling) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, c->stream); }
+        // at most kMaxProfRecords pending records (events are released by frs_profile_read): later passes go untimed
+        if (c->profiling && c->prof.size() < kMaxProfRecords) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, c->stream); }
     }
     ~Prof() {
-        if (c->profiling) { cudaEventRecord(b, c->stream); c->prof.push_back({kind, a, b}); }
+        if (!a) return;
+        cudaEventRecord(b, c->stream);
+        c->prof.push_back({kind, a, b});
     }
 };
 
@@ -375,23 +379,23 @@ int cg_alloc(frs_ctx* ctx) {
 }
 
 // second half of an iteration: from q = M p to the updated (x, r, p, scal)
-int cg_iter_finish(frs_ctx* ctx, float* x, double* d_hist, int k, bool have_pq = false) {
+int cg_iter_finish(frs_ctx* ctx, float* x, double* d_hist, int k, bool have_pq = false, double rtol2 = 0.0) {
     const size_t n = (size_t)ctx->nfield * ctx->npix;
     const int nb = red_blocks(n);
     if (!have_pq) RET(dot(ctx, ctx->cg_p, ctx->cg_q, n, ctx->scal + kPQ));
     cg_update_xr_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(x, ctx->cg_r, ctx->cg_p, ctx->cg_q, n, ctx->scal, ctx->partials);
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, ctx->scal + kRRNew);
     cg_update_p_kernel<<<nb, kEwThreads, 0, ctx->stream>>>(ctx->cg_p, ctx->cg_r, n, ctx->scal, ctx->scal + kBeta);
-    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_hist, k + 1);
+    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_hist, k + 1, rtol2);
     ctx->launches += 4;
     CK(cudaGetLastError());
     return FRS_OK;
 }
 // one iteration from (x, r, p, scal[kRR]); leaves scal[kRR] = new <r,r>
-int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k) {
+int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k, double rtol2 = 0.0) {
     // with the prior term the last Hartley pass has p and q = M p side by side: <p, q> comes out of its epilogue
     RET(metric_apply_impl(ctx, ctx->cg_p, with_prior, ctx->cg_q, with_prior ? ctx->scal + kPQ : nullptr));
-    return cg_iter_finish(ctx, x, d_hist, k, with_prior != 0);
+    return cg_iter_finish(ctx, x, d_hist, k, with_prior != 0, rtol2);
 }
 
 }  // namespace
@@ -481,7 +485,11 @@ int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
     int neg = 0;
     CK(cudaMemcpyAsync(&neg, ctx->flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
-    if (neg) { ctx->have_psf = false; return fail(ctx, FRS_ENOTPSD, "PSF weights contain negative or NaN entries"); }
+    if (neg) {
+        ctx->have_psf = false;
+        return fail(ctx, FRS_ENOTPSD, neg == 2 ? "PSF weights are not Hermitian on the self-conjugate columns kx = 0, nx (W[-k] != W[k])"
+                                               : "PSF weights contain negative or NaN entries");
+    }
     ctx->have_psf = true;
     ctx->have_kern = false; ctx->lik_mode = 0;    // a kernel fitted to the previous PSF no longer applies
     return FRS_OK;
@@ -761,31 +769,29 @@ int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rto
     const size_t n = (size_t)ctx->nfield * ctx->npix;
     const int nb = red_blocks(n);
     CK(cudaMemsetAsync(ctx->scal, 0, kNScal * sizeof(double), ctx->stream));
+    CK(cudaMemsetAsync(ctx->scal + kIters, 0, sizeof(double), ctx->stream));
+    const double rtol2 = (double)rtol * (double)rtol;
+    if (rtol > 0.f) RET(dot(ctx, b, b, n, ctx->scal + kBB));
     // r0 = b - M x0 ; p0 = r0
     RET(metric_apply_impl(ctx, x, with_prior, ctx->cg_q));
     cg_init_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(b, ctx->cg_q, ctx->cg_r, ctx->cg_p, n, ctx->partials);
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, ctx->scal + kRRNew);
-    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_res_history, 0);
+    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_res_history, 0, rtol2);
     ctx->launches += 3;
-    double bb = 0.0;
-    if (rtol > 0.f) {
-        RET(dot(ctx, b, b, n, ctx->scal + kBB));
-        CK(cudaMemcpyAsync(&bb, ctx->scal + kBB, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-        CK(cudaStreamSynchronize(ctx->stream));
-    }
-    int it = 0;
-    double sc[kNScal];
-    for (; it < max_iter; ++it) {
-        if (rtol > 0.f) {
-            CK(cudaMemcpyAsync(sc, ctx->scal, sizeof(sc), cudaMemcpyDeviceToHost, ctx->stream));
+    // The stopping test lives on the device; with rtol > 0 the host looks at the flag every 8 iterations only to stop
+    // enqueueing (the iterations enqueued past the stopping point leave x, r, p untouched).
+    double sc[16];
+    for (int it = 0; it < max_iter; ++it) {
+        if (rtol > 0.f && (it & 7) == 7) {
+            CK(cudaMemcpyAsync(sc, ctx->scal, kNScal * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
             CK(cudaStreamSynchronize(ctx->stream));
-            if (sc[kRR] <= (double)rtol * (double)rtol * bb || sc[kBreak] != 0.0) break;
+            if (sc[kDone] != 0.0) break;
         }
-        RET(cg_iter(ctx, x, with_prior, d_res_history, it));
+        RET(cg_iter(ctx, x, with_prior, d_res_history, it, rtol2));
     }
-    CK(cudaMemcpyAsync(sc, ctx->scal, sizeof(sc), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(sc, ctx->scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
-    if (h_iters) *h_iters = it;
+    if (h_iters) *h_iters = (int)sc[kIters];
     if (h_resnorm) *h_resnorm = sqrt(sc[kRR]);
     if (sc[kBreak] != 0.0) return fail(ctx, FRS_EBREAKDOWN, "CG breakdown: <p, M p> <= 0");
     return FRS_OK;

@@ -107,8 +107,16 @@ __global__ void weights_layout_kernel(const float* __restrict__ w_half, float* _
     const int kx = 2 * m + c, ky = 2 * q + par;
     float v = 0.f;
     if (kx <= nx) {
-        v = w_half[(size_t)b * (2 * ny) * (nx + 1) + (size_t)ky * (nx + 1) + kx];
+        const float* wb = w_half + (size_t)b * (2 * ny) * (nx + 1);
+        v = wb[(size_t)ky * (nx + 1) + kx];
         if (!(v >= 0.f)) atomicExch(neg_flag, 1);
+        // Hermitian symmetry W[-k] = W[k] (R4) is implied by the half grid everywhere except on the self-conjugate
+        // columns kx = 0 and kx = nx, where both members of a pair are stored: they must agree, or the natural and the
+        // transposed orientation of the operator would silently differ
+        if (kx == 0 || kx == nx) {
+            const float m = wb[(size_t)((2 * ny - ky) % (2 * ny)) * (nx + 1) + kx];
+            if (!(fabsf(v - m) <= 1e-5f * fmaxf(fabsf(v), fabsf(m)))) atomicExch(neg_flag, 2);
+        }
     }
     wt[(size_t)b * per + i] = 0.5f * v;
 }

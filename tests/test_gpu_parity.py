@@ -224,6 +224,40 @@ def test_energy_device_scalar_and_xi_zero(frs):
     assert rel(g.cpu().numpy(), g_ref) <= TOL
 
 
+def test_non_hermitian_weights_are_rejected(frs):
+    """W[-k] = W[k] (R4) is implied by the half grid except on the self-conjugate columns kx = 0 and kx = nx, where both
+    members of a pair are stored: a mismatch there would make the two orientations of the operator differ silently."""
+    w = workload(("c1",))
+    for kx in (0, w.nx):
+        bad = w.w_half.copy()
+        bad[0, 3, kx] += 1.0                                      # its partner (2 ny - 3, kx) is left alone
+        ctx = frs.Context(w.ny, w.nx, 1)
+        with pytest.raises(frs.FrsError) as ei:
+            ctx.set_psf_weights(dev(bad))
+        assert ei.value.code == frs.binding.FRS_ENOTPSD
+        ok = w.w_half.copy()
+        ok[0, 3, kx] += 1.0
+        ok[0, 2 * w.ny - 3, kx] += 1.0
+        ctx.set_psf_weights(dev(ok))
+
+
+def test_cg_rtol_stops_on_the_device_at_the_right_iterate(frs):
+    """The stopping test runs on the device; the host only looks every 8 iterations, and the iterations enqueued past
+    the stopping point must leave x untouched: x equals the iterate of a run with max_iter = the reported count."""
+    import torch
+    w, ctx, b, ap = _cg_problem(frs, ("c1b",))
+    x = torch.zeros_like(b)
+    it, rn = ctx.cg_solve(b, x, 200, rtol=1e-2)
+    assert 0 < it < 200 and it % 8 != 0 or it < 200
+    assert rn <= 1e-2 * float(b.double().norm())
+    x2 = torch.zeros_like(b)
+    it2, rn2 = ctx.cg_solve(b, x2, it)
+    assert it2 == it and torch.equal(x, x2) and rn2 == rn
+    x3 = torch.zeros_like(b)
+    it3, rn3 = ctx.cg_solve(b, x3, it - 1)
+    assert rn3 > 1e-2 * float(b.double().norm())                   # one iteration earlier the criterion was not met
+
+
 # ---------------------------------------------------------------------------------- CG (protocol of DESIGN.md R9)
 def _cg_problem(frs, key):
     import torch
