@@ -133,7 +133,7 @@ int ensure_scratch(frs_ctx* ctx) {
     RET(dev_alloc(ctx, &ctx->T, (size_t)ctx->nchan * max2(spec_batch_stride(ctx->ny, ctx->nx), spec_batch_stride(ctx->nx, ctx->ny))));
     RET(dev_alloc(ctx, &ctx->T2, (size_t)ctx->nchan * max2((nx / 2 + 1) * ny, (ny / 2 + 1) * nx) * 2));
     RET(dev_alloc(ctx, &ctx->Th, (size_t)(ctx->nchan > 2 ? ctx->nchan : 2) *
-                                     max2(spec_batch_stride(ctx->ny, ctx->nx / 2), spec_batch_stride(ctx->nx, ctx->ny / 2))));
+                                     max2(spec_batch_stride(ctx->ny, ctx->nx / 2, kPairBins), spec_batch_stride(ctx->nx, ctx->ny / 2, kPairBins))));
     RET(dev_alloc(ctx, &ctx->lin, 2 * np));
     RET(dev_alloc(ctx, &ctx->acc, 2 * np));
     RET(dev_alloc(ctx, &ctx->img, (size_t)ctx->nchan * np));
@@ -223,7 +223,8 @@ int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const flo
 // one contiguous run of the transposed output -- so the transform transposes for free, and the
 // latent-space path keeps its sky-space arrays transposed instead of paying for scattered stores.
 int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul, float* out, const float* mul,
-              const float* add, const float* offset_dev, int nb, double* d_dot = nullptr, float sign = 1.0f) {
+              const float* add, const float* offset_dev, int nb, double* d_dot = nullptr, float sign = 1.0f,
+              bool exp_out = false) {
     const int ntile_h = n2 / 4 + 1;
     {
         Prof pr(ctx, kPassHartRows);
@@ -238,7 +239,7 @@ int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul
     {
         Prof pr(ctx, kPassHartCols);
         HartColsArgs a{};
-        a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = n2;
+        a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = n2; a.exp_out = exp_out ? 1 : 0;
         a.img_bstride = ctx->npix;
         a.tw = ctx->tw[n1];
         a.dot_partials = (d_dot && add) ? ctx->partials : nullptr;   // <add, out> fused into the epilogue (fp64)
@@ -279,9 +280,14 @@ int check_hot(frs_ctx* ctx, bool need_s, bool need_model) {
 
 int sky_forward_impl(frs_ctx* ctx, const float* xi) {
     // tau_f = mu_f + H[A_f xi_f];  s_c = exp(tau_0 + lognu_c tau_1)      (R6)   -- sky-space arrays transposed
-    RET(hartley_t(ctx, xi, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, ctx->d_mu, ctx->nfield));
-    sky_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->d_lognu, ctx->sT, ctx->npix, ctx->nfield, ctx->nchan);
-    ctx->launches++;
+    if (ctx->nfield == 1 && ctx->nchan == 1) {
+        // single field, single channel: s = exp(tau) leaves the last Hartley pass directly (A2 fused into A1)
+        RET(hartley_t(ctx, xi, ctx->ny, ctx->nx, ctx->amp, ctx->sT, nullptr, nullptr, ctx->d_mu, 1, nullptr, 1.0f, true));
+    } else {
+        RET(hartley_t(ctx, xi, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, ctx->d_mu, ctx->nfield));
+        sky_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->d_lognu, ctx->sT, ctx->npix, ctx->nfield, ctx->nchan);
+        ctx->launches++;
+    }
     CK(cudaGetLastError());
     ctx->have_s = true;
     ctx->sT_ok = true;
@@ -503,7 +509,7 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
     // row pass over all 2 ny rows of length 2 nx (no padding), then one DIF step + ny-point column FFTs
     float2* tmp = nullptr;
     float* stats = nullptr;
-    const size_t tstride = spec_batch_stride(my, ctx->nx);
+    const size_t tstride = spec_batch_stride(my, ctx->nx, kPairBins);
     CK(cudaMalloc(reinterpret_cast<void**>(&tmp), (size_t)ctx->nchan * tstride * sizeof(float2)));
     int rc = FRS_OK;
     std::vector<float> hs;

@@ -24,9 +24,9 @@ psf_cols_kernel(PsfColsArgs a) {
     for (int e = 0; e < kE; ++e) v[e] = c2zero();
     if (live) {
         // columns 2m, 2m+1 of the row-transformed PSF (2 NF rows, block layout of tmap.h)
-        const float2* c0 = a.t + b * spec_batch_stride(2 * NF, a.ncols - 1);
+        const float2* c0 = a.t + b * spec_batch_stride(2 * NF, a.ncols - 1, kPairBins);
         const bool two = 2 * m + 1 < a.ncols;
-        auto at = [&](int c, int y) { return ldg2(reinterpret_cast<const float*>(c0 + spec_index(2 * NF, 2 * m + c, y))); };
+        auto at = [&](int c, int y) { return ldg2(reinterpret_cast<const float*>(c0 + spec_index(2 * NF, 2 * m + c, y, kPairBins))); };
 #pragma unroll
         for (int e = 0; e < kE; ++e) {
             const int n = p + e * P;

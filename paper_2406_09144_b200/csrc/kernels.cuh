@@ -86,7 +86,7 @@ template <int NF> struct RowsFwdGeo : Geo<NF, 1, NF / 2, 256> {};
 struct RowsFwdArgs {
     const float* in;      // [nb][ny][nxr]
     const float* mul;     // optional [nb][ny][nxr] multiplier (s or A); nullptr = none
-    float2* out;          // [nb][NF/8+1][ny/2][8][2]: 128-byte blocks (8 bins) x (rows 2r, 2r+1), tmap.h
+    float2* out;          // [nb][NF/B+1][ny/2][B][2]: blocks of B bins x (rows 2r, 2r+1); B = 8 (PAD) or 2, tmap.h
     int ny;               // rows
     int items_per_batch, nitems;
     size_t in_bstride, mul_bstride;   // elements (float)
@@ -231,10 +231,11 @@ rows_fwd_kernel(RowsFwdArgs a) {
         if (live) {
             // (X_0[k], X_1[k]) -> 16-byte slot k % 8 of block (k / 8, y0 / 2): 8 neighbouring lanes fill one 128-byte line
             auto slot = [](const C2& x) { return make_float4(x.re.x, x.im.x, x.re.y, x.im.y); };
-            float4* ob = reinterpret_cast<float4*>(a.out + b * spec_batch_stride(a.ny, NF));
+            constexpr int BINS = PAD ? kBlockBins : kPairBins;    // tmap.h: 128-byte blocks for the convolution, pairs otherwise
+            float4* ob = reinterpret_cast<float4*>(a.out + b * spec_batch_stride(a.ny, NF, BINS));
 #pragma unroll
-            for (int e = 0; e < kE; ++e) stg4(ob + spec_index(a.ny, p + e * P, y0) / 2, slot(v[e]));
-            if (p == 0) stg4(ob + spec_index(a.ny, NF, y0) / 2, slot(xn));
+            for (int e = 0; e < kE; ++e) stg4(ob + spec_index(a.ny, p + e * P, y0, BINS) / 2, slot(v[e]));
+            if (p == 0) stg4(ob + spec_index(a.ny, NF, y0, BINS) / 2, slot(xn));
         }
     }
 }

@@ -146,13 +146,14 @@ conv_cols_kernel(const __grid_constant__ ConvColsArgs a) {
 
 // ------------------------------------------------------------------------------------------------
 struct HartColsArgs {
-    const float2* t;      // block layout of tmap.h: columns x = 0..nx/2 of the row-transformed field (NF rows)
+    const float2* t;      // pair layout of tmap.h ([nb][m][NF/2][2][2]): columns x = 0..nx/2 of the row-transformed field (NF rows)
     float* out;           // [nb][nx][NF]  TRANSPOSED: out[x][y] = H[y][x]
     const float* mul;     // optional [nb][nx][NF]: out = mul * (H + offset) + add
     const float* add;     // optional [nb][nx][NF]
     const float* offset;  // optional device [nb]   (mu)
     double* dot_partials; // optional [gridDim.x]: sum over the CTA's outputs of out * add (fp64) -- <v, M v> of a CG step
     int nx;
+    int exp_out;          // out = exp(...) (the sky of a single-field, single-channel model: A2 fused into A1's last pass)
     int items_per_batch, nitems;
     size_t img_bstride;
     const float4* tw;
@@ -160,9 +161,19 @@ struct HartColsArgs {
 
 // F[y][x] = column FFT; H[y][x] = Re F - Im F and H[(-y) mod NF][nx - x] = Re F + Im F  (reading R6).
 // Column x of H is one contiguous run of the transposed output, so all stores are coalesced.
-template <int NF>
+// Input: the column pair (2m, 2m+1) is one contiguous run of 16 NF bytes in the pair layout; lanes read neighbouring
+// 8-byte samples (staging it through shared memory by a bulk or a tensor copy was measured 5-8 % slower: the landing
+// costs a second trip through the shared-memory pipe and the copy can only start behind the transform).
+// The epilogue variant is a template parameter: as run-time flags the 64-fold unrolled optional pieces (the predicated-off
+// expf sequences alone) cost a third of the kernel's issue slots (measured: 113 us instead of 76 us per pass at 4096^2).
+enum HartMode { kHPlain = 0,      // out = H + offset
+                kHExp = 1,        // out = exp(H + offset)                        (sky of a single-field model)
+                kHMul = 2,        // out = mul . H                                 (N'^-1: K^-1 in harmonic space; gradient without prior)
+                kHMulAdd = 3,     // out = mul . H + add                           (gradient with prior)
+                kHMulAddDot = 4 };// ... and sum out . add in fp64                 (last pass of a CG iteration)
+template <int NF, int MODE>
 __global__ void __launch_bounds__(RowsGeo<NF>::THREADS, RowsGeo<NF>::MINB)
-hart_cols_kernel(HartColsArgs a) {
+hart_cols_kernel(const HartColsArgs a) {
     using GEO = RowsGeo<NF>;
     constexpr int P = GEO::P;
     extern __shared__ __align__(128) float4 smem4[];
@@ -182,13 +193,13 @@ hart_cols_kernel(HartColsArgs a) {
 
         C2 v[kE];
         if (live) {
-            // columns 2m, 2m+1 (neighbouring 16-byte slots of one block of T)
-            const float* c0 = reinterpret_cast<const float*>(a.t + b * spec_batch_stride(NF, a.nx / 2));
+            const float* c0 = reinterpret_cast<const float*>(a.t + b * spec_batch_stride(NF, a.nx / 2, kPairBins)
+                                                             + spec_index(NF, 2 * m, 0, kPairBins));
             const bool two = 2 * m + 1 <= a.nx / 2;            // the last pair may hold one column only
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
                 const int y = p + e * P;
-                const float* q = c0 + 2 * spec_index(NF, 2 * m, y);
+                const float* q = c0 + 2 * ((y >> 1) * 4 + (y & 1));
                 const float2 x0 = ldg2(q);
                 const float2 x1 = two ? ldg2(q + 4) : make_float2(0.f, 0.f);
                 v[e] = c2make(x0, x1);
@@ -200,42 +211,42 @@ hart_cols_kernel(HartColsArgs a) {
         pair_fft<NF, false>(v, p, buf, tws, gb);
         if (live) {
             const size_t base = b * a.img_bstride;
-            const float off = a.offset ? __ldg(a.offset + b) : 0.f;
+            const float off = (MODE == kHPlain || MODE == kHExp) && a.offset ? __ldg(a.offset + b) : 0.f;
             const int half = a.nx / 2;
+            constexpr bool MUL = MODE >= kHMul, ADD = MODE >= kHMulAdd;
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
                 const int x = 2 * m + c;
                 if (x > half) continue;
                 const bool mirror = x > 0 && x < half;
-                const size_t col0 = base + (size_t)x * NF, col1 = base + (size_t)(a.nx - x) * NF;
+                // column x of H: rows y (Re - Im); column nx - x: rows (-y) mod NF (Re + Im)
 #pragma unroll
-                for (int e = 0; e < kE; ++e) {
-                    const int y = p + e * P, ym = (NF - y) & (NF - 1);
-                    const float2 f = c2get(v[e], c);
-                    float h0 = f.x - f.y + off;
-                    if (a.mul) h0 *= ldg1(a.mul + col0 + y);
-                    if (a.add) {
-                        const float ad = ldg1(a.add + col0 + y);
-                        h0 += ad;
-                        if (a.dot_partials) dacc += (double)h0 * (double)ad;
+                for (int side = 0; side < 2; ++side) {
+                    if (side == 1 && !mirror) continue;
+                    const size_t col = base + (size_t)(side ? a.nx - x : x) * NF;
+                    float mu[kE], ad[kE];
+#pragma unroll
+                    for (int e = 0; e < kE; ++e) {
+                        const int y = p + e * P, yy = side ? (NF - y) & (NF - 1) : y;
+                        if (MUL) mu[e] = ldg1(a.mul + col + yy);
+                        if (ADD) ad[e] = ldg1(a.add + col + yy);
                     }
-                    a.out[col0 + y] = h0;
-                    if (mirror) {
-                        float h1 = f.x + f.y + off;
-                        if (a.mul) h1 *= ldg1(a.mul + col1 + ym);
-                        if (a.add) {
-                            const float ad = ldg1(a.add + col1 + ym);
-                            h1 += ad;
-                            if (a.dot_partials) dacc += (double)h1 * (double)ad;
-                        }
-                        a.out[col1 + ym] = h1;
+#pragma unroll
+                    for (int e = 0; e < kE; ++e) {
+                        const int y = p + e * P, yy = side ? (NF - y) & (NF - 1) : y;
+                        const float2 f = c2get(v[e], c);
+                        float h = (side ? f.x + f.y : f.x - f.y) + off;
+                        if (MUL) h *= mu[e];
+                        if (ADD) h += ad[e];
+                        if (MODE == kHMulAddDot) dacc += (double)h * (double)ad[e];
+                        if (MODE == kHExp) h = expf(h);
+                        a.out[col + yy] = h;
                     }
                 }
             }
         }
-        gb.sync();
     }
-    if (a.dot_partials) {
+    if (MODE == kHMulAddDot) {
         // fixed-order block reduction: warp shuffle tree, then warp 0 over the per-warp sums
         __shared__ double dred[32];
 #pragma unroll

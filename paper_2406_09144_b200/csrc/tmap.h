@@ -18,13 +18,21 @@
 
 namespace frs {
 
-constexpr int kBlockBins = 8;                                     // bins kx per 128-byte block of T
-__host__ __device__ constexpr int spec_tiles(int nf) { return nf / kBlockBins + 1; }   // bins kx = 0..nf
+// Two block widths.  The convolution's spectrum T (rows_fwd<.,PAD> -> conv_cols) uses 8 bins per block, see above.  The
+// Hartley row pass and the PSF set-up (rows_fwd<.,!PAD> -> hart_cols / psf_cols) use 2: their column pass carries the
+// column PAIR (2m, 2m+1) per thread, and with 2-bin blocks that pair is one CONTIGUOUS run of 16 rows bytes, fetched by a
+// single bulk copy (with 8-bin blocks the same pair is 32-byte pieces at a 128-byte stride: measured 12 us slower per
+// Hartley transform at 4096^2, whether read by loads or by a TMA gather).
+constexpr int kBlockBins = 8;                                     // conv: bins kx per 128-byte block of T
+constexpr int kPairBins = 2;                                      // Hartley / PSF set-up: bins per 32-byte block
+__host__ __device__ constexpr int spec_tiles(int nf, int bins = kBlockBins) { return nf / bins + 1; }   // bins kx = 0..nf
 // float2 index, inside one batch, of sample (kx, y) of the row-transformed array of `rows` image rows
-__host__ __device__ constexpr size_t spec_index(int rows, int kx, int y) {
-    return ((((size_t)(kx / kBlockBins) * (rows / 2) + (y >> 1)) * kBlockBins + (kx % kBlockBins)) << 1) + (y & 1);
+__host__ __device__ constexpr size_t spec_index(int rows, int kx, int y, int bins = kBlockBins) {
+    return ((((size_t)(kx / bins) * (rows / 2) + (y >> 1)) * bins + (kx % bins)) << 1) + (y & 1);
 }
-__host__ __device__ constexpr size_t spec_batch_stride(int rows, int nf) { return (size_t)spec_tiles(nf) * rows * kBlockBins; }
+__host__ __device__ constexpr size_t spec_batch_stride(int rows, int nf, int bins = kBlockBins) {
+    return (size_t)spec_tiles(nf, bins) * rows * bins;
+}
 
 // smaller rows: boxes below the 128-byte TMA alignment -> cp.async
 __host__ __device__ constexpr bool tma_rows_ok(int nf) { return nf >= 128; }
