@@ -174,6 +174,12 @@ int frs_selftest_dif_exchange(int n, int* out);
  * 16-byte slots of the exchange buffer the row gather lands in, 1 if rows of nf bins use TMA. */
 int frs_selftest_tma_geometry(int nf, int rows, int* out);
 
+/* The tensor-core measurement north_star asks for before a DFT-as-GEMM stage may be used (needs a GPU; FRS_ECUDA without):
+ * SM cycles per tcgen05.mma kind::tf32 instruction of shape M = 128, K = 8, N = n_out (32 or 64), operands in shared
+ * memory, accumulator in TMEM, one CTA per SM, `mmas_per_commit` instructions per commit/wait, `iters` repetitions.
+ * A radix-16 stage of one column pair with the 3-term TF32 split is 24 such instructions at N = 64. */
+int frs_selftest_tcgen05_stage(int n_out, int mmas_per_commit, int iters, double* clk_per_mma);
+
 #ifdef __cplusplus
 }
 #endif

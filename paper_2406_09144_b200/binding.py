@@ -50,6 +50,7 @@ EXPORTS = {
     "frs_selftest_tma_geometry": (_i, [_i, _i, C.POINTER(_i)]),
     "frs_selftest_dif_host": (_i, [_i, _i, _vp, _vp]),
     "frs_selftest_dif_exchange": (_i, [_i, C.POINTER(_i)]),
+    "frs_selftest_tcgen05_stage": (_i, [_i, _i, _i, C.POINTER(_d)]),
 }
 
 _lib = None
@@ -109,6 +110,15 @@ def selftest_dif_exchange(n):
     if rc != 0:
         raise FrsError(rc, "selftest_dif_exchange")
     return tuple(int(v) for v in out)
+
+
+def selftest_tcgen05_stage(n_out=64, mmas_per_commit=24, iters=2000):
+    """SM cycles per tcgen05.mma kind::tf32 (M = 128, K = 8, N = n_out) -- the tensor-core measurement of DESIGN.md section 5."""
+    out = _d(0.0)
+    rc = lib().frs_selftest_tcgen05_stage(int(n_out), int(mmas_per_commit), int(iters), C.byref(out))
+    if rc != 0:
+        raise FrsError(rc, "selftest_tcgen05_stage")
+    return out.value
 
 
 def _ptr(t, dtype=None, numel=None, name="tensor"):

@@ -212,3 +212,89 @@ extern "C" int frs_selftest_tma_geometry(int nf, int rows, int* out) {
     out[5] = frs::tma_rows_ok(nf) ? 1 : 0;
     return 0;
 }
+
+// ---- tensor-core measurement owed by north_star ("tensor cores only if a DFT-as-GEMM stage is MEASURED to beat the radix
+// passes"): throughput of tcgen05.mma kind::tf32 at the shape a radix-16 DFT stage needs -- M = 128 positions per
+// instruction, K = 8, N = 32 or 64 real outputs, operands in shared memory, accumulator in TMEM, one CTA per SM.
+// A stage of one column pair is 256 positions x K = 96 (3-term TF32 split of a 32-real input: hi.hi + lo.hi + hi.lo,
+// needed for the 1e-5 parity bar) x N = 64 (even- and odd-bin outputs) = 24 such instructions.
+// compares the result with the 640 SM-cycles the packed-FP32 butterflies of the same stage take.
+namespace frs {
+__device__ __forceinline__ unsigned st_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned long long st_make_desc(unsigned addr, unsigned lbo, unsigned sbo) {
+    unsigned long long d = 0;                                       // SWIZZLE_NONE, K-major (canonical 8 x 16-byte core matrices)
+    d |= (unsigned long long)((addr >> 4) & 0x3FFF);
+    d |= (unsigned long long)((lbo >> 4) & 0x3FFF) << 16;
+    d |= (unsigned long long)((sbo >> 4) & 0x3FFF) << 32;
+    d |= 1ull << 46;                                                // descriptor version of sm_100
+    return d;
+}
+template <int N>
+__global__ void __launch_bounds__(128, 1) tcgen05_stage_kernel(int iters, int nmma, long long* cyc) {
+    __shared__ __align__(1024) float a_s[128 * 8 * 2];
+    __shared__ __align__(1024) float b_s[64 * 8 * 2];
+    __shared__ unsigned tmem_base;
+    __shared__ __align__(8) unsigned long long bar;
+    for (int i = threadIdx.x; i < 128 * 16; i += 128) a_s[i] = 0.001f * (i % 97);
+    for (int i = threadIdx.x; i < 64 * 16; i += 128) b_s[i] = 0.002f * (i % 89);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(st_smem_u32(&bar)) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (threadIdx.x < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 64;" :: "r"(st_smem_u32(&tmem_base)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const unsigned tmem = tmem_base;
+    // instruction descriptor: D = F32 (bit 4), A = B = TF32 (2 at bits 7 and 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+    const unsigned idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(N >> 3) << 17) | ((unsigned)(128 >> 4) << 24);
+    const unsigned long long da = st_make_desc(st_smem_u32(a_s), 128, 256), db = st_make_desc(st_smem_u32(b_s), 128, 256);
+    unsigned parity = 0;
+    if (threadIdx.x == 0) {
+        const long long t0 = clock64();
+        for (int it = 0; it < iters; ++it) {
+            for (int j = 0; j < nmma; ++j) {
+                const unsigned acc = j > 0;
+                asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                             :: "r"(tmem), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(st_smem_u32(&bar)) : "memory");
+            unsigned ok = 0, spins = 0;
+            while (!ok) {
+                asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                             : "=r"(ok) : "r"(st_smem_u32(&bar)), "r"(parity) : "memory");
+                if (!ok && ++spins > (1u << 24)) __trap();
+            }
+            parity ^= 1u;
+        }
+        if (blockIdx.x == 0) *cyc = clock64() - t0;
+    }
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    if (threadIdx.x < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 64;" :: "r"(tmem) : "memory");
+}
+}  // namespace frs
+
+extern "C" int frs_selftest_tcgen05_stage(int n_out, int mmas_per_commit, int iters, double* clk_per_mma) {
+    if (!clk_per_mma || (n_out != 32 && n_out != 64) || mmas_per_commit < 1 || iters < 1) return FRS_EINVAL;
+    int ndev = 0, sms = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return FRS_ECUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
+    long long* d = nullptr;
+    if (cudaMalloc(reinterpret_cast<void**>(&d), sizeof(long long)) != cudaSuccess) return FRS_ECUDA;
+    for (int pass = 0; pass < 2; ++pass) {                          // warm-up, then the timed launch
+        const int it = pass ? iters : 4;
+        if (n_out == 32) frs::tcgen05_stage_kernel<32><<<sms, 128>>>(it, mmas_per_commit, d);
+        else frs::tcgen05_stage_kernel<64><<<sms, 128>>>(it, mmas_per_commit, d);
+        if (cudaDeviceSynchronize() != cudaSuccess) { cudaFree(d); return FRS_ECUDA; }
+    }
+    long long h = 0;
+    cudaMemcpy(&h, d, sizeof(h), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    *clk_per_mma = (double)h / iters / mmas_per_commit;
+    return 0;
+}

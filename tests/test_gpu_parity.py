@@ -531,3 +531,12 @@ def test_config2_as_stated_outer_steps_teacher_forced(frs):
             scale *= 0.5
         assert e1 < e
         xi = (xi + scale * d).contiguous()
+
+
+def test_tensor_core_stage_measurement_runs(frs):
+    """The measurement behind the decision not to run DFT stages on the tensor cores: tcgen05.mma
+    kind::tf32 at the shape of a radix-16 stage.  24 instructions (3-term split, both output parities) per column pair
+    against the 640 SM-cycles of the packed-FP32 butterflies: recorded in profiles/r2_tensor_core_stage.md."""
+    clk = frs.selftest_tcgen05_stage(64, 24, 500)
+    assert 8.0 < clk < 1000.0
+    print(f"tcgen05.mma kind::tf32 M=128 K=8 N=64: {clk:.1f} clk per instruction -> {24 * clk:.0f} clk per stage and column pair")

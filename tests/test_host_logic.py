@@ -113,3 +113,29 @@ def test_no_cpu_fallback(library):
     assert library.frs_create(64, 64, 1, 0, None, C.byref(h)) == frs.FRS_ECUDA
     assert library.frs_create(48, 64, 1, 0, None, C.byref(h)) == frs.FRS_EINVAL      # not a power of two
     assert library.frs_create(64, 8192, 1, 0, None, C.byref(h)) == frs.FRS_EINVAL
+
+
+def test_tf32_dft_stage_needs_the_three_term_split():
+    """Arithmetic of the tensor-core alternative: a radix-16 DFT stage as a TF32 GEMM.  One pass of
+    TF32 (10-bit mantissa, fp32 accumulate) misses the 1e-5 parity bar by two orders of magnitude; the 3-term split
+    x_hi W_hi + x_lo W_hi + x_hi W_lo meets it -- at three times the tensor-core work.  Emulated in numpy."""
+    def tf32(a):
+        b = np.asarray(a, np.float32).view(np.uint32)
+        b = (b + np.uint32(0x1000)) & np.uint32(0xFFFFE000)          # round to 10 explicit mantissa bits
+        return b.view(np.float32)
+    rng = np.random.default_rng(16)
+    x = rng.normal(size=(4096, 16)) + 1j * rng.normal(size=(4096, 16))
+    w = np.exp(-2j * np.pi * np.outer(np.arange(16), np.arange(16)) / 16)
+    ref = x @ w
+    xr = np.concatenate([x.real, x.imag], 1).astype(np.float32)      # [p][32] real form
+    wr = np.block([[w.real, w.imag], [-w.imag, w.real]]).astype(np.float32)   # [32][32]
+    def gemm(a, b):                                                  # exact products of tf32 operands, fp32 accumulate
+        return (a.astype(np.float64) @ b.astype(np.float64)).astype(np.float32)
+    def err(y):
+        return np.linalg.norm((y[:, :16] + 1j * y[:, 16:]) - ref) / np.linalg.norm(ref)
+    one = gemm(tf32(xr), tf32(wr))
+    xh, wh = tf32(xr), tf32(wr)
+    xl, wl = tf32(xr - xh), tf32(wr - wh)
+    three = gemm(xh, wh) + gemm(xl, wh) + gemm(xh, wl)
+    assert err(one) > 1e-4                                           # ~3e-4: fails the bar on its own
+    assert err(three) < 2e-6                                         # the split restores fp32-class accuracy
