@@ -294,6 +294,52 @@ def metric_apply_eq9(w_half, kern, amp, mu, lognu, xi, v, with_prior=True, s=Non
 
 
 # =============================================================================
+# MGVI: posterior samples and the sample-averaged KL ("Metric Gaussian Variational Inference"; reading R15)
+# =============================================================================
+def ninv_sqrt_apply(kern, x):
+    """N'^-1/2 x = FFT^-1[ K^-1/2 . FFT x ] (periodic, as Eq. 18): the symmetric square root of N'^-1."""
+    return np.real(np.fft.ifft2(np.fft.fft2(np.asarray(x, dtype=F64)) / np.sqrt(np.asarray(kern, dtype=F64))))
+
+
+def sample_source_eq9(w_half, kern, amp, lognu, s, eta_xi, eta_d):
+    """m = eta_xi + J^T C N'^-1/2 eta_d  with white eta_xi [nfield,ny,nx], eta_d [nchan,ny,nx]:  Cov m = 1 + J^T C N'^-1 C J = M,
+    the metric of Eq. 9 at the position with sky s (MGVI draws its samples as M^-1 m, Knollmueller & Ensslin 2019)."""
+    t = np.stack([psf_apply(w_half[c], ninv_sqrt_apply(kern[c], eta_d[c])) for c in range(s.shape[0])])
+    return np.asarray(eta_xi, dtype=F64) + vjp(amp, lognu, s, t)
+
+
+def draw_sample_eq9(w_half, kern, amp, mu, lognu, xi, eta_xi, eta_d, cg_iters):
+    """One posterior sample around xi: sigma = M(xi)^-1 m by `cg_iters` CG iterations from 0 (Cov sigma -> M^-1)."""
+    s = sky(xi, amp, mu, lognu)
+    m = sample_source_eq9(w_half, kern, amp, lognu, s, eta_xi, eta_d)
+    sol = cg(lambda v: metric_apply_eq9(w_half, kern, amp, mu, lognu, xi, v, True, s=s), m, max_iter=cg_iters)
+    return sol["x"], m
+
+
+def kl_energy_grad_eq9(w_half, kern, dirty, amp, mu, lognu, xi, samples, mirrored=True):
+    """Sample-averaged KL and its gradient: mean over the positions xi + sigma_i (and xi - sigma_i if mirrored) of
+    E_tot and grad E_tot (Eq. 9 likelihood + standard-normal prior)."""
+    xi = np.asarray(xi, dtype=F64)
+    pos = [xi + np.asarray(sg, F64) for sg in samples] + ([xi - np.asarray(sg, F64) for sg in samples] if mirrored else [])
+    e, g = 0.0, np.zeros_like(xi)
+    for q in pos:
+        ei, gi = energy_grad_eq9(w_half, kern, dirty, amp, mu, lognu, q, True)
+        e += ei
+        g += gi
+    return e / len(pos), g / len(pos)
+
+
+def kl_metric_apply_eq9(w_half, kern, amp, mu, lognu, xi, samples, v, mirrored=True):
+    """Sample-averaged metric: mean over the same positions of M(xi +- sigma_i) v."""
+    xi = np.asarray(xi, dtype=F64)
+    pos = [xi + np.asarray(sg, F64) for sg in samples] + ([xi - np.asarray(sg, F64) for sg in samples] if mirrored else [])
+    out = np.zeros_like(np.asarray(v, dtype=F64))
+    for q in pos:
+        out += metric_apply_eq9(w_half, kern, amp, mu, lognu, q, v, True)
+    return out / len(pos)
+
+
+# =============================================================================
 # Conjugate gradient (paper silent; reading R9: textbook Hestenes-Stiefel)
 # =============================================================================
 def cg_step(apply, x, r, p, rr):

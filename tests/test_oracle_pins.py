@@ -497,3 +497,66 @@ def test_eq9_gradient_metric_and_limits(which, small, multi):
     e_big = o.energy_grad_eq9(w.w_half, kbig, w.dirty, w.amp, w.mu, w.lognu, xi, False)[0]
     r2 = sum(np.sum((w.dirty[c] - o.psf_apply(w.w_half[c], s[c])) ** 2) for c in range(w.nchan))
     assert abs(big * e_big - 0.5 * r2) <= 1e-9 * r2
+
+
+# ------------------------------------------------------------------ MGVI samples and the sample-averaged KL (R15)
+def test_mgvi_sample_source_has_the_metric_as_covariance():
+    """Cov(eta_xi + J^T C N'^-1/2 eta_d) = 1 + J^T C N'^-1 C J = M: checked against the dense metric of a 4x4 problem,
+    entry by entry, both by the exact linear map (m is linear in eta) and by Monte Carlo."""
+    w = wl.make_config(1, n=4, npts=300)
+    n = w.ny * w.nx
+    eps = 1e-2 * float(np.sum(o.full_spectrum(w.w_half[0])))
+    kern = np.stack([o.noise_kernel_from_psf(w.w_half[0], eps)])
+    rng = np.random.default_rng(40)
+    xi = 0.3 * rng.normal(size=(1, w.ny, w.nx))
+    s = o.sky(xi, w.amp, w.mu, w.lognu)
+    dense = np.stack([o.metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, e.reshape(1, w.ny, w.nx), True).ravel()
+                      for e in np.eye(n)], axis=1)
+    # m = eta_xi + A eta_d with A = J^T C N'^-1/2: assemble A column by column, Cov m = 1 + A A^T exactly
+    z = np.zeros((1, w.ny, w.nx))
+    a_mat = np.stack([o.sample_source_eq9(w.w_half, kern, w.amp, w.lognu, s, z, e.reshape(1, w.ny, w.nx)).ravel() for e in np.eye(n)], axis=1)
+    assert np.allclose(np.eye(n) + a_mat @ a_mat.T, dense, rtol=1e-10, atol=1e-10 * np.abs(dense).max())
+    assert np.allclose(o.sample_source_eq9(w.w_half, kern, w.amp, w.lognu, s, xi, 0 * z), xi)       # eta_xi enters with weight 1
+    draws = np.stack([o.sample_source_eq9(w.w_half, kern, w.amp, w.lognu, s, rng.normal(size=z.shape), rng.normal(size=z.shape)).ravel()
+                      for _ in range(4000)])
+    emp = draws.T @ draws / len(draws)
+    assert np.linalg.norm(emp - dense) / np.linalg.norm(dense) < 0.08
+    # N'^-1/2 is the symmetric square root of N'^-1
+    x = rng.normal(size=(w.ny, w.nx))
+    assert np.allclose(o.ninv_sqrt_apply(kern[0], o.ninv_sqrt_apply(kern[0], x)), o.ninv_apply(kern[0], x), atol=1e-12)
+    # a sample solves M sigma = m: against the dense solve
+    eta_xi, eta_d = rng.normal(size=z.shape), rng.normal(size=z.shape)
+    sg, m = o.draw_sample_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, eta_xi, eta_d, cg_iters=3 * n)
+    assert np.allclose(sg.ravel(), np.linalg.solve(dense, m.ravel()), rtol=1e-8, atol=1e-10)
+
+
+def test_kl_average_gradient_and_metric(multi):
+    w = multi
+    rng = np.random.default_rng(41)
+    eps = 1e-2 * float(np.sum(o.full_spectrum(w.w_half[0])))
+    kern = np.stack([o.noise_kernel_from_psf(w.w_half[c], eps) for c in range(w.nchan)])
+    xi = 0.2 * rng.normal(size=(w.nfield, w.ny, w.nx))
+    samples = [0.1 * rng.normal(size=xi.shape) for _ in range(2)]
+    kl, g = o.kl_energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi, samples, True)
+    # written out: the mean over the four positions xi +- sigma_i
+    es = [o.energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi + sg * sgn, True)[0] for sg in samples for sgn in (1, -1)]
+    assert abs(kl - np.mean(es)) <= 1e-12 * abs(kl)
+    # mirrored: invariant under sigma -> -sigma; one sample at sigma = 0 is the plain energy
+    kl2, g2 = o.kl_energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi, [-sg for sg in samples], True)
+    assert abs(kl - kl2) <= 1e-12 * abs(kl) and rel(g2, g) < 1e-12
+    e0, g0 = o.energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi, True)
+    kl0, gk0 = o.kl_energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi, [0 * xi], False)
+    assert kl0 == e0 and np.array_equal(gk0, g0)
+    for _ in range(3):                                               # gradient of the KL by central differences
+        d = rng.normal(size=xi.shape)
+        h = 1e-5 * np.linalg.norm(xi) / np.linalg.norm(d)
+        kp = o.kl_energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi + h * d, samples, True)[0]
+        km = o.kl_energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi - h * d, samples, True)[0]
+        fd = (kp - km) / (2 * h)
+        assert abs(fd - np.sum(g * d)) <= 1e-6 * max(abs(fd), np.linalg.norm(g) * np.linalg.norm(d) * 1e-3)
+    v, u = rng.normal(size=xi.shape), rng.normal(size=xi.shape)
+    mv = o.kl_metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, samples, v, True)
+    mu_ = o.kl_metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, samples, u, True)
+    assert abs(np.sum(u * mv) - np.sum(mu_ * v)) <= 1e-10 * abs(np.sum(u * mv)) and np.sum(v * mv) >= np.sum(v * v)
+    one = np.mean([o.metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi + sg * sgn, v, True) for sg in samples for sgn in (1, -1)], axis=0)
+    assert rel(mv, one) < 1e-13
