@@ -136,6 +136,24 @@ int frs_ninv_apply(frs_ctx* ctx, const float* x, float* y);
  * Affects frs_energy_grad, frs_metric_apply, frs_cg_solve / _step / _step_begin. */
 int frs_set_likelihood(frs_ctx* ctx, int mode);
 
+/* ---- MGVI: posterior samples and the sample-averaged KL (reading R15) ------------
+ * MGVI approximates the posterior by N(xi, M(xi)^-1), M the metric above, and minimises the KL estimated on samples
+ * xi +- sigma_i, sigma_i ~ N(0, M^-1).  The random numbers are INPUTS (white N(0,1) arrays drawn by the caller). */
+
+/* One sample at the cached position (Eq. 9 likelihood, mode 1, only): m = eta_xi + J^T C N'^-1/2 eta_d has covariance M;
+ * sample = M^-1 m by CG from 0 (max_iter, rtol as frs_cg_solve).  eta_xi [nfield][ny][nx], eta_d [nchan][ny][nx] white
+ * noise (device); sample [nfield][ny][nx].  h_iters (host, may be NULL).  Synchronises.  Errors: FRS_ESTATE in mode 0
+ * (the square root of C needs noise on the padded grid: not provided) or without a position. */
+int frs_draw_sample(frs_ctx* ctx, const float* eta_xi, const float* eta_d, int max_iter, float rtol, float* sample, int* h_iters);
+/* Sample-averaged KL and gradient: mean over the positions xi + sigma_i (and xi - sigma_i if mirrored) of E_tot and
+ * grad E_tot (likelihood of the current mode + prior).  samples: device [nsamples][nfield][ny][nx].  Energy outputs
+ * as frs_energy_grad.  Leaves the cached position at xi. */
+int frs_kl_energy_grad(frs_ctx* ctx, const float* xi, const float* samples, int nsamples, int mirrored, double* d_energy,
+                       double* h_energy, float* grad);
+/* out = mean over the same positions of M(xi +- sigma_i) v (with the prior term): the metric of the KL's Newton-CG step.
+ * Recomputes the sky at every position (2 nsamples sky evaluations and metric applies per call).  Leaves the position at xi. */
+int frs_kl_metric_apply(frs_ctx* ctx, const float* xi, const float* samples, int nsamples, int mirrored, const float* v, float* out);
+
 /* ---- host-buffer entry points (end-to-end measurements: copies are part of the call) -------- */
 
 /* y = s . C (s . x) with x, y in HOST memory (pinned or pageable), [nchan][ny][nx].

@@ -41,6 +41,9 @@ EXPORTS = {
     "frs_get_noise_kernel": (_i, [_vp, _vp]),
     "frs_ninv_apply": (_i, [_vp, _vp, _vp]),
     "frs_set_likelihood": (_i, [_vp, _i]),
+    "frs_draw_sample": (_i, [_vp, _vp, _vp, _i, _f, _vp, C.POINTER(_i)]),
+    "frs_kl_energy_grad": (_i, [_vp, _vp, _vp, _i, _i, _vp, C.POINTER(_d), _vp]),
+    "frs_kl_metric_apply": (_i, [_vp, _vp, _vp, _i, _i, _vp, _vp]),
     "frs_sky_metric_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_psf_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_launch_count": (C.c_longlong, [_vp]),
@@ -245,6 +248,30 @@ class Context:
 
     def set_likelihood(self, mode):
         self._ck(lib().frs_set_likelihood(self._h, int(mode)))
+
+    # ---- MGVI
+    def draw_sample(self, eta_xi, eta_d, sample, max_iter, rtol=0.0):
+        it = _i(0)
+        self._ck(lib().frs_draw_sample(self._h, _ptr(eta_xi, self.f32, self.nfield * self.npix, "eta_xi"),
+                                       _ptr(eta_d, self.f32, self.nchan * self.npix, "eta_d"), int(max_iter), float(rtol),
+                                       _ptr(sample, self.f32, self.nfield * self.npix, "sample"), C.byref(it)))
+        return it.value
+
+    def kl_energy_grad(self, xi, samples, grad, mirrored=True):
+        h = _d(0.0)
+        ns = samples.shape[0]
+        self._ck(lib().frs_kl_energy_grad(self._h, _ptr(xi, self.f32, self.nfield * self.npix, "xi"),
+                                          _ptr(samples, self.f32, ns * self.nfield * self.npix, "samples"), ns, int(mirrored),
+                                          None, C.byref(h), _ptr(grad, self.f32, self.nfield * self.npix, "grad")))
+        return h.value
+
+    def kl_metric_apply(self, xi, samples, v, out, mirrored=True):
+        ns = samples.shape[0]
+        self._ck(lib().frs_kl_metric_apply(self._h, _ptr(xi, self.f32, self.nfield * self.npix, "xi"),
+                                           _ptr(samples, self.f32, ns * self.nfield * self.npix, "samples"), ns, int(mirrored),
+                                           _ptr(v, self.f32, self.nfield * self.npix, "v"),
+                                           _ptr(out, self.f32, self.nfield * self.npix, "out")))
+        return out
 
     # ---- hot path
     def sky_forward(self, xi, sky=None):

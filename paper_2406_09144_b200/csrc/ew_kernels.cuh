@@ -115,7 +115,8 @@ __global__ void energy_final_kernel(const double* __restrict__ sc_sc, const doub
 // (ny/2, nx/2):  Re FFT(t)[k] = (H[k] + H[-k]) / 2, conj FFT(I_delta)[k] = (-1)^(ky+kx), + eps from the eps I_delta term:
 //   K = max((-1)^(ky+kx) (H[k] + H[-k]) / 2 + eps, eps);   kern[ky][kx] = K;  kinv = 1 / (K ny nx) in both orientations
 __global__ void noise_kernel_finish_kernel(const float* __restrict__ ht, float eps, float* __restrict__ kern,
-                                           float* __restrict__ kinv_n, float* __restrict__ kinv_t, int ny, int nx) {
+                                           float* __restrict__ kinv_n, float* __restrict__ kinv_t, float* __restrict__ kisq_n,
+                                           int ny, int nx) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, npix = (size_t)ny * nx;
     if (i >= npix) return;
     const size_t b = blockIdx.y * npix;
@@ -128,10 +129,12 @@ __global__ void noise_kernel_finish_kernel(const float* __restrict__ ht, float e
     const float inv = 1.0f / (k * (float)ny * (float)nx);
     kinv_n[b + i] = inv;
     kinv_t[b + (size_t)kx * ny + ky] = inv;
+    kisq_n[b + i] = rsqrtf(k) / ((float)ny * (float)nx);          // N'^-1/2 (MGVI sample source, R15)
 }
 // a caller-supplied kernel: flags non-positive / NaN entries and departures from K[-k] = K[k] beyond 1e-5 max-free relative
 __global__ void noise_kernel_from_array_kernel(const float* __restrict__ kern, float* __restrict__ kinv_n,
-                                               float* __restrict__ kinv_t, int ny, int nx, int* __restrict__ bad) {
+                                               float* __restrict__ kinv_t, float* __restrict__ kisq_n, int ny, int nx,
+                                               int* __restrict__ bad) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, npix = (size_t)ny * nx;
     if (i >= npix) return;
     const size_t b = blockIdx.y * npix;
@@ -141,6 +144,26 @@ __global__ void noise_kernel_from_array_kernel(const float* __restrict__ kern, f
     const float inv = 1.0f / (k * (float)ny * (float)nx);
     kinv_n[b + i] = inv;
     kinv_t[b + (size_t)kx * ny + ky] = inv;
+    kisq_n[b + i] = rsqrtf(k) / ((float)ny * (float)nx);
+}
+// out = x + sgn y  (a position xi +- sigma of the sample-averaged KL), n a multiple of 4
+__global__ void __launch_bounds__(kEwThreads) add_scaled_kernel(const float* __restrict__ x, const float* __restrict__ y, float sgn,
+                                                                 float* __restrict__ out, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i * 4 >= n) return;
+    const float4 a = reinterpret_cast<const float4*>(x)[i], b = reinterpret_cast<const float4*>(y)[i];
+    reinterpret_cast<float4*>(out)[i] = make_float4(fmaf(sgn, b.x, a.x), fmaf(sgn, b.y, a.y), fmaf(sgn, b.z, a.z), fmaf(sgn, b.w, a.w));
+}
+// acc = (first ? 0 : acc) + w g ;  the energies likewise in fp64: e_acc = (first ? 0 : e_acc) + w e
+__global__ void __launch_bounds__(kEwThreads) accumulate_kernel(float* __restrict__ acc, const float* __restrict__ g, float w, int first,
+                                                                 size_t n, double* __restrict__ e_acc, const double* __restrict__ e) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0 && e_acc) *e_acc = (first ? 0.0 : *e_acc) + (double)w * (*e);
+    if (i * 4 >= n) return;
+    const float4 b = reinterpret_cast<const float4*>(g)[i];
+    float4 a = first ? make_float4(0.f, 0.f, 0.f, 0.f) : reinterpret_cast<float4*>(acc)[i];
+    a.x = fmaf(w, b.x, a.x); a.y = fmaf(w, b.y, a.y); a.z = fmaf(w, b.z, a.z); a.w = fmaf(w, b.w, a.w);
+    reinterpret_cast<float4*>(acc)[i] = a;
 }
 __global__ void set_delta_kernel(float* __restrict__ img, size_t npix, size_t pos) { img[blockIdx.x * npix + pos] = 1.0f; }
 // E = 0.5 <r, N'^-1 r> + 0.5 with_prior <xi, xi>

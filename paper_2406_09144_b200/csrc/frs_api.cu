@@ -41,7 +41,8 @@ struct frs_ctx {
     std::vector<MapKey> maps;  // spectrum tensor maps (tmap.h), built on first use
     float *lin = nullptr, *img = nullptr, *acc = nullptr;
     // Eq. 9 with the fitted noise kernel (R14): K, 1/(K ny nx) in both orientations, two more image-sized scratch arrays
-    float *kern = nullptr, *kinvN = nullptr, *kinvT = nullptr, *img2 = nullptr, *img3 = nullptr;
+    float *kern = nullptr, *kinvN = nullptr, *kinvT = nullptr, *kisqN = nullptr, *img2 = nullptr, *img3 = nullptr;
+    float *lat1 = nullptr, *lat2 = nullptr;   // latent-sized scratch of the MGVI calls (sample source, positions xi +- sigma)
     bool have_kern = false;
     int lik_mode = 0;                // 0: N' = R' limit, 1: Eq. 9 with N'^-1 of Eq. 18
     float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
@@ -404,6 +405,23 @@ int cg_iter(frs_ctx* ctx, float* x, int with_prior, double* d_hist, int k, doubl
     return cg_iter_finish(ctx, x, d_hist, k, with_prior != 0, rtol2);
 }
 
+float* ctx_lat1(frs_ctx* ctx) { return ctx->lat1; }
+
+// positions xi + sigma_i (and xi - sigma_i): visit(position, weight, first)
+template <typename F>
+int for_each_position(frs_ctx* ctx, const float* xi, const float* samples, int ns, int mirrored, F visit) {
+    const size_t n = (size_t)ctx->nfield * ctx->npix;
+    const int npos = ns * (mirrored ? 2 : 1);
+    int k = 0;
+    for (int i = 0; i < ns; ++i)
+        for (int sgn = 1; sgn >= (mirrored ? -1 : 1); sgn -= 2, ++k) {
+            add_scaled_kernel<<<ew_grid(n), kEwThreads, 0, ctx->stream>>>(xi, samples + (size_t)i * n, (float)sgn, ctx_lat1(ctx), n);
+            ctx->launches++;
+            RET(visit(ctx_lat1(ctx), 1.0f / (float)npos, k == 0));
+        }
+    return FRS_OK;
+}
+
 }  // namespace
 
 // =================================================================================================
@@ -457,7 +475,7 @@ void frs_destroy(frs_ctx* ctx) {
     for (auto& kv : ctx->tw) cudaFree(kv.second);
     for (auto& kv : ctx->twd) cudaFree(kv.second);
     for (auto& kv : ctx->twist) cudaFree(kv.second);
-    void* ptrs[] = {ctx->kern, ctx->kinvN, ctx->kinvT, ctx->img2, ctx->img3, ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
+    void* ptrs[] = {ctx->kern, ctx->kinvN, ctx->kinvT, ctx->kisqN, ctx->lat1, ctx->lat2, ctx->img2, ctx->img3, ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -633,11 +651,18 @@ int frs_sky_metric_apply(frs_ctx* ctx, const float* x, float* y) {
     return FRS_OK;
 }
 
+static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, double* d_energy, double* h_energy, float* grad);
+
 int frs_energy_grad(frs_ctx* ctx, const float* xi, int with_prior, double* d_energy, double* h_energy, float* grad) {
     if (!ctx || !xi || !grad || !aligned16(xi) || !aligned16(grad)) return fail(ctx, FRS_EINVAL, "frs_energy_grad: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(check_hot(ctx, false, true));
     if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
+    return energy_grad_impl(ctx, xi, with_prior, d_energy, h_energy, grad);
+}
+
+// the energy is left in ctx->scal[11] (device)
+static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, double* d_energy, double* h_energy, float* grad) {
     RET(sky_forward_impl(ctx, xi));
     const Orient o = orient(ctx, true);                       // sky-space arrays transposed on this path
     if (ctx->lik_mode == 1) {
@@ -765,12 +790,20 @@ int frs_cg_step_end(frs_ctx* ctx, float* x, int with_prior) {
     return cg_iter_finish(ctx, x, nullptr, 0);
 }
 
+static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,
+                         double* h_resnorm, double* d_res_history);
+
 int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,
                  double* h_resnorm, double* d_res_history) {
     if (!ctx || !b || !x || !aligned16(b) || !aligned16(x) || max_iter < 0 || rtol < 0.f || b == x)
         return fail(ctx, FRS_EINVAL, "frs_cg_solve: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(check_hot(ctx, true, true));
+    return cg_solve_impl(ctx, b, x, max_iter, rtol, with_prior, h_iters, h_resnorm, d_res_history);
+}
+
+static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,
+                         double* h_resnorm, double* d_res_history) {
     RET(cg_alloc(ctx));
     const size_t n = (size_t)ctx->nfield * ctx->npix;
     const int nb = red_blocks(n);
@@ -803,12 +836,95 @@ int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rto
     return FRS_OK;
 }
 
+// ---- MGVI: posterior samples and the sample-averaged KL (reading R15) ------------------------
+static int latent_scratch(frs_ctx* ctx) {
+    RET(dev_alloc(ctx, &ctx->lat1, 2 * ctx->npix));
+    RET(dev_alloc(ctx, &ctx->lat2, 2 * ctx->npix));
+    return FRS_OK;
+}
+
+int frs_draw_sample(frs_ctx* ctx, const float* eta_xi, const float* eta_d, int max_iter, float rtol, float* sample, int* h_iters) {
+    if (!ctx || !eta_xi || !eta_d || !sample || !aligned16(eta_xi) || !aligned16(eta_d) || !aligned16(sample) || max_iter < 0 ||
+        rtol < 0.f || sample == eta_xi)
+        return fail(ctx, FRS_EINVAL, "frs_draw_sample: bad argument");
+    if (ctx->lik_mode != 1) return fail(ctx, FRS_ESTATE, "frs_draw_sample needs the Eq. 9 likelihood (frs_set_likelihood(ctx, 1))");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, true));
+    RET(ensure_scratch9(ctx));
+    RET(latent_scratch(ctx));
+    const Orient o = orient(ctx, true);
+    RET(need_s_transposed(ctx));
+    // m = eta_xi + J^T C N'^-1/2 eta_d  (Cov m = M): the sky-space chain runs in the transposed orientation
+    RET(transpose(ctx, eta_d, ctx->img2, ctx->ny, ctx->nx, ctx->nchan));
+    RET(hartley_t(ctx, ctx->img2, ctx->nx, ctx->ny, nullptr, ctx->img3, ctx->kisqN, nullptr, nullptr, ctx->nchan));
+    RET(hartley_t(ctx, ctx->img3, ctx->ny, ctx->nx, nullptr, ctx->img, nullptr, nullptr, nullptr, ctx->nchan));
+    RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
+    RET(conv_cols(ctx, o));
+    const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
+    RET(conv_rows_inv(ctx, o, simple ? ctx->acc : ctx->img, kMulS, ctx->sT, nullptr, nullptr));
+    if (!simple) {
+        vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
+                                                                               ctx->nfield, ctx->nchan);
+        ctx->launches++;
+    }
+    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, ctx->lat1, ctx->amp, eta_xi, nullptr, ctx->nfield));
+    // sigma = M^-1 m by CG from 0
+    CK(cudaMemsetAsync(sample, 0, (size_t)ctx->nfield * ctx->npix * sizeof(float), ctx->stream));
+    return cg_solve_impl(ctx, ctx->lat1, sample, max_iter, rtol, 1, h_iters, nullptr, nullptr);
+}
+
+int frs_kl_energy_grad(frs_ctx* ctx, const float* xi, const float* samples, int nsamples, int mirrored, double* d_energy,
+                       double* h_energy, float* grad) {
+    if (!ctx || !xi || !samples || !grad || nsamples < 1 || !aligned16(xi) || !aligned16(samples) || !aligned16(grad) || grad == xi)
+        return fail(ctx, FRS_EINVAL, "frs_kl_energy_grad: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, false, true));
+    if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
+    RET(latent_scratch(ctx));
+    const size_t n = (size_t)ctx->nfield * ctx->npix;
+    RET(for_each_position(ctx, xi, samples, nsamples, mirrored, [&](const float* q, float w, bool first) -> int {
+        RET(energy_grad_impl(ctx, q, 1, nullptr, nullptr, ctx->lat2));
+        accumulate_kernel<<<ew_grid(n), kEwThreads, 0, ctx->stream>>>(grad, ctx->lat2, w, first ? 1 : 0, n, ctx->scal + 13, ctx->scal + 11);
+        ctx->launches++;
+        return FRS_OK;
+    }));
+    RET(sky_forward_impl(ctx, xi));                           // leave the position at the mean
+    CK(cudaGetLastError());
+    if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 13, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    if (h_energy) {
+        CK(cudaMemcpyAsync(h_energy, ctx->scal + 13, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    return FRS_OK;
+}
+
+int frs_kl_metric_apply(frs_ctx* ctx, const float* xi, const float* samples, int nsamples, int mirrored, const float* v, float* out) {
+    if (!ctx || !xi || !samples || !v || !out || nsamples < 1 || !aligned16(xi) || !aligned16(samples) || !aligned16(v) ||
+        !aligned16(out) || out == v || out == xi)
+        return fail(ctx, FRS_EINVAL, "frs_kl_metric_apply: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, false, true));
+    RET(latent_scratch(ctx));
+    const size_t n = (size_t)ctx->nfield * ctx->npix;
+    RET(for_each_position(ctx, xi, samples, nsamples, mirrored, [&](const float* q, float w, bool first) -> int {
+        RET(sky_forward_impl(ctx, q));
+        RET(metric_apply_impl(ctx, v, 1, ctx->lat2));
+        accumulate_kernel<<<ew_grid(n), kEwThreads, 0, ctx->stream>>>(out, ctx->lat2, w, first ? 1 : 0, n, nullptr, nullptr);
+        ctx->launches++;
+        return FRS_OK;
+    }));
+    RET(sky_forward_impl(ctx, xi));
+    CK(cudaGetLastError());
+    return FRS_OK;
+}
+
 // ---- the paper's literal likelihood: noise kernel of Eq. 15-18 ------------------------------------
 static int kernel_arrays(frs_ctx* ctx) {
     const size_t n = (size_t)ctx->nchan * ctx->npix;
     RET(dev_alloc(ctx, &ctx->kern, n));
     RET(dev_alloc(ctx, &ctx->kinvN, n));
     RET(dev_alloc(ctx, &ctx->kinvT, n));
+    RET(dev_alloc(ctx, &ctx->kisqN, n));
     return ensure_scratch9(ctx);
 }
 
@@ -828,7 +944,7 @@ int frs_set_noise_kernel(frs_ctx* ctx, float eps) {
     RET(conv_rows_inv(ctx, o, ctx->img, kPlain, nullptr, nullptr, nullptr));
     RET(hartley_t(ctx, ctx->img, ctx->ny, ctx->nx, nullptr, ctx->img3, nullptr, nullptr, nullptr, ctx->nchan));   // [nx][ny]
     dim3 grid((unsigned)((ctx->npix + 255) / 256), ctx->nchan);
-    noise_kernel_finish_kernel<<<grid, 256, 0, ctx->stream>>>(ctx->img3, eps, ctx->kern, ctx->kinvN, ctx->kinvT, ctx->ny, ctx->nx);
+    noise_kernel_finish_kernel<<<grid, 256, 0, ctx->stream>>>(ctx->img3, eps, ctx->kern, ctx->kinvN, ctx->kinvT, ctx->kisqN, ctx->ny, ctx->nx);
     ctx->launches++;
     CK(cudaGetLastError());
     ctx->have_kern = true;
@@ -844,7 +960,7 @@ int frs_set_noise_kernel_array(frs_ctx* ctx, const float* kern) {
     CK(cudaMemcpyAsync(ctx->kern, kern, n * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaMemsetAsync(ctx->flag, 0, sizeof(int), ctx->stream));
     dim3 grid((unsigned)((ctx->npix + 255) / 256), ctx->nchan);
-    noise_kernel_from_array_kernel<<<grid, 256, 0, ctx->stream>>>(ctx->kern, ctx->kinvN, ctx->kinvT, ctx->ny, ctx->nx, ctx->flag);
+    noise_kernel_from_array_kernel<<<grid, 256, 0, ctx->stream>>>(ctx->kern, ctx->kinvN, ctx->kinvT, ctx->kisqN, ctx->ny, ctx->nx, ctx->flag);
     ctx->launches++;
     int bad = 0;
     CK(cudaMemcpyAsync(&bad, ctx->flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
