@@ -340,6 +340,35 @@ def kl_metric_apply_eq9(w_half, kern, amp, mu, lognu, xi, samples, v, mirrored=T
 
 
 # =============================================================================
+# Major cycle with the exact response on a list of uv points (Eq. 1 coplanar, Alg. 1, Eq. 20-22; R16)
+# =============================================================================
+def exact_response(uv, x, my, mx):
+    """R x: V_k = sum_pixels x[y][x] exp(-2 pi i (u_k x / Mx + v_k y / My)), (u, v) in cell units of the padded grid,
+    NOT rounded to cells (Eq. 1 for a coplanar array, unit primary beam) -- the direct sum, O(nvis npix)."""
+    x = np.asarray(x, dtype=F64)
+    ny, nx = x.shape
+    uv = np.asarray(uv, dtype=F64)
+    ex = np.exp(-2j * np.pi * np.outer(uv[:, 0], np.arange(nx)) / mx)      # [nvis, nx]
+    ey = np.exp(-2j * np.pi * np.outer(uv[:, 1], np.arange(ny)) / my)      # [nvis, ny]
+    return np.einsum("ky,yx,kx->k", ey, x, ex)
+
+
+def exact_adjoint(uv, wgt, vis, ny, nx, my, mx):
+    """R^dagger N^-1 V with every visibility and its conjugate (the convention of the weight grid, R5):
+    image[y][x] = sum_k 2 w_k Re( V_k exp(+2 pi i (u_k x / Mx + v_k y / My)) )."""
+    uv = np.asarray(uv, dtype=F64)
+    ex = np.exp(2j * np.pi * np.outer(uv[:, 0], np.arange(nx)) / mx)
+    ey = np.exp(2j * np.pi * np.outer(uv[:, 1], np.arange(ny)) / my)
+    return 2.0 * np.real(np.einsum("k,ky,kx->yx", np.asarray(wgt, F64) * np.asarray(vis, np.complex128), ey, ex))
+
+
+def major_cycle_residual(uv, wgt, dirty_full, sky_i, my, mx):
+    """d_{i+1} = I^D - R^dagger N^-1 R I_i with the exact response (Eq. 20, 22)."""
+    ny, nx = np.asarray(sky_i).shape
+    return np.asarray(dirty_full, F64) - exact_adjoint(uv, wgt, exact_response(uv, sky_i, my, mx), ny, nx, my, mx)
+
+
+# =============================================================================
 # Conjugate gradient (paper silent; reading R9: textbook Hestenes-Stiefel)
 # =============================================================================
 def cg_step(apply, x, r, p, rr):

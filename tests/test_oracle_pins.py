@@ -560,3 +560,38 @@ def test_kl_average_gradient_and_metric(multi):
     assert abs(np.sum(u * mv) - np.sum(mu_ * v)) <= 1e-10 * abs(np.sum(u * mv)) and np.sum(v * mv) >= np.sum(v * v)
     one = np.mean([o.metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi + sg * sgn, v, True) for sg in samples for sgn in (1, -1)], axis=0)
     assert rel(mv, one) < 1e-13
+
+
+# ------------------------------------------------------------------ exact response and the major cycle (Eq. 1, Eq. 20-22; R16)
+def test_exact_response_closed_forms_and_grid_limit():
+    ny, nx = 8, 16
+    my, mx = 2 * ny, 2 * nx
+    rng = np.random.default_rng(60)
+    # one visibility, one pixel: the plane wave of Eq. 1
+    uv = np.array([[2.3, -1.7]])
+    d = np.zeros((ny, nx)); d[3, 5] = 2.0
+    assert np.allclose(o.exact_response(uv, d, my, mx), 2.0 * np.exp(-2j * np.pi * (2.3 * 5 / mx - 1.7 * 3 / my)), atol=1e-14)
+    # R^dagger N^-1 R delta = 2 w cos(2 pi (u dx / Mx + v dy / My)): the PSF of one visibility and its conjugate
+    img = o.exact_adjoint(uv, [0.5], o.exact_response(uv, d, my, mx), ny, nx, my, mx)
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    assert np.allclose(img, 2.0 * 2 * 0.5 * np.cos(2 * np.pi * (2.3 * (xx - 5) / mx - 1.7 * (yy - 3) / my)), atol=1e-13)
+    # adjointness <R x, N^-1 V> summed with the conjugates = <x, R^dagger N^-1 V>
+    uvs = np.stack(wl.uv_gaussian(rng, 40, my, mx, 0.2), axis=1)
+    w = rng.uniform(0.5, 1.5, 40)
+    x = rng.normal(size=(ny, nx))
+    v = rng.normal(size=40) + 1j * rng.normal(size=40)
+    lhs = 2.0 * np.real(np.sum(np.conj(o.exact_response(uvs, x, my, mx)) * w * v))
+    assert abs(lhs - np.sum(x * o.exact_adjoint(uvs, w, v, ny, nx, my, mx))) <= 1e-12 * abs(lhs)
+    # uv points ON grid cells: R^dagger N^-1 R is exactly the PSF convolution with the gridded weights (R5), so a major
+    # cycle returns the residual of the minor cycle's own model, d = I^D - C I
+    uvg = np.rint(uvs)
+    wgrid = np.zeros((my, mx))
+    for (u, vv), wk in zip(uvg, w):
+        wgrid[int(vv) % my, int(u) % mx] += wk
+        wgrid[int(-vv) % my, int(-u) % mx] += wk
+    cx = o.psf_apply(wgrid[:, : nx + 1], x)
+    assert np.allclose(o.exact_adjoint(uvg, w, o.exact_response(uvg, x, my, mx), ny, nx, my, mx), cx, rtol=1e-11, atol=1e-11 * np.abs(cx).max())
+    dirty = rng.normal(size=(ny, nx))
+    assert np.allclose(o.major_cycle_residual(uvg, w, dirty, x, my, mx), dirty - cx, atol=1e-10 * np.abs(cx).max())
+    # off the grid the two differ (that difference is what the major cycle corrects)
+    assert rel(o.exact_adjoint(uvs, w, o.exact_response(uvs, x, my, mx), ny, nx, my, mx), cx) > 1e-2
