@@ -154,6 +154,21 @@ int frs_kl_energy_grad(frs_ctx* ctx, const float* xi, const float* samples, int 
  * Recomputes the sky at every position (2 nsamples sky evaluations and metric applies per call).  Leaves the position at xi. */
 int frs_kl_metric_apply(frs_ctx* ctx, const float* xi, const float* samples, int nsamples, int mirrored, const float* v, float* out);
 
+/* ---- major cycle: exact response on a list of uv points (Alg. 1, Eq. 20-22; Eq. 1; reading R16) ----
+ * One channel at a time: images are [ny][nx] (any channel of a context), ny, nx <= 1024 (direct sums, O(nvis npix);
+ * else FRS_EINVAL).  uv: DEVICE float [nvis][2] = (u, v) in cell units of the padded (2ny x 2nx) grid, NOT rounded to
+ * cells; wgt: DEVICE float [nvis] = N^-1 (natural weighting: the scale w0 of the weight grid); vis: DEVICE float
+ * [nvis][2] = (Re, Im).  A minor cycle on the residual d_i uses frs_set_dirty(d_i + C s_{i-1}) (R13). */
+
+/* vis = R x:  V_k = sum_pixels x[y][x] exp(-2 pi i (u_k x / (2 nx) + v_k y / (2 ny))). */
+int frs_exact_response(frs_ctx* ctx, const float* uv, int nvis, const float* x, float* vis);
+/* y = R^dagger N^-1 vis, each visibility with its conjugate (the convention of the weight grid, R5):
+ * y[y][x] = sum_k 2 w_k Re(V_k exp(+2 pi i (u_k x / (2 nx) + v_k y / (2 ny)))).  The dirty image is frs_exact_adjoint(V). */
+int frs_exact_adjoint(frs_ctx* ctx, const float* uv, const float* wgt, int nvis, const float* vis, float* y);
+/* d_next = dirty_full - R^dagger N^-1 R sky   (Eq. 20, 22).  d_next may alias dirty_full. */
+int frs_major_cycle_residual(frs_ctx* ctx, const float* uv, const float* wgt, int nvis, const float* dirty_full, const float* sky,
+                             float* d_next);
+
 /* ---- host-buffer entry points (end-to-end measurements: copies are part of the call) -------- */
 
 /* y = s . C (s . x) with x, y in HOST memory (pinned or pageable), [nchan][ny][nx].

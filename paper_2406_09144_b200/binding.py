@@ -44,6 +44,9 @@ EXPORTS = {
     "frs_draw_sample": (_i, [_vp, _vp, _vp, _i, _f, _vp, C.POINTER(_i)]),
     "frs_kl_energy_grad": (_i, [_vp, _vp, _vp, _i, _i, _vp, C.POINTER(_d), _vp]),
     "frs_kl_metric_apply": (_i, [_vp, _vp, _vp, _i, _i, _vp, _vp]),
+    "frs_exact_response": (_i, [_vp, _vp, _i, _vp, _vp]),
+    "frs_exact_adjoint": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
+    "frs_major_cycle_residual": (_i, [_vp, _vp, _vp, _i, _vp, _vp, _vp]),
     "frs_sky_metric_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_psf_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_launch_count": (C.c_longlong, [_vp]),
@@ -248,6 +251,26 @@ class Context:
 
     def set_likelihood(self, mode):
         self._ck(lib().frs_set_likelihood(self._h, int(mode)))
+
+    # ---- major cycle (exact response on uv points; images are single-channel [ny][nx])
+    def exact_response(self, uv, x, vis):
+        nvis = uv.shape[0]
+        self._ck(lib().frs_exact_response(self._h, _ptr(uv, self.f32, 2 * nvis, "uv"), nvis, _ptr(x, self.f32, self.npix, "x"),
+                                          _ptr(vis, self.f32, 2 * nvis, "vis")))
+        return vis
+
+    def exact_adjoint(self, uv, wgt, vis, y):
+        nvis = uv.shape[0]
+        self._ck(lib().frs_exact_adjoint(self._h, _ptr(uv, self.f32, 2 * nvis, "uv"), _ptr(wgt, self.f32, nvis, "wgt"), nvis,
+                                         _ptr(vis, self.f32, 2 * nvis, "vis"), _ptr(y, self.f32, self.npix, "y")))
+        return y
+
+    def major_cycle_residual(self, uv, wgt, dirty_full, sky, d_next):
+        nvis = uv.shape[0]
+        self._ck(lib().frs_major_cycle_residual(self._h, _ptr(uv, self.f32, 2 * nvis, "uv"), _ptr(wgt, self.f32, nvis, "wgt"), nvis,
+                                                _ptr(dirty_full, self.f32, self.npix, "dirty_full"),
+                                                _ptr(sky, self.f32, self.npix, "sky"), _ptr(d_next, self.f32, self.npix, "d_next")))
+        return d_next
 
     # ---- MGVI
     def draw_sample(self, eta_xi, eta_d, sample, max_iter, rtol=0.0):

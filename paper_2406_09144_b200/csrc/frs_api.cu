@@ -11,6 +11,7 @@
 #include "../../include/frs.h"
 #include "ew_kernels.cuh"
 #include "launch.h"
+#include "response.h"
 #include "setup.h"
 #include "tables.h"
 
@@ -42,7 +43,8 @@ struct frs_ctx {
     float *lin = nullptr, *img = nullptr, *acc = nullptr;
     // Eq. 9 with the fitted noise kernel (R14): K, 1/(K ny nx) in both orientations, two more image-sized scratch arrays
     float *kern = nullptr, *kinvN = nullptr, *kinvT = nullptr, *kisqN = nullptr, *img2 = nullptr, *img3 = nullptr;
-    float *lat1 = nullptr, *lat2 = nullptr;   // latent-sized scratch of the MGVI calls (sample source, positions xi +- sigma)
+    float *lat1 = nullptr, *lat2 = nullptr;
+    float* visbuf = nullptr; size_t visbuf_n = 0;   // visibilities of the exact response (major cycle)   // latent-sized scratch of the MGVI calls (sample source, positions xi +- sigma)
     bool have_kern = false;
     int lik_mode = 0;                // 0: N' = R' limit, 1: Eq. 9 with N'^-1 of Eq. 18
     float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
@@ -475,7 +477,7 @@ void frs_destroy(frs_ctx* ctx) {
     for (auto& kv : ctx->tw) cudaFree(kv.second);
     for (auto& kv : ctx->twd) cudaFree(kv.second);
     for (auto& kv : ctx->twist) cudaFree(kv.second);
-    void* ptrs[] = {ctx->kern, ctx->kinvN, ctx->kinvT, ctx->kisqN, ctx->lat1, ctx->lat2, ctx->img2, ctx->img3, ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
+    void* ptrs[] = {ctx->visbuf, ctx->kern, ctx->kinvN, ctx->kinvT, ctx->kisqN, ctx->lat1, ctx->lat2, ctx->img2, ctx->img3, ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -915,6 +917,51 @@ int frs_kl_metric_apply(frs_ctx* ctx, const float* xi, const float* samples, int
     }));
     RET(sky_forward_impl(ctx, xi));
     CK(cudaGetLastError());
+    return FRS_OK;
+}
+
+// ---- major cycle: exact response on uv points (Alg. 1, Eq. 20-22; reading R16) ----------------------
+static int response_args(frs_ctx* ctx, const float* uv, const float* wgt, int nvis, const char* who) {
+    if (!ctx) return FRS_EINVAL;
+    if (!uv || nvis < 1 || (reinterpret_cast<uintptr_t>(uv) & 7u) || (wgt && (reinterpret_cast<uintptr_t>(wgt) & 3u))) return fail(ctx, FRS_EINVAL, who);
+    if (ctx->ny > kMaxResponseSide || ctx->nx > kMaxResponseSide)
+        return fail(ctx, FRS_EINVAL, "exact response: direct sums are provided for ny, nx <= 1024 (O(nvis npix); larger fields need a gridder)");
+    return FRS_OK;
+}
+
+int frs_exact_response(frs_ctx* ctx, const float* uv, int nvis, const float* x, float* vis) {
+    RET(response_args(ctx, uv, nullptr, nvis, "frs_exact_response: bad argument"));
+    if (!x || !vis || (reinterpret_cast<uintptr_t>(vis) & 7u)) return fail(ctx, FRS_EINVAL, "frs_exact_response: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    CKL(launch_exact_degrid(ctx->stream, uv, nvis, x, ctx->ny, ctx->nx, vis));
+    ctx->launches++;
+    return FRS_OK;
+}
+
+int frs_exact_adjoint(frs_ctx* ctx, const float* uv, const float* wgt, int nvis, const float* vis, float* y) {
+    RET(response_args(ctx, uv, wgt, nvis, "frs_exact_adjoint: bad argument"));
+    if (!wgt || !vis || !y || (reinterpret_cast<uintptr_t>(vis) & 7u)) return fail(ctx, FRS_EINVAL, "frs_exact_adjoint: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    CKL(launch_exact_grid(ctx->stream, uv, wgt, vis, nvis, ctx->ny, ctx->nx, nullptr, 1.0f, y));
+    ctx->launches++;
+    return FRS_OK;
+}
+
+int frs_major_cycle_residual(frs_ctx* ctx, const float* uv, const float* wgt, int nvis, const float* dirty_full, const float* sky,
+                             float* d_next) {
+    RET(response_args(ctx, uv, wgt, nvis, "frs_major_cycle_residual: bad argument"));
+    if (!wgt || !dirty_full || !sky || !d_next) return fail(ctx, FRS_EINVAL, "frs_major_cycle_residual: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    if (ctx->visbuf_n < (size_t)nvis) {
+        if (ctx->visbuf) CK(cudaFree(ctx->visbuf));
+        ctx->visbuf = nullptr;
+        CK(cudaMalloc(reinterpret_cast<void**>(&ctx->visbuf), (size_t)nvis * 2 * sizeof(float)));
+        ctx->visbuf_n = (size_t)nvis;
+    }
+    // d_{i+1} = I^D - R^+ N^-1 R I_i
+    CKL(launch_exact_degrid(ctx->stream, uv, nvis, sky, ctx->ny, ctx->nx, ctx->visbuf));
+    CKL(launch_exact_grid(ctx->stream, uv, wgt, ctx->visbuf, nvis, ctx->ny, ctx->nx, dirty_full, -1.0f, d_next));
+    ctx->launches += 2;
     return FRS_OK;
 }
 
