@@ -4,8 +4,8 @@
 // FFT core of fft_dif.cuh: the spectrum between the forward and the inverse transform stays in the permuted
 // order of that core (the weights are stored in it, k_setup.cu weights_permute), every exchange overwrites the
 // slots the thread has just read, and one exchange of each transform stays inside C neighbouring lanes.  Per
-// column a group passes TWO blocking barriers (eight in the sorting core) plus one release barrier that only
-// its first warp waits on.
+// column a group passes TWO blocking barriers (eight in the sorting core).  The staging buffer holds columns only
+// (the next one is in flight for a whole column time); the weights come from L2 straight into registers.
 template <int NF> struct ColsDifGeo {
     using D = Dif<NF>;
     static constexpr int P = D::P;
@@ -13,7 +13,6 @@ template <int NF> struct ColsDifGeo {
     static constexpr int THREADS = P >= WANT ? P : WANT;
     static constexpr int G = THREADS / P;                               // groups (columns in flight) per CTA
     static constexpr bool OWN_BAR = (P % 32 == 0) && G <= 15;           // named barrier 1 + g per group (exchange)
-    static constexpr bool SPLIT_RELEASE = OWN_BAR && P >= 64 && 2 * G <= 15;   // barrier 1 + G + g: first warp waits, the others only arrive
     static constexpr int TW = D::TW_TOTAL;                              // float4 slots, multiple of 8
     static constexpr int STAGE = NF / 2;                                // float4 slots of the staging buffer (NF float2)
     static constexpr int GROUP_SLOTS = D::XLEN + STAGE;
@@ -52,13 +51,11 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
         live = item < a.nitems && kx < a.ncols;
         w = a.wt + b * a.w_bstride + (size_t)kx * NF * 2;
     };
-    auto fetch_weights = [&](const void* src, bool live) {       // one bulk copy of 8 NF bytes into the staging buffer
-        if (t == 0 && live) {
-            fence_proxy_async();
-            mbar_expect_tx(bar, NF * 8);
-            bulk_g2s(stage, src, NF * 8, bar);
-        }
-        __syncwarp();
+    // this column's weights do not pass through shared memory: their 8 NF bytes are pulled into L2 one column ahead
+    // (one bulk prefetch) and read from there straight into registers, so that the staging buffer belongs to the
+    // columns alone and the NEXT column is in flight for a whole column time
+    auto prefetch_weights = [&](const void* src, bool live) {
+        if (t == 0 && live) bulk_prefetch_l2(src, NF * 8);
     };
     auto fetch_column = [&](int b, int kx, bool live) {          // column kx lands as NF contiguous samples
         if (t == 0 && live) {
@@ -69,21 +66,13 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
         if (t < NCOPY && live) tensor_g2s_5d(stage + 2 * BOXR * t, &a.tmap, 0, kx % kBlockBins, BOXR * t, kx / kBlockBins, b, bar);
         __syncwarp();
     };
-    // every thread of the group has consumed the staging buffer: only the issuing warp has to know
-    auto release_stage = [&]() {
-        if constexpr (GEO::SPLIT_RELEASE) {
-            if (t < 32) asm volatile("bar.sync %0, %1;" :: "r"(1 + GEO::G + g), "r"(P) : "memory");
-            else asm volatile("bar.arrive %0, %1;" :: "r"(1 + GEO::G + g), "r"(P) : "memory");
-        } else {
-            gb.sync();
-        }
-    };
     unsigned parity = 0;
     __syncthreads();
     {
         bool live; int b, kx; const float* w;
         column(blockIdx.x, live, b, kx, w);
         fetch_column(b, kx, live);
+        prefetch_weights(w, live);
     }
 
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
@@ -104,26 +93,24 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
             for (int e = 0; e < kE; ++e) v[e] = c2zero();
         }
         dif_fwd_0<NF>(v, t, X, tws);
-        gb.sync();                                  // X1 written; and every thread has picked up its samples
-        fetch_weights(w, live);
+        gb.sync();                                  // X1 written; and every thread has picked up its samples:
+        {                                           // the next column may land
+            bool nlive; int nb_, nkx; const float* nw;
+            column(item + gridDim.x, nlive, nb_, nkx, nw);
+            fetch_column(nb_, nkx, nlive);
+            prefetch_weights(nw, nlive);
+        }
         dif_fwd_1<NF>(v, t, X, tws);
         dif_warp_sync();
         dif_fwd_2<NF>(v, t, X);
         if (live) {
-            mbar_wait(bar, parity);
-            parity ^= 1u;
+            const float* wp = w + 2 * t;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 ww = stage[t + e * P];                   // (even-bin weight, odd-bin weight) of register e
+                const float2 ww = ldg2(wp + 2 * e * P);               // (even-bin weight, odd-bin weight) of register e
                 v[e].re = f2mul(v[e].re, ww);
                 v[e].im = f2mul(v[e].im, ww);
             }
-        }
-        release_stage();                            // the weights have been consumed: the next column may land
-        {
-            bool nlive; int nb_, nkx; const float* nw;
-            column(item + gridDim.x, nlive, nb_, nkx, nw);
-            fetch_column(nb_, nkx, nlive);
         }
         dif_inv_0<NF>(v, t, X);
         dif_warp_sync();
