@@ -71,6 +71,10 @@ class ClockSampler:
                                           "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
+            t0 = time.time()                      # nvidia-smi needs a moment to start: wait for its first line
+            while not self.lines and time.time() - t0 < 3.0:
+                time.sleep(0.01)
+            self.n0 = len(self.lines)
         except Exception:
             self.proc = None
 
@@ -78,13 +82,26 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.lines.append(line.strip())
 
-    def stop(self):
+    def stop(self, load=None, sync=None):
+        """load/sync: the timed step and a device synchronise.  The timed region of the default run is shorter than
+        a few sampling periods (20 ms), so the very same step loop keeps running, untimed, for another 0.4 s while
+        the sampler goes on: the clocks reported are those of this kernel sequence under load."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
+        window = "timed region"
+        if load is not None:
+            t_end, i = time.time() + 0.4, 0
+            while time.time() < t_end:
+                for _ in range(16):
+                    load(i)
+                    i += 1
+                sync()
+            window = "timed region + 0.4 s of the same step loop (untimed)"
+        else:
+            time.sleep(0.15)
         self.proc.terminate()
         sm, mx, reasons = [], [], set()
-        for l in self.lines:
+        for l in self.lines[getattr(self, "n0", 0):]:
             f = [x.strip() for x in l.split(",")]
             if len(f) < 9:
                 continue
@@ -97,7 +114,7 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "window": window}
 
 
 # ----------------------------------------------------------------------------------------- oracle arm
@@ -218,7 +235,7 @@ def run_cuda(args):
         sampler.start()
     ms = timed(step, args.steps, args.warmup)
     launches = ctx.launch_count() - l_after_warmup
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop(step, torch.cuda.synchronize) if rank == 0 else None
     ms_step = ms / args.steps
     value = world * args.steps / (ms * 1e-3)
 
@@ -295,16 +312,25 @@ def run_cuda(args):
             extra["energy_grad_ms"] = m / k2
             b = (-g).contiguous()
             sol = torch.zeros_like(b)
-            iters = 10
+            iters = 20
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            ctx.cg_solve(b, sol, 2)
+            ctx.cg_solve(b, sol, iters)                                    # warm-up: also builds the iteration graph
             sol.zero_()
             e0.record()
             ctx.cg_solve(b, sol, iters)
             e1.record()
             torch.cuda.synchronize()
             extra["ms_per_cg_iter"] = e0.elapsed_time(e1) / (iters + 1)   # + the initial M x0 apply
+            ctx.set_cuda_graphs(False)                                     # the same solve with plain launches
+            ctx.cg_solve(b, sol, 2)
+            sol.zero_()
+            e0.record()
+            ctx.cg_solve(b, sol, iters)
+            e1.record()
+            torch.cuda.synchronize()
+            extra["ms_per_cg_iter_plain_launches"] = e0.elapsed_time(e1) / (iters + 1)
+            ctx.set_cuda_graphs(True)
             # the paper's literal likelihood (Eq. 9 with the fitted noise kernel): J^T C N'^-1 C J + 1
             ctx.set_noise_kernel(1e-2 * float(np.sum(w.w_half[0][:, 0]) + 2 * np.sum(w.w_half[0][:, 1:-1]) + np.sum(w.w_half[0][:, -1])))
             ctx.set_likelihood(1)

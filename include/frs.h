@@ -97,6 +97,12 @@ int frs_metric_apply(frs_ctx* ctx, const float* v, int with_prior, float* out);
  * Synchronises at the end.  FRS_EBREAKDOWN if <p, M p> <= 0 was met (x is the last good iterate). */
 int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior,
                  int* h_iters, double* h_resnorm, double* d_res_history);
+/* frs_cg_solve (and the solves inside frs_draw_sample) run iteration 0 with plain launches and replay every later
+ * iteration as ONE captured CUDA graph (the iteration index lives on the device), rebuilt only when a frozen argument
+ * (x, with_prior, likelihood mode, history pointer, rtol, number of fields) changes.  on = 0 turns that off (plain
+ * launches throughout: what the profiling events of frs_profile_enable need, and the comparison arm of bench.py).
+ * The results are the same kernels on the same data either way.  Default: on. */
+int frs_set_cuda_graphs(frs_ctx* ctx, int on);
 /* Copy out the CG state of the last frs_cg_solve / frs_cg_step: r, p, q (DEVICE pointers,
  * [nfield][ny][nx] each, any may be NULL) and the scalar block scal_host (HOST double[8], may be NULL:
  * rr, pq, rr_new, alpha, beta, breakdown, bb, -).  Synchronises. */

@@ -41,6 +41,7 @@ EXPORTS = {
     "frs_get_noise_kernel": (_i, [_vp, _vp]),
     "frs_ninv_apply": (_i, [_vp, _vp, _vp]),
     "frs_set_likelihood": (_i, [_vp, _i]),
+    "frs_set_cuda_graphs": (_i, [_vp, _i]),
     "frs_draw_sample": (_i, [_vp, _vp, _vp, _i, _f, _vp, C.POINTER(_i)]),
     "frs_kl_energy_grad": (_i, [_vp, _vp, _vp, _i, _i, _vp, C.POINTER(_d), _vp]),
     "frs_kl_metric_apply": (_i, [_vp, _vp, _vp, _i, _i, _vp, _vp]),
@@ -251,6 +252,9 @@ class Context:
 
     def set_likelihood(self, mode):
         self._ck(lib().frs_set_likelihood(self._h, int(mode)))
+
+    def set_cuda_graphs(self, on):
+        self._ck(lib().frs_set_cuda_graphs(self._h, int(bool(on))))
 
     # ---- major cycle (exact response on uv points; images are single-channel [ny][nx])
     def exact_response(self, uv, x, vis):

@@ -176,7 +176,7 @@ __global__ void energy9_final_kernel(const double* __restrict__ ru, const double
 // scal[kIters] = completed iterations.  The stopping test runs on the DEVICE (cg_shift_kernel): once `done` is set the
 // vector updates of the iterations still enqueued turn into no-ops, so the host never has to synchronise inside the loop
 // and x is exactly the iterate at which the criterion was met.
-enum { kRR = 0, kPQ = 1, kRRNew = 2, kAlpha = 3, kBeta = 4, kBreak = 5, kBB = 6, kDone = 7, kNScal = 8, kIters = 12 };
+enum { kRR = 0, kPQ = 1, kRRNew = 2, kAlpha = 3, kBeta = 4, kBreak = 5, kBB = 6, kDone = 7, kNScal = 8, kIters = 12, kStep = 13 };
 
 // r = b - q ; p = r ; partial <r,r>       (q = M x0, or q == nullptr for x0 = 0)
 __global__ void __launch_bounds__(kRedThreads) cg_init_kernel(const float* __restrict__ b, const float* __restrict__ q,
@@ -256,8 +256,12 @@ __global__ void __launch_bounds__(kEwThreads) add_inplace_kernel(float* __restri
     }
 }
 // end of iteration k (k = 0: initialisation): rr <- rr_new, count it, and decide whether to stop:
-// ||r||^2 <= rtol2 <b,b>  (rtol2 = 0: never)  or  breakdown <p, M p> <= 0
+// ||r||^2 <= rtol2 <b,b>  (rtol2 = 0: never)  or  breakdown <p, M p> <= 0.
+// k < 0: the iteration index is the device-side counter scal[kStep] + 1, so that one captured iteration (a CUDA graph
+// whose kernel arguments are frozen) can be replayed for every k.
 __global__ void cg_shift_kernel(double* __restrict__ scal, double* __restrict__ hist, int k, double rtol2) {
+    if (k < 0) k = (int)scal[kStep] + 1;
+    scal[kStep] = (double)k;
     if (scal[kDone] == 0.0) {
         scal[kRR] = scal[kRRNew];
         scal[kIters] = (double)k;

@@ -53,6 +53,12 @@ struct frs_ctx {
     int* flag = nullptr;
     bool have_psf = false, have_dirty = false, have_amp = false, have_s = false;
     long long launches = 0;
+    // one CG iteration captured as a CUDA graph (cg_solve_impl): replayed while the key (every frozen argument) matches
+    struct CgGraphKey { const float* x; int with_prior, nfield, lik_mode; double* hist; double rtol2; bool sT_ok; } cg_key = {};
+    cudaGraphExec_t cg_exec = nullptr;
+    cudaStream_t cap_stream = nullptr;  // capture runs on a stream of the ctx's own (the caller's may be the legacy default stream)
+    long long cg_graph_launches = 0;   // kernels per replay
+    int use_graphs = 1;
     bool profiling = false;
     std::vector<ProfRec> prof;
     char err[512] = "no error";
@@ -395,7 +401,7 @@ int cg_iter_finish(frs_ctx* ctx, float* x, double* d_hist, int k, bool have_pq =
     cg_update_xr_kernel<<<nb, kRedThreads, 0, ctx->stream>>>(x, ctx->cg_r, ctx->cg_p, ctx->cg_q, n, ctx->scal, ctx->partials);
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, nb, 1, 0, ctx->scal + kRRNew);
     cg_update_p_kernel<<<nb, kEwThreads, 0, ctx->stream>>>(ctx->cg_p, ctx->cg_r, n, ctx->scal, ctx->scal + kBeta);
-    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_hist, k + 1, rtol2);
+    cg_shift_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal, d_hist, k < 0 ? -1 : k + 1, rtol2);
     ctx->launches += 4;
     CK(cudaGetLastError());
     return FRS_OK;
@@ -481,6 +487,8 @@ void frs_destroy(frs_ctx* ctx) {
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    if (ctx->cg_exec) cudaGraphExecDestroy(ctx->cg_exec);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     delete ctx;
 }
 
@@ -795,6 +803,12 @@ int frs_cg_step_end(frs_ctx* ctx, float* x, int with_prior) {
 static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,
                          double* h_resnorm, double* d_res_history);
 
+int frs_set_cuda_graphs(frs_ctx* ctx, int on) {
+    if (!ctx) return FRS_EINVAL;
+    ctx->use_graphs = on ? 1 : 0;
+    return FRS_OK;
+}
+
 int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,
                  double* h_resnorm, double* d_res_history) {
     if (!ctx || !b || !x || !aligned16(b) || !aligned16(x) || max_iter < 0 || rtol < 0.f || b == x)
@@ -822,13 +836,54 @@ static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, f
     // The stopping test lives on the device; with rtol > 0 the host looks at the flag every 8 iterations only to stop
     // enqueueing (the iterations enqueued past the stopping point leave x, r, p untouched).
     double sc[16];
-    for (int it = 0; it < max_iter; ++it) {
+    // Iteration 0 runs eagerly (it triggers every lazy allocation, tensor map and shared-memory opt-in); the following
+    // iterations replay ONE captured iteration as a CUDA graph: at configs 1-2 an iteration is 13 launches of a few
+    // microseconds each and the host cannot enqueue them as fast as the device runs them.
+    int it = 0;
+    if (it < max_iter) {
+        RET(cg_iter(ctx, x, with_prior, d_res_history, -1, rtol2));
+        ++it;
+    }
+    const bool graphs = ctx->use_graphs && !ctx->profiling && max_iter - it >= 2;
+    if (graphs) {
+        const frs_ctx::CgGraphKey key = {x, with_prior, ctx->nfield, ctx->lik_mode, d_res_history, rtol2, ctx->sT_ok};
+        const frs_ctx::CgGraphKey& k0 = ctx->cg_key;
+        const bool same = ctx->cg_exec && k0.x == key.x && k0.with_prior == key.with_prior && k0.nfield == key.nfield &&
+                          k0.lik_mode == key.lik_mode && k0.hist == key.hist && k0.rtol2 == key.rtol2 && k0.sT_ok == key.sT_ok;
+        if (!same) {
+            if (ctx->cg_exec) { cudaGraphExecDestroy(ctx->cg_exec); ctx->cg_exec = nullptr; }
+            cudaGraph_t g = nullptr;
+            const long long l0 = ctx->launches;
+            if (!ctx->cap_stream) CK(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+            cudaStream_t user = ctx->stream;
+            CK(cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+            ctx->stream = ctx->cap_stream;
+            const int rc = cg_iter(ctx, x, with_prior, d_res_history, -1, rtol2);
+            ctx->stream = user;
+            const cudaError_t ce = cudaStreamEndCapture(ctx->cap_stream, &g);
+            ctx->cg_graph_launches = ctx->launches - l0;
+            ctx->launches = l0;                     // nothing ran during the capture
+            if (rc == FRS_OK && ce == cudaSuccess && g && cudaGraphInstantiate(&ctx->cg_exec, g, 0) == cudaSuccess) {
+                ctx->cg_key = key;
+            } else {
+                ctx->cg_exec = nullptr;
+                cudaGetLastError();                 // capture refused: fall back to eager launches below
+            }
+            if (g) cudaGraphDestroy(g);
+        }
+    }
+    for (; it < max_iter; ++it) {
         if (rtol > 0.f && (it & 7) == 7) {
             CK(cudaMemcpyAsync(sc, ctx->scal, kNScal * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
             CK(cudaStreamSynchronize(ctx->stream));
             if (sc[kDone] != 0.0) break;
         }
-        RET(cg_iter(ctx, x, with_prior, d_res_history, it, rtol2));
+        if (graphs && ctx->cg_exec) {
+            CK(cudaGraphLaunch(ctx->cg_exec, ctx->stream));
+            ctx->launches += ctx->cg_graph_launches;
+        } else {
+            RET(cg_iter(ctx, x, with_prior, d_res_history, -1, rtol2));
+        }
     }
     CK(cudaMemcpyAsync(sc, ctx->scal, 16 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));

@@ -258,6 +258,36 @@ def test_cg_rtol_stops_on_the_device_at_the_right_iterate(frs):
     assert rn3 > 1e-2 * float(b.double().norm())                   # one iteration earlier the criterion was not met
 
 
+def test_cg_graph_replay_equals_plain_launches(frs):
+    """frs_cg_solve replays iterations 1.. as one captured CUDA graph (the iteration index lives on the device): same
+    kernels on the same data, so x, the residual history and the iteration count must be bit-identical to plain
+    launches -- without and with the stopping test, single- and multi-channel, and in the Eq. 9 mode."""
+    import torch
+    for key, mode in ((("c1b",), 0), (("multi", 64, 3), 0), (("c1b",), 1)):
+        w, ctx, b, ap = _cg_problem(frs, key)
+        if mode == 1:
+            ctx.set_noise_kernel(1e-2 * float(np.sum(w.w_half[0][:, 0]) + 2 * np.sum(w.w_half[0][:, 1:-1]) + np.sum(w.w_half[0][:, -1])))
+            ctx.set_likelihood(1)
+        out = {}
+        for on in (1, 0, 1):
+            ctx.set_cuda_graphs(on)
+            l0 = ctx.launch_count()
+            x = torch.zeros_like(b)
+            hist = torch.zeros(21, dtype=torch.float64, device="cuda")
+            it, rn = ctx.cg_solve(b, x, 20, res_history=hist)
+            xr = torch.zeros_like(b)
+            itr, rnr = ctx.cg_solve(b, xr, 200, rtol=1e-2)
+            res = (x.clone(), hist.clone(), it, rn, xr.clone(), itr, rnr, ctx.launch_count() - l0)
+            if on in out and on == 1:
+                prev = out[1]                                      # the cached graph of the first round is reused
+                assert torch.equal(prev[0], res[0]) and torch.equal(prev[4], res[4])
+            out[on] = res
+        g, e = out[1], out[0]
+        assert torch.equal(g[0], e[0]) and torch.equal(g[1], e[1]) and g[2] == e[2] == 20 and g[3] == e[3]
+        assert torch.equal(g[4], e[4]) and g[5] == e[5] and g[6] == e[6]
+        assert g[7] == e[7] > 0                                    # the launch count is kept honest under replay
+
+
 # ---------------------------------------------------------------------------------- CG (protocol of DESIGN.md R9)
 def _cg_problem(frs, key):
     import torch
