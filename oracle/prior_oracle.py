@@ -1,0 +1,208 @@
+"""ORACLE -- test infrastructure, not product code.
+
+NEXT-3 of SURVEY.md section 8(f): the learned amplitude spectrum of the diffuse-emission prior and the inverse-gamma
+point-source pixels (parameters of Table A.1 / B.1).  The paper defers the
+definitions to Arras et al. (2021a), which is not in the container, so what is written out here is the reading
+DESIGN.md lists as R17 (amplitude model) and R18 (point sources), in float64, in the order of that reading.
+Shares no code with the CUDA path; imported only by tests/.
+
+R17 in one place (ny x nx harmonic grid, standard-normal latent vector theta):
+  bins      b(pixel) = rint(|k|), |k| = sqrt(fy^2 + fx^2) in cycles per LONGER field side, f = min(k, n - k) scaled by
+            nmax / n;  nb = max b + 1;  mult_b = pixels in bin b;  t_b = ln b (b >= 1)
+  theta     [xi_fluct, xi_slope, xi_flex, xi_asp, xi_zm, zeta_1 .. zeta_{nb-2}, eta_1 .. eta_{nb-2}]
+  hyper     (offset, zm_mean, zm_std, fl_mean, fl_std, sl_mean, sl_std, fx_mean, fx_std, as_mean, as_std)   Table A.1
+  lognormal LN(xi; m, s) = m / sqrt(1 + (s/m)^2) * exp(sqrt(ln(1 + (s/m)^2)) xi): mean m, standard deviation s
+  fluct = LN(xi_fluct), slope = sl_mean + sl_std xi_slope, flex = LN(xi_flex), asp = LN(xi_asp), zm = LN(xi_zm)
+  walk      dev_1 = vel_1 = 0;  D_j = t_{j+1} - t_j;
+            dev_{j+1} = dev_j + vel_j D_j + flex asp sqrt(D_j) eta_j;  vel_{j+1} = vel_j + flex sqrt(D_j) zeta_j
+  spectrum  ln P_b = slope t_b + dev_b;  a_b = exp(ln P_b / 2);  S = sum_{b>=1} mult_b a_b^2
+  amplitude A[pixel] = fluct a_b / sqrt(S) (b >= 1),  A[zero mode] = zm      =>  sum_pixels A^2 = fluct^2 + zm^2
+  sky       s = exp(offset + H[A . xi])   (frs_oracle.sky with mu = offset)
+"""
+from __future__ import annotations
+
+import numpy as np
+
+NHYPER = 11
+NSCALAR = 5          # xi_fluct, xi_slope, xi_flex, xi_asp, xi_zm
+
+
+# ----------------------------------------------------------------------------------------------- bins
+def bins(ny, nx):
+    """b[ky, kx] = rint(|k|) (int64), mult[b], t[b] = ln b (t[0] unused = 0)."""
+    nmax = max(ny, nx)
+    fy = np.minimum(np.arange(ny), ny - np.arange(ny)) * (nmax // ny)
+    fx = np.minimum(np.arange(nx), nx - np.arange(nx)) * (nmax // nx)
+    k2 = fy[:, None].astype(np.int64) ** 2 + fx[None, :].astype(np.int64) ** 2
+    b = np.rint(np.sqrt(k2.astype(np.float64))).astype(np.int64)
+    nb = int(b.max()) + 1
+    mult = np.bincount(b.ravel(), minlength=nb).astype(np.float64)
+    t = np.zeros(nb)
+    t[1:] = np.log(np.arange(1, nb))
+    return b, mult, t
+
+
+def ntheta(nb):
+    return NSCALAR + 2 * (nb - 2)
+
+
+# ----------------------------------------------------------------------------------------------- scalars
+def lognormal(xi, mean, std):
+    """Log-normal variable with the given mean and standard deviation as a function of a standard normal xi."""
+    r = 1.0 + (std / mean) ** 2
+    return mean / np.sqrt(r) * np.exp(np.sqrt(np.log(r)) * xi)
+
+
+def unpack(theta, nb):
+    theta = np.asarray(theta)
+    n = nb - 2
+    return theta[:NSCALAR], theta[NSCALAR:NSCALAR + n], theta[NSCALAR + n:NSCALAR + 2 * n]
+
+
+# ----------------------------------------------------------------------------------------------- forward
+def bin_amplitudes(theta, hyper, mult, t):
+    """A_b for b = 0 .. nb-1 (the walk written as the plain loop of the reading).  Works for complex theta too
+    (used by the complex-step derivative below), hence no float() casts."""
+    nb = len(t)
+    sc, zeta, eta = unpack(theta, nb)
+    _, zm_m, zm_s, fl_m, fl_s, sl_m, sl_s, fx_m, fx_s, as_m, as_s = hyper
+    fluct = lognormal(sc[0], fl_m, fl_s)
+    slope = sl_m + sl_s * sc[1]
+    flex = lognormal(sc[2], fx_m, fx_s)
+    asp = lognormal(sc[3], as_m, as_s)
+    zm = lognormal(sc[4], zm_m, zm_s)
+    dtype = np.result_type(np.asarray(theta).dtype, np.float64)
+    dev = np.zeros(nb, dtype)
+    vel = np.zeros(nb, dtype)
+    for j in range(1, nb - 1):
+        d = t[j + 1] - t[j]
+        dev[j + 1] = dev[j] + vel[j] * d + flex * asp * np.sqrt(d) * eta[j - 1]
+        vel[j + 1] = vel[j] + flex * np.sqrt(d) * zeta[j - 1]
+    a = np.zeros(nb, dtype)
+    a[1:] = np.exp(0.5 * (slope * t[1:] + dev[1:]))
+    s = np.sum(mult[1:] * a[1:] ** 2)
+    out = np.zeros(nb, dtype)
+    out[1:] = fluct * a[1:] / np.sqrt(s)
+    out[0] = zm
+    return out
+
+
+def amplitude(theta, hyper, ny, nx):
+    """A [ny, nx] (harmonic order) of the reading R17."""
+    b, mult, t = bins(ny, nx)
+    return bin_amplitudes(theta, hyper, mult, t)[b]
+
+
+# ----------------------------------------------------------------------------------------------- derivatives
+def amplitude_jvp(theta, dtheta, hyper, ny, nx, h=1e-30):
+    """dA = (dA/dtheta) dtheta by the complex-step derivative of the forward function: exact to rounding and
+    independent of any hand-derived formula (the forward map is analytic in theta)."""
+    b, mult, t = bins(ny, nx)
+    z = np.asarray(theta, np.complex128) + 1j * h * np.asarray(dtheta, np.float64)
+    return (np.imag(bin_amplitudes(z, hyper, mult, t)) / h)[b]
+
+
+def bin_jacobian(theta, hyper, mult, t):
+    """Dense dA_b / dtheta_i [nb, ntheta], column by column with the complex step (small nb only)."""
+    nb = len(t)
+    n = ntheta(nb)
+    jac = np.zeros((nb, n))
+    for i in range(n):
+        z = np.asarray(theta, np.complex128).copy()
+        z[i] += 1e-30j
+        jac[:, i] = np.imag(bin_amplitudes(z, hyper, mult, t)) / 1e-30
+    return jac
+
+
+def amplitude_vjp(theta, g_a, hyper, ny, nx):
+    """g_theta = (dA/dtheta)^T g_A, the adjoint of the reading written out (reverse sweep of the walk)."""
+    b, mult, t = bins(ny, nx)
+    nb = len(t)
+    g = np.bincount(b.ravel(), weights=np.asarray(g_a, np.float64).ravel(), minlength=nb)    # G_b = sum over the bin
+    sc, zeta, eta = unpack(np.asarray(theta, np.float64), nb)
+    _, zm_m, zm_s, fl_m, fl_s, sl_m, sl_s, fx_m, fx_s, as_m, as_s = hyper
+    sig = lambda m, s: np.sqrt(np.log(1.0 + (s / m) ** 2))  # noqa: E731
+    flex = lognormal(sc[2], fx_m, fx_s)
+    asp = lognormal(sc[3], as_m, as_s)
+    zm = lognormal(sc[4], zm_m, zm_s)
+    a_b = bin_amplitudes(theta, hyper, mult, t)
+    # A_b = fluct a_b / sqrt(S):  dA_b = A_b (dfluct / fluct + dlnP_b / 2 - dS / (2 S)),  dS / S = sum_b w_b dlnP_b
+    q = a_b * g
+    q[0] = 0.0
+    qsum = np.sum(q)
+    w = mult * a_b ** 2
+    w[0] = 0.0
+    w /= np.sum(w)                                        # = mult_b a_b^2 / S  (the fluct^2 cancels)
+    lbar = 0.5 * q - 0.5 * qsum * w                       # adjoint of ln P_b
+    out = np.zeros(ntheta(nb))
+    out[0] = sig(fl_m, fl_s) * qsum
+    out[1] = sl_s * np.sum(lbar * t)
+    out[4] = zm * sig(zm_m, zm_s) * g[0]
+    dbar = np.zeros(nb + 1)                               # D_b = sum_{b' >= b} lbar_b'
+    for bb in range(nb - 1, 0, -1):
+        dbar[bb] = dbar[bb + 1] + lbar[bb]
+    vbar = np.zeros(nb + 1)                               # adjoint of vel_b
+    fxbar = asbar = 0.0
+    n = nb - 2
+    for j in range(nb - 2, 0, -1):
+        d = t[j + 1] - t[j]
+        vbar[j] = vbar[j + 1] + d * dbar[j + 1]
+        out[NSCALAR + n + (j - 1)] = flex * asp * np.sqrt(d) * dbar[j + 1]          # eta_j
+        out[NSCALAR + (j - 1)] = flex * np.sqrt(d) * vbar[j + 1]                    # zeta_j
+        fxbar += np.sqrt(d) * (asp * eta[j - 1] * dbar[j + 1] + zeta[j - 1] * vbar[j + 1])
+        asbar += np.sqrt(d) * flex * eta[j - 1] * dbar[j + 1]
+    out[2] = flex * sig(fx_m, fx_s) * fxbar
+    out[3] = asp * sig(as_m, as_s) * asbar
+    return out
+
+
+# ----------------------------------------------------------------------------------------------- joint model
+# Likelihood of DESIGN.md R1 (E_lh = 1/2 <s, C s> - <j, s>, single channel, one field) on the joint latent vector
+# (xi, theta), prior 1/2 <xi, xi> + 1/2 <theta, theta>.  The convolution and the Hartley transform are the ones of
+# frs_oracle (pinned there); what is new is the dependence of A on theta.
+def _fo():
+    from oracle import frs_oracle as fo
+    return fo
+
+
+def sky_joint(w_unused, hyper, xi, theta):
+    fo = _fo()
+    ny, nx = xi.shape
+    a = amplitude(theta, hyper, ny, nx)
+    return np.exp(hyper[0] + fo.hartley2(a * np.asarray(xi, np.float64))), a
+
+
+def energy_grad_joint(w_half_c, dirty, hyper, xi, theta, with_prior=True):
+    """E(xi, theta), dE/dxi [ny, nx], dE/dtheta [ntheta]."""
+    fo = _fo()
+    xi = np.asarray(xi, np.float64)
+    theta = np.asarray(theta, np.float64)
+    ny, nx = xi.shape
+    s, a = sky_joint(None, hyper, xi, theta)
+    cs = fo.psf_apply(w_half_c, s)
+    e = 0.5 * np.sum(s * cs) - np.sum(np.asarray(dirty, np.float64) * s)
+    h = fo.hartley2(s * (cs - dirty))
+    g_xi = a * h
+    g_th = amplitude_vjp(theta, xi * h, hyper, ny, nx)
+    if with_prior:
+        e += 0.5 * np.sum(xi * xi) + 0.5 * np.sum(theta * theta)
+        g_xi = g_xi + xi
+        g_th = g_th + theta
+    return float(e), g_xi, g_th
+
+
+def metric_apply_joint(w_half_c, hyper, xi, theta, dxi, dtheta, with_prior=True):
+    """Fisher metric J^T C J (+ 1) of the joint model applied to (dxi, dtheta); J = ds/d(xi, theta)."""
+    fo = _fo()
+    xi = np.asarray(xi, np.float64)
+    ny, nx = xi.shape
+    s, a = sky_joint(None, hyper, xi, theta)
+    da = amplitude_jvp(theta, dtheta, hyper, ny, nx)
+    dtau = fo.hartley2(a * np.asarray(dxi, np.float64) + da * xi)
+    h = fo.hartley2(s * fo.psf_apply(w_half_c, s * dtau))
+    o_xi = a * h
+    o_th = amplitude_vjp(theta, xi * h, hyper, ny, nx)
+    if with_prior:
+        o_xi = o_xi + dxi
+        o_th = o_th + np.asarray(dtheta, np.float64)
+    return o_xi, o_th

@@ -1,0 +1,146 @@
+"""Pins of oracle/prior_oracle.py (NEXT-3, readings R17): everything here is CPU-only and checks the oracle against
+things other than itself -- a hand-worked fixture, closed forms, quadrature, finite differences, dense Jacobians."""
+import os
+
+import numpy as np
+
+from oracle import frs_oracle as fo
+from oracle import prior_oracle as po
+
+HYPER = (18.0, 1.0, 0.1, 5.0, 1.0, -2.0, 0.2, 1.2, 0.4, 0.2, 0.2)      # Table A.1, S band
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def test_bins_hand_worked_4x4():
+    rows = [l.split() for l in open(os.path.join(GOLD, "hand_bins_4x4.txt")) if l.strip() and not l.startswith("#")]
+    b_ref = np.array(rows[:4], dtype=np.int64)
+    mult_ref = np.array(rows[4], dtype=np.float64)
+    b, mult, t = po.bins(4, 4)
+    assert np.array_equal(b, b_ref) and np.array_equal(mult, mult_ref)
+    assert t[0] == 0.0 and np.allclose(t[1:], np.log([1.0, 2.0, 3.0]), rtol=0, atol=1e-15)
+
+
+def test_bins_rectangle_uses_the_longer_side_and_is_even():
+    b, mult, t = po.bins(8, 32)
+    assert b[1, 0] == 4 and b[0, 1] == 1 and b[4, 16] == np.rint(np.hypot(16, 16))      # fy scaled by 32 / 8
+    assert np.array_equal(b, b[(-np.arange(8)) % 8][:, (-np.arange(32)) % 32])           # b[-k] = b[k]: A is even (R6)
+    assert mult.sum() == 8 * 32 and mult[0] == 1
+
+
+def test_lognormal_has_the_stated_mean_and_std():
+    x, w = np.polynomial.hermite_e.hermegauss(80)
+    w = w / np.sqrt(2 * np.pi)
+    for m, s in ((5.0, 1.0), (1.2, 0.4), (0.2, 0.2), (1.0, 0.1)):
+        v = po.lognormal(x, m, s)
+        mean = np.sum(w * v)
+        assert abs(mean - m) <= 1e-10 * m and abs(np.sqrt(np.sum(w * v * v) - mean ** 2) - s) <= 1e-8 * s
+
+
+def test_total_fluctuation_variance_and_zero_mode():
+    rng = np.random.default_rng(0)
+    ny, nx = 16, 32
+    _, _, t = po.bins(ny, nx)
+    th = rng.normal(size=po.ntheta(len(t)))
+    a = po.amplitude(th, HYPER, ny, nx)
+    fl, zm = po.lognormal(th[0], 5.0, 1.0), po.lognormal(th[4], 1.0, 0.1)
+    assert abs(np.sum(a ** 2) - (fl ** 2 + zm ** 2)) <= 1e-12 * fl ** 2 and a[0, 0] == zm and np.all(a > 0)
+    # Var(lin[x]) = sum A^2 (frs_oracle pin "Correlated field"): Monte Carlo over white xi at one pixel, ~1 %
+    xi = rng.normal(size=(4000, ny, nx))
+    lin0 = np.einsum("nyx,yx->n", xi, a)                    # H[A xi] at x = 0: cas = 1 for every mode
+    assert abs(lin0.var() / (fl ** 2 + zm ** 2) - 1.0) < 0.08
+
+
+def test_pure_power_law_without_walk():
+    ny = nx = 32
+    b, mult, t = po.bins(ny, nx)
+    th = np.zeros(po.ntheta(len(t)))
+    th[1] = 0.7
+    slope = -2.0 + 0.2 * 0.7
+    a = po.amplitude(th, HYPER, ny, nx)
+    k = np.maximum(b, 1).astype(np.float64)
+    ref = k ** (slope / 2)
+    ref[0, 0] = 0.0
+    ref *= po.lognormal(0.0, 5.0, 1.0) / np.sqrt(np.sum(ref ** 2))
+    ref[0, 0] = po.lognormal(0.0, 1.0, 0.1)
+    assert np.max(np.abs(a - ref)) <= 1e-13 * ref.max()
+
+
+def test_walk_single_kick_closed_forms():
+    """One zeta_j = 1: vel jumps by flex sqrt(D_j) at j+1, so dev_b = flex sqrt(D_j) (t_b - t_{j+1}) for b > j.
+    One eta_j = 1: dev jumps by flex asp sqrt(D_j) and stays."""
+    ny = nx = 32
+    b, mult, t = po.bins(ny, nx)
+    nb, n, j = len(t), len(t) - 2, 5
+    flex, asp = po.lognormal(0.0, 1.2, 0.4), po.lognormal(0.0, 0.2, 0.2)
+    d = t[j + 1] - t[j]
+    for kind in (0, 1):
+        th = np.zeros(po.ntheta(nb))
+        th[po.NSCALAR + kind * n + (j - 1)] = 1.0
+        ab = po.bin_amplitudes(th, HYPER, mult, t)
+        dev = 2.0 * np.log(ab[1:] / ab[1]) - (-2.0) * t[1:]                 # ln P_b - slope t_b, relative to b = 1
+        ref = np.zeros(nb - 1)
+        bb = np.arange(1, nb)
+        ref[bb > j] = flex * np.sqrt(d) * (t[bb[bb > j]] - t[j + 1]) if kind == 0 else flex * asp * np.sqrt(d)
+        assert np.max(np.abs(dev - ref)) <= 1e-12
+
+
+def test_jvp_vjp_against_finite_differences_dense_jacobian_and_each_other():
+    rng = np.random.default_rng(3)
+    ny, nx = 16, 16
+    b, mult, t = po.bins(ny, nx)
+    nb = len(t)
+    th = 0.5 * rng.normal(size=po.ntheta(nb))
+    d = rng.normal(size=po.ntheta(nb))
+    g = rng.normal(size=(ny, nx))
+    jv = po.amplitude_jvp(th, d, HYPER, ny, nx)
+    h = 1e-6
+    fd = (po.amplitude(th + h * d, HYPER, ny, nx) - po.amplitude(th - h * d, HYPER, ny, nx)) / (2 * h)
+    assert np.linalg.norm(fd - jv) <= 1e-6 * np.linalg.norm(jv)
+    jac = po.bin_jacobian(th, HYPER, mult, t)
+    vj = po.amplitude_vjp(th, g, HYPER, ny, nx)
+    ref = jac.T @ np.bincount(b.ravel(), weights=g.ravel(), minlength=nb)
+    assert np.max(np.abs(vj - ref)) <= 1e-12 * np.max(np.abs(ref))
+    assert abs(np.sum(jv * g) - np.sum(d * vj)) <= 1e-12 * abs(np.sum(jv * g))
+
+
+def _problem(n=16, seed=5):
+    from gen import workloads as wl
+    w = wl.make_config(1, n=n, seed=seed)
+    rng = np.random.default_rng(seed)
+    _, _, t = po.bins(n, n)
+    hyper = (float(np.log(np.median(w.sky_true))), 1.0, 0.1, 1.0, 0.3, -3.0, 0.2, 0.5, 0.2, 0.2, 0.1)
+    xi = 0.3 * rng.normal(size=(n, n))
+    th = 0.3 * rng.normal(size=po.ntheta(len(t)))
+    return w, hyper, xi, th, rng
+
+
+def test_joint_gradient_against_central_differences():
+    w, hyper, xi, th, rng = _problem()
+    e, gx, gt = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi, th)
+    for _ in range(4):
+        dx, dt = rng.normal(size=xi.shape), rng.normal(size=th.shape)
+        h = 1e-5
+        ep = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi + h * dx, th + h * dt)[0]
+        em = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi - h * dx, th - h * dt)[0]
+        lin = np.sum(gx * dx) + np.sum(gt * dt)
+        assert abs((ep - em) / (2 * h) - lin) <= 1e-6 * max(abs(lin), np.linalg.norm(gx) + np.linalg.norm(gt))
+    # theta fixed: the joint model is the fixed-amplitude model of frs_oracle at A(theta)
+    a = po.amplitude(th, hyper, *xi.shape)
+    e0, g0 = fo.energy_grad(w.w_half, w.dirty, a[None], [hyper[0]], w.lognu, xi[None], True)
+    assert abs(e0 + 0.5 * np.sum(th * th) - e) <= 1e-12 * abs(e) and np.max(np.abs(g0[0] - gx)) <= 1e-10 * np.max(np.abs(gx))
+
+
+def test_joint_metric_symmetric_and_at_least_identity():
+    w, hyper, xi, th, rng = _problem()
+    u = (rng.normal(size=xi.shape), rng.normal(size=th.shape))
+    v = (rng.normal(size=xi.shape), rng.normal(size=th.shape))
+    mu = po.metric_apply_joint(w.w_half[0], hyper, xi, th, *u)
+    mv = po.metric_apply_joint(w.w_half[0], hyper, xi, th, *v)
+    a, b = np.sum(v[0] * mu[0]) + np.sum(v[1] * mu[1]), np.sum(u[0] * mv[0]) + np.sum(u[1] * mv[1])
+    assert abs(a - b) <= 1e-11 * abs(a)
+    assert np.sum(u[0] * mu[0]) + np.sum(u[1] * mu[1]) >= np.sum(u[0] ** 2) + np.sum(u[1] ** 2)
+    # dtheta = 0 reduces to the fixed-amplitude metric of frs_oracle
+    am = po.amplitude(th, hyper, *xi.shape)
+    m0 = fo.metric_apply(w.w_half, am[None], [hyper[0]], w.lognu, xi[None], u[0][None], True)
+    mj = po.metric_apply_joint(w.w_half[0], hyper, xi, th, u[0], np.zeros_like(th))
+    assert np.max(np.abs(m0[0] - mj[0])) <= 1e-10 * np.max(np.abs(m0))
