@@ -142,6 +142,40 @@ int frs_ninv_apply(frs_ctx* ctx, const float* x, float* y);
  * Affects frs_energy_grad, frs_metric_apply, frs_cg_solve / _step / _step_begin. */
 int frs_set_likelihood(frs_ctx* ctx, int mode);
 
+/* ---- NEXT-3: learned amplitude spectrum of the diffuse-emission prior (parameters of Table A.1 / B.1,
+ * P:536-566; the paper defers the definition to Arras et al. 2021a -- DESIGN.md reading R17 states the one built) ----
+ * The amplitude A of frs_set_amplitude becomes a function of a standard-normal latent vector theta:
+ *   radial bins b(mode) = rint(|k|) (cycles per longer field side), nb bins, t_b = ln b;
+ *   theta = [xi_fluct, xi_slope, xi_flex, xi_asp, xi_zm, zeta_1..zeta_{nb-2}, eta_1..eta_{nb-2}]  (ntheta = 5 + 2 (nb - 2));
+ *   fluct, flex, asp, zm log-normal with the given mean / std, slope = mean + std xi_slope;
+ *   dev_1 = vel_1 = 0, dev_{j+1} = dev_j + vel_j D_j + flex asp sqrt(D_j) eta_j, vel_{j+1} = vel_j + flex sqrt(D_j) zeta_j,
+ *   D_j = t_{j+1} - t_j;  ln P_b = slope t_b + dev_b;  a_b = exp(ln P_b / 2);  A = fluct a_b / sqrt(sum mult_b a_b^2) on
+ *   bin b >= 1, A = zm on the zero mode;  sky = exp(offset + H[A . xi]).
+ * Single channel, one field.  The spectrum (a few thousand bins) is evaluated in fp64 on the device; A is fp32. */
+
+/* Host arithmetic only: number of bins and length of theta for an ny x nx grid (either pointer may be NULL). */
+int frs_amp_model_size(int ny, int nx, int* nb, int* ntheta);
+/* hyper_host: HOST float[11] = offset, zero-mode mean, std, fluctuations mean, std, loglogavgslope mean, std,
+ * flexibility mean, std, asperity mean, std (the rows of Table A.1).  Builds the bin index of the grid on first use.
+ * Switches the context to nfield = 1 with mu = offset and invalidates amplitude and position; frs_set_amplitude
+ * switches back.  Errors: FRS_ESTATE for nchan != 1, FRS_EINVAL for a non-positive log-normal mean or a negative std. */
+int frs_set_amplitude_model(frs_ctx* ctx, const float* hyper_host);
+/* A(theta) becomes the context's amplitude (theta: device float[ntheta], copied); amp_out: device [ny][nx] or NULL.
+ * Invalidates the cached position. */
+int frs_amplitude_forward(frs_ctx* ctx, const float* theta, float* amp_out);
+/* d_amp [ny][nx] = (dA/dtheta) dtheta and g_theta [ntheta] = (dA/dtheta)^T g_amp at the theta of the last forward. */
+int frs_amplitude_jvp(frs_ctx* ctx, const float* dtheta, float* d_amp);
+int frs_amplitude_vjp(frs_ctx* ctx, const float* g_amp, float* g_theta);
+/* Energy of the likelihood in use (frs_set_likelihood) at the joint position (xi, theta), prior 1/2 <xi,xi> + 1/2
+ * <theta,theta> if with_prior, and its gradient with respect to both (grad_xi [ny][nx], grad_theta [ntheta]).
+ * Sets the joint position.  h_energy: host double or NULL (non-NULL synchronises). */
+int frs_energy_grad_joint(frs_ctx* ctx, const float* xi, const float* theta, int with_prior, double* h_energy, float* grad_xi,
+                          float* grad_theta);
+/* Fisher metric of the joint model at the joint position: (out_xi, out_theta) = J^T C J (dxi, dtheta) (+ (dxi, dtheta)),
+ * J = d sky / d (xi, theta) = diag(s) H [diag(A) . + diag(xi) dA/dtheta .]   (mode 1: C N'^-1 C in the middle).
+ * FRS_ESTATE without a joint position. */
+int frs_metric_apply_joint(frs_ctx* ctx, const float* dxi, const float* dtheta, int with_prior, float* out_xi, float* out_theta);
+
 /* ---- MGVI: posterior samples and the sample-averaged KL (reading R15) ------------
  * MGVI approximates the posterior by N(xi, M(xi)^-1), M the metric above, and minimises the KL estimated on samples
  * xi +- sigma_i, sigma_i ~ N(0, M^-1).  The random numbers are INPUTS (white N(0,1) arrays drawn by the caller). */

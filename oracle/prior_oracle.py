@@ -172,16 +172,23 @@ def sky_joint(w_unused, hyper, xi, theta):
     return np.exp(hyper[0] + fo.hartley2(a * np.asarray(xi, np.float64))), a
 
 
-def energy_grad_joint(w_half_c, dirty, hyper, xi, theta, with_prior=True):
-    """E(xi, theta), dE/dxi [ny, nx], dE/dtheta [ntheta]."""
+def energy_grad_joint(w_half_c, dirty, hyper, xi, theta, with_prior=True, kern=None):
+    """E(xi, theta), dE/dxi [ny, nx], dE/dtheta [ntheta].  kern = None: the N' = R' likelihood (R1); kern = K [ny, nx]:
+    Eq. 9 with N'^-1 of Eq. 18 (R14), E_lh = 1/2 r^T N'^-1 r, r = j - C s."""
     fo = _fo()
     xi = np.asarray(xi, np.float64)
     theta = np.asarray(theta, np.float64)
     ny, nx = xi.shape
     s, a = sky_joint(None, hyper, xi, theta)
     cs = fo.psf_apply(w_half_c, s)
-    e = 0.5 * np.sum(s * cs) - np.sum(np.asarray(dirty, np.float64) * s)
-    h = fo.hartley2(s * (cs - dirty))
+    if kern is None:
+        e = 0.5 * np.sum(s * cs) - np.sum(np.asarray(dirty, np.float64) * s)
+        h = fo.hartley2(s * (cs - dirty))
+    else:
+        r = np.asarray(dirty, np.float64) - cs
+        u = fo.ninv_apply(kern, r)
+        e = 0.5 * np.sum(r * u)
+        h = -fo.hartley2(s * fo.psf_apply(w_half_c, u))
     g_xi = a * h
     g_th = amplitude_vjp(theta, xi * h, hyper, ny, nx)
     if with_prior:
@@ -191,15 +198,19 @@ def energy_grad_joint(w_half_c, dirty, hyper, xi, theta, with_prior=True):
     return float(e), g_xi, g_th
 
 
-def metric_apply_joint(w_half_c, hyper, xi, theta, dxi, dtheta, with_prior=True):
-    """Fisher metric J^T C J (+ 1) of the joint model applied to (dxi, dtheta); J = ds/d(xi, theta)."""
+def metric_apply_joint(w_half_c, hyper, xi, theta, dxi, dtheta, with_prior=True, kern=None):
+    """Fisher metric J^T C J (+ 1) of the joint model applied to (dxi, dtheta); J = ds/d(xi, theta).
+    kern given: J^T C N'^-1 C J (+ 1)."""
     fo = _fo()
     xi = np.asarray(xi, np.float64)
     ny, nx = xi.shape
     s, a = sky_joint(None, hyper, xi, theta)
     da = amplitude_jvp(theta, dtheta, hyper, ny, nx)
     dtau = fo.hartley2(a * np.asarray(dxi, np.float64) + da * xi)
-    h = fo.hartley2(s * fo.psf_apply(w_half_c, s * dtau))
+    cj = fo.psf_apply(w_half_c, s * dtau)
+    if kern is not None:
+        cj = fo.psf_apply(w_half_c, fo.ninv_apply(kern, cj))
+    h = fo.hartley2(s * cj)
     o_xi = a * h
     o_th = amplitude_vjp(theta, xi * h, hyper, ny, nx)
     if with_prior:

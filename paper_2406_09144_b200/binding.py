@@ -42,6 +42,13 @@ EXPORTS = {
     "frs_ninv_apply": (_i, [_vp, _vp, _vp]),
     "frs_set_likelihood": (_i, [_vp, _i]),
     "frs_set_cuda_graphs": (_i, [_vp, _i]),
+    "frs_amp_model_size": (_i, [_i, _i, C.POINTER(_i), C.POINTER(_i)]),
+    "frs_set_amplitude_model": (_i, [_vp, C.POINTER(_f)]),
+    "frs_amplitude_forward": (_i, [_vp, _vp, _vp]),
+    "frs_amplitude_jvp": (_i, [_vp, _vp, _vp]),
+    "frs_amplitude_vjp": (_i, [_vp, _vp, _vp]),
+    "frs_energy_grad_joint": (_i, [_vp, _vp, _vp, _i, C.POINTER(_d), _vp, _vp]),
+    "frs_metric_apply_joint": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
     "frs_draw_sample": (_i, [_vp, _vp, _vp, _i, _f, _vp, C.POINTER(_i)]),
     "frs_kl_energy_grad": (_i, [_vp, _vp, _vp, _i, _i, _vp, C.POINTER(_d), _vp]),
     "frs_kl_metric_apply": (_i, [_vp, _vp, _vp, _i, _i, _vp, _vp]),
@@ -252,6 +259,36 @@ class Context:
 
     def set_likelihood(self, mode):
         self._ck(lib().frs_set_likelihood(self._h, int(mode)))
+
+    # ---- learned amplitude spectrum (NEXT-3, reading R17)
+    def set_amplitude_model(self, hyper):
+        h = (_f * 11)(*[float(x) for x in hyper])
+        self._ck(lib().frs_set_amplitude_model(self._h, h))
+        nb, nt = _i(0), _i(0)
+        self._ck(lib().frs_amp_model_size(self.ny, self.nx, C.byref(nb), C.byref(nt)))
+        self.nfield, self.nb, self.ntheta = 1, nb.value, nt.value
+
+    def amplitude_forward(self, theta, amp_out=None):
+        self._ck(lib().frs_amplitude_forward(self._h, _ptr(theta, self.f32, self.ntheta, "theta"),
+                                             _ptr(amp_out, self.f32, self.npix, "amp_out")))
+
+    def amplitude_jvp(self, dtheta, d_amp):
+        self._ck(lib().frs_amplitude_jvp(self._h, _ptr(dtheta, self.f32, self.ntheta, "dtheta"), _ptr(d_amp, self.f32, self.npix, "d_amp")))
+
+    def amplitude_vjp(self, g_amp, g_theta):
+        self._ck(lib().frs_amplitude_vjp(self._h, _ptr(g_amp, self.f32, self.npix, "g_amp"), _ptr(g_theta, self.f32, self.ntheta, "g_theta")))
+
+    def energy_grad_joint(self, xi, theta, grad_xi, grad_theta, with_prior=True):
+        e = _d(0.0)
+        self._ck(lib().frs_energy_grad_joint(self._h, _ptr(xi, self.f32, self.npix, "xi"), _ptr(theta, self.f32, self.ntheta, "theta"),
+                                             int(with_prior), C.byref(e), _ptr(grad_xi, self.f32, self.npix, "grad_xi"),
+                                             _ptr(grad_theta, self.f32, self.ntheta, "grad_theta")))
+        return e.value
+
+    def metric_apply_joint(self, dxi, dtheta, out_xi, out_theta, with_prior=True):
+        self._ck(lib().frs_metric_apply_joint(self._h, _ptr(dxi, self.f32, self.npix, "dxi"), _ptr(dtheta, self.f32, self.ntheta, "dtheta"),
+                                              int(with_prior), _ptr(out_xi, self.f32, self.npix, "out_xi"),
+                                              _ptr(out_theta, self.f32, self.ntheta, "out_theta")))
 
     def set_cuda_graphs(self, on):
         self._ck(lib().frs_set_cuda_graphs(self._h, int(bool(on))))

@@ -11,6 +11,7 @@
 #include "../../include/frs.h"
 #include "ew_kernels.cuh"
 #include "launch.h"
+#include "prior.h"
 #include "response.h"
 #include "setup.h"
 #include "tables.h"
@@ -59,6 +60,10 @@ struct frs_ctx {
     cudaStream_t cap_stream = nullptr;  // capture runs on a stream of the ctx's own (the caller's may be the legacy default stream)
     long long cg_graph_launches = 0;   // kernels per replay
     int use_graphs = 1;
+    // NEXT-3: learned amplitude spectrum (prior.h).  plain_latent: the joint calls run the latent-space passes without
+    // the fused (.A, + v) prologue / epilogue and apply their own
+    AmpModel am;
+    bool have_amp_model = false, plain_latent = false;
     bool profiling = false;
     std::vector<ProfRec> prof;
     char err[512] = "no error";
@@ -323,7 +328,7 @@ int metric_apply9_impl(frs_ctx* ctx, const float* v, int with_prior, float* out,
     const Orient o = orient(ctx, true);
     RET(need_s_transposed(ctx));
     RET(ensure_scratch9(ctx));
-    RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
+    RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->plain_latent ? nullptr : ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
     const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
     if (simple) {
         RET(conv_rows_fwd(ctx, o, ctx->lin, ctx->sT));
@@ -346,8 +351,9 @@ int metric_apply9_impl(frs_ctx* ctx, const float* v, int with_prior, float* out,
                                                                                ctx->nfield, ctx->nchan);
         ctx->launches++;
     }
-    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield,
-                  with_prior ? d_vmv : nullptr));
+    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->plain_latent ? nullptr : ctx->amp,
+                  (with_prior && !ctx->plain_latent) ? v : nullptr, nullptr, ctx->nfield,
+                  (with_prior && !ctx->plain_latent) ? d_vmv : nullptr));
     CK(cudaGetLastError());
     return FRS_OK;
 }
@@ -358,7 +364,7 @@ int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, 
     const Orient o = orient(ctx, true);
     RET(need_s_transposed(ctx));
     // lin_f = H[A_f v_f]   (transposed)
-    RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
+    RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->plain_latent ? nullptr : ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
     const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
     if (simple) {
         RET(conv_rows_fwd(ctx, o, ctx->lin, ctx->sT));             // s . lin fused into the row pass
@@ -378,8 +384,9 @@ int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, 
         ctx->launches++;
     }
     // out_f = A_f . H[acc_f] (+ v_f)   (transposes back to the latent layout)
-    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->amp, with_prior ? v : nullptr, nullptr, ctx->nfield,
-                  with_prior ? d_vmv : nullptr));
+    RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, out, ctx->plain_latent ? nullptr : ctx->amp,
+                  (with_prior && !ctx->plain_latent) ? v : nullptr, nullptr, ctx->nfield,
+                  (with_prior && !ctx->plain_latent) ? d_vmv : nullptr));
     CK(cudaGetLastError());
     return FRS_OK;
 }
@@ -488,6 +495,11 @@ void frs_destroy(frs_ctx* ctx) {
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     if (ctx->cg_exec) cudaGraphExecDestroy(ctx->cg_exec);
+    {
+        AmpModel& m = ctx->am;
+        void* mp[] = {m.pindex, m.mult, m.d_hyper, m.theta, m.ab, m.wn, m.abf, m.dabf, m.gbin, m.work, m.sc, m.xi};
+        for (void* q : mp) if (q) cudaFree(q);
+    }
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     delete ctx;
 }
@@ -602,6 +614,7 @@ int frs_set_amplitude(frs_ctx* ctx, int nfield, const float* amp, const float* m
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->nfield = nfield;
     ctx->have_amp = true;
+    ctx->have_amp_model = false;          // a fixed amplitude array replaces the learned spectrum
     ctx->have_s = ctx->s_ok = ctx->sT_ok = false;
     return FRS_OK;
 }
@@ -695,8 +708,8 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
                                                                                    ctx->nfield, ctx->nchan);
             ctx->launches++;
         }
-        RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, grad, ctx->amp, with_prior ? xi : nullptr, nullptr, ctx->nfield,
-                      nullptr, -1.0f));
+        RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, grad, ctx->plain_latent ? nullptr : ctx->amp,
+                      (with_prior && !ctx->plain_latent) ? xi : nullptr, nullptr, ctx->nfield, nullptr, -1.0f));
         CK(cudaGetLastError());
         if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
         if (h_energy) {
@@ -723,7 +736,8 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
         ctx->launches++;
         accp = ctx->acc;
     }
-    RET(hartley_t(ctx, accp, ctx->nx, ctx->ny, nullptr, grad, ctx->amp, with_prior ? xi : nullptr, nullptr, ctx->nfield));
+    RET(hartley_t(ctx, accp, ctx->nx, ctx->ny, nullptr, grad, ctx->plain_latent ? nullptr : ctx->amp,
+                  (with_prior && !ctx->plain_latent) ? xi : nullptr, nullptr, ctx->nfield));
     CK(cudaGetLastError());
     if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     if (h_energy) {
@@ -890,6 +904,152 @@ static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, f
     if (h_iters) *h_iters = (int)sc[kIters];
     if (h_resnorm) *h_resnorm = sqrt(sc[kRR]);
     if (sc[kBreak] != 0.0) return fail(ctx, FRS_EBREAKDOWN, "CG breakdown: <p, M p> <= 0");
+    return FRS_OK;
+}
+
+static int latent_scratch(frs_ctx* ctx);
+// ---- NEXT-3: learned amplitude spectrum and the joint latent vector (xi, theta)  (Table A.1; reading R17) ----
+int frs_amp_model_size(int ny, int nx, int* nb, int* ntheta) {
+    if (!pow2_in(ny, 32, 4096) || !pow2_in(nx, 32, 4096) || (!nb && !ntheta)) return FRS_EINVAL;
+    const int n = amp_num_bins(ny, nx);
+    if (nb) *nb = n;
+    if (ntheta) *ntheta = kAmpScalars + 2 * (n - 2);
+    return FRS_OK;
+}
+
+int frs_set_amplitude_model(frs_ctx* ctx, const float* hyper_host) {
+    if (!ctx || !hyper_host) return fail(ctx, FRS_EINVAL, "frs_set_amplitude_model: bad argument");
+    if (ctx->nchan != 1) return fail(ctx, FRS_ESTATE, "frs_set_amplitude_model: single-channel contexts only");
+    // means of the log-normal parameters must be positive, every standard deviation non-negative
+    for (int i = 1; i < kAmpHyper; i += 2)
+        if (i != 5 && !(hyper_host[i] > 0.f)) return fail(ctx, FRS_EINVAL, "frs_set_amplitude_model: log-normal mean <= 0");
+    for (int i = 2; i < kAmpHyper; i += 2)
+        if (!(hyper_host[i] >= 0.f)) return fail(ctx, FRS_EINVAL, "frs_set_amplitude_model: negative standard deviation");
+    CK(cudaSetDevice(ctx->device));
+    AmpModel& m = ctx->am;
+    if (!m.pindex) {
+        m.ny = ctx->ny; m.nx = ctx->nx; m.nb = amp_num_bins(ctx->ny, ctx->nx);
+        if (m.nb > kAmpMaxBins || m.nb < 4) return fail(ctx, FRS_EINVAL, "frs_set_amplitude_model: unsupported grid");
+        RET(dev_alloc(ctx, &m.pindex, ctx->npix));
+        RET(dev_alloc(ctx, &m.mult, (size_t)m.nb));
+        RET(dev_alloc(ctx, &m.d_hyper, (size_t)kAmpHyper));
+        RET(dev_alloc(ctx, &m.theta, (size_t)m.ntheta()));
+        RET(dev_alloc(ctx, &m.ab, (size_t)m.nb));
+        RET(dev_alloc(ctx, &m.wn, (size_t)m.nb));
+        RET(dev_alloc(ctx, &m.abf, (size_t)m.nb));
+        RET(dev_alloc(ctx, &m.dabf, (size_t)m.nb));
+        RET(dev_alloc(ctx, &m.gbin, (size_t)m.nb));
+        RET(dev_alloc(ctx, &m.work, (size_t)4 * m.nb));
+        RET(dev_alloc(ctx, &m.sc, (size_t)8));
+        RET(dev_alloc(ctx, &m.xi, ctx->npix));
+        CKL(launch_amp_bins(ctx->stream, m));
+        ctx->launches += 2;
+    }
+    for (int i = 0; i < kAmpHyper; ++i) m.hyper[i] = (double)hyper_host[i];
+    CK(cudaMemcpyAsync(m.d_hyper, m.hyper, sizeof(m.hyper), cudaMemcpyHostToDevice, ctx->stream));
+    RET(dev_alloc(ctx, &ctx->amp, 2 * ctx->npix));
+    const float mu[2] = {hyper_host[0], 0.f};
+    CK(cudaMemcpyAsync(ctx->d_mu, mu, sizeof(mu), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->nfield = 1;
+    ctx->have_amp_model = true;
+    m.have_theta = m.have_xi = false;
+    ctx->have_amp = false;
+    ctx->have_s = ctx->s_ok = ctx->sT_ok = false;
+    return FRS_OK;
+}
+
+static int amp_forward_impl(frs_ctx* ctx, const float* theta) {
+    AmpModel& m = ctx->am;
+    if (theta != m.theta) CK(cudaMemcpyAsync(m.theta, theta, (size_t)m.ntheta() * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    CKL(launch_amp_forward(ctx->stream, m));
+    CKL(launch_amp_gather(ctx->stream, m, m.abf, ctx->amp));
+    ctx->launches += 2;
+    m.have_theta = true;
+    ctx->have_amp = true;
+    ctx->have_s = ctx->s_ok = ctx->sT_ok = false;        // the cached sky belongs to the previous amplitude
+    m.have_xi = false;
+    return FRS_OK;
+}
+
+int frs_amplitude_forward(frs_ctx* ctx, const float* theta, float* amp_out) {
+    if (!ctx || !theta || (amp_out && !aligned16(amp_out))) return fail(ctx, FRS_EINVAL, "frs_amplitude_forward: bad argument");
+    if (!ctx->have_amp_model) return fail(ctx, FRS_ESTATE, "amplitude model not set (frs_set_amplitude_model)");
+    CK(cudaSetDevice(ctx->device));
+    RET(amp_forward_impl(ctx, theta));
+    if (amp_out) CK(cudaMemcpyAsync(amp_out, ctx->amp, ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    return FRS_OK;
+}
+
+int frs_amplitude_jvp(frs_ctx* ctx, const float* dtheta, float* d_amp) {
+    if (!ctx || !dtheta || !d_amp || !aligned16(d_amp)) return fail(ctx, FRS_EINVAL, "frs_amplitude_jvp: bad argument");
+    if (!ctx->have_amp_model || !ctx->am.have_theta) return fail(ctx, FRS_ESTATE, "no amplitude position (frs_amplitude_forward)");
+    CK(cudaSetDevice(ctx->device));
+    CKL(launch_amp_tangent(ctx->stream, ctx->am, dtheta));
+    CKL(launch_amp_gather(ctx->stream, ctx->am, ctx->am.dabf, d_amp));
+    ctx->launches += 2;
+    return FRS_OK;
+}
+
+int frs_amplitude_vjp(frs_ctx* ctx, const float* g_amp, float* g_theta) {
+    if (!ctx || !g_amp || !g_theta || !aligned16(g_amp)) return fail(ctx, FRS_EINVAL, "frs_amplitude_vjp: bad argument");
+    if (!ctx->have_amp_model || !ctx->am.have_theta) return fail(ctx, FRS_ESTATE, "no amplitude position (frs_amplitude_forward)");
+    CK(cudaSetDevice(ctx->device));
+    CKL(launch_amp_bin_reduce(ctx->stream, ctx->am, g_amp));
+    CKL(launch_amp_adjoint(ctx->stream, ctx->am, nullptr, g_theta, nullptr));
+    ctx->launches += 2;
+    return FRS_OK;
+}
+
+int frs_energy_grad_joint(frs_ctx* ctx, const float* xi, const float* theta, int with_prior, double* h_energy, float* grad_xi,
+                          float* grad_theta) {
+    if (!ctx || !xi || !theta || !grad_xi || !grad_theta || !aligned16(xi) || !aligned16(grad_xi) || xi == grad_xi)
+        return fail(ctx, FRS_EINVAL, "frs_energy_grad_joint: bad argument");
+    if (!ctx->have_amp_model) return fail(ctx, FRS_ESTATE, "amplitude model not set (frs_set_amplitude_model)");
+    CK(cudaSetDevice(ctx->device));
+    RET(amp_forward_impl(ctx, theta));
+    RET(check_hot(ctx, false, true));
+    if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
+    RET(latent_scratch(ctx));
+    AmpModel& m = ctx->am;
+    CK(cudaMemcpyAsync(m.xi, xi, ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    m.have_xi = true;
+    // h = H[s (C s - j)] (mode 0) or -H[s C N'^-1 r] (mode 1): the latent-space passes without their fused . A + xi
+    ctx->plain_latent = true;
+    const int rc = energy_grad_impl(ctx, xi, with_prior, nullptr, nullptr, ctx->lat1);
+    ctx->plain_latent = false;
+    RET(rc);
+    // grad_xi = A . h (+ xi);  G_b = bin sums of xi . h;  grad_theta = (dA/dtheta)^T G (+ theta);  E += 1/2 <theta, theta>
+    CKL(launch_joint_epilogue(ctx->stream, m, ctx->lat1, xi, with_prior ? xi : nullptr, grad_xi));
+    CKL(launch_amp_adjoint(ctx->stream, m, with_prior ? m.theta : nullptr, grad_theta, with_prior ? ctx->scal + 11 : nullptr));
+    ctx->launches += 2;
+    if (h_energy) {
+        CK(cudaMemcpyAsync(h_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    return FRS_OK;
+}
+
+int frs_metric_apply_joint(frs_ctx* ctx, const float* dxi, const float* dtheta, int with_prior, float* out_xi, float* out_theta) {
+    if (!ctx || !dxi || !dtheta || !out_xi || !out_theta || !aligned16(dxi) || !aligned16(out_xi) || dxi == out_xi)
+        return fail(ctx, FRS_EINVAL, "frs_metric_apply_joint: bad argument");
+    if (!ctx->have_amp_model || !ctx->am.have_theta || !ctx->am.have_xi)
+        return fail(ctx, FRS_ESTATE, "no joint position (frs_energy_grad_joint)");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, true));
+    RET(latent_scratch(ctx));
+    AmpModel& m = ctx->am;
+    // u = A . dxi + dA(dtheta) . xi;  h = H[s C s H[u]] (mode 0; mode 1 with N'^-1 in the middle)
+    CKL(launch_amp_tangent(ctx->stream, m, dtheta));
+    CKL(launch_joint_prologue(ctx->stream, m, dxi, m.xi, ctx->lat1));
+    ctx->launches += 2;
+    ctx->plain_latent = true;
+    const int rc = metric_apply_impl(ctx, ctx->lat1, with_prior, ctx->lat2);
+    ctx->plain_latent = false;
+    RET(rc);
+    CKL(launch_joint_epilogue(ctx->stream, m, ctx->lat2, m.xi, with_prior ? dxi : nullptr, out_xi));
+    CKL(launch_amp_adjoint(ctx->stream, m, with_prior ? dtheta : nullptr, out_theta, nullptr));
+    ctx->launches += 2;
     return FRS_OK;
 }
 

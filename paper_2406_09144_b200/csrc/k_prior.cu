@@ -1,0 +1,374 @@
+// k_prior.cu -- learned amplitude spectrum (NEXT-3, Table A.1; reading R17).
+//
+// Two kinds of kernels.  The spectrum itself lives on nb = O(N) radial bins: its walk, normalisation, tangent and
+// adjoint are prefix sums of a few thousand doubles, done by ONE CTA in fp64 with a fixed association order
+// (chunk per thread, shuffle scan over the thread totals).  The image-sized work is a gather A[pixel] = A_b[bin] and its
+// adjoint, a reduction of an image onto the bins (shared-memory histogram of doubles, flushed with fp64 atomics: the
+// result depends on the order of arrival only in the last bits of a double).
+#include <cmath>
+#include "prior.h"
+
+namespace frs {
+
+namespace {
+constexpr int kScanThreads = 1024;
+
+__host__ __device__ inline int fold_freq(int k, int n) { return k < n - k ? k : n - k; }
+
+// b = rint(sqrt(fy^2 + fx^2)), frequencies in cycles per LONGER side; the decision is taken in fp64 on an exact
+// integer argument (the oracle does the same), so host, device and oracle agree bit for bit
+__host__ __device__ inline int bin_of(int ky, int kx, int ny, int nx) {
+    const int nmax = ny > nx ? ny : nx;
+    const long long fy = (long long)fold_freq(ky, ny) * (nmax / ny), fx = (long long)fold_freq(kx, nx) * (nmax / nx);
+    return (int)rint(sqrt((double)(fy * fy + fx * fx)));
+}
+
+__global__ void amp_bins_kernel(unsigned short* __restrict__ pindex, unsigned int* __restrict__ count, int ny, int nx) {
+    const size_t n = (size_t)ny * nx;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int b = bin_of((int)(i / nx), (int)(i % nx), ny, nx);
+        pindex[i] = (unsigned short)b;
+        atomicAdd(count + b, 1u);                     // integer: exact and order-independent
+    }
+}
+__global__ void amp_mult_kernel(const unsigned int* __restrict__ count, double* __restrict__ mult, int nb) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < nb) mult[b] = (double)count[b];
+}
+
+// inclusive prefix sums of v[0..n) in place, one CTA of kScanThreads; returns the total to every thread
+__device__ double block_scan(double* v, int n, double* wtot) {
+    const int chunk = (n + kScanThreads - 1) / kScanThreads;
+    const int i0 = threadIdx.x * chunk, i1 = min(n, i0 + chunk);
+    double s = 0.0;
+    for (int i = i0; i < i1; ++i) { s += v[i]; v[i] = s; }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double x = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    __syncthreads();                                  // wtot may still be read by a previous scan
+    if (lane == 31) wtot[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+        double w = wtot[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double y = __shfl_up_sync(0xffffffffu, w, o);
+            if (lane >= o) w += y;
+        }
+        wtot[lane] = w;
+    }
+    __syncthreads();
+    const double off = x - s + (warp > 0 ? wtot[warp - 1] : 0.0);
+    for (int i = i0; i < i1; ++i) v[i] += off;
+    const double total = wtot[31];
+    __syncthreads();
+    return total;
+}
+
+struct Scalars { double fluct, slope, flex, asp, zm, sig_f, sig_x, sig_a, sig_z, sl_s; };
+__device__ inline double ln_sigma(double m, double s) { return sqrt(log(1.0 + (s / m) * (s / m))); }
+__device__ inline double lognormal(double xi, double m, double s) {
+    const double r = 1.0 + (s / m) * (s / m);
+    return m / sqrt(r) * exp(sqrt(log(r)) * xi);
+}
+// hyper: offset, zm mean/std, fluct mean/std, slope mean/std, flex mean/std, asp mean/std
+__device__ inline Scalars scalars_of(const float* __restrict__ th, const double* __restrict__ hy) {
+    Scalars s;
+    s.fluct = lognormal(th[0], hy[3], hy[4]);
+    s.slope = hy[5] + hy[6] * th[1];
+    s.flex = lognormal(th[2], hy[7], hy[8]);
+    s.asp = lognormal(th[3], hy[9], hy[10]);
+    s.zm = lognormal(th[4], hy[1], hy[2]);
+    s.sig_f = ln_sigma(hy[3], hy[4]); s.sig_x = ln_sigma(hy[7], hy[8]); s.sig_a = ln_sigma(hy[9], hy[10]);
+    s.sig_z = ln_sigma(hy[1], hy[2]); s.sl_s = hy[6];
+    return s;
+}
+__device__ inline double tlog(int b) { return b >= 1 ? log((double)b) : 0.0; }
+__device__ inline double dstep(int j) { return log((double)(j + 1)) - log((double)j); }      // D_j = t_{j+1} - t_j
+
+// theta -> A_b, wn_b = mult_b a_b^2 / S, scalars.  work: [2 nb] doubles.
+__global__ void __launch_bounds__(kScanThreads) amp_forward_kernel(const float* __restrict__ th, const double* __restrict__ hy,
+                                                                    const double* __restrict__ mult, int nb, double* __restrict__ work,
+                                                                    double* __restrict__ ab, double* __restrict__ wn,
+                                                                    float* __restrict__ abf, double* __restrict__ sc) {
+    __shared__ double wtot[32];
+    const Scalars s = scalars_of(th, hy);
+    const float* zeta = th + kAmpScalars;
+    const float* eta = zeta + (nb - 2);
+    double* w0 = work;
+    double* w1 = work + nb;
+    // vel_b = sum_{j < b} flex sqrt(D_j) zeta_j
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) w0[b] = (b >= 1 && b <= nb - 2) ? s.flex * sqrt(dstep(b)) * (double)zeta[b - 1] : 0.0;
+    __syncthreads();
+    block_scan(w0, nb, wtot);
+    // dev_b = sum_{j < b} (vel_j D_j + flex asp sqrt(D_j) eta_j),  vel_j = w0[j - 1]
+    for (int b = threadIdx.x; b < nb; b += kScanThreads)
+        w1[b] = (b >= 1 && b <= nb - 2) ? w0[b - 1] * dstep(b) + s.flex * s.asp * sqrt(dstep(b)) * (double)eta[b - 1] : 0.0;
+    __syncthreads();
+    block_scan(w1, nb, wtot);
+    // a_b = exp((slope t_b + dev_b) / 2), dev_b = w1[b - 1];  S = sum mult_b a_b^2
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) {
+        const double a = b >= 1 ? exp(0.5 * (s.slope * tlog(b) + w1[b - 1])) : 0.0;
+        ab[b] = a;
+        w0[b] = mult[b] * a * a;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) wn[b] = w0[b];
+    __syncthreads();
+    const double S = block_scan(w0, nb, wtot);
+    const double rs = 1.0 / sqrt(S);
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) {
+        const double a = b >= 1 ? s.fluct * ab[b] * rs : s.zm;
+        ab[b] = a;
+        abf[b] = (float)a;
+        wn[b] = b >= 1 ? wn[b] / S : 0.0;
+    }
+    if (threadIdx.x == 0) { sc[0] = s.fluct; sc[1] = s.slope; sc[2] = s.flex; sc[3] = s.asp; sc[4] = s.zm; sc[5] = S; }
+}
+
+// dA_b for dtheta at the stored theta:  dA_b = A_b (dfluct/fluct + dlnP_b / 2 - sum_b' wn_b' dlnP_b' / 2),  dA_0 = dzm
+__global__ void __launch_bounds__(kScanThreads) amp_tangent_kernel(const float* __restrict__ th, const float* __restrict__ dth,
+                                                                    const double* __restrict__ hy, int nb, double* __restrict__ work,
+                                                                    const double* __restrict__ ab, const double* __restrict__ wn,
+                                                                    float* __restrict__ dabf) {
+    __shared__ double wtot[32];
+    const Scalars s = scalars_of(th, hy);
+    const float *zeta = th + kAmpScalars, *eta = zeta + (nb - 2), *dzeta = dth + kAmpScalars, *deta = dzeta + (nb - 2);
+    const double dlnf = s.sig_f * dth[0], dsl = s.sl_s * dth[1], dfx = s.flex * s.sig_x * dth[2], das = s.asp * s.sig_a * dth[3],
+                 dzm = s.zm * s.sig_z * dth[4];
+    double *w0 = work, *w1 = work + nb, *w2 = work + 2 * nb;
+    for (int b = threadIdx.x; b < nb; b += kScanThreads)
+        w0[b] = (b >= 1 && b <= nb - 2) ? sqrt(dstep(b)) * (dfx * (double)zeta[b - 1] + s.flex * (double)dzeta[b - 1]) : 0.0;
+    __syncthreads();
+    block_scan(w0, nb, wtot);
+    for (int b = threadIdx.x; b < nb; b += kScanThreads)
+        w1[b] = (b >= 1 && b <= nb - 2)
+                    ? w0[b - 1] * dstep(b) + sqrt(dstep(b)) * ((dfx * s.asp + s.flex * das) * (double)eta[b - 1] + s.flex * s.asp * (double)deta[b - 1])
+                    : 0.0;
+    __syncthreads();
+    block_scan(w1, nb, wtot);
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) {
+        const double dl = b >= 1 ? dsl * tlog(b) + w1[b - 1] : 0.0;
+        w2[b] = dl;
+        w0[b] = wn[b] * dl;
+    }
+    __syncthreads();
+    const double r = block_scan(w0, nb, wtot);
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) dabf[b] = (float)(b >= 1 ? ab[b] * (dlnf + 0.5 * w2[b] - 0.5 * r) : dzm);
+}
+
+// g_theta = (dA/dtheta)^T G (+ theta_add), G = bin sums of the adjoint image.  work: [4 nb] doubles.
+__global__ void __launch_bounds__(kScanThreads) amp_adjoint_kernel(const float* __restrict__ th, const double* __restrict__ hy, int nb,
+                                                                    double* __restrict__ work, const double* __restrict__ ab,
+                                                                    const double* __restrict__ wn, const double* __restrict__ gbin,
+                                                                    const float* __restrict__ theta_add, float* __restrict__ gth,
+                                                                    double* __restrict__ energy_acc) {
+    __shared__ double wtot[32];
+    const Scalars s = scalars_of(th, hy);
+    const float *zeta = th + kAmpScalars, *eta = zeta + (nb - 2);
+    double *w0 = work, *w1 = work + nb, *w2 = work + 2 * nb, *w3 = work + 3 * nb;
+    if (energy_acc && theta_add) {                    // + 1/2 <theta, theta> of the prior on theta (2 nb + 1 <= 4 nb values)
+        const int nt = kAmpScalars + 2 * (nb - 2);
+        for (int i = threadIdx.x; i < nt; i += kScanThreads) w0[i] = (double)theta_add[i] * (double)theta_add[i];
+        __syncthreads();
+        const double tt = block_scan(w0, nt, wtot);
+        if (threadIdx.x == 0) energy_acc[0] += 0.5 * tt;
+        __syncthreads();
+    }
+    // Q = sum_b>=1 A_b G_b
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) { w1[b] = b >= 1 ? ab[b] * gbin[b] : 0.0; w0[b] = w1[b]; }
+    __syncthreads();
+    const double Q = block_scan(w0, nb, wtot);
+    // lbar_b = q_b / 2 - Q wn_b / 2 (adjoint of ln P_b);  slope:  sum lbar_b t_b
+    for (int b = threadIdx.x; b < nb; b += kScanThreads) {
+        const double lb = 0.5 * w1[b] - 0.5 * Q * wn[b];
+        w1[b] = lb;
+        w0[b] = lb * tlog(b);
+        w2[nb - 1 - b] = lb;                          // reversed: suffix sums D_b = sum_{b' >= b} lbar_b'
+    }
+    __syncthreads();
+    const double slbar = block_scan(w0, nb, wtot);
+    block_scan(w2, nb, wtot);                         // D_b = w2[nb - 1 - b]
+    // V_b = sum_{j >= b} D_j D_{j+1}-weighted steps:  c_j = D_j(step) * Dbar_{j+1}, j = 1 .. nb-2  (reversed again)
+    for (int b = threadIdx.x; b < nb; b += kScanThreads)
+        w3[nb - 1 - b] = (b >= 1 && b <= nb - 2) ? dstep(b) * w2[nb - 1 - (b + 1)] : 0.0;
+    __syncthreads();
+    block_scan(w3, nb, wtot);                         // V_b = w3[nb - 1 - b]
+    // eta_j, zeta_j and the two sums for flex and asp
+    for (int j = threadIdx.x; j < nb; j += kScanThreads) {
+        double fxb = 0.0, asb = 0.0;
+        if (j >= 1 && j <= nb - 2) {
+            const double sq = sqrt(dstep(j)), dn = w2[nb - 1 - (j + 1)], vn = w3[nb - 1 - (j + 1)];
+            const double gz = s.flex * sq * vn, ge = s.flex * s.asp * sq * dn;
+            gth[kAmpScalars + (j - 1)] = (float)(gz + (theta_add ? (double)theta_add[kAmpScalars + (j - 1)] : 0.0));
+            gth[kAmpScalars + (nb - 2) + (j - 1)] = (float)(ge + (theta_add ? (double)theta_add[kAmpScalars + (nb - 2) + (j - 1)] : 0.0));
+            fxb = sq * (s.asp * (double)eta[j - 1] * dn + (double)zeta[j - 1] * vn);
+            asb = sq * s.flex * (double)eta[j - 1] * dn;
+        }
+        w0[j] = fxb;
+        w1[j] = asb;
+    }
+    __syncthreads();
+    const double fxbar = block_scan(w0, nb, wtot);
+    const double asbar = block_scan(w1, nb, wtot);
+    if (threadIdx.x == 0) {
+        const double g[kAmpScalars] = {s.sig_f * Q, s.sl_s * slbar, s.flex * s.sig_x * fxbar, s.asp * s.sig_a * asbar,
+                                       s.zm * s.sig_z * gbin[0]};
+        for (int i = 0; i < kAmpScalars; ++i) gth[i] = (float)(g[i] + (theta_add ? (double)theta_add[i] : 0.0));
+    }
+}
+
+// ---- image-sized passes ---------------------------------------------------------------------------------------------
+constexpr int kImgThreads = 256;
+constexpr int kStrip = 8;             // consecutive modes per thread: neighbours along kx mostly share a bin
+
+__global__ void __launch_bounds__(kImgThreads) amp_gather_kernel(const unsigned short* __restrict__ pindex, const float* __restrict__ table,
+                                                                  float* __restrict__ out, size_t n) {
+    const size_t n8 = n / kStrip;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
+        const uint4 pb = reinterpret_cast<const uint4*>(pindex)[i];
+        const unsigned w[4] = {pb.x, pb.y, pb.z, pb.w};
+        float o[kStrip];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { o[2 * k] = __ldg(table + (w[k] & 0xffffu)); o[2 * k + 1] = __ldg(table + (w[k] >> 16)); }
+        reinterpret_cast<float4*>(out)[2 * i] = make_float4(o[0], o[1], o[2], o[3]);
+        reinterpret_cast<float4*>(out)[2 * i + 1] = make_float4(o[4], o[5], o[6], o[7]);
+    }
+}
+
+// u = A . dxi + dA . xi
+__global__ void __launch_bounds__(kImgThreads) joint_prologue_kernel(const unsigned short* __restrict__ pindex, const float* __restrict__ abf,
+                                                                      const float* __restrict__ dabf, const float* __restrict__ dxi,
+                                                                      const float* __restrict__ xi, float* __restrict__ u, size_t n) {
+    const size_t n8 = n / kStrip;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
+        const uint4 pb = reinterpret_cast<const uint4*>(pindex)[i];
+        const unsigned w[4] = {pb.x, pb.y, pb.z, pb.w};
+        const float4 d0 = reinterpret_cast<const float4*>(dxi)[2 * i], d1 = reinterpret_cast<const float4*>(dxi)[2 * i + 1];
+        const float4 x0 = reinterpret_cast<const float4*>(xi)[2 * i], x1 = reinterpret_cast<const float4*>(xi)[2 * i + 1];
+        const float d[kStrip] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w}, x[kStrip] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+        float o[kStrip];
+#pragma unroll
+        for (int k = 0; k < kStrip; ++k) {
+            const unsigned b = (k & 1) ? (w[k >> 1] >> 16) : (w[k >> 1] & 0xffffu);
+            o[k] = fmaf(__ldg(abf + b), d[k], __ldg(dabf + b) * x[k]);
+        }
+        reinterpret_cast<float4*>(u)[2 * i] = make_float4(o[0], o[1], o[2], o[3]);
+        reinterpret_cast<float4*>(u)[2 * i + 1] = make_float4(o[4], o[5], o[6], o[7]);
+    }
+}
+
+// bin sums of val = (xi ? xi . h : h) into gbin (fp64), and optionally out = A . h (+ add).
+// Shared-memory histogram of doubles per CTA; a thread merges the run of equal bins inside its strip first.
+__global__ void __launch_bounds__(kImgThreads) bin_reduce_kernel(const unsigned short* __restrict__ pindex, const float* __restrict__ h,
+                                                                  const float* __restrict__ xi, const float* __restrict__ add,
+                                                                  const float* __restrict__ abf, float* __restrict__ out,
+                                                                  double* __restrict__ gbin, int nb, size_t n) {
+    extern __shared__ double hist[];
+    for (int b = threadIdx.x; b < nb; b += kImgThreads) hist[b] = 0.0;
+    __syncthreads();
+    const size_t n8 = n / kStrip;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
+        const uint4 pb = reinterpret_cast<const uint4*>(pindex)[i];
+        const unsigned w[4] = {pb.x, pb.y, pb.z, pb.w};
+        const float4 h0 = reinterpret_cast<const float4*>(h)[2 * i], h1 = reinterpret_cast<const float4*>(h)[2 * i + 1];
+        const float hv[kStrip] = {h0.x, h0.y, h0.z, h0.w, h1.x, h1.y, h1.z, h1.w};
+        float xv[kStrip], av[kStrip];
+        if (xi) {
+            const float4 x0 = reinterpret_cast<const float4*>(xi)[2 * i], x1 = reinterpret_cast<const float4*>(xi)[2 * i + 1];
+            xv[0] = x0.x; xv[1] = x0.y; xv[2] = x0.z; xv[3] = x0.w; xv[4] = x1.x; xv[5] = x1.y; xv[6] = x1.z; xv[7] = x1.w;
+        }
+        if (out && add) {
+            const float4 a0 = reinterpret_cast<const float4*>(add)[2 * i], a1 = reinterpret_cast<const float4*>(add)[2 * i + 1];
+            av[0] = a0.x; av[1] = a0.y; av[2] = a0.z; av[3] = a0.w; av[4] = a1.x; av[5] = a1.y; av[6] = a1.z; av[7] = a1.w;
+        }
+        float o[kStrip];
+        unsigned cur = w[0] & 0xffffu;
+        double acc = 0.0;
+#pragma unroll
+        for (int k = 0; k < kStrip; ++k) {
+            const unsigned b = (k & 1) ? (w[k >> 1] >> 16) : (w[k >> 1] & 0xffffu);
+            if (b != cur) { atomicAdd(hist + cur, acc); acc = 0.0; cur = b; }
+            acc += xi ? (double)xv[k] * (double)hv[k] : (double)hv[k];
+            if (out) o[k] = add ? fmaf(__ldg(abf + b), hv[k], av[k]) : __ldg(abf + b) * hv[k];
+        }
+        atomicAdd(hist + cur, acc);
+        if (out) {
+            reinterpret_cast<float4*>(out)[2 * i] = make_float4(o[0], o[1], o[2], o[3]);
+            reinterpret_cast<float4*>(out)[2 * i + 1] = make_float4(o[4], o[5], o[6], o[7]);
+        }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nb; b += kImgThreads)
+        if (hist[b] != 0.0) atomicAdd(gbin + b, hist[b]);
+}
+
+int img_grid(size_t n) {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const size_t want = (n / kStrip + kImgThreads - 1) / kImgThreads;
+    const size_t cap = (size_t)sms * 8;
+    return (int)(want < cap ? (want ? want : 1) : cap);
+}
+}  // namespace
+
+int amp_num_bins(int ny, int nx) { return bin_of(ny / 2, nx / 2, ny, nx) + 1; }
+
+int launch_amp_bins(cudaStream_t st, const AmpModel& m) {
+    unsigned int* count = nullptr;
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&count), m.nb * sizeof(unsigned int));
+    if (e != cudaSuccess) return (int)e;
+    cudaMemsetAsync(count, 0, m.nb * sizeof(unsigned int), st);
+    const size_t n = (size_t)m.ny * m.nx;
+    amp_bins_kernel<<<img_grid(n * kStrip), kImgThreads, 0, st>>>(m.pindex, count, m.ny, m.nx);
+    amp_mult_kernel<<<(m.nb + 255) / 256, 256, 0, st>>>(count, m.mult, m.nb);
+    e = cudaStreamSynchronize(st);
+    cudaFree(count);
+    return e != cudaSuccess ? (int)e : (int)cudaGetLastError();
+}
+int launch_amp_forward(cudaStream_t st, const AmpModel& m) {
+    amp_forward_kernel<<<1, kScanThreads, 0, st>>>(m.theta, m.d_hyper, m.mult, m.nb, m.work, m.ab, m.wn, m.abf, m.sc);
+    return (int)cudaGetLastError();
+}
+int launch_amp_tangent(cudaStream_t st, const AmpModel& m, const float* dtheta) {
+    amp_tangent_kernel<<<1, kScanThreads, 0, st>>>(m.theta, dtheta, m.d_hyper, m.nb, m.work, m.ab, m.wn, m.dabf);
+    return (int)cudaGetLastError();
+}
+int launch_amp_adjoint(cudaStream_t st, const AmpModel& m, const float* theta_add, float* g_theta, double* energy_acc) {
+    amp_adjoint_kernel<<<1, kScanThreads, 0, st>>>(m.theta, m.d_hyper, m.nb, m.work, m.ab, m.wn, m.gbin, theta_add, g_theta, energy_acc);
+    return (int)cudaGetLastError();
+}
+int launch_amp_gather(cudaStream_t st, const AmpModel& m, const float* table, float* out) {
+    const size_t n = (size_t)m.ny * m.nx;
+    amp_gather_kernel<<<img_grid(n), kImgThreads, 0, st>>>(m.pindex, table, out, n);
+    return (int)cudaGetLastError();
+}
+static int reduce_launch(cudaStream_t st, const AmpModel& m, const float* h, const float* xi, const float* add, float* out) {
+    const size_t n = (size_t)m.ny * m.nx;
+    const int smem = m.nb * (int)sizeof(double);
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(bin_reduce_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return (int)e;
+    }
+    cudaError_t e = cudaMemsetAsync(m.gbin, 0, m.nb * sizeof(double), st);
+    if (e != cudaSuccess) return (int)e;
+    bin_reduce_kernel<<<img_grid(n), kImgThreads, smem, st>>>(m.pindex, h, xi, add, m.abf, out,
+                                                            m.gbin, m.nb, n);
+    return (int)cudaGetLastError();
+}
+int launch_amp_bin_reduce(cudaStream_t st, const AmpModel& m, const float* img) { return reduce_launch(st, m, img, nullptr, nullptr, nullptr); }
+int launch_joint_prologue(cudaStream_t st, const AmpModel& m, const float* dxi, const float* xi, float* u) {
+    const size_t n = (size_t)m.ny * m.nx;
+    joint_prologue_kernel<<<img_grid(n), kImgThreads, 0, st>>>(m.pindex, m.abf, m.dabf, dxi, xi, u, n);
+    return (int)cudaGetLastError();
+}
+int launch_joint_epilogue(cudaStream_t st, const AmpModel& m, const float* h, const float* xi, const float* add, float* out_xi) {
+    return reduce_launch(st, m, h, xi, add, out_xi);
+}
+
+}  // namespace frs

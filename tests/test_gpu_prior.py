@@ -1,0 +1,160 @@
+"""GPU parity of the learned amplitude spectrum and the joint (xi, theta) model (NEXT-3, reading R17)
+against oracle/prior_oracle.py, through the C ABI.  Tolerances: the spectrum is evaluated in fp64 on the device and
+rounded once (<= 2e-7 relative per value); image-sized results rel-L2 <= 1e-5 as everywhere (north_star)."""
+import numpy as np
+import pytest
+
+from gen import workloads as wl
+from oracle import prior_oracle as po
+
+pytestmark = pytest.mark.gpu
+
+HYPER = (18.0, 1.0, 0.1, 5.0, 1.0, -2.0, 0.2, 1.2, 0.4, 0.2, 0.2)        # Table A.1, S band
+
+
+def rel(a, b):
+    a, b = np.asarray(a, np.float64), np.asarray(b, np.float64)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+@pytest.fixture(scope="module")
+def frs():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2406_09144_b200 as m
+    m.load_library()
+    return m
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def theta_of(nb, seed, scale=0.5):
+    return (scale * np.random.default_rng(seed).normal(size=po.ntheta(nb))).astype(np.float32)
+
+
+@pytest.mark.parametrize("shape", [(32, 32), (64, 128), (512, 512), (256, 1024), (4096, 4096)])
+def test_amplitude_forward_jvp_vjp(frs, shape):
+    import torch
+    ny, nx = shape
+    ctx = frs.Context(ny, nx, 1)
+    ctx.set_amplitude_model(HYPER)
+    b, mult, t = po.bins(ny, nx)
+    assert ctx.nb == len(t) and ctx.ntheta == po.ntheta(len(t))
+    th = theta_of(len(t), 1)
+    amp = torch.empty(1, ny, nx, device="cuda")
+    ctx.amplitude_forward(dev(th), amp)
+    ref = po.amplitude(th.astype(np.float64), HYPER, ny, nx)
+    got = amp.cpu().numpy()[0].astype(np.float64)
+    assert np.max(np.abs(got - ref) / ref) <= 2e-7                 # every mode, relative: one fp32 rounding
+    dth = theta_of(len(t), 2, 1.0)
+    da = torch.empty(1, ny, nx, device="cuda")
+    ctx.amplitude_jvp(dev(dth), da)
+    ref_j = po.amplitude_jvp(th.astype(np.float64), dth.astype(np.float64), HYPER, ny, nx)
+    assert np.max(np.abs(da.cpu().numpy()[0] - ref_j)) <= 3e-7 * np.max(np.abs(ref_j))
+    g = np.random.default_rng(3).normal(size=(ny, nx)).astype(np.float32)
+    gt = torch.empty(ctx.ntheta, device="cuda")
+    ctx.amplitude_vjp(dev(g[None]), gt)
+    ref_v = po.amplitude_vjp(th.astype(np.float64), g.astype(np.float64), HYPER, ny, nx)
+    assert np.max(np.abs(gt.cpu().numpy() - ref_v)) <= 3e-7 * np.max(np.abs(ref_v))
+    # adjointness of what the GPU computes, in fp64 on the host
+    lhs = float((da.double() * dev(g[None]).double()).sum())
+    rhs = float((dev(dth).double() * gt.double()).sum())
+    assert abs(lhs - rhs) <= 1e-5 * abs(lhs)
+
+
+def _problem(n, seed=5, ny=None, nx=None):
+    w = wl.make_config(1, n=n, seed=seed) if ny is None else wl.make_config(3, ny=ny, nx=nx, seed=seed)
+    rng = np.random.default_rng(seed)
+    _, _, t = po.bins(w.ny, w.nx)
+    hyper = (float(np.log(np.median(w.sky_true))), 1.0, 0.1, 1.0, 0.3, -3.0, 0.2, 0.5, 0.2, 0.2, 0.1)
+    xi = (0.3 * rng.normal(size=(w.ny, w.nx))).astype(np.float32)
+    th = (0.3 * rng.normal(size=po.ntheta(len(t)))).astype(np.float32)
+    return w, hyper, xi, th, rng
+
+
+@pytest.mark.parametrize("size", [(128, None, None), (0, 64, 256), (512, None, None)])
+@pytest.mark.parametrize("with_prior", [True, False])
+def test_joint_energy_gradient_and_metric(frs, size, with_prior):
+    import torch
+    w, hyper, xi, th, rng = _problem(size[0], ny=size[1], nx=size[2])
+    ctx = frs.Context(w.ny, w.nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    ctx.set_amplitude_model(hyper)
+    gx = torch.empty(1, w.ny, w.nx, device="cuda")
+    gt = torch.empty(ctx.ntheta, device="cuda")
+    e = ctx.energy_grad_joint(dev(xi[None]), dev(th), gx, gt, with_prior)
+    e_ref, gx_ref, gt_ref = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi, th, with_prior)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
+    assert rel(gx.cpu().numpy()[0], gx_ref) <= 1e-5
+    assert rel(gt.cpu().numpy(), gt_ref) <= 1e-5
+    # the sky of the joint position
+    s = ctx.new_image()
+    ctx.sky_forward(dev(xi[None]), s)
+    assert rel(s.cpu().numpy()[0], po.sky_joint(None, hyper, xi, th)[0]) <= 1e-5
+    dxi = rng.normal(size=xi.shape).astype(np.float32)
+    dth = rng.normal(size=th.shape).astype(np.float32)
+    ox = torch.empty(1, w.ny, w.nx, device="cuda")
+    ot = torch.empty(ctx.ntheta, device="cuda")
+    ctx.energy_grad_joint(dev(xi[None]), dev(th), gx, gt, with_prior)      # position (sky_forward kept it; explicit here)
+    ctx.metric_apply_joint(dev(dxi[None]), dev(dth), ox, ot, with_prior)
+    ox_ref, ot_ref = po.metric_apply_joint(w.w_half[0], hyper, xi, th, dxi, dth, with_prior)
+    assert rel(ox.cpu().numpy()[0], ox_ref) <= 1e-5
+    assert rel(ot.cpu().numpy(), ot_ref) <= 1e-5
+
+
+def test_joint_model_with_the_eq9_likelihood(frs):
+    """Mode 1 (Eq. 9 with the fitted noise kernel, R14) under the joint model: the oracle runs on the GPU's K."""
+    import torch
+    from oracle import frs_oracle as fo
+    w, hyper, xi, th, rng = _problem(128)
+    ctx = frs.Context(w.ny, w.nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    ctx.set_amplitude_model(hyper)
+    ctx.set_noise_kernel(1e-2 * float(fo.psf_from_weights(w.w_half[0])[0, 0]))
+    ctx.set_likelihood(1)
+    kern = ctx.get_noise_kernel().cpu().numpy()[0].astype(np.float64)
+    gx, gt = torch.empty(1, w.ny, w.nx, device="cuda"), torch.empty(ctx.ntheta, device="cuda")
+    e = ctx.energy_grad_joint(dev(xi[None]), dev(th), gx, gt, True)
+    e_ref, gx_ref, gt_ref = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi, th, True, kern)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref) and rel(gx.cpu().numpy()[0], gx_ref) <= 1e-5 and rel(gt.cpu().numpy(), gt_ref) <= 1e-5
+    dxi, dth = rng.normal(size=xi.shape).astype(np.float32), rng.normal(size=th.shape).astype(np.float32)
+    ox, ot = torch.empty_like(gx), torch.empty_like(gt)
+    ctx.metric_apply_joint(dev(dxi[None]), dev(dth), ox, ot, True)
+    ox_ref, ot_ref = po.metric_apply_joint(w.w_half[0], hyper, xi, th, dxi, dth, True, kern)
+    assert rel(ox.cpu().numpy()[0], ox_ref) <= 1e-5 and rel(ot.cpu().numpy(), ot_ref) <= 1e-5
+
+
+def test_joint_model_state_errors_and_switch_back(frs):
+    import torch
+    w, hyper, xi, th, rng = _problem(64)
+    ctx = frs.Context(w.ny, w.nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    gx, gt = torch.empty(1, w.ny, w.nx, device="cuda"), torch.empty(po.ntheta(len(po.bins(64, 64)[2])), device="cuda")
+    ctx.ntheta = gt.numel()
+    with pytest.raises(frs.FrsError):
+        ctx.energy_grad_joint(dev(xi[None]), dev(th), gx, gt)               # no model set
+    ctx.set_amplitude_model(hyper)
+    with pytest.raises(frs.FrsError):
+        ctx.metric_apply_joint(dev(xi[None]), dev(th), gx, gt)              # no joint position yet
+    with pytest.raises(frs.FrsError):
+        ctx.set_amplitude_model((1.0, -1.0) + tuple(hyper[2:]))             # log-normal mean <= 0
+    e = ctx.energy_grad_joint(dev(xi[None]), dev(th), gx, gt)
+    # a fixed amplitude array switches the learned spectrum off again; the fixed-amplitude path at A(theta) agrees
+    amp = torch.empty(1, w.ny, w.nx, device="cuda")
+    ctx.amplitude_forward(dev(th), amp)
+    ctx.set_amplitude(amp, [hyper[0]])
+    g2 = ctx.new_latent()
+    e2 = ctx.energy_grad(dev(xi[None]), g2, with_prior=True)
+    assert abs(e2 + 0.5 * float(np.sum(th.astype(np.float64) ** 2)) - e) <= 1e-6 * abs(e)
+    assert rel(g2.cpu().numpy(), gx.cpu().numpy()) <= 1e-6
+    with pytest.raises(frs.FrsError):
+        ctx.energy_grad_joint(dev(xi[None]), dev(th), gx, gt)
+    multi = frs.Context(64, 64, 2)
+    with pytest.raises(frs.FrsError):
+        multi.set_amplitude_model(hyper)

@@ -139,3 +139,17 @@ def test_tf32_dft_stage_needs_the_three_term_split():
     three = gemm(xh, wh) + gemm(xl, wh) + gemm(xh, wl)
     assert err(one) > 1e-4                                           # ~3e-4: fails the bar on its own
     assert err(three) < 2e-6                                         # the split restores fp32-class accuracy
+
+
+def test_amp_model_size_matches_oracle_bins():
+    """frs_amp_model_size is host arithmetic (no GPU): bins and theta length of the radial grid equal the oracle's."""
+    import ctypes as C
+    from oracle import prior_oracle as po
+    import paper_2406_09144_b200 as frs
+    lib = frs.load_library()
+    for ny, nx in ((32, 32), (64, 256), (512, 128), (1024, 1024)):
+        nb, nt = C.c_int(0), C.c_int(0)
+        assert lib.frs_amp_model_size(ny, nx, C.byref(nb), C.byref(nt)) == 0
+        t = po.bins(ny, nx)[2]
+        assert nb.value == len(t) and nt.value == po.ntheta(len(t))
+    assert lib.frs_amp_model_size(48, 32, C.byref(nb), C.byref(nt)) != 0

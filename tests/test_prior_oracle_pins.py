@@ -144,3 +144,20 @@ def test_joint_metric_symmetric_and_at_least_identity():
     m0 = fo.metric_apply(w.w_half, am[None], [hyper[0]], w.lognu, xi[None], u[0][None], True)
     mj = po.metric_apply_joint(w.w_half[0], hyper, xi, th, u[0], np.zeros_like(th))
     assert np.max(np.abs(m0[0] - mj[0])) <= 1e-10 * np.max(np.abs(m0))
+
+
+def test_joint_eq9_gradient_against_central_differences_and_metric_symmetry():
+    w, hyper, xi, th, rng = _problem()
+    kern = fo.noise_kernel_from_psf(w.w_half[0], 1e-2 * float(fo.psf_from_weights(w.w_half[0])[0, 0]))
+    e, gx, gt = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi, th, True, kern)
+    dx, dt = rng.normal(size=xi.shape), rng.normal(size=th.shape)
+    h = 1e-5
+    ep = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi + h * dx, th + h * dt, True, kern)[0]
+    em = po.energy_grad_joint(w.w_half[0], w.dirty[0], hyper, xi - h * dx, th - h * dt, True, kern)[0]
+    lin = np.sum(gx * dx) + np.sum(gt * dt)
+    assert abs((ep - em) / (2 * h) - lin) <= 1e-6 * max(abs(lin), np.linalg.norm(gx) + np.linalg.norm(gt))
+    u = (rng.normal(size=xi.shape), rng.normal(size=th.shape))
+    mu = po.metric_apply_joint(w.w_half[0], hyper, xi, th, dx, dt, True, kern)
+    mv = po.metric_apply_joint(w.w_half[0], hyper, xi, th, u[0], u[1], True, kern)
+    a, b = np.sum(u[0] * mu[0]) + np.sum(u[1] * mu[1]), np.sum(dx * mv[0]) + np.sum(dt * mv[1])
+    assert abs(a - b) <= 1e-11 * abs(a)
