@@ -217,3 +217,91 @@ def metric_apply_joint(w_half_c, hyper, xi, theta, dxi, dtheta, with_prior=True,
         o_xi = o_xi + dxi
         o_th = o_th + np.asarray(dtheta, np.float64)
     return o_xi, o_th
+
+
+# ----------------------------------------------------------------------------------------------- point sources (R18)
+# P:92 "pixels are independently modeled with an inverse gamma prior for their intensity ... the locations currently
+# need to be manually set"; P:294 two such pixels in the core of Cygnus A.  The paper gives no formula; reading R18:
+# flux_p = F^-1(Phi(xi_p)) with F the CDF of the inverse-gamma distribution pdf(x) ~ x^(-alpha-1) exp(-q / x) and Phi the
+# standard normal CDF (so that xi_p is standard normal), added to the diffuse sky at pixel (y_p, x_p):
+#   s = exp(offset + H[A xi]) + sum_p flux_p e_p.
+# scipy's incomplete-gamma inverses are the library step (pinned in tests by the alpha = 1 closed form and by moments).
+def point_flux(xi_p, alpha, q):
+    from scipy import special
+    xi_p = np.asarray(xi_p, np.float64)
+    # F(x) = Q(alpha, q / x) (regularised upper incomplete gamma).  Solve in the tail that keeps precision:
+    # xi >= 0: P(alpha, y) = Phi(-xi);  xi < 0: Q(alpha, y) = Phi(xi);  flux = q / y
+    lo = special.gammaincinv(alpha, special.ndtr(-np.abs(xi_p)))          # for xi >= 0
+    hi = special.gammainccinv(alpha, special.ndtr(-np.abs(xi_p)))         # for xi < 0
+    return q / np.where(xi_p >= 0, lo, hi)
+
+
+def point_flux_prime(xi_p, alpha, q):
+    """d flux / d xi = phi(xi) / pdf(flux), pdf(x) = q^alpha / Gamma(alpha) x^(-alpha-1) exp(-q / x)."""
+    from scipy import special
+    xi_p = np.asarray(xi_p, np.float64)
+    x = point_flux(xi_p, alpha, q)
+    logpdf = alpha * np.log(q) - special.gammaln(alpha) - (alpha + 1.0) * np.log(x) - q / x
+    return np.exp(-0.5 * xi_p ** 2 - 0.5 * np.log(2 * np.pi) - logpdf)
+
+
+def sky_full(hyper, xi, theta_amp, pts, xi_pts):
+    """Diffuse sky plus point sources.  pts = (yx [npts, 2] int, alpha, q)."""
+    s, a = sky_joint(None, hyper, xi, theta_amp)
+    s_diff = s.copy()
+    yx, alpha, q = pts
+    fl = point_flux(xi_pts, alpha, q)
+    for (y, x), f in zip(yx, fl):
+        s[y, x] += f
+    return s, s_diff, a
+
+
+def energy_grad_full(w_half_c, dirty, hyper, xi, theta_amp, pts, xi_pts, with_prior=True, kern=None):
+    """E and its gradient with respect to (xi, theta_amp, xi_pts)."""
+    fo = _fo()
+    xi = np.asarray(xi, np.float64)
+    theta_amp = np.asarray(theta_amp, np.float64)
+    xi_pts = np.asarray(xi_pts, np.float64)
+    ny, nx = xi.shape
+    s, s_diff, a = sky_full(hyper, xi, theta_amp, pts, xi_pts)
+    cs = fo.psf_apply(w_half_c, s)
+    if kern is None:
+        e = 0.5 * np.sum(s * cs) - np.sum(np.asarray(dirty, np.float64) * s)
+        gs = cs - dirty                                   # dE / ds
+    else:
+        r = np.asarray(dirty, np.float64) - cs
+        u = fo.ninv_apply(kern, r)
+        e = 0.5 * np.sum(r * u)
+        gs = -fo.psf_apply(w_half_c, u)
+    h = fo.hartley2(s_diff * gs)
+    g_xi = a * h
+    g_th = amplitude_vjp(theta_amp, xi * h, hyper, ny, nx)
+    yx, alpha, q = pts
+    g_pt = point_flux_prime(xi_pts, alpha, q) * np.array([gs[y, x] for y, x in yx])
+    if with_prior:
+        e += 0.5 * np.sum(xi * xi) + 0.5 * np.sum(theta_amp ** 2) + 0.5 * np.sum(xi_pts ** 2)
+        g_xi, g_th, g_pt = g_xi + xi, g_th + theta_amp, g_pt + xi_pts
+    return float(e), g_xi, g_th, g_pt
+
+
+def metric_apply_full(w_half_c, hyper, xi, theta_amp, pts, xi_pts, dxi, dtheta, dpts, with_prior=True, kern=None):
+    fo = _fo()
+    xi = np.asarray(xi, np.float64)
+    ny, nx = xi.shape
+    s, s_diff, a = sky_full(hyper, xi, theta_amp, pts, xi_pts)
+    yx, alpha, q = pts
+    fp = point_flux_prime(xi_pts, alpha, q)
+    da = amplitude_jvp(theta_amp, dtheta, hyper, ny, nx)
+    ds = s_diff * fo.hartley2(a * np.asarray(dxi, np.float64) + da * xi)          # J (dxi, dtheta, dpts)
+    for (y, x), f, d in zip(yx, fp, np.asarray(dpts, np.float64)):
+        ds[y, x] += f * d
+    c = fo.psf_apply(w_half_c, ds)
+    if kern is not None:
+        c = fo.psf_apply(w_half_c, fo.ninv_apply(kern, c))
+    h = fo.hartley2(s_diff * c)
+    o_xi = a * h
+    o_th = amplitude_vjp(theta_amp, xi * h, hyper, ny, nx)
+    o_pt = fp * np.array([c[y, x] for y, x in yx])
+    if with_prior:
+        o_xi, o_th, o_pt = o_xi + dxi, o_th + np.asarray(dtheta, np.float64), o_pt + np.asarray(dpts, np.float64)
+    return o_xi, o_th, o_pt

@@ -161,3 +161,65 @@ def test_joint_eq9_gradient_against_central_differences_and_metric_symmetry():
     mv = po.metric_apply_joint(w.w_half[0], hyper, xi, th, u[0], u[1], True, kern)
     a, b = np.sum(u[0] * mu[0]) + np.sum(u[1] * mu[1]), np.sum(dx * mv[0]) + np.sum(dt * mv[1])
     assert abs(a - b) <= 1e-11 * abs(a)
+
+
+# ---------------------------------------------------------------------------------- point sources (reading R18)
+def test_point_flux_closed_form_moments_and_derivative():
+    from scipy import integrate, special
+    xi = np.array([-8.0, -3.0, -1.0, 0.0, 0.5, 2.0, 5.0, 8.0])
+    # alpha = 1: F(x) = exp(-q / x)  =>  flux = -q / ln Phi(xi), written for each tail without cancellation
+    ref = -2.0 / np.where(xi < 0, np.log(special.ndtr(xi)), np.log1p(-special.ndtr(-xi)))
+    assert np.max(np.abs(po.point_flux(xi, 1.0, 2.0) / ref - 1.0)) <= 1e-12
+    # monotone, positive, median = q / Q^-1(alpha, 1/2)
+    f = po.point_flux(np.linspace(-8, 8, 201), 0.5, 1e-4)
+    assert np.all(f > 0) and np.all(np.diff(f) > 0)
+    # alpha = 3, q = 2: mean q / (alpha - 1) = 1, variance q^2 / ((alpha-1)^2 (alpha-2)) = 1  (xi standard normal)
+    phi = lambda t: np.exp(-0.5 * t * t) / np.sqrt(2 * np.pi)  # noqa: E731
+    m1 = integrate.quad(lambda t: po.point_flux(t, 3.0, 2.0) * phi(t), -14, 14, limit=400)[0]
+    m2 = integrate.quad(lambda t: po.point_flux(t, 3.0, 2.0) ** 2 * phi(t), -14, 14, limit=400)[0]
+    assert abs(m1 - 1.0) <= 1e-7 and abs(m2 - m1 * m1 - 1.0) <= 1e-4
+    h = 1e-6
+    fd = (po.point_flux(xi + h, 0.5, 1e-4) - po.point_flux(xi - h, 0.5, 1e-4)) / (2 * h)
+    assert np.max(np.abs(po.point_flux_prime(xi, 0.5, 1e-4) / fd - 1.0)) <= 1e-6
+
+
+def _full_problem():
+    w, hyper, xi, th, rng = _problem()
+    n = xi.shape[0]
+    pts = (np.array([[n // 2, n // 2], [n // 2 + 1, n // 2 - 2], [0, n - 1]]), 0.5, 0.05 * float(np.median(w.sky_true)))
+    xp = np.array([0.8, -0.4, 1.5])
+    return w, hyper, xi, th, pts, xp, rng
+
+
+def test_full_model_gradient_against_central_differences():
+    w, hyper, xi, th, pts, xp, rng = _full_problem()
+    for kern in (None, fo.noise_kernel_from_psf(w.w_half[0], 1e-2 * float(fo.psf_from_weights(w.w_half[0])[0, 0]))):
+        e, gx, gt, gp = po.energy_grad_full(w.w_half[0], w.dirty[0], hyper, xi, th, pts, xp, True, kern)
+        for _ in range(3):
+            dx, dt, dp = rng.normal(size=xi.shape), rng.normal(size=th.shape), rng.normal(size=xp.shape)
+            h = 1e-5
+            ep = po.energy_grad_full(w.w_half[0], w.dirty[0], hyper, xi + h * dx, th + h * dt, pts, xp + h * dp, True, kern)[0]
+            em = po.energy_grad_full(w.w_half[0], w.dirty[0], hyper, xi - h * dx, th - h * dt, pts, xp - h * dp, True, kern)[0]
+            lin = np.sum(gx * dx) + np.sum(gt * dt) + np.sum(gp * dp)
+            assert abs((ep - em) / (2 * h) - lin) <= 1e-6 * max(abs(lin), np.linalg.norm(gx) + np.linalg.norm(gt) + np.linalg.norm(gp))
+    # the sky has the fluxes added exactly at the listed pixels
+    s, s_diff, _ = po.sky_full(hyper, xi, th, pts, xp)
+    d = s - s_diff
+    fl = po.point_flux(xp, pts[1], pts[2])
+    assert np.count_nonzero(d) == 3 and all(abs(d[y, x] - f) <= 1e-12 * f for (y, x), f in zip(pts[0], fl))
+
+
+def test_full_model_metric_symmetric_and_reduces_to_joint():
+    w, hyper, xi, th, pts, xp, rng = _full_problem()
+    u = (rng.normal(size=xi.shape), rng.normal(size=th.shape), rng.normal(size=xp.shape))
+    v = (rng.normal(size=xi.shape), rng.normal(size=th.shape), rng.normal(size=xp.shape))
+    mu = po.metric_apply_full(w.w_half[0], hyper, xi, th, pts, xp, *u)
+    mv = po.metric_apply_full(w.w_half[0], hyper, xi, th, pts, xp, *v)
+    a = sum(np.sum(p * q) for p, q in zip(v, mu))
+    b = sum(np.sum(p * q) for p, q in zip(u, mv))
+    assert abs(a - b) <= 1e-11 * abs(a)
+    assert sum(np.sum(p * q) for p, q in zip(u, mu)) >= sum(np.sum(p * p) for p in u)
+    none = (np.zeros((0, 2), np.int64), 0.5, 1.0)
+    m0 = po.metric_apply_full(w.w_half[0], hyper, xi, th, none, np.zeros(0), u[0], u[1], np.zeros(0))
+    mj = po.metric_apply_joint(w.w_half[0], hyper, xi, th, u[0], u[1])
+    assert np.array_equal(m0[0], mj[0]) and np.array_equal(m0[1], mj[1])
