@@ -166,6 +166,14 @@ int frs_amplitude_forward(frs_ctx* ctx, const float* theta, float* amp_out);
 /* d_amp [ny][nx] = (dA/dtheta) dtheta and g_theta [ntheta] = (dA/dtheta)^T g_amp at the theta of the last forward. */
 int frs_amplitude_jvp(frs_ctx* ctx, const float* dtheta, float* d_amp);
 int frs_amplitude_vjp(frs_ctx* ctx, const float* g_amp, float* g_theta);
+/* Inverse-gamma point-source pixels ("pixels independently modeled with an inverse gamma prior ... locations
+ * manually set"; reading R18): flux_p = F^-1(Phi(xi_p)), F the CDF of pdf(x) ~ x^(-alpha-1) exp(-q / x), is
+ * added to the diffuse sky at pixel (y_p, x_p).  yx_host: HOST int[npts][2]; npts = 0 removes them; npts <= 1024.
+ * With point sources set, theta of the joint calls below is [amplitude part (frs_amp_model_size) | xi_p, p < npts] and
+ * so are grad_theta, dtheta, out_theta; frs_sky_forward adds the fluxes of the last joint position (xi_p = 0 before
+ * one), and every latent-space call uses the diffuse sky as the Jacobian of the diffuse part at those pixels.
+ * Errors: FRS_EINVAL (pixel outside the field, repeated pixel, alpha or q <= 0), FRS_ESTATE for nchan != 1. */
+int frs_set_point_sources(frs_ctx* ctx, int npts, const int* yx_host, float alpha, float q);
 /* Energy of the likelihood in use (frs_set_likelihood) at the joint position (xi, theta), prior 1/2 <xi,xi> + 1/2
  * <theta,theta> if with_prior, and its gradient with respect to both (grad_xi [ny][nx], grad_theta [ntheta]).
  * Sets the joint position.  h_energy: host double or NULL (non-NULL synchronises). */

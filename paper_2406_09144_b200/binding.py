@@ -47,6 +47,7 @@ EXPORTS = {
     "frs_amplitude_forward": (_i, [_vp, _vp, _vp]),
     "frs_amplitude_jvp": (_i, [_vp, _vp, _vp]),
     "frs_amplitude_vjp": (_i, [_vp, _vp, _vp]),
+    "frs_set_point_sources": (_i, [_vp, _i, C.POINTER(_i), _f, _f]),
     "frs_energy_grad_joint": (_i, [_vp, _vp, _vp, _i, C.POINTER(_d), _vp, _vp]),
     "frs_metric_apply_joint": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
     "frs_draw_sample": (_i, [_vp, _vp, _vp, _i, _f, _vp, C.POINTER(_i)]),
@@ -268,8 +269,19 @@ class Context:
         self._ck(lib().frs_amp_model_size(self.ny, self.nx, C.byref(nb), C.byref(nt)))
         self.nfield, self.nb, self.ntheta = 1, nb.value, nt.value
 
+    def set_point_sources(self, yx, alpha, q):
+        """yx: sequence of (y, x) pixels; the joint calls then take theta = [amplitude part | one latent per pixel]."""
+        flat = [int(v) for p in yx for v in p]
+        arr = (_i * max(1, len(flat)))(*flat)
+        self._ck(lib().frs_set_point_sources(self._h, len(flat) // 2, arr, float(alpha), float(q)))
+        self.npts = len(flat) // 2
+
+    @property
+    def ntheta_joint(self):
+        return self.ntheta + getattr(self, "npts", 0)
+
     def amplitude_forward(self, theta, amp_out=None):
-        self._ck(lib().frs_amplitude_forward(self._h, _ptr(theta, self.f32, self.ntheta, "theta"),
+        self._ck(lib().frs_amplitude_forward(self._h, _ptr(theta, self.f32, None, "theta"),
                                              _ptr(amp_out, self.f32, self.npix, "amp_out")))
 
     def amplitude_jvp(self, dtheta, d_amp):
@@ -280,15 +292,15 @@ class Context:
 
     def energy_grad_joint(self, xi, theta, grad_xi, grad_theta, with_prior=True):
         e = _d(0.0)
-        self._ck(lib().frs_energy_grad_joint(self._h, _ptr(xi, self.f32, self.npix, "xi"), _ptr(theta, self.f32, self.ntheta, "theta"),
+        self._ck(lib().frs_energy_grad_joint(self._h, _ptr(xi, self.f32, self.npix, "xi"), _ptr(theta, self.f32, self.ntheta_joint, "theta"),
                                              int(with_prior), C.byref(e), _ptr(grad_xi, self.f32, self.npix, "grad_xi"),
-                                             _ptr(grad_theta, self.f32, self.ntheta, "grad_theta")))
+                                             _ptr(grad_theta, self.f32, self.ntheta_joint, "grad_theta")))
         return e.value
 
     def metric_apply_joint(self, dxi, dtheta, out_xi, out_theta, with_prior=True):
-        self._ck(lib().frs_metric_apply_joint(self._h, _ptr(dxi, self.f32, self.npix, "dxi"), _ptr(dtheta, self.f32, self.ntheta, "dtheta"),
+        self._ck(lib().frs_metric_apply_joint(self._h, _ptr(dxi, self.f32, self.npix, "dxi"), _ptr(dtheta, self.f32, self.ntheta_joint, "dtheta"),
                                               int(with_prior), _ptr(out_xi, self.f32, self.npix, "out_xi"),
-                                              _ptr(out_theta, self.f32, self.ntheta, "out_theta")))
+                                              _ptr(out_theta, self.f32, self.ntheta_joint, "out_theta")))
 
     def set_cuda_graphs(self, on):
         self._ck(lib().frs_set_cuda_graphs(self._h, int(bool(on))))

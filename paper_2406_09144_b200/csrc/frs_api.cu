@@ -64,6 +64,12 @@ struct frs_ctx {
     // the fused (.A, + v) prologue / epilogue and apply their own
     AmpModel am;
     bool have_amp_model = false, plain_latent = false;
+    // inverse-gamma point-source pixels (reading R18): fluxes added to the cached sky; the latent-space passes patch the
+    // few pixels where the Jacobian of the diffuse part differs from the total sky (points_pre / points_post)
+    PointSources pts;
+    const float* pts_dv = nullptr;      // tangent of the point latents (joint metric), else null = 0
+    const float* pts_add = nullptr;     // prior term added to the point outputs (joint calls with the prior), else null
+    float* pts_out = nullptr;           // where the point outputs go (joint calls), else the scratch pts.out
     bool profiling = false;
     std::vector<ProfRec> prof;
     char err[512] = "no error";
@@ -303,9 +309,32 @@ int sky_forward_impl(frs_ctx* ctx, const float* xi) {
         ctx->launches++;
     }
     CK(cudaGetLastError());
+    if (ctx->pts.n > 0) {
+        CKL(launch_points_flux(ctx->stream, ctx->pts));
+        CKL(launch_points_add(ctx->stream, ctx->pts, ctx->sT));
+        ctx->launches += 2;
+        ctx->pts.in_sky = true;
+    }
     ctx->have_s = true;
     ctx->sT_ok = true;
     ctx->s_ok = false;
+    return FRS_OK;
+}
+
+// point-source pixels around the fused . s passes (no-ops without point sources in the cached sky)
+int points_pre(frs_ctx* ctx, float* lin) {
+    if (ctx->pts.n > 0 && ctx->pts.in_sky) {
+        CKL(launch_points_pre(ctx->stream, ctx->pts, lin, ctx->pts_dv));
+        ctx->launches++;
+    }
+    return FRS_OK;
+}
+int points_post(frs_ctx* ctx, float* acc, double sign, double* energy_acc) {
+    if (ctx->pts.n > 0 && ctx->pts.in_sky) {
+        CKL(launch_points_post(ctx->stream, ctx->pts, acc, ctx->pts_add, ctx->pts_out ? ctx->pts_out : ctx->pts.out, sign,
+                               ctx->pts_add ? energy_acc : nullptr));
+        ctx->launches++;
+    }
     return FRS_OK;
 }
 
@@ -331,6 +360,7 @@ int metric_apply9_impl(frs_ctx* ctx, const float* v, int with_prior, float* out,
     RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->plain_latent ? nullptr : ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
     const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
     if (simple) {
+        RET(points_pre(ctx, ctx->lin));
         RET(conv_rows_fwd(ctx, o, ctx->lin, ctx->sT));
     } else {
         jvp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->sT, ctx->d_lognu, ctx->img,
@@ -345,6 +375,7 @@ int metric_apply9_impl(frs_ctx* ctx, const float* v, int with_prior, float* out,
     RET(conv_cols(ctx, o));
     if (simple) {
         RET(conv_rows_inv(ctx, o, ctx->acc, kMulS, ctx->sT, nullptr, nullptr));
+        RET(points_post(ctx, ctx->acc, 1.0, nullptr));
     } else {
         RET(conv_rows_inv(ctx, o, ctx->img, kMulS, ctx->sT, nullptr, nullptr));
         vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
@@ -367,6 +398,7 @@ int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, 
     RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->plain_latent ? nullptr : ctx->amp, ctx->lin, nullptr, nullptr, nullptr, ctx->nfield));
     const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
     if (simple) {
+        RET(points_pre(ctx, ctx->lin));
         RET(conv_rows_fwd(ctx, o, ctx->lin, ctx->sT));             // s . lin fused into the row pass
     } else {
         jvp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->sT, ctx->d_lognu, ctx->img,
@@ -377,6 +409,7 @@ int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, 
     RET(conv_cols(ctx, o));
     if (simple) {
         RET(conv_rows_inv(ctx, o, ctx->acc, kMulS, ctx->sT, nullptr, nullptr));      // acc = s . C(...)
+        RET(points_post(ctx, ctx->acc, 1.0, nullptr));
     } else {
         RET(conv_rows_inv(ctx, o, ctx->img, kMulS, ctx->sT, nullptr, nullptr));
         vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
@@ -497,6 +530,9 @@ void frs_destroy(frs_ctx* ctx) {
     if (ctx->cg_exec) cudaGraphExecDestroy(ctx->cg_exec);
     {
         AmpModel& m = ctx->am;
+        PointSources& ps = ctx->pts;
+        void* pp[] = {ps.idx, ps.xi, ps.out, ps.flux, ps.dflux, ps.sdiff, ps.stot};
+        for (void* q : pp) if (q) cudaFree(q);
         void* mp[] = {m.pindex, m.mult, m.d_hyper, m.theta, m.ab, m.wn, m.abf, m.dabf, m.gbin, m.work, m.sc, m.xi};
         for (void* q : mp) if (q) cudaFree(q);
     }
@@ -635,6 +671,7 @@ int frs_set_sky(frs_ctx* ctx, const float* sky) {
     CK(cudaMemcpyAsync(ctx->s, sky, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
     ctx->have_s = ctx->s_ok = true;
     ctx->sT_ok = false;
+    ctx->pts.in_sky = false;              // a sky supplied by the caller has no point-source bookkeeping
     return FRS_OK;
 }
 
@@ -703,6 +740,7 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
         RET(conv_cols(ctx, o));
         const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
         RET(conv_rows_inv(ctx, o, simple ? ctx->acc : ctx->img, kMulS, ctx->sT, nullptr, nullptr));   // s . C u
+        if (simple) RET(points_post(ctx, ctx->acc, -1.0, ctx->scal + 11));
         if (!simple) {
             vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
                                                                                    ctx->nfield, ctx->nchan);
@@ -730,6 +768,7 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
     energy_final_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal + 8, ctx->scal + 9, ctx->scal + 10, with_prior, ctx->scal + 11);
     ctx->launches++;
     const float* accp = ctx->img;
+    if (ctx->nchan == 1 && ctx->nfield == 1) RET(points_post(ctx, ctx->img, 1.0, ctx->scal + 11));
     if (!(ctx->nchan == 1 && ctx->nfield == 1)) {
         vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
                                                                                ctx->nfield, ctx->nchan);
@@ -1001,6 +1040,36 @@ int frs_amplitude_vjp(frs_ctx* ctx, const float* g_amp, float* g_theta) {
     return FRS_OK;
 }
 
+int frs_set_point_sources(frs_ctx* ctx, int npts, const int* yx_host, float alpha, float q) {
+    if (!ctx || npts < 0 || npts > kMaxPoints || (npts > 0 && (!yx_host || !(alpha > 0.f) || !(q > 0.f))))
+        return fail(ctx, FRS_EINVAL, "frs_set_point_sources: bad argument");
+    if (ctx->nchan != 1) return fail(ctx, FRS_ESTATE, "frs_set_point_sources: single-channel contexts only");
+    CK(cudaSetDevice(ctx->device));
+    std::vector<int> idx((size_t)npts);
+    for (int i = 0; i < npts; ++i) {
+        const int y = yx_host[2 * i], x = yx_host[2 * i + 1];
+        if (y < 0 || y >= ctx->ny || x < 0 || x >= ctx->nx) return fail(ctx, FRS_EINVAL, "frs_set_point_sources: pixel outside the field");
+        idx[i] = x * ctx->ny + y;                       // the latent-space path keeps the sky transposed
+        for (int k = 0; k < i; ++k)
+            if (idx[k] == idx[i]) return fail(ctx, FRS_EINVAL, "frs_set_point_sources: the same pixel twice");
+    }
+    PointSources& p = ctx->pts;
+    RET(dev_alloc(ctx, &p.idx, (size_t)kMaxPoints));
+    RET(dev_alloc(ctx, &p.xi, (size_t)kMaxPoints));
+    RET(dev_alloc(ctx, &p.out, (size_t)kMaxPoints));
+    RET(dev_alloc(ctx, &p.flux, (size_t)kMaxPoints));
+    RET(dev_alloc(ctx, &p.dflux, (size_t)kMaxPoints));
+    RET(dev_alloc(ctx, &p.sdiff, (size_t)kMaxPoints));
+    RET(dev_alloc(ctx, &p.stot, (size_t)kMaxPoints));
+    if (npts) CK(cudaMemcpyAsync(p.idx, idx.data(), (size_t)npts * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemsetAsync(p.xi, 0, (size_t)kMaxPoints * sizeof(float), ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    p.n = npts; p.alpha = alpha; p.q = q; p.in_sky = false;
+    ctx->have_s = ctx->s_ok = ctx->sT_ok = false;
+    ctx->am.have_xi = false;
+    return FRS_OK;
+}
+
 int frs_energy_grad_joint(frs_ctx* ctx, const float* xi, const float* theta, int with_prior, double* h_energy, float* grad_xi,
                           float* grad_theta) {
     if (!ctx || !xi || !theta || !grad_xi || !grad_theta || !aligned16(xi) || !aligned16(grad_xi) || xi == grad_xi)
@@ -1012,12 +1081,18 @@ int frs_energy_grad_joint(frs_ctx* ctx, const float* xi, const float* theta, int
     if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
     RET(latent_scratch(ctx));
     AmpModel& m = ctx->am;
+    const int npts = ctx->pts.n, nta = m.ntheta();      // theta = [amplitude part | point latents]
+    if (npts) CK(cudaMemcpyAsync(ctx->pts.xi, theta + nta, (size_t)npts * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaMemcpyAsync(m.xi, xi, ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
     m.have_xi = true;
     // h = H[s (C s - j)] (mode 0) or -H[s C N'^-1 r] (mode 1): the latent-space passes without their fused . A + xi
     ctx->plain_latent = true;
+    ctx->pts_add = (npts && with_prior) ? ctx->pts.xi : nullptr;
+    ctx->pts_out = npts ? grad_theta + nta : nullptr;
     const int rc = energy_grad_impl(ctx, xi, with_prior, nullptr, nullptr, ctx->lat1);
     ctx->plain_latent = false;
+    ctx->pts_add = nullptr;
+    ctx->pts_out = nullptr;
     RET(rc);
     // grad_xi = A . h (+ xi);  G_b = bin sums of xi . h;  grad_theta = (dA/dtheta)^T G (+ theta);  E += 1/2 <theta, theta>
     CKL(launch_joint_epilogue(ctx->stream, m, ctx->lat1, xi, with_prior ? xi : nullptr, grad_xi));
@@ -1043,9 +1118,15 @@ int frs_metric_apply_joint(frs_ctx* ctx, const float* dxi, const float* dtheta, 
     CKL(launch_amp_tangent(ctx->stream, m, dtheta));
     CKL(launch_joint_prologue(ctx->stream, m, dxi, m.xi, ctx->lat1));
     ctx->launches += 2;
+    const int npts = ctx->pts.n, nta = m.ntheta();
     ctx->plain_latent = true;
+    ctx->pts_dv = npts ? dtheta + nta : nullptr;
+    ctx->pts_add = (npts && with_prior) ? dtheta + nta : nullptr;
+    ctx->pts_out = npts ? out_theta + nta : nullptr;
     const int rc = metric_apply_impl(ctx, ctx->lat1, with_prior, ctx->lat2);
     ctx->plain_latent = false;
+    ctx->pts_dv = ctx->pts_add = nullptr;
+    ctx->pts_out = nullptr;
     RET(rc);
     CKL(launch_joint_epilogue(ctx->stream, m, ctx->lat2, m.xi, with_prior ? dxi : nullptr, out_xi));
     CKL(launch_amp_adjoint(ctx->stream, m, with_prior ? dtheta : nullptr, out_theta, nullptr));

@@ -371,4 +371,110 @@ int launch_joint_epilogue(cudaStream_t st, const AmpModel& m, const float* h, co
     return reduce_launch(st, m, h, xi, add, out_xi);
 }
 
+
+// ---- inverse-gamma point sources (reading R18) -------------------------------------------------------------------------
+namespace {
+// regularised incomplete gamma functions P(a, y) (series) and Q(a, y) (continued fraction, modified Lentz), fp64
+__device__ double gamma_p_series(double a, double y, double lga1) {        // lga1 = lgamma(a + 1)
+    double term = 1.0, sum = 1.0;
+    for (int n = 1; n < 2000; ++n) {
+        term *= y / (a + n);
+        sum += term;
+        if (term < sum * 1e-17) break;
+    }
+    return exp(a * log(y) - y - lga1) * sum;
+}
+__device__ double gamma_q_cf(double a, double y, double lga) {             // lga = lgamma(a)
+    const double tiny = 1e-300;
+    double b = y + 1.0 - a, c = 1.0 / tiny, d = 1.0 / b, h = d;
+    for (int i = 1; i < 2000; ++i) {
+        const double an = -i * (i - a);
+        b += 2.0;
+        d = an * d + b; if (fabs(d) < tiny) d = tiny;
+        c = b + an / c; if (fabs(c) < tiny) c = tiny;
+        d = 1.0 / d;
+        const double del = d * c;
+        h *= del;
+        if (fabs(del - 1.0) < 1e-16) break;
+    }
+    return exp(a * log(y) - y - lga) * h;
+}
+__device__ double gamma_p(double a, double y, double lga) {
+    return y < a + 1.0 ? gamma_p_series(a, y, lga + log(a)) : 1.0 - gamma_q_cf(a, y, lga);
+}
+__device__ double gamma_q(double a, double y, double lga) {
+    return y < a + 1.0 ? 1.0 - gamma_p_series(a, y, lga + log(a)) : gamma_q_cf(a, y, lga);
+}
+// flux = q / y with  P(alpha, y) = Phi(-xi) (xi >= 0)  or  Q(alpha, y) = Phi(xi) (xi < 0): each tail without cancellation.
+// Bisection on ln y (both functions are monotone in y); dflux = phi(xi) / pdf(flux).
+__global__ void points_flux_kernel(const float* __restrict__ xi, int n, double alpha, double q, double* __restrict__ flux,
+                                   double* __restrict__ dflux) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double x = (double)xi[i], lga = lgamma(alpha);
+    const double p = 0.5 * erfc(fabs(x) * 0.70710678118654752440);          // Phi(-|xi|)
+    const bool upper = x >= 0.0;
+    double lo = -1500.0, hi = 8.0;                                           // ln y
+    for (int it = 0; it < 90; ++it) {
+        const double mid = 0.5 * (lo + hi), y = exp(mid);
+        // P increases with y, Q decreases
+        const bool too_small = upper ? gamma_p(alpha, y, lga) < p : gamma_q(alpha, y, lga) > p;
+        if (too_small) lo = mid; else hi = mid;
+    }
+    const double y = exp(0.5 * (lo + hi)), f = q / y;
+    const double logpdf = alpha * log(q) - lga - (alpha + 1.0) * log(f) - q / f;
+    flux[i] = f;
+    dflux[i] = exp(-0.5 * x * x - 0.91893853320467274178 - logpdf);
+}
+__global__ void points_add_kernel(const int* __restrict__ idx, const double* __restrict__ flux, int n, float* __restrict__ sky,
+                                  double* __restrict__ sdiff, double* __restrict__ stot) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double d = (double)sky[idx[i]];
+    const float t = (float)(d + flux[i]);
+    sdiff[i] = d;
+    stot[i] = (double)t;                           // the value the fused passes will multiply by
+    sky[idx[i]] = t;
+}
+__global__ void points_pre_kernel(const int* __restrict__ idx, const double* __restrict__ dflux, const double* __restrict__ sdiff,
+                                  const double* __restrict__ stot, int n, float* __restrict__ lin, const float* __restrict__ dv) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    lin[idx[i]] = (float)((sdiff[i] * (double)lin[idx[i]] + (dv ? dflux[i] * (double)dv[i] : 0.0)) / stot[i]);
+}
+__global__ void points_post_kernel(const int* __restrict__ idx, const double* __restrict__ dflux, const double* __restrict__ sdiff,
+                                   const double* __restrict__ stot, int n, float* __restrict__ acc, const float* __restrict__ add,
+                                   float* __restrict__ out, double sign, double* __restrict__ energy_acc) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        const double c = (double)acc[idx[i]] / stot[i];
+        if (out) out[i] = (float)(sign * dflux[i] * c + (add ? (double)add[i] : 0.0));
+        acc[idx[i]] = (float)(sdiff[i] * c);
+    }
+    if (energy_acc && add && i == 0) {
+        double t = 0.0;
+        for (int k = 0; k < n; ++k) t += (double)add[k] * (double)add[k];
+        energy_acc[0] += 0.5 * t;
+    }
+}
+}  // namespace
+
+int launch_points_flux(cudaStream_t st, const PointSources& p) {
+    points_flux_kernel<<<(p.n + 63) / 64, 64, 0, st>>>(p.xi, p.n, p.alpha, p.q, p.flux, p.dflux);
+    return (int)cudaGetLastError();
+}
+int launch_points_add(cudaStream_t st, const PointSources& p, float* sky) {
+    points_add_kernel<<<(p.n + 63) / 64, 64, 0, st>>>(p.idx, p.flux, p.n, sky, p.sdiff, p.stot);
+    return (int)cudaGetLastError();
+}
+int launch_points_pre(cudaStream_t st, const PointSources& p, float* lin, const float* dv) {
+    points_pre_kernel<<<(p.n + 63) / 64, 64, 0, st>>>(p.idx, p.dflux, p.sdiff, p.stot, p.n, lin, dv);
+    return (int)cudaGetLastError();
+}
+int launch_points_post(cudaStream_t st, const PointSources& p, float* acc, const float* add, float* out, double sign,
+                       double* energy_acc) {
+    points_post_kernel<<<(p.n + 63) / 64, 64, 0, st>>>(p.idx, p.dflux, p.sdiff, p.stot, p.n, acc, add, out, sign, energy_acc);
+    return (int)cudaGetLastError();
+}
+
 }  // namespace frs

@@ -32,6 +32,32 @@ struct AmpModel {
     int ntheta() const { return kAmpScalars + 2 * (nb - 2); }
 };
 
+// ---- inverse-gamma point-source pixels (reading R18) ----
+constexpr int kMaxPoints = 1024;
+struct PointSources {
+    int n = 0;
+    double alpha = 0.0, q = 0.0;
+    int* idx = nullptr;             // [n] position in the TRANSPOSED sky arrays: x ny + y
+    float* xi = nullptr;            // [n] latent values of the current position (zeros until a joint call sets them)
+    float* dv = nullptr;            // [n] tangent input of the metric (joint calls)
+    float* out = nullptr;           // [n] gradient / metric output of the point latents
+    double* flux = nullptr;         // [n] F^-1(Phi(xi))
+    double* dflux = nullptr;        // [n] d flux / d xi
+    double* sdiff = nullptr;        // [n] diffuse sky at the pixel
+    double* stot = nullptr;         // [n] diffuse + flux
+    bool in_sky = false;            // the cached sky contains the fluxes
+};
+// flux, dflux from p.xi
+int launch_points_flux(cudaStream_t st, const PointSources& p);
+// sky[idx] += flux, remembering the diffuse and the total value  (sky: transposed [nx][ny])
+int launch_points_add(cudaStream_t st, const PointSources& p, float* sky);
+// the fused passes multiply by the TOTAL sky; at a point-source pixel the Jacobian of the diffuse part is the diffuse sky
+// and the point latent enters with dflux:  lin[idx] <- (sdiff lin[idx] + dflux dv) / stot   (dv may be null: 0)
+int launch_points_pre(cudaStream_t st, const PointSources& p, float* lin, const float* dv);
+// acc holds stot . c at the pixel:  out = sign dflux c (+ add);  acc[idx] <- sdiff c;  energy_acc (may be null) += 1/2 |add|^2
+int launch_points_post(cudaStream_t st, const PointSources& p, float* acc, const float* add, float* out, double sign,
+                       double* energy_acc);
+
 int launch_amp_bins(cudaStream_t st, const AmpModel& m);
 // theta -> A_b (and the state kept for the derivatives)
 int launch_amp_forward(cudaStream_t st, const AmpModel& m);

@@ -158,3 +158,74 @@ def test_joint_model_state_errors_and_switch_back(frs):
     multi = frs.Context(64, 64, 2)
     with pytest.raises(frs.FrsError):
         multi.set_amplitude_model(hyper)
+
+
+# ---------------------------------------------------------------------------------- point sources (reading R18)
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("size", [(128, None, None), (0, 64, 256)])
+def test_full_model_with_point_sources(frs, size, mode):
+    import torch
+    from oracle import frs_oracle as fo
+    w, hyper, xi, th, rng = _problem(size[0], ny=size[1], nx=size[2])
+    ny, nx = w.ny, w.nx
+    yx = np.array([[ny // 2, nx // 2], [ny // 2 + 1, nx // 2 - 2], [0, nx - 1], [ny - 1, 0]])
+    alpha, q = 0.5, 0.05 * float(np.median(w.sky_true))
+    pts = (yx, alpha, q)
+    xp = np.array([0.8, -0.4, 2.5, -3.0], np.float32)
+    ctx = frs.Context(ny, nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    ctx.set_amplitude_model(hyper)
+    ctx.set_point_sources(yx, alpha, q)
+    kern = None
+    if mode == 1:
+        ctx.set_noise_kernel(1e-2 * float(fo.psf_from_weights(w.w_half[0])[0, 0]))
+        ctx.set_likelihood(1)
+        kern = ctx.get_noise_kernel().cpu().numpy()[0].astype(np.float64)
+    theta = np.concatenate([th, xp]).astype(np.float32)
+    assert ctx.ntheta_joint == theta.size
+    gx, gt = torch.empty(1, ny, nx, device="cuda"), torch.empty(theta.size, device="cuda")
+    e = ctx.energy_grad_joint(dev(xi[None]), dev(theta), gx, gt, True)
+    e_ref, gx_ref, gt_ref, gp_ref = po.energy_grad_full(w.w_half[0], w.dirty[0], hyper, xi, th, pts, xp, True, kern)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
+    assert rel(gx.cpu().numpy()[0], gx_ref) <= 1e-5
+    got = gt.cpu().numpy()
+    assert rel(got[:th.size], gt_ref) <= 1e-5
+    # each point gradient is dflux x (C s - j)[pixel]: a difference of two image values, held to 1e-5 of its operands
+    s_ref = po.sky_full(hyper, xi, th, pts, xp)[0]
+    cs = fo.psf_apply(w.w_half[0], s_ref)
+    scale = po.point_flux_prime(xp, alpha, q) * np.array([abs(cs[y, x]) + abs(w.dirty[0][y, x]) for y, x in yx]) + np.abs(xp)
+    if mode == 0:
+        assert np.all(np.abs(got[th.size:] - gp_ref) <= 1e-5 * scale)
+    else:
+        assert rel(got[th.size:], gp_ref) <= 1e-4
+    # the cached sky carries the fluxes, in the natural orientation too
+    s = ctx.new_image()
+    ctx.sky_forward(dev(xi[None]), s)
+    assert rel(s.cpu().numpy()[0], s_ref) <= 1e-5
+    for (y, x), f in zip(yx, po.point_flux(xp, alpha, q)):
+        assert abs(float(s[0, y, x]) - s_ref[y, x]) <= 2e-6 * s_ref[y, x]
+    dxi = rng.normal(size=xi.shape).astype(np.float32)
+    dth = rng.normal(size=theta.shape).astype(np.float32)
+    ox, ot = torch.empty_like(gx), torch.empty_like(gt)
+    ctx.energy_grad_joint(dev(xi[None]), dev(theta), gx, gt, True)
+    ctx.metric_apply_joint(dev(dxi[None]), dev(dth), ox, ot, True)
+    ox_ref, ot_ref, op_ref = po.metric_apply_full(w.w_half[0], hyper, xi, th, pts, xp, dxi, dth[:th.size], dth[th.size:], True, kern)
+    assert rel(ox.cpu().numpy()[0], ox_ref) <= 1e-5
+    assert rel(ot.cpu().numpy()[:th.size], ot_ref) <= 1e-5
+    assert rel(ot.cpu().numpy()[th.size:], op_ref) <= 1e-5
+    # the xi-block operators of the fixed-amplitude API see the same Jacobian (diffuse sky at the point pixels)
+    out = ctx.new_latent()
+    ctx.metric_apply(dev(dxi[None]), out, with_prior=True)
+    ref0 = po.metric_apply_full(w.w_half[0], hyper, xi, th, pts, xp, dxi, np.zeros_like(th), np.zeros(4), True, kern)[0]
+    assert rel(out.cpu().numpy()[0], ref0) <= 1e-5
+
+
+def test_point_source_argument_errors(frs):
+    ctx = frs.Context(64, 64, 1)
+    for bad in ([[64, 0]], [[0, -1]], [[3, 4], [3, 4]]):
+        with pytest.raises(frs.FrsError):
+            ctx.set_point_sources(bad, 0.5, 1.0)
+    with pytest.raises(frs.FrsError):
+        ctx.set_point_sources([[1, 1]], 0.0, 1.0)
+    ctx.set_point_sources([], 0.5, 1.0)
