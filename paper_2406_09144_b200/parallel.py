@@ -94,3 +94,67 @@ class ChannelShard:
             self.ctx.cg_step_end(x, with_prior=with_prior)
         r, p, q, sc = self.ctx.cg_read_state()
         return float(sc[0]) ** 0.5
+
+
+# ---- MGVI samples over ranks (the replica axis of the single-channel configs) ------------------------
+def partition_samples(nsamp: int, world: int, rank: int) -> range:
+    """Contiguous, balanced block of sample indices for `rank` (same rule as the channels)."""
+    return partition_channels(nsamp, world, rank)
+
+
+class SampleShard:
+    """One rank's share of the MGVI samples of a single-channel problem (reading R15).
+
+    Every rank holds the WHOLE problem (PSF spectrum, dirty image, model: replicas) and draws / evaluates only its
+    own samples: drawing a sample is an independent CG solve, and the sample-averaged KL, its gradient and its metric
+    are means over samples, so the only exchange is ONE all-reduce (sum) of a latent-sized vector (plus the energy
+    scalar) per KL evaluation or metric apply; a rank weights its local mean by n_local / n_total before the sum.
+    `ctx` is a ready Context (or any object with draw_sample / kl_energy_grad / kl_metric_apply).
+    """
+
+    def __init__(self, ctx, nsamp, group=None):
+        import torch.distributed as dist
+        self.dist, self.group, self.ctx = dist, group, ctx
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.nsamp = int(nsamp)
+        self.mine = partition_samples(self.nsamp, self.world, self.rank)
+        self.samples = None
+
+    def _sum(self, t):
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
+        return t
+
+    def draw(self, eta_xi, eta_d, max_iter, rtol=0.0):
+        """eta_xi [nsamp, nfield, ny, nx], eta_d [nsamp, nchan, ny, nx]: the white-noise inputs of ALL samples (every rank
+        sees the same arrays, e.g. from a counter-based generator); the rank solves for its own block only."""
+        import torch
+        loc = [torch.zeros_like(eta_xi[0]) for _ in self.mine]
+        for out, i in zip(loc, self.mine):
+            self.ctx.draw_sample(eta_xi[i].contiguous(), eta_d[i].contiguous(), out, max_iter, rtol)
+        self.samples = torch.stack(loc) if loc else eta_xi[:0].clone()
+        return self.samples
+
+    def kl_energy_grad(self, xi, grad, mirrored=True):
+        """KL estimate over ALL samples and its gradient (identical on every rank)."""
+        import torch
+        n = len(self.mine)
+        e = 0.0
+        if n:
+            e = self.ctx.kl_energy_grad(xi, self.samples, grad, mirrored) * n / self.nsamp
+            grad.mul_(n / self.nsamp)
+        else:
+            grad.zero_()
+        et = torch.tensor([e], dtype=torch.float64, device=grad.device)
+        self._sum(et)
+        self._sum(grad)
+        return float(et.item())
+
+    def kl_metric_apply(self, xi, v, out, mirrored=True):
+        n = len(self.mine)
+        if n:
+            self.ctx.kl_metric_apply(xi, self.samples, v, out, mirrored)
+            out.mul_(n / self.nsamp)
+        else:
+            out.zero_()
+        self._sum(out)
+        return out

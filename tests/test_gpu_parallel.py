@@ -71,6 +71,42 @@ def test_channel_shard_real_context_nccl_world1(nccl_world1):
     assert abs(rn - ref["res"][-1]) <= 1e-3 * ref["res"][-1]
 
 
+def test_sample_shard_real_context_nccl_world1(nccl_world1):
+    """MGVI samples over ranks (SampleShard) with the real context and NCCL at world size 1: draw -> KL energy / gradient
+    -> all_reduce -> KL metric, against the oracle running on the GPU's noise kernel and the GPU's own samples."""
+    import torch
+    import paper_2406_09144_b200 as frs
+    from paper_2406_09144_b200.parallel import SampleShard
+    frs.load_library()
+    w = wl.make_config(1, n=64, sigma_rel=0.1)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).cuda()  # noqa: E731
+    ctx = frs.Context(w.ny, w.nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    ctx.set_amplitude(dev(w.amp), w.mu)
+    ctx.set_noise_kernel(1e-2 * float(o.psf_from_weights(w.w_half[0])[0, 0]))
+    ctx.set_likelihood(1)
+    kern = ctx.get_noise_kernel().cpu().numpy().astype(np.float64)
+    rng = np.random.default_rng(11)
+    xi = (0.2 * rng.normal(size=(1, w.ny, w.nx))).astype(np.float32)
+    ctx.sky_forward(dev(xi))
+    nsamp = 2
+    eta_xi = rng.normal(size=(nsamp, 1, w.ny, w.nx)).astype(np.float32)
+    eta_d = rng.normal(size=(nsamp, 1, w.ny, w.nx)).astype(np.float32)
+    sh = SampleShard(ctx, nsamp)
+    assert list(sh.mine) == [0, 1]
+    samples = sh.draw(dev(eta_xi), dev(eta_d), 30)
+    g = ctx.new_latent()
+    e = sh.kl_energy_grad(dev(xi), g, True)
+    smp = samples.cpu().numpy().astype(np.float64)
+    e_ref, g_ref = o.kl_energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi, smp, True)
+    assert abs(e - e_ref) <= 1e-5 * abs(e_ref) and rel(g.cpu().numpy(), g_ref) <= 1e-5
+    v = rng.normal(size=xi.shape).astype(np.float32)
+    out = ctx.new_latent()
+    sh.kl_metric_apply(dev(xi), dev(v), out, True)
+    assert rel(out.cpu().numpy(), o.kl_metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, smp, v, True)) <= 1e-5
+
+
 def test_two_devices_if_present():
     """Contexts on two devices in one process (per-device launch caches); skipped on a one-GPU box."""
     import torch

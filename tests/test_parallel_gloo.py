@@ -13,7 +13,7 @@ import torch.multiprocessing as mp
 
 from gen import workloads as wl
 from oracle import frs_oracle as o
-from paper_2406_09144_b200.parallel import ChannelShard, partition_channels
+from paper_2406_09144_b200.parallel import ChannelShard, SampleShard, partition_channels
 
 
 def test_partition_is_a_balanced_cover():
@@ -130,3 +130,73 @@ def test_sharded_operators_equal_the_full_oracle_world2():
     assert nloc == 2                                   # rank 0 owns 2 of the 3 channels
     assert de <= 1e-12 and dg <= 1e-12 and dm <= 1e-12, res
     assert dx <= 1e-9 and rn > 0, res
+
+
+# ---------------------------------------------------------------------------------- MGVI samples over ranks
+class OracleKlCtx:
+    """Stand-in with the MGVI methods of binding.Context, arithmetic from the oracle (Eq. 9 likelihood, R14 / R15)."""
+
+    def __init__(self, w, kern):
+        self.w, self.kern = w, kern
+
+    def draw_sample(self, eta_xi, eta_d, sample, max_iter, rtol=0.0):
+        s = o.draw_sample_eq9(self.w.w_half, self.kern, self.w.amp, self.w.mu, self.w.lognu, self.xi, eta_xi.numpy(), eta_d.numpy(), max_iter)[0]
+        sample.copy_(torch.from_numpy(s))
+
+    def kl_energy_grad(self, xi, samples, grad, mirrored=True):
+        e, g = o.kl_energy_grad_eq9(self.w.w_half, self.kern, self.w.dirty, self.w.amp, self.w.mu, self.w.lognu, xi.numpy(),
+                                    samples.numpy(), mirrored)
+        grad.copy_(torch.from_numpy(g))
+        return e
+
+    def kl_metric_apply(self, xi, samples, v, out, mirrored=True):
+        out.copy_(torch.from_numpy(o.kl_metric_apply_eq9(self.w.w_half, self.kern, self.w.amp, self.w.mu, self.w.lognu, xi.numpy(),
+                                                         samples.numpy(), v.numpy(), mirrored)))
+
+
+def _kl_worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = wl.make_config(1, n=16, seed=2)
+        kern = o.noise_kernel_from_psf(w.w_half[0], 1e-2 * float(o.psf_from_weights(w.w_half[0])[0, 0]))[None]
+        rng = np.random.default_rng(7)                                  # the same stream on every rank
+        xi = 0.2 * rng.normal(size=(1, w.ny, w.nx))
+        nsamp = 3                                                       # 3 samples over 2 ranks: uneven split
+        eta_xi, eta_d = rng.normal(size=(nsamp, 1, w.ny, w.nx)), rng.normal(size=(nsamp, 1, w.ny, w.nx))
+        ctx = OracleKlCtx(w, kern)
+        ctx.xi = xi
+        sh = SampleShard(ctx, nsamp)
+        sh.draw(torch.from_numpy(eta_xi), torch.from_numpy(eta_d), 8)
+        g = torch.zeros(1, w.ny, w.nx, dtype=torch.float64)
+        e = sh.kl_energy_grad(torch.from_numpy(xi), g, True)
+        v = rng.normal(size=xi.shape)
+        mv = torch.zeros_like(g)
+        sh.kl_metric_apply(torch.from_numpy(xi), torch.from_numpy(v), mv, True)
+        if rank == 0:
+            full = np.stack([o.draw_sample_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, eta_xi[i], eta_d[i], 8)[0] for i in range(nsamp)])
+            e_ref, g_ref = o.kl_energy_grad_eq9(w.w_half, kern, w.dirty, w.amp, w.mu, w.lognu, xi, full, True)
+            m_ref = o.kl_metric_apply_eq9(w.w_half, kern, w.amp, w.mu, w.lognu, xi, full, v, True)
+            rel = lambda a, r: float(np.linalg.norm(a - r) / np.linalg.norm(r))   # noqa: E731
+            out.put((len(sh.mine), abs(e - e_ref) / abs(e_ref), rel(g.numpy(), g_ref), rel(mv.numpy(), m_ref)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_sample_sharded_kl_equals_the_full_oracle_world2():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_kl_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = out.get(timeout=240)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    nloc, de, dg, dm = res
+    assert nloc == 2 and de <= 1e-12 and dg <= 1e-12 and dm <= 1e-12, res
