@@ -52,6 +52,22 @@ const char* frs_version(void);
  * requires max|Im W| <= 1e-5 max W and min Re W >= -1e-5 max W, else FRS_ENOTPSD (R4; P:191:
  * a covariance kernel must be real and positive).  Stores max(Re W, 0).  Synchronises. */
 int frs_set_psf(frs_ctx* ctx, const float* psf);
+/* ---- images that are not a power of two (3600^2) by embedding; reading R19 ----
+ * Eq. 14 is a LINEAR convolution of the ny_img x nx_img image with a PSF twice its size: any padded grid of at least
+ * twice the image computes it exactly.  The context is created on the next power of two (ny, nx); every image-sized
+ * array of the other calls stays [ny][nx] with the image in its corner [0, ny_img) x [0, nx_img); the correlated field
+ * lives on the whole grid and the sky is its crop: frs_sky_forward / frs_set_sky zero it outside the image, and with it
+ * every fused . s of the gradient and the metric.  (Mode 1 applies Eq. 18 on the embedding grid.) */
+
+/* psf_img: device [nchan][2 ny_img][2 nx_img], origin at [0][0], negative offsets wrapped.  Copies it to the offsets
+ * |dy| < ny_img, |dx| < nx_img of the context's padded grid (zero elsewhere), takes its spectrum as frs_set_psf does --
+ * but keeps the sign of Re W (the truncated PSF is real and even, not a covariance on the larger grid; FRS_ENOTPSD only
+ * for max|Im W| > 1e-5 max W) -- and sets the field of view.  Synchronises. */
+int frs_set_psf_embedded(frs_ctx* ctx, const float* psf_img, int ny_img, int nx_img);
+/* The sky is zero outside [0, ny_img) x [0, nx_img) from now on (ny_img = ny, nx_img = nx: whole grid again).  For PSFs
+ * given as weights on the context's own padded grid.  Invalidates the cached position. */
+int frs_set_field_of_view(frs_ctx* ctx, int ny_img, int nx_img);
+
 /* PSF given as its real, non-negative half spectrum W [nchan][2ny][nx+1] (the gridded, Hermitian-
  * symmetrised visibility weights; P:180 'FFT[I^PSF]', R3: (C x)[n] = sum_k W[k] xhat[k] e^{+2 pi i k.n/M},
  * so the PSF peak equals sum W).  Negative entries -> FRS_ENOTPSD.  Synchronises. */

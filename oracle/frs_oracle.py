@@ -438,3 +438,42 @@ def newton_cg_step(w_half, dirty, amp, mu, lognu, xi, cg_iters=50):
             break
         d = 0.5 * d
     return xi + d, e0, e1
+
+
+# =============================================================================
+# Image sizes that are not powers of two (3600^2) by embedding -- DESIGN.md reading R19
+# =============================================================================
+# The convolution of Eq. 14 is a LINEAR convolution of the ny_i x nx_i image with the (2 ny_i) x (2 nx_i) PSF; any padded
+# grid of at least twice the image size computes it exactly.  The correlated field lives on the embedding grid
+# (ny x nx, the next power of two); the sky is its crop to the image, everything outside is not part of the model:
+#   s = crop(exp(mu + H[A xi])),   E = 1/2 <s, C s> - <j, s> (+ 1/2 <xi, xi>),   C on the ny_i x nx_i image.
+def embed(x, ny, nx):
+    out = np.zeros(x.shape[:-2] + (ny, nx))
+    out[..., :x.shape[-2], :x.shape[-1]] = x
+    return out
+
+
+def energy_grad_embedded(w_half_img, dirty_img, amp, mu, xi, with_prior=True):
+    """w_half_img [2 ny_i, nx_i + 1], dirty_img [ny_i, nx_i]: the image-sized problem; amp, xi [ny, nx]: the field on the
+    embedding grid.  Returns E and dE/dxi [ny, nx]."""
+    xi = np.asarray(xi, dtype=F64)
+    ny, nx = xi.shape
+    nyi, nxi = dirty_img.shape
+    s_full = np.exp(mu + hartley2(np.asarray(amp, F64) * xi))
+    s = s_full[:nyi, :nxi]
+    cs = psf_apply(w_half_img, s)
+    e = 0.5 * np.sum(s * cs) - np.sum(np.asarray(dirty_img, F64) * s)
+    g = np.asarray(amp, F64) * hartley2(embed(s * (cs - dirty_img), ny, nx))
+    if with_prior:
+        e += 0.5 * np.sum(xi * xi)
+        g = g + xi
+    return float(e), g
+
+
+def metric_apply_embedded(w_half_img, nyi, nxi, amp, mu, xi, v, with_prior=True):
+    xi = np.asarray(xi, dtype=F64)
+    ny, nx = xi.shape
+    s = np.exp(mu + hartley2(np.asarray(amp, F64) * xi))[:nyi, :nxi]
+    jv = s * hartley2(np.asarray(amp, F64) * np.asarray(v, F64))[:nyi, :nxi]
+    out = np.asarray(amp, F64) * hartley2(embed(s * psf_apply(w_half_img, jv), ny, nx))
+    return out + v if with_prior else out

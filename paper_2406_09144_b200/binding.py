@@ -42,6 +42,8 @@ EXPORTS = {
     "frs_ninv_apply": (_i, [_vp, _vp, _vp]),
     "frs_set_likelihood": (_i, [_vp, _i]),
     "frs_set_cuda_graphs": (_i, [_vp, _i]),
+    "frs_set_psf_embedded": (_i, [_vp, _vp, _i, _i]),
+    "frs_set_field_of_view": (_i, [_vp, _i, _i]),
     "frs_amp_model_size": (_i, [_i, _i, C.POINTER(_i), C.POINTER(_i)]),
     "frs_set_amplitude_model": (_i, [_vp, C.POINTER(_f)]),
     "frs_amplitude_forward": (_i, [_vp, _vp, _vp]),
@@ -301,6 +303,14 @@ class Context:
         self._ck(lib().frs_metric_apply_joint(self._h, _ptr(dxi, self.f32, self.npix, "dxi"), _ptr(dtheta, self.f32, self.ntheta_joint, "dtheta"),
                                               int(with_prior), _ptr(out_xi, self.f32, self.npix, "out_xi"),
                                               _ptr(out_theta, self.f32, self.ntheta_joint, "out_theta")))
+
+    # ---- images smaller than the (power-of-two) grid: embedding, reading R19
+    def set_psf_embedded(self, psf_img, ny_img, nx_img):
+        self._ck(lib().frs_set_psf_embedded(self._h, _ptr(psf_img, self.f32, self.nchan * 4 * ny_img * nx_img, "psf_img"),
+                                            int(ny_img), int(nx_img)))
+
+    def set_field_of_view(self, ny_img, nx_img):
+        self._ck(lib().frs_set_field_of_view(self._h, int(ny_img), int(nx_img)))
 
     def set_cuda_graphs(self, on):
         self._ck(lib().frs_set_cuda_graphs(self._h, int(bool(on))))

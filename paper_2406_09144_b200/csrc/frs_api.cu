@@ -67,6 +67,7 @@ struct frs_ctx {
     // inverse-gamma point-source pixels (reading R18): fluxes added to the cached sky; the latent-space passes patch the
     // few pixels where the Jacobian of the diffuse part differs from the total sky (points_pre / points_post)
     PointSources pts;
+    int fov_y = 0, fov_x = 0;           // image smaller than the grid (reading R19): the sky is zero outside [0,fov_y) x [0,fov_x); 0 = whole grid
     const float* pts_dv = nullptr;      // tangent of the point latents (joint metric), else null = 0
     const float* pts_add = nullptr;     // prior term added to the point outputs (joint calls with the prior), else null
     float* pts_out = nullptr;           // where the point outputs go (joint calls), else the scratch pts.out
@@ -314,6 +315,10 @@ int sky_forward_impl(frs_ctx* ctx, const float* xi) {
         CKL(launch_points_add(ctx->stream, ctx->pts, ctx->sT));
         ctx->launches += 2;
         ctx->pts.in_sky = true;
+    }
+    if (ctx->fov_y) {                        // sT is [nx][ny]
+        CKL(launch_mask_outside(ctx->stream, ctx->sT, ctx->nx, ctx->ny, ctx->fov_x, ctx->fov_y, ctx->nchan));
+        ctx->launches++;
     }
     ctx->have_s = true;
     ctx->sT_ok = true;
@@ -577,9 +582,43 @@ int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
     return FRS_OK;
 }
 
+static int set_psf_impl(frs_ctx* ctx, const float* psf, bool covariance);
 int frs_set_psf(frs_ctx* ctx, const float* psf) {
     if (!ctx || !psf || !aligned16(psf)) return fail(ctx, FRS_EINVAL, "frs_set_psf: bad argument");
     CK(cudaSetDevice(ctx->device));
+    return set_psf_impl(ctx, psf, true);
+}
+
+int frs_set_field_of_view(frs_ctx* ctx, int ny_img, int nx_img) {
+    if (!ctx || ny_img < 1 || nx_img < 1 || ny_img > ctx->ny || nx_img > ctx->nx)
+        return fail(ctx, FRS_EINVAL, "frs_set_field_of_view: bad argument");
+    const bool whole = ny_img == ctx->ny && nx_img == ctx->nx;
+    ctx->fov_y = whole ? 0 : ny_img;
+    ctx->fov_x = whole ? 0 : nx_img;
+    ctx->have_s = ctx->s_ok = ctx->sT_ok = false;
+    ctx->am.have_xi = false;
+    return FRS_OK;
+}
+
+int frs_set_psf_embedded(frs_ctx* ctx, const float* psf_img, int ny_img, int nx_img) {
+    if (!ctx || !psf_img || !aligned16(psf_img) || ny_img < 1 || nx_img < 1 || ny_img > ctx->ny || nx_img > ctx->nx)
+        return fail(ctx, FRS_EINVAL, "frs_set_psf_embedded: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    float* big = nullptr;
+    CK(cudaMalloc(reinterpret_cast<void**>(&big), (size_t)ctx->nchan * 4 * ctx->npix * sizeof(float)));
+    int rc = FRS_OK;
+    const int e = launch_embed_psf(ctx->stream, psf_img, big, ny_img, nx_img, ctx->ny, ctx->nx, ctx->nchan);
+    if (e) rc = cuda_fail(ctx, (cudaError_t)e, "launch_embed_psf");
+    ctx->launches++;
+    // the truncated PSF is real and even but need not be a covariance on the larger grid: its spectrum keeps its sign
+    if (rc == FRS_OK) rc = set_psf_impl(ctx, big, false);
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(big);
+    if (rc != FRS_OK) return rc;
+    return frs_set_field_of_view(ctx, ny_img, nx_img);
+}
+
+static int set_psf_impl(frs_ctx* ctx, const float* psf, bool covariance) {
     const int my = 2 * ctx->ny, mx = 2 * ctx->nx;
     RET(dev_alloc(ctx, &ctx->wt, (size_t)ctx->nchan * ctx->ntile * 2 * ctx->ny * 2));
     // row pass over all 2 ny rows of length 2 nx (no padding), then one DIF step + ny-point column FFTs
@@ -601,6 +640,7 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
         CKL(launch_psf_cols(ctx->stream, ctx->ny, c, ctx->nchan, &gx));   // grid size only
         CK(cudaMalloc(reinterpret_cast<void**>(&stats), (size_t)ctx->nchan * gx * 3 * sizeof(float)));
         c.t = tmp; c.wt = ctx->wt; c.stats = stats; c.scale = 1.0f / ((float)my * (float)mx);
+        c.floor = covariance ? 0.f : -3.0e38f;
         c.ncols = ctx->nx + 1; c.w_bstride = (size_t)ctx->ntile * 2 * ctx->ny * 2;
         c.tw = ctx->tw[ctx->ny]; c.twist = ctx->twist[ctx->ny];
         CKL(launch_psf_cols(ctx->stream, ctx->ny, c, ctx->nchan, nullptr));
@@ -619,7 +659,7 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
     for (size_t i = 0; i < hs.size(); i += 3) {
         max_im = fmaxf(max_im, hs[i]); min_re = fminf(min_re, hs[i + 1]); max_re = fmaxf(max_re, hs[i + 2]);
     }
-    if (!(max_im <= 1e-5f * max_re) || !(min_re >= -1e-5f * max_re)) {
+    if (!(max_im <= 1e-5f * max_re) || (covariance && !(min_re >= -1e-5f * max_re))) {
         ctx->have_psf = false;
         snprintf(ctx->err, sizeof(ctx->err), "PSF spectrum not real/non-negative: max|Im|=%g min Re=%g max Re=%g", max_im, min_re, max_re);
         return FRS_ENOTPSD;
@@ -669,6 +709,10 @@ int frs_set_sky(frs_ctx* ctx, const float* sky) {
     CK(cudaSetDevice(ctx->device));
     RET(ensure_scratch(ctx));
     CK(cudaMemcpyAsync(ctx->s, sky, (size_t)ctx->nchan * ctx->npix * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream));
+    if (ctx->fov_y) {
+        CKL(launch_mask_outside(ctx->stream, ctx->s, ctx->ny, ctx->nx, ctx->fov_y, ctx->fov_x, ctx->nchan));
+        ctx->launches++;
+    }
     ctx->have_s = ctx->s_ok = true;
     ctx->sT_ok = false;
     ctx->pts.in_sky = false;              // a sky supplied by the caller has no point-source bookkeeping

@@ -51,8 +51,8 @@ psf_cols_kernel(PsfColsArgs a) {
             max_im = fmaxf(max_im, fmaxf(fabsf(v[e].im.x), fabsf(v[e].im.y)) * a.scale);
             min_re = fminf(min_re, fminf(re0, re1));
             max_re = fmaxf(max_re, fmaxf(re0, re1));
-            w[(size_t)(p + e * P) * 2] = 0.5f * fmaxf(re0, 0.f);
-            w[(size_t)(NF + p + e * P) * 2] = 0.5f * fmaxf(re1, 0.f);
+            w[(size_t)(p + e * P) * 2] = 0.5f * fmaxf(re0, a.floor);
+            w[(size_t)(NF + p + e * P) * 2] = 0.5f * fmaxf(re1, a.floor);
         }
     }
     __shared__ float red[3][32];
@@ -204,6 +204,39 @@ __global__ void transpose_kernel(const float* __restrict__ in, float* __restrict
 int launch_transpose(cudaStream_t st, const float* in, float* out, int rows, int cols, int nb) {
     dim3 grid((cols + 31) / 32, (rows + 31) / 32, nb), block(32, 8);
     transpose_kernel<<<grid, block, 0, st>>>(in, out, rows, cols);
+    return (int)cudaGetLastError();
+}
+
+__global__ void embed_psf_kernel(const float* __restrict__ small, float* __restrict__ big, int nyi, int nxi, int ny, int nx) {
+    const int my = 2 * ny, mx = 2 * nx;
+    const size_t n = (size_t)my * mx;
+    const float* sb = small + (size_t)blockIdx.y * 4 * nyi * nxi;
+    float* bb = big + (size_t)blockIdx.y * n;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int y = (int)(i / mx), x = (int)(i % mx);
+        const int sy = y < ny ? y : y - my, sx = x < nx ? x : x - mx;             // signed offsets
+        float v = 0.f;
+        if (sy > -nyi && sy < nyi && sx > -nxi && sx < nxi)
+            v = sb[(size_t)((sy + 2 * nyi) % (2 * nyi)) * (2 * nxi) + (sx + 2 * nxi) % (2 * nxi)];
+        bb[i] = v;
+    }
+}
+int launch_embed_psf(cudaStream_t st, const float* small, float* big, int nyi, int nxi, int ny, int nx, int nb) {
+    embed_psf_kernel<<<dim3(1184, nb), 256, 0, st>>>(small, big, nyi, nxi, ny, nx);
+    return (int)cudaGetLastError();
+}
+__global__ void mask_outside_kernel(float* __restrict__ img, int rows, int cols, int rows_in, int cols_in) {
+    float* b = img + (size_t)blockIdx.y * rows * cols;
+    // the strip right of the kept block, then the rows below it: only what has to be zeroed is touched
+    const size_t right = (size_t)rows_in * (cols - cols_in), below = (size_t)(rows - rows_in) * cols;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < right + below; i += (size_t)gridDim.x * blockDim.x) {
+        if (i < right) b[(i / (cols - cols_in)) * cols + cols_in + i % (cols - cols_in)] = 0.f;
+        else b[(size_t)rows_in * cols + (i - right)] = 0.f;
+    }
+}
+int launch_mask_outside(cudaStream_t st, float* img, int rows, int cols, int rows_in, int cols_in, int nb) {
+    if (rows_in == rows && cols_in == cols) return 0;
+    mask_outside_kernel<<<dim3(592, nb), 256, 0, st>>>(img, rows, cols, rows_in, cols_in);
     return (int)cudaGetLastError();
 }
 

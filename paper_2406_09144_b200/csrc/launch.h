@@ -24,6 +24,7 @@ struct PsfColsArgs {
     float* stats;         // [nb][gridDim.x][3]: max |Im W|, min Re W, max Re W   (unscaled by fold)
     int ntile;
     float scale;          // 1 / (My Mx)
+    float floor;          // W is stored as max(Re W, floor): 0 for a covariance kernel, -FLT_MAX for an embedded PSF
     size_t w_bstride;
     const float4* tw;
     const float2* twist;

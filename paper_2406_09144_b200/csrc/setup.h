@@ -8,4 +8,9 @@ int launch_weights_transpose(cudaStream_t st, const float* wt, float* wtT, int n
 int launch_weights_permute(cudaStream_t st, float* wt, int nf, int cols, int nb);
 // out[b][j][i] = in[b][i][j], in [nb][rows][cols]
 int launch_transpose(cudaStream_t st, const float* in, float* out, int rows, int cols, int nb);
+// Embedding of an image that is smaller than the grid (reading R19).
+// big [nb][2 ny][2 nx] <- small [nb][2 nyi][2 nxi]: the PSF copied to the offsets |dy| < nyi, |dx| < nxi (wrapped), zero elsewhere
+int launch_embed_psf(cudaStream_t st, const float* small, float* big, int nyi, int nxi, int ny, int nx, int nb);
+// img [nb][rows][cols] <- 0 outside [0, rows_in) x [0, cols_in)
+int launch_mask_outside(cudaStream_t st, float* img, int rows, int cols, int rows_in, int cols_in, int nb);
 }

@@ -595,3 +595,49 @@ def test_exact_response_closed_forms_and_grid_limit():
     assert np.allclose(o.major_cycle_residual(uvg, w, dirty, x, my, mx), dirty - cx, atol=1e-10 * np.abs(cx).max())
     # off the grid the two differ (that difference is what the major cycle corrects)
     assert rel(o.exact_adjoint(uvs, w, o.exact_response(uvs, x, my, mx), ny, nx, my, mx), cx) > 1e-2
+
+
+# ---------------------------------------------------------------------------------- embedding (reading R19)
+def test_embedded_convolution_is_the_image_sized_convolution():
+    """A 12 x 10 image in a 16 x 16 embedding: the linear convolution with the 24 x 20 PSF, computed on the 32 x 32 padded
+    grid with the PSF copied to the offsets |d| < image size and zero elsewhere, equals the image-sized operator
+    (checked against the O(N^4) direct sum) -- any padding of at least twice the image computes Eq. 14 exactly."""
+    rng = np.random.default_rng(0)
+    nyi, nxi, ny, nx = 12, 10, 16, 16
+    w = wl.make_config(3, ny=nyi, nx=nxi, npts=400)
+    psf = o.psf_from_weights(w.w_half[0])                      # [24, 20]
+    x = rng.normal(size=(nyi, nxi))
+    ref = o.conv_direct(psf, x)
+    assert np.max(np.abs(o.psf_apply(w.w_half[0], x) - ref)) <= 1e-12 * np.max(np.abs(ref))
+    big = np.zeros((2 * ny, 2 * nx))
+    for dy in range(-nyi + 1, nyi):
+        for dx in range(-nxi + 1, nxi):
+            big[dy % (2 * ny), dx % (2 * nx)] = psf[dy % (2 * nyi), dx % (2 * nxi)]
+    wbig = np.fft.rfft2(big) / (4 * ny * nx)
+    assert np.max(np.abs(wbig.imag)) <= 1e-12 * np.max(np.abs(wbig.real))
+    got = o.psf_apply(wbig.real, o.embed(x, ny, nx))[:nyi, :nxi]
+    assert np.max(np.abs(got - ref)) <= 1e-12 * np.max(np.abs(ref))
+
+
+def test_embedded_energy_gradient_and_metric():
+    rng = np.random.default_rng(1)
+    nyi, nxi, ny, nx = 12, 10, 16, 16
+    w = wl.make_config(3, ny=nyi, nx=nxi, npts=400)
+    wf = wl.make_config(1, n=16)
+    amp, mu = wf.amp[0], float(np.log(np.median(w.sky_true)))
+    xi = 0.3 * rng.normal(size=(ny, nx))
+    e, g = o.energy_grad_embedded(w.w_half[0], w.dirty[0], amp, mu, xi)
+    for _ in range(3):
+        d = rng.normal(size=xi.shape)
+        h = 1e-5
+        fd = (o.energy_grad_embedded(w.w_half[0], w.dirty[0], amp, mu, xi + h * d)[0]
+              - o.energy_grad_embedded(w.w_half[0], w.dirty[0], amp, mu, xi - h * d)[0]) / (2 * h)
+        assert abs(fd - np.sum(g * d)) <= 1e-6 * max(abs(fd), np.linalg.norm(g))
+    u, v = rng.normal(size=xi.shape), rng.normal(size=xi.shape)
+    mu_, mv = (o.metric_apply_embedded(w.w_half[0], nyi, nxi, amp, mu, xi, t) for t in (u, v))
+    assert abs(np.sum(v * mu_) - np.sum(u * mv)) <= 1e-12 * abs(np.sum(v * mu_)) and np.sum(u * mu_) >= np.sum(u * u)
+    # image = embedding grid: the plain functions
+    w16 = wl.make_config(1, n=16)
+    e0, g0 = o.energy_grad(w16.w_half, w16.dirty, w16.amp, [mu], w16.lognu, xi[None])
+    e1, g1 = o.energy_grad_embedded(w16.w_half[0], w16.dirty[0], w16.amp[0], mu, xi)
+    assert abs(e0 - e1) <= 1e-12 * abs(e0) and np.max(np.abs(g0[0] - g1)) <= 1e-12 * np.max(np.abs(g1))
