@@ -10,7 +10,8 @@ Library primitives used as steps: numpy.fft (pinned in tests against the O(n^2) 
 out below and against the O(N^4) direct convolution), numpy.linalg.solve (CG pin only).
 
 Pins: tests/test_oracle_pins.py (every function, incl. sky / log_sky / channel_coeff through the
-hand-worked fixture tests/golden/hand_sky_two_fields.txt, and the Eq. 9 / Eq. 15-18 functions).
+hand-worked fixture tests/golden/hand_sky_two_fields.txt, the Eq. 9 / Eq. 15-18 functions, and the embedded
+(non-power-of-two) functions of reading R19 through the O(N^4) direct sum and finite differences).
 "parity unpinned": the absolute values of E and grad on real data -- the paper prints no operator
 value (last pin row); they are pinned only through the identities tested there.
 
