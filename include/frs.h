@@ -200,6 +200,29 @@ int frs_energy_grad_joint(frs_ctx* ctx, const float* xi, const float* theta, int
  * FRS_ESTATE without a joint position. */
 int frs_metric_apply_joint(frs_ctx* ctx, const float* dxi, const float* dtheta, int with_prior, float* out_xi, float* out_theta);
 
+/* ---- building blocks of composed sky models: several Gaussian processes on patches ("each of these sources with a
+ * separate exponentiated Gaussian process ... a third Gaussian process model for the background", Fig. 10; R20) ----
+ * s = sum_k insert_k( exp(mu_k + H_k[A_k xi_k]) ): one context per component (its own power-of-two grid, amplitude, offset) and
+ * one context of the full field that owns PSF, dirty image and likelihood.  These calls are the two halves the fused calls
+ * above combine; `PatchModel` in paper_2406_09144_b200/patches.py strings them together (no arithmetic in Python). */
+
+/* Likelihood energy (NO prior term) of a caller-supplied sky and its derivative with respect to the sky:
+ * mode 0: E = 1/2 <s, C s> - <j, s>, grad_sky = C s - j;  mode 1: E = 1/2 r^T N'^-1 r, grad_sky = -C N'^-1 r, r = j - C s.
+ * sky, grad_sky: device [nchan][ny][nx], natural orientation.  Sets the sky as frs_set_sky does.  h_energy: host double
+ * or NULL (non-NULL synchronises). */
+int frs_sky_energy_grad(frs_ctx* ctx, const float* sky, double* h_energy, float* grad_sky);
+/* Jacobian of one log-normal field at the cached position (frs_sky_forward), single channel, one field:
+ * dsky [ny][nx] = s . H[A v]   and   out [ny][nx] = A . H[s . w_sky] (+ add if non-NULL). */
+int frs_latent_jvp(frs_ctx* ctx, const float* v, float* dsky);
+int frs_latent_vjp(frs_ctx* ctx, const float* w_sky, const float* add, float* out);
+/* *h_out = <a, b> over n device floats (n a multiple of 4, 16-byte aligned), accumulated in fp64 in a fixed order (the prior
+ * terms 1/2 <xi_k, xi_k> of a composed model).  Synchronises. */
+int frs_dot(frs_ctx* ctx, const float* a, const float* b, long long n, double* h_out);
+/* field [ny][nx] of THIS context: field[y0 + y][x0 + x] += patch[y][x], patch [nyp][nxp]; and the crop patch = field[...].
+ * FRS_EINVAL if the patch does not lie inside the field. */
+int frs_patch_insert_add(frs_ctx* ctx, const float* patch, int nyp, int nxp, int y0, int x0, float* field);
+int frs_patch_crop(frs_ctx* ctx, const float* field, int nyp, int nxp, int y0, int x0, float* patch);
+
 /* ---- MGVI: posterior samples and the sample-averaged KL (reading R15) ------------
  * MGVI approximates the posterior by N(xi, M(xi)^-1), M the metric above, and minimises the KL estimated on samples
  * xi +- sigma_i, sigma_i ~ N(0, M^-1).  The random numbers are INPUTS (white N(0,1) arrays drawn by the caller). */

@@ -3,7 +3,8 @@
 NEXT-3 of SURVEY.md section 8(f): the learned amplitude spectrum of the diffuse-emission prior and the inverse-gamma
 point-source pixels (parameters of Table A.1 / B.1).  The paper defers the
 definitions to Arras et al. (2021a), which is not in the container, so what is written out here is the reading
-DESIGN.md lists as R17 (amplitude model) and R18 (point sources), in float64, in the order of that reading.
+DESIGN.md lists as R17 (amplitude model), R18 (point sources) and R20 (several GPs on patches), in float64, in the order
+of that reading.  Pins: tests/test_prior_oracle_pins.py.
 Shares no code with the CUDA path; imported only by tests/.
 
 R17 in one place (ny x nx harmonic grid, standard-normal latent vector theta):
@@ -305,3 +306,64 @@ def metric_apply_full(w_half_c, hyper, xi, theta_amp, pts, xi_pts, dxi, dtheta, 
     if with_prior:
         o_xi, o_th, o_pt = o_xi + dxi, o_th + np.asarray(dtheta, np.float64), o_pt + np.asarray(dpts, np.float64)
     return o_xi, o_th, o_pt
+
+
+# ----------------------------------------------------------------------------------------------- several GPs on patches (R20)
+# P:369 "We model each of these sources with a separate exponentiated Gaussian process ... a third Gaussian process model
+# to represent all the background sources" (Fig. 10: two source patches inside a background field).  Reading R20: component k
+# has its own grid (ny_k x nx_k), amplitude A_k, offset mu_k and excitations xi_k; its sky exp(mu_k + H_k[A_k xi_k]) is ADDED
+# into the full field at the patch position (y0_k, x0_k); the components may overlap (the background covers everything).
+#   s = sum_k insert_k( exp(mu_k + H_k[A_k xi_k]) ),   E = E_lh(s) + 1/2 sum_k <xi_k, xi_k>.
+# comps: list of (amp_k [ny_k, nx_k], mu_k, y0_k, x0_k).
+def sky_patches(comps, xis, ny, nx):
+    fo = _fo()
+    s = np.zeros((ny, nx))
+    parts = []
+    for (amp, mu, y0, x0), xi in zip(comps, xis):
+        sk = np.exp(mu + fo.hartley2(np.asarray(amp, np.float64) * np.asarray(xi, np.float64)))
+        parts.append(sk)
+        s[y0:y0 + sk.shape[0], x0:x0 + sk.shape[1]] += sk
+    return s, parts
+
+
+def _dE_ds(w_half_c, dirty, s, kern):
+    fo = _fo()
+    cs = fo.psf_apply(w_half_c, s)
+    if kern is None:
+        return 0.5 * np.sum(s * cs) - np.sum(np.asarray(dirty, np.float64) * s), cs - dirty
+    r = np.asarray(dirty, np.float64) - cs
+    u = fo.ninv_apply(kern, r)
+    return 0.5 * np.sum(r * u), -fo.psf_apply(w_half_c, u)
+
+
+def energy_grad_patches(w_half_c, dirty, comps, xis, with_prior=True, kern=None):
+    """E and the list of dE/dxi_k."""
+    fo = _fo()
+    ny, nx = dirty.shape
+    s, parts = sky_patches(comps, xis, ny, nx)
+    e, gs = _dE_ds(w_half_c, dirty, s, kern)
+    grads = []
+    for (amp, mu, y0, x0), xi, sk in zip(comps, xis, parts):
+        g = np.asarray(amp, np.float64) * fo.hartley2(sk * gs[y0:y0 + sk.shape[0], x0:x0 + sk.shape[1]])
+        if with_prior:
+            e += 0.5 * np.sum(np.asarray(xi, np.float64) ** 2)
+            g = g + xi
+        grads.append(g)
+    return float(e), grads
+
+
+def metric_apply_patches(w_half_c, ny, nx, comps, xis, vs, with_prior=True, kern=None):
+    """Fisher metric J^T C J (+ 1) (kern: J^T C N'^-1 C J) of the patch model applied to the list vs."""
+    fo = _fo()
+    _, parts = sky_patches(comps, xis, ny, nx)
+    ds = np.zeros((ny, nx))
+    for (amp, mu, y0, x0), v, sk in zip(comps, vs, parts):
+        ds[y0:y0 + sk.shape[0], x0:x0 + sk.shape[1]] += sk * fo.hartley2(np.asarray(amp, np.float64) * np.asarray(v, np.float64))
+    c = fo.psf_apply(w_half_c, ds)
+    if kern is not None:
+        c = fo.psf_apply(w_half_c, fo.ninv_apply(kern, c))
+    outs = []
+    for (amp, mu, y0, x0), v, sk in zip(comps, vs, parts):
+        o_ = np.asarray(amp, np.float64) * fo.hartley2(sk * c[y0:y0 + sk.shape[0], x0:x0 + sk.shape[1]])
+        outs.append(o_ + v if with_prior else o_)
+    return outs

@@ -42,6 +42,12 @@ EXPORTS = {
     "frs_ninv_apply": (_i, [_vp, _vp, _vp]),
     "frs_set_likelihood": (_i, [_vp, _i]),
     "frs_set_cuda_graphs": (_i, [_vp, _i]),
+    "frs_sky_energy_grad": (_i, [_vp, _vp, C.POINTER(_d), _vp]),
+    "frs_dot": (_i, [_vp, _vp, _vp, C.c_longlong, C.POINTER(_d)]),
+    "frs_latent_jvp": (_i, [_vp, _vp, _vp]),
+    "frs_latent_vjp": (_i, [_vp, _vp, _vp, _vp]),
+    "frs_patch_insert_add": (_i, [_vp, _vp, _i, _i, _i, _i, _vp]),
+    "frs_patch_crop": (_i, [_vp, _vp, _i, _i, _i, _i, _vp]),
     "frs_set_psf_embedded": (_i, [_vp, _vp, _i, _i]),
     "frs_set_field_of_view": (_i, [_vp, _i, _i]),
     "frs_amp_model_size": (_i, [_i, _i, C.POINTER(_i), C.POINTER(_i)]),
@@ -311,6 +317,35 @@ class Context:
 
     def set_field_of_view(self, ny_img, nx_img):
         self._ck(lib().frs_set_field_of_view(self._h, int(ny_img), int(nx_img)))
+
+    # ---- building blocks of composed sky models (several GPs on patches, reading R20)
+    def sky_energy_grad(self, sky, grad_sky):
+        e = _d(0.0)
+        self._ck(lib().frs_sky_energy_grad(self._h, _ptr(sky, self.f32, self.nchan * self.npix, "sky"), C.byref(e),
+                                           _ptr(grad_sky, self.f32, self.nchan * self.npix, "grad_sky")))
+        return e.value
+
+    def dot(self, a, b):
+        out = _d(0.0)
+        self._ck(lib().frs_dot(self._h, _ptr(a, self.f32, None, "a"), _ptr(b, self.f32, a.numel(), "b"), a.numel(), C.byref(out)))
+        return out.value
+
+    def latent_jvp(self, v, dsky):
+        self._ck(lib().frs_latent_jvp(self._h, _ptr(v, self.f32, self.npix, "v"), _ptr(dsky, self.f32, self.npix, "dsky")))
+
+    def latent_vjp(self, w_sky, out, add=None):
+        self._ck(lib().frs_latent_vjp(self._h, _ptr(w_sky, self.f32, self.npix, "w_sky"), _ptr(add, self.f32, self.npix, "add"),
+                                      _ptr(out, self.f32, self.npix, "out")))
+
+    def patch_insert_add(self, patch, y0, x0, field):
+        nyp, nxp = patch.shape[-2], patch.shape[-1]
+        self._ck(lib().frs_patch_insert_add(self._h, _ptr(patch, self.f32, nyp * nxp, "patch"), nyp, nxp, int(y0), int(x0),
+                                            _ptr(field, self.f32, self.npix, "field")))
+
+    def patch_crop(self, field, y0, x0, patch):
+        nyp, nxp = patch.shape[-2], patch.shape[-1]
+        self._ck(lib().frs_patch_crop(self._h, _ptr(field, self.f32, self.npix, "field"), nyp, nxp, int(y0), int(x0),
+                                      _ptr(patch, self.f32, nyp * nxp, "patch")))
 
     def set_cuda_graphs(self, on):
         self._ck(lib().frs_set_cuda_graphs(self._h, int(bool(on))))

@@ -166,6 +166,15 @@ __global__ void __launch_bounds__(kEwThreads) accumulate_kernel(float* __restric
     reinterpret_cast<float4*>(acc)[i] = a;
 }
 __global__ void set_delta_kernel(float* __restrict__ img, size_t npix, size_t pos) { img[blockIdx.x * npix + pos] = 1.0f; }
+// a *= b, n a multiple of 4
+__global__ void __launch_bounds__(kEwThreads) mul_inplace_kernel(float* __restrict__ a, const float* __restrict__ b, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i * 4 >= n) return;
+    float4 x = reinterpret_cast<float4*>(a)[i];
+    const float4 y = reinterpret_cast<const float4*>(b)[i];
+    x.x *= y.x; x.y *= y.y; x.z *= y.z; x.w *= y.w;
+    reinterpret_cast<float4*>(a)[i] = x;
+}
 // E = 0.5 <r, N'^-1 r> + 0.5 with_prior <xi, xi>
 __global__ void energy9_final_kernel(const double* __restrict__ ru, const double* __restrict__ xx, int with_prior,
                                      double* __restrict__ e) {

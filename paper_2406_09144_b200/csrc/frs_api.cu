@@ -1178,6 +1178,109 @@ int frs_metric_apply_joint(frs_ctx* ctx, const float* dxi, const float* dtheta, 
     return FRS_OK;
 }
 
+// ---- building blocks of composed sky models: several Gaussian processes on patches (reading R20) --------------
+// A composed model keeps one context per component (its own grid, amplitude and position) and one for the full field;
+// these calls expose the two halves the existing calls fuse: the sky-space derivative of the likelihood and the Jacobian
+// of one log-normal field.
+int frs_sky_energy_grad(frs_ctx* ctx, const float* sky, double* h_energy, float* grad_sky) {
+    if (!ctx || !sky || !grad_sky || !aligned16(sky) || !aligned16(grad_sky) || sky == grad_sky)
+        return fail(ctx, FRS_EINVAL, "frs_sky_energy_grad: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(frs_set_sky(ctx, sky));
+    RET(check_hot(ctx, true, false));
+    if (!ctx->have_dirty) return fail(ctx, FRS_ESTATE, "dirty image not set (frs_set_dirty)");
+    const Orient o = orient(ctx, false);
+    const size_t n = (size_t)ctx->nchan * ctx->npix;
+    const unsigned eg = (unsigned)((n / 4 + kEwThreads - 1) / kEwThreads);
+    RET(ensure_scratch9(ctx));
+    RET(conv_rows_fwd(ctx, o, ctx->s, nullptr));
+    RET(conv_cols(ctx, o));
+    RET(conv_rows_inv(ctx, o, ctx->img2, kResid, nullptr, ctx->dirty, nullptr));            // r = j - C s
+    if (ctx->lik_mode == 0) {
+        // E = 1/2 <s, C s> - <j, s> = -1/2 <s, r> - 1/2 <j, s>;  dE/ds = C s - j = -r
+        RET(dot(ctx, ctx->s, ctx->img2, n, ctx->scal + 8));
+        RET(dot(ctx, ctx->dirty, ctx->s, n, ctx->scal + 9));
+        accumulate_kernel<<<eg, kEwThreads, 0, ctx->stream>>>(grad_sky, ctx->img2, -1.0f, 1, n, nullptr, nullptr);
+        ctx->launches++;
+    } else {
+        // E = 1/2 r^T N'^-1 r;  dE/ds = -C N'^-1 r
+        if (!ctx->have_kern) return fail(ctx, FRS_ESTATE, "noise kernel not set (frs_set_noise_kernel)");
+        RET(hartley_t(ctx, ctx->img2, ctx->ny, ctx->nx, nullptr, ctx->img3, ctx->kinvT, nullptr, nullptr, ctx->nchan));
+        RET(hartley_t(ctx, ctx->img3, ctx->nx, ctx->ny, nullptr, ctx->img, nullptr, nullptr, nullptr, ctx->nchan));   // u
+        RET(dot(ctx, ctx->img2, ctx->img, n, ctx->scal + 8));
+        RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
+        RET(conv_cols(ctx, o));
+        RET(conv_rows_inv(ctx, o, ctx->img3, kPlain, nullptr, nullptr, nullptr));
+        accumulate_kernel<<<eg, kEwThreads, 0, ctx->stream>>>(grad_sky, ctx->img3, -1.0f, 1, n, nullptr, nullptr);
+        ctx->launches++;
+    }
+    CK(cudaGetLastError());
+    if (h_energy) {
+        double sc[2];
+        CK(cudaMemcpyAsync(sc, ctx->scal + 8, sizeof(sc), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        *h_energy = ctx->lik_mode == 0 ? -0.5 * sc[0] - 0.5 * sc[1] : 0.5 * sc[0];
+    }
+    return FRS_OK;
+}
+
+// dsky = s . H[A v] at the cached position (natural orientation)
+int frs_latent_jvp(frs_ctx* ctx, const float* v, float* dsky) {
+    if (!ctx || !v || !dsky || !aligned16(v) || !aligned16(dsky)) return fail(ctx, FRS_EINVAL, "frs_latent_jvp: bad argument");
+    if (ctx->nchan != 1 || ctx->nfield != 1) return fail(ctx, FRS_ESTATE, "frs_latent_jvp: single channel, one field");
+    CK(cudaSetDevice(ctx->device));
+    if (!ctx->have_amp || !ctx->have_s) return fail(ctx, FRS_ESTATE, "no position (frs_sky_forward)");
+    RET(ensure_scratch(ctx));
+    RET(need_s_transposed(ctx));
+    RET(hartley_t(ctx, v, ctx->ny, ctx->nx, ctx->amp, ctx->lin, nullptr, nullptr, nullptr, 1));      // [nx][ny]
+    mul_inplace_kernel<<<(unsigned)((ctx->npix / 4 + kEwThreads - 1) / kEwThreads), kEwThreads, 0, ctx->stream>>>(ctx->lin, ctx->sT, ctx->npix);
+    ctx->launches++;
+    RET(transpose(ctx, ctx->lin, dsky, ctx->nx, ctx->ny, 1));
+    return FRS_OK;
+}
+
+// out = A . H[s . w] (+ add) at the cached position; w in the natural orientation
+int frs_latent_vjp(frs_ctx* ctx, const float* w_sky, const float* add, float* out) {
+    if (!ctx || !w_sky || !out || !aligned16(w_sky) || !aligned16(out) || (add && !aligned16(add)))
+        return fail(ctx, FRS_EINVAL, "frs_latent_vjp: bad argument");
+    if (ctx->nchan != 1 || ctx->nfield != 1) return fail(ctx, FRS_ESTATE, "frs_latent_vjp: single channel, one field");
+    CK(cudaSetDevice(ctx->device));
+    if (!ctx->have_amp || !ctx->have_s) return fail(ctx, FRS_ESTATE, "no position (frs_sky_forward)");
+    RET(ensure_scratch(ctx));
+    RET(need_s_transposed(ctx));
+    RET(transpose(ctx, w_sky, ctx->img, ctx->ny, ctx->nx, 1));                                       // [nx][ny]
+    RET(hartley_t(ctx, ctx->img, ctx->nx, ctx->ny, ctx->sT, out, ctx->amp, add, nullptr, 1));
+    return FRS_OK;
+}
+
+// <a, b> over n floats (n a multiple of 4), accumulated in fp64 with the fixed-order reduction of the CG scalars
+int frs_dot(frs_ctx* ctx, const float* a, const float* b, long long n, double* h_out) {
+    if (!ctx || !a || !b || !h_out || n <= 0 || (n & 3) || !aligned16(a) || !aligned16(b)) return fail(ctx, FRS_EINVAL, "frs_dot: bad argument");
+    CK(cudaSetDevice(ctx->device));
+    RET(ensure_scratch(ctx));
+    RET(dot(ctx, a, b, (size_t)n, ctx->scal + 14));
+    CK(cudaMemcpyAsync(h_out, ctx->scal + 14, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return FRS_OK;
+}
+
+int frs_patch_insert_add(frs_ctx* ctx, const float* patch, int nyp, int nxp, int y0, int x0, float* field) {
+    if (!ctx || !patch || !field || nyp < 1 || nxp < 1 || y0 < 0 || x0 < 0 || y0 + nyp > ctx->ny || x0 + nxp > ctx->nx)
+        return fail(ctx, FRS_EINVAL, "frs_patch_insert_add: patch outside the field");
+    CK(cudaSetDevice(ctx->device));
+    CKL(launch_patch_copy(ctx->stream, field, ctx->ny, ctx->nx, const_cast<float*>(patch), nyp, nxp, y0, x0, 1));
+    ctx->launches++;
+    return FRS_OK;
+}
+int frs_patch_crop(frs_ctx* ctx, const float* field, int nyp, int nxp, int y0, int x0, float* patch) {
+    if (!ctx || !patch || !field || nyp < 1 || nxp < 1 || y0 < 0 || x0 < 0 || y0 + nyp > ctx->ny || x0 + nxp > ctx->nx)
+        return fail(ctx, FRS_EINVAL, "frs_patch_crop: patch outside the field");
+    CK(cudaSetDevice(ctx->device));
+    CKL(launch_patch_copy(ctx->stream, const_cast<float*>(field), ctx->ny, ctx->nx, patch, nyp, nxp, y0, x0, 0));
+    ctx->launches++;
+    return FRS_OK;
+}
+
 // ---- MGVI: posterior samples and the sample-averaged KL (reading R15) ------------------------
 static int latent_scratch(frs_ctx* ctx) {
     RET(dev_alloc(ctx, &ctx->lat1, 2 * ctx->npix));

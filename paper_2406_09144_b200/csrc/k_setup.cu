@@ -225,6 +225,18 @@ int launch_embed_psf(cudaStream_t st, const float* small, float* big, int nyi, i
     embed_psf_kernel<<<dim3(1184, nb), 256, 0, st>>>(small, big, nyi, nxi, ny, nx);
     return (int)cudaGetLastError();
 }
+__global__ void patch_copy_kernel(float* __restrict__ field, int nx, float* __restrict__ patch, int nyp, int nxp, int y0, int x0, int add) {
+    const size_t n = (size_t)nyp * nxp;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t f = (size_t)(y0 + i / nxp) * nx + x0 + i % nxp;
+        if (add) field[f] += patch[i]; else patch[i] = field[f];
+    }
+}
+int launch_patch_copy(cudaStream_t st, float* field, int ny, int nx, float* patch, int nyp, int nxp, int y0, int x0, int add) {
+    (void)ny;
+    patch_copy_kernel<<<592, 256, 0, st>>>(field, nx, patch, nyp, nxp, y0, x0, add);
+    return (int)cudaGetLastError();
+}
 __global__ void mask_outside_kernel(float* __restrict__ img, int rows, int cols, int rows_in, int cols_in) {
     float* b = img + (size_t)blockIdx.y * rows * cols;
     // the strip right of the kept block, then the rows below it: only what has to be zeroed is touched

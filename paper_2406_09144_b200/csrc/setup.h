@@ -11,6 +11,8 @@ int launch_transpose(cudaStream_t st, const float* in, float* out, int rows, int
 // Embedding of an image that is smaller than the grid (reading R19).
 // big [nb][2 ny][2 nx] <- small [nb][2 nyi][2 nxi]: the PSF copied to the offsets |dy| < nyi, |dx| < nxi (wrapped), zero elsewhere
 int launch_embed_psf(cudaStream_t st, const float* small, float* big, int nyi, int nxi, int ny, int nx, int nb);
+// field[y0 + y][x0 + x] += patch[y][x] (add = 1)  or  patch[y][x] = field[y0 + y][x0 + x] (add = 0); patch [nyp][nxp], field [ny][nx]
+int launch_patch_copy(cudaStream_t st, float* field, int ny, int nx, float* patch, int nyp, int nxp, int y0, int x0, int add);
 // img [nb][rows][cols] <- 0 outside [0, rows_in) x [0, cols_in)
 int launch_mask_outside(cudaStream_t st, float* img, int rows, int cols, int rows_in, int cols_in, int nb);
 }

@@ -4,6 +4,7 @@ import os
 
 import numpy as np
 
+from gen import workloads as wl
 from oracle import frs_oracle as fo
 from oracle import prior_oracle as po
 
@@ -223,3 +224,43 @@ def test_full_model_metric_symmetric_and_reduces_to_joint():
     m0 = po.metric_apply_full(w.w_half[0], hyper, xi, th, none, np.zeros(0), u[0], u[1], np.zeros(0))
     mj = po.metric_apply_joint(w.w_half[0], hyper, xi, th, u[0], u[1])
     assert np.array_equal(m0[0], mj[0]) and np.array_equal(m0[1], mj[1])
+
+
+# ---------------------------------------------------------------------------------- several GPs on patches (reading R20)
+def _patch_problem():
+    w = wl.make_config(1, n=32, seed=4)
+    rng = np.random.default_rng(9)
+    mu = float(np.log(np.median(w.sky_true)))
+    amp32 = w.amp[0]
+    amp16 = wl.make_config(1, n=16, seed=4).amp[0]
+    amp8x16 = wl.make_config(3, ny=8, nx=16, npts=300).amp[0]
+    comps = [(amp32, mu - 1.0, 0, 0), (amp16, mu, 4, 10), (amp8x16, mu + 0.5, 20, 2)]
+    xis = [0.3 * rng.normal(size=c[0].shape) for c in comps]
+    return w, comps, xis, rng
+
+
+def test_patch_model_gradient_metric_and_reduction():
+    w, comps, xis, rng = _patch_problem()
+    for kern in (None, fo.noise_kernel_from_psf(w.w_half[0], 1e-2 * float(fo.psf_from_weights(w.w_half[0])[0, 0]))):
+        e, gs = po.energy_grad_patches(w.w_half[0], w.dirty[0], comps, xis, True, kern)
+        ds = [rng.normal(size=x.shape) for x in xis]
+        h = 1e-5
+        ep = po.energy_grad_patches(w.w_half[0], w.dirty[0], comps, [x + h * d for x, d in zip(xis, ds)], True, kern)[0]
+        em = po.energy_grad_patches(w.w_half[0], w.dirty[0], comps, [x - h * d for x, d in zip(xis, ds)], True, kern)[0]
+        lin = sum(np.sum(g * d) for g, d in zip(gs, ds))
+        assert abs((ep - em) / (2 * h) - lin) <= 1e-6 * max(abs(lin), sum(np.linalg.norm(g) for g in gs))
+        us = [rng.normal(size=x.shape) for x in xis]
+        mu_ = po.metric_apply_patches(w.w_half[0], 32, 32, comps, xis, us, True, kern)
+        md = po.metric_apply_patches(w.w_half[0], 32, 32, comps, xis, ds, True, kern)
+        a, b = sum(np.sum(p * q) for p, q in zip(ds, mu_)), sum(np.sum(p * q) for p, q in zip(us, md))
+        assert abs(a - b) <= 1e-11 * abs(a)
+    # the sky is the sum of the inserted parts; one full-field component is the plain model of frs_oracle
+    s, parts = po.sky_patches(comps, xis, 32, 32)
+    ref = np.zeros((32, 32))
+    ref[:, :] += parts[0]
+    ref[4:20, 10:26] += parts[1]
+    ref[20:28, 2:18] += parts[2]
+    assert np.array_equal(s, ref)
+    e1, g1 = po.energy_grad_patches(w.w_half[0], w.dirty[0], comps[:1], xis[:1])
+    e0, g0 = fo.energy_grad(w.w_half, w.dirty, comps[0][0][None], [comps[0][1]], w.lognu, xis[0][None])
+    assert abs(e1 - e0) <= 1e-12 * abs(e0) and np.max(np.abs(g1[0] - g0[0])) <= 1e-12 * np.max(np.abs(g0))
