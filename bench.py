@@ -337,6 +337,17 @@ def run_cuda(args):
             m = timed(lambda i: ctx.metric_apply(v, out, True), k2, 3)
             extra["eq9_metric_apply_ms"] = m / k2
             ctx.set_likelihood(0)
+            if w.nchan == 1:
+                # learned amplitude spectrum (NEXT-3, reading R17): joint (xi, theta) energy + gradient and metric apply
+                ctx.set_amplitude_model((float(w.mu[0]), 1.0, 0.1, 1.0, 0.3, -3.0, 0.2, 0.5, 0.2, 0.2, 0.1))
+                th = dev(0.3 * rng.normal(size=ctx.ntheta))
+                gth, oth = torch.empty_like(th), torch.empty_like(th)
+                m = timed(lambda i: ctx.energy_grad_joint(xi, th, g, gth, True), k2, 3)
+                extra["joint_energy_grad_ms"] = m / k2
+                dth = dev(rng.normal(size=ctx.ntheta))
+                m = timed(lambda i: ctx.metric_apply_joint(v, dth, out, oth, True), k2, 3)
+                extra["joint_metric_apply_ms"] = m / k2
+                extra["joint_ntheta"] = int(ctx.ntheta)
 
     if world > 1:
         dist.barrier()
