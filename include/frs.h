@@ -261,6 +261,12 @@ int frs_major_cycle_residual(frs_ctx* ctx, const float* uv, const float* wgt, in
 /* y = s . C (s . x) with x, y in HOST memory (pinned or pageable), [nchan][ny][nx].
  * Copies x to the device, runs frs_sky_metric_apply, copies y back, synchronises. */
 int frs_sky_metric_apply_host(frs_ctx* ctx, const float* x_host, float* y_host);
+/* n independent applies y_k = s . C (s . x_k) with HOST buffers (x_hosts, y_hosts: host arrays of n host pointers; the
+ * buffers should be pinned, pageable memory makes the copies synchronous).  The copies of neighbouring items overlap the
+ * kernels: host -> device of item k + 1 and device -> host of item k - 1 run on two copy streams of the context while
+ * item k computes (two device buffers each way), so the throughput is that of the slowest of the three.  The same x or y
+ * buffer may appear again only two items later.  Synchronises at the end. */
+int frs_sky_metric_apply_host_batch(frs_ctx* ctx, int n, const float* const* x_hosts, float* const* y_hosts);
 /* y = C x with HOST buffers. */
 int frs_psf_apply_host(frs_ctx* ctx, const float* x_host, float* y_host);
 

@@ -66,6 +66,7 @@ EXPORTS = {
     "frs_major_cycle_residual": (_i, [_vp, _vp, _vp, _i, _vp, _vp, _vp]),
     "frs_sky_metric_apply_host": (_i, [_vp, _vp, _vp]),
     "frs_psf_apply_host": (_i, [_vp, _vp, _vp]),
+    "frs_sky_metric_apply_host_batch": (_i, [_vp, _i, C.POINTER(_vp), C.POINTER(_vp)]),
     "frs_launch_count": (C.c_longlong, [_vp]),
     "frs_profile_enable": (_i, [_vp, _i]),
     "frs_profile_read": (_i, [_vp, C.POINTER(_d), C.POINTER(C.c_longlong)]),
@@ -462,6 +463,14 @@ class Context:
     def sky_metric_apply_host(self, x_host, y_host):
         self._ck(lib().frs_sky_metric_apply_host(self._h, _vp(x_host.data_ptr()), _vp(y_host.data_ptr())))
         return y_host
+
+    def sky_metric_apply_host_batch(self, x_hosts, y_hosts):
+        """Lists of (pinned) CPU tensors; copies and kernels of neighbouring items overlap inside the library."""
+        n = len(x_hosts)
+        xs = (_vp * max(1, n))(*[x.data_ptr() for x in x_hosts])
+        ys = (_vp * max(1, n))(*[y.data_ptr() for y in y_hosts])
+        self._ck(lib().frs_sky_metric_apply_host_batch(self._h, n, xs, ys))
+        return y_hosts
 
     def psf_apply_host(self, x_host, y_host):
         self._ck(lib().frs_psf_apply_host(self._h, _vp(x_host.data_ptr()), _vp(y_host.data_ptr())))

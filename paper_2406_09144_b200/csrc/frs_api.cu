@@ -49,7 +49,9 @@ struct frs_ctx {
     bool have_kern = false;
     int lik_mode = 0;                // 0: N' = R' limit, 1: Eq. 9 with N'^-1 of Eq. 18
     float *cg_r = nullptr, *cg_p = nullptr, *cg_q = nullptr;
-    float *hx = nullptr, *hy = nullptr;
+    float *hx = nullptr, *hy = nullptr, *hx2 = nullptr, *hy2 = nullptr;
+    cudaStream_t s_in = nullptr, s_out = nullptr;      // copy streams of frs_sky_metric_apply_host_batch
+    cudaEvent_t ev_in[2] = {}, ev_comp[2] = {}, ev_out[2] = {};
     double *partials = nullptr, *scal = nullptr;   // scal: [0..7] CG, [8] sum s.c, [9] sum j.s, [10] <xi,xi>, [11] E
     int* flag = nullptr;
     bool have_psf = false, have_dirty = false, have_amp = false, have_s = false;
@@ -542,6 +544,12 @@ void frs_destroy(frs_ctx* ctx) {
         for (void* q : mp) if (q) cudaFree(q);
     }
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+    if (ctx->s_in) {
+        cudaStreamDestroy(ctx->s_in); cudaStreamDestroy(ctx->s_out);
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(ctx->ev_in[i]); cudaEventDestroy(ctx->ev_comp[i]); cudaEventDestroy(ctx->ev_out[i]); }
+    }
+    if (ctx->hx2) cudaFree(ctx->hx2);
+    if (ctx->hy2) cudaFree(ctx->hy2);
     delete ctx;
 }
 
@@ -1503,6 +1511,57 @@ static int host_apply(frs_ctx* ctx, const float* xh, float* yh, bool with_s) {
     return FRS_OK;
 }
 int frs_sky_metric_apply_host(frs_ctx* ctx, const float* x_host, float* y_host) { return host_apply(ctx, x_host, y_host, true); }
+
+// n independent applies with the copies of neighbouring items overlapping the kernels: host -> device of item k + 1 and
+// device -> host of item k - 1 run on two copy streams of the ctx's own while item k computes (two device buffers each way)
+int frs_sky_metric_apply_host_batch(frs_ctx* ctx, int n, const float* const* x_hosts, float* const* y_hosts) {
+    if (!ctx || n < 0 || (n > 0 && (!x_hosts || !y_hosts))) return fail(ctx, FRS_EINVAL, "frs_sky_metric_apply_host_batch: bad argument");
+    for (int k = 0; k < n; ++k)
+        if (!x_hosts[k] || !y_hosts[k]) return fail(ctx, FRS_EINVAL, "frs_sky_metric_apply_host_batch: null buffer");
+    CK(cudaSetDevice(ctx->device));
+    RET(check_hot(ctx, true, false));
+    const size_t cnt = (size_t)ctx->nchan * ctx->npix;
+    RET(dev_alloc(ctx, &ctx->hx, cnt));
+    RET(dev_alloc(ctx, &ctx->hy, cnt));
+    RET(dev_alloc(ctx, &ctx->hx2, cnt));
+    RET(dev_alloc(ctx, &ctx->hy2, cnt));
+    if (!ctx->s_in) {
+        CK(cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CK(cudaEventCreateWithFlags(&ctx->ev_in[i], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&ctx->ev_comp[i], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&ctx->ev_out[i], cudaEventDisableTiming));
+        }
+    }
+    RET(need_s_natural(ctx));
+    const Orient o = orient(ctx, false);
+    float* hx[2] = {ctx->hx, ctx->hx2};
+    float* hy[2] = {ctx->hy, ctx->hy2};
+    // everything enqueued so far on the ctx's stream (the sky, the spectrum) precedes the first copy
+    CK(cudaEventRecord(ctx->ev_comp[0], ctx->stream));
+    CK(cudaEventRecord(ctx->ev_comp[1], ctx->stream));
+    bool out_used[2] = {false, false};
+    for (int k = 0; k < n; ++k) {
+        const int b = k & 1;
+        CK(cudaStreamWaitEvent(ctx->s_in, ctx->ev_comp[b], 0));               // item k - 2 has read hx[b]
+        CK(cudaMemcpyAsync(hx[b], x_hosts[k], cnt * sizeof(float), cudaMemcpyHostToDevice, ctx->s_in));
+        CK(cudaEventRecord(ctx->ev_in[b], ctx->s_in));
+        CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_in[b], 0));
+        if (out_used[b]) CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_out[b], 0));   // item k - 2 has left hy[b]
+        RET(conv_rows_fwd(ctx, o, hx[b], ctx->s));
+        RET(conv_cols(ctx, o));
+        RET(conv_rows_inv(ctx, o, hy[b], kMulS, ctx->s, nullptr, nullptr));
+        CK(cudaEventRecord(ctx->ev_comp[b], ctx->stream));
+        CK(cudaStreamWaitEvent(ctx->s_out, ctx->ev_comp[b], 0));
+        CK(cudaMemcpyAsync(y_hosts[k], hy[b], cnt * sizeof(float), cudaMemcpyDeviceToHost, ctx->s_out));
+        CK(cudaEventRecord(ctx->ev_out[b], ctx->s_out));
+        out_used[b] = true;
+    }
+    CK(cudaStreamSynchronize(ctx->s_out));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return FRS_OK;
+}
 int frs_psf_apply_host(frs_ctx* ctx, const float* x_host, float* y_host) { return host_apply(ctx, x_host, y_host, false); }
 
 int frs_profile_enable(frs_ctx* ctx, int on) {

@@ -570,3 +570,30 @@ def test_tensor_core_stage_measurement_runs(frs):
     clk = frs.selftest_tcgen05_stage(64, 24, 500)
     assert 8.0 < clk < 1000.0
     print(f"tcgen05.mma kind::tf32 M=128 K=8 N=64: {clk:.1f} clk per instruction -> {24 * clk:.0f} clk per stage and column pair")
+
+
+def test_host_batch_apply_equals_single_calls(frs):
+    """frs_sky_metric_apply_host_batch overlaps copies and kernels of neighbouring items on its own streams: every result
+    must be bit-identical to the one-apply-per-call entry point, also when buffers are reused two items later."""
+    import torch
+    w = workload(("sq", 2, 512))
+    ctx = make_ctx(frs, w)
+    xi = (0.3 * np.random.default_rng(0).normal(size=(1, w.ny, w.nx))).astype(np.float32)
+    ctx.sky_forward(dev(xi))
+    rng = np.random.default_rng(1)
+    xs = [torch.from_numpy(rng.normal(size=(1, w.ny, w.nx)).astype(np.float32)).pin_memory() for _ in range(5)]
+    ref = []
+    for x in xs:
+        y = torch.empty_like(x).pin_memory()
+        ctx.sky_metric_apply_host(x, y)
+        ref.append(y.clone())
+    ys = [torch.empty_like(xs[0]).pin_memory() for _ in range(5)]
+    ctx.sky_metric_apply_host_batch(xs, ys)
+    assert all(torch.equal(a, b) for a, b in zip(ys, ref))
+    # two input and two output buffers rotated: the last two results survive
+    ctx.sky_metric_apply_host_batch([xs[0], xs[1], xs[2], xs[3]], [ys[0], ys[1], ys[0], ys[1]])
+    assert torch.equal(ys[0], ref[2]) and torch.equal(ys[1], ref[3])
+    ctx.sky_metric_apply_host_batch([], [])
+    y_dev = ctx.new_image()
+    ctx.sky_metric_apply(xs[4].cuda(), y_dev)
+    assert torch.equal(y_dev.cpu(), ref[4])
