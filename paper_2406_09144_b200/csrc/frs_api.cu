@@ -57,7 +57,8 @@ struct frs_ctx {
     bool have_psf = false, have_dirty = false, have_amp = false, have_s = false;
     long long launches = 0;
     // one CG iteration captured as a CUDA graph (cg_solve_impl): replayed while the key (every frozen argument) matches
-    struct CgGraphKey { const float* x; int with_prior, nfield, lik_mode; double* hist; double rtol2; bool sT_ok; } cg_key = {};
+    struct CgGraphKey { const float* x; int with_prior, nfield, lik_mode; double* hist; double rtol2; bool sT_ok; long long epoch; } cg_key = {};
+    long long cfg_epoch = 0;           // bumped by every setter that can change the launch sequence of an iteration
     cudaGraphExec_t cg_exec = nullptr;
     cudaStream_t cap_stream = nullptr;  // capture runs on a stream of the ctx's own (the caller's may be the legacy default stream)
     long long cg_graph_launches = 0;   // kernels per replay
@@ -570,6 +571,7 @@ static int build_transposed_weights(frs_ctx* ctx) {
 }
 
 int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !w_half || !aligned16(w_half)) return fail(ctx, FRS_EINVAL, "frs_set_psf_weights: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(dev_alloc(ctx, &ctx->wt, (size_t)ctx->nchan * ctx->ntile * 2 * ctx->ny * 2));
@@ -592,12 +594,14 @@ int frs_set_psf_weights(frs_ctx* ctx, const float* w_half) {
 
 static int set_psf_impl(frs_ctx* ctx, const float* psf, bool covariance);
 int frs_set_psf(frs_ctx* ctx, const float* psf) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !psf || !aligned16(psf)) return fail(ctx, FRS_EINVAL, "frs_set_psf: bad argument");
     CK(cudaSetDevice(ctx->device));
     return set_psf_impl(ctx, psf, true);
 }
 
 int frs_set_field_of_view(frs_ctx* ctx, int ny_img, int nx_img) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || ny_img < 1 || nx_img < 1 || ny_img > ctx->ny || nx_img > ctx->nx)
         return fail(ctx, FRS_EINVAL, "frs_set_field_of_view: bad argument");
     const bool whole = ny_img == ctx->ny && nx_img == ctx->nx;
@@ -609,6 +613,7 @@ int frs_set_field_of_view(frs_ctx* ctx, int ny_img, int nx_img) {
 }
 
 int frs_set_psf_embedded(frs_ctx* ctx, const float* psf_img, int ny_img, int nx_img) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !psf_img || !aligned16(psf_img) || ny_img < 1 || nx_img < 1 || ny_img > ctx->ny || nx_img > ctx->nx)
         return fail(ctx, FRS_EINVAL, "frs_set_psf_embedded: bad argument");
     CK(cudaSetDevice(ctx->device));
@@ -688,6 +693,7 @@ int frs_set_dirty(frs_ctx* ctx, const float* j) {
 }
 
 int frs_set_amplitude(frs_ctx* ctx, int nfield, const float* amp, const float* mu_host) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !amp || !mu_host || !aligned16(amp) || nfield < 1 || nfield > 2)
         return fail(ctx, FRS_EINVAL, "frs_set_amplitude: bad argument");
     CK(cudaSetDevice(ctx->device));
@@ -704,6 +710,7 @@ int frs_set_amplitude(frs_ctx* ctx, int nfield, const float* amp, const float* m
 }
 
 int frs_set_channel_lognu(frs_ctx* ctx, const float* lognu_host) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !lognu_host) return fail(ctx, FRS_EINVAL, "frs_set_channel_lognu: bad argument");
     CK(cudaSetDevice(ctx->device));
     CK(cudaMemcpyAsync(ctx->d_lognu, lognu_host, ctx->nchan * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
@@ -713,6 +720,7 @@ int frs_set_channel_lognu(frs_ctx* ctx, const float* lognu_host) {
 }
 
 int frs_set_sky(frs_ctx* ctx, const float* sky) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !sky || !aligned16(sky)) return fail(ctx, FRS_EINVAL, "frs_set_sky: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(ensure_scratch(ctx));
@@ -951,10 +959,10 @@ static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, f
     }
     const bool graphs = ctx->use_graphs && !ctx->profiling && max_iter - it >= 2;
     if (graphs) {
-        const frs_ctx::CgGraphKey key = {x, with_prior, ctx->nfield, ctx->lik_mode, d_res_history, rtol2, ctx->sT_ok};
+        const frs_ctx::CgGraphKey key = {x, with_prior, ctx->nfield, ctx->lik_mode, d_res_history, rtol2, ctx->sT_ok, ctx->cfg_epoch};
         const frs_ctx::CgGraphKey& k0 = ctx->cg_key;
         const bool same = ctx->cg_exec && k0.x == key.x && k0.with_prior == key.with_prior && k0.nfield == key.nfield &&
-                          k0.lik_mode == key.lik_mode && k0.hist == key.hist && k0.rtol2 == key.rtol2 && k0.sT_ok == key.sT_ok;
+                          k0.lik_mode == key.lik_mode && k0.hist == key.hist && k0.rtol2 == key.rtol2 && k0.sT_ok == key.sT_ok && k0.epoch == key.epoch;
         if (!same) {
             if (ctx->cg_exec) { cudaGraphExecDestroy(ctx->cg_exec); ctx->cg_exec = nullptr; }
             cudaGraph_t g = nullptr;
@@ -1009,6 +1017,7 @@ int frs_amp_model_size(int ny, int nx, int* nb, int* ntheta) {
 }
 
 int frs_set_amplitude_model(frs_ctx* ctx, const float* hyper_host) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !hyper_host) return fail(ctx, FRS_EINVAL, "frs_set_amplitude_model: bad argument");
     if (ctx->nchan != 1) return fail(ctx, FRS_ESTATE, "frs_set_amplitude_model: single-channel contexts only");
     // means of the log-normal parameters must be positive, every standard deviation non-negative
@@ -1093,6 +1102,7 @@ int frs_amplitude_vjp(frs_ctx* ctx, const float* g_amp, float* g_theta) {
 }
 
 int frs_set_point_sources(frs_ctx* ctx, int npts, const int* yx_host, float alpha, float q) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || npts < 0 || npts > kMaxPoints || (npts > 0 && (!yx_host || !(alpha > 0.f) || !(q > 0.f))))
         return fail(ctx, FRS_EINVAL, "frs_set_point_sources: bad argument");
     if (ctx->nchan != 1) return fail(ctx, FRS_ESTATE, "frs_set_point_sources: single-channel contexts only");
@@ -1427,6 +1437,7 @@ static int kernel_arrays(frs_ctx* ctx) {
 }
 
 int frs_set_noise_kernel(frs_ctx* ctx, float eps) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !(eps > 0.f)) return fail(ctx, FRS_EINVAL, "frs_set_noise_kernel: eps must be > 0");
     CK(cudaSetDevice(ctx->device));
     RET(check_hot(ctx, false, false));
@@ -1450,6 +1461,7 @@ int frs_set_noise_kernel(frs_ctx* ctx, float eps) {
 }
 
 int frs_set_noise_kernel_array(frs_ctx* ctx, const float* kern) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || !kern || !aligned16(kern)) return fail(ctx, FRS_EINVAL, "frs_set_noise_kernel_array: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(ensure_scratch(ctx));
@@ -1487,6 +1499,7 @@ int frs_ninv_apply(frs_ctx* ctx, const float* x, float* y) {
 }
 
 int frs_set_likelihood(frs_ctx* ctx, int mode) {
+    if (ctx) ctx->cfg_epoch++;
     if (!ctx || (mode != 0 && mode != 1)) return fail(ctx, FRS_EINVAL, "frs_set_likelihood: mode must be 0 or 1");
     if (mode == 1 && !ctx->have_kern) return fail(ctx, FRS_ESTATE, "noise kernel not set (frs_set_noise_kernel)");
     ctx->lik_mode = mode;

@@ -229,3 +229,31 @@ def test_point_source_argument_errors(frs):
     with pytest.raises(frs.FrsError):
         ctx.set_point_sources([[1, 1]], 0.0, 1.0)
     ctx.set_point_sources([], 0.5, 1.0)
+
+
+def test_cg_graph_is_rebuilt_when_the_model_changes(frs):
+    """The captured CG iteration freezes the launch sequence; adding point sources changes it (two patch kernels per
+    apply): the same solve into the same x must match plain launches bit for bit after the change."""
+    import torch
+    w, hyper, xi, th, rng = _problem(128)
+    ctx = frs.Context(w.ny, w.nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    ctx.set_amplitude_model(hyper)
+    gx, gt = torch.empty(1, w.ny, w.nx, device="cuda"), torch.empty(ctx.ntheta, device="cuda")
+    ctx.energy_grad_joint(dev(xi[None]), dev(th), gx, gt)
+    b = (-gx).contiguous()
+    x = torch.zeros_like(b)
+    ctx.cg_solve(b, x, 8)
+    x1 = x.clone()
+    ctx.set_point_sources([[64, 64], [10, 100]], 0.5, 0.05 * float(np.median(w.sky_true)))
+    theta = torch.cat([dev(th), dev(np.array([1.5, 2.0], np.float32))])
+    gt2 = torch.empty(theta.numel(), device="cuda")
+    ctx.energy_grad_joint(dev(xi[None]), theta, gx, gt2)
+    x.zero_()
+    ctx.cg_solve(b, x, 8)                      # same x pointer, same arguments: only the model changed
+    x2 = x.clone()
+    ctx.set_cuda_graphs(False)
+    x.zero_()
+    ctx.cg_solve(b, x, 8)
+    assert torch.equal(x, x2) and not torch.equal(x1, x2)
