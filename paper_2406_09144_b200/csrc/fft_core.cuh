@@ -3,9 +3,13 @@
 // Each thread owns kE = 16 complex elements of an N-point transform in the CANONICAL
 // distribution  reg e  <->  position p + e*P  (p = thread index inside the group).  A stage of
 // radix R does 16/R butterflies per thread fully in registers; between stages the group
-// exchanges through a padded shared-memory buffer (pad 1 float2 per 16 -> conflict-free 64-bit
-// accesses).  Input and output are both in natural order
-// in the canonical distribution, so forward -> pointwise -> inverse needs no reordering.
+// exchanges through a padded shared-memory buffer: one float4 slot per position (the pair of transforms a
+// thread carries), one slot of padding per 16 (xpad).  The scatters and gathers of the stages are free of bank
+// conflicts; a phase of 8 lanes that straddles a padding step is not -- that is the case for the mirror reads
+// Z[N - k] of the row passes (kernels.cuh), whose phases are offset by one position: 2-way conflicts in half of
+// their phases, 7 % of the shared-memory wavefronts of rows_fwd (profiles/r2_l1_apply_ncu.md, source page).
+// Input and output are both in natural order in the canonical distribution, so forward -> pointwise -> inverse
+// needs no reordering.
 //
 // The stage arithmetic is __host__ __device__: csrc/selftest.cu replays it thread by thread on
 // the CPU so that the index maps and twiddle tables are tested without a GPU.
