@@ -5,9 +5,9 @@
 // radix R does 16/R butterflies per thread fully in registers; between stages the group
 // exchanges through a padded shared-memory buffer: one float4 slot per position (the pair of transforms a
 // thread carries), one slot of padding per 16 (xpad).  The scatters and gathers of the stages are free of bank
-// conflicts; a phase of 8 lanes that straddles a padding step is not -- that is the case for the mirror reads
-// Z[N - k] of the row passes (kernels.cuh), whose phases are offset by one position: 2-way conflicts in half of
-// their phases, 7 % of the shared-memory wavefronts of rows_fwd (profiles/r2_l1_apply_ncu.md, source page).
+// conflicts; a phase of 8 lanes that straddles a padding step is not -- which is why the mirror reads Z[N - k] of
+// rows_fwd (kernels.cuh), whose phases are offset by one position, go through a DENSE parking layout instead (in the
+// padded one they conflicted 2-way in half of their phases: 7 % of that kernel's shared-memory wavefronts).
 // Input and output are both in natural order in the canonical distribution, so forward -> pointwise -> inverse
 // needs no reordering.
 //

@@ -205,14 +205,18 @@ rows_fwd_kernel(RowsFwdArgs a) {
             }
         }
         pair_fft<NF, false>(v, p, buf, tws, gb);
-        canon_scatter2<NF>(v, p, buf);            // park Z: slot xpad(k) = Z_0[k], Z_1[k]
+        // park Z DENSELY: slot k = (Z_0[k], Z_1[k]).  The mirror reads below walk the slots downwards in phases of 8 lanes that
+        // are offset by one position; in the padded layout of the exchanges such a phase straddles a padding step and
+        // conflicts 2-way (7 % of this kernel's shared-memory wavefronts, profiles/); any 8 consecutive dense slots do not
+#pragma unroll
+        for (int e = 0; e < kE; ++e) buf[p + e * P] = pack(v[e]);
         gb.sync();
         // X[k] scale = (Z[k] + conj Z[NF-k]) - i twist[k] (Z[k] - conj Z[NF-k]),  k = p + e P (and k = NF from Z[0])
         C2 xn = c2zero();
 #pragma unroll
         for (int e = 0; e < kE; ++e) {
             const int k = p + e * P;
-            const C2 zm = unpack(buf[xpad((NF - k) & (NF - 1))]);
+            const C2 zm = unpack(buf[(NF - k) & (NF - 1)]);
             const float2 w0 = __ldg(a.twist + k);
             const float2 w = make_float2(w0.x * a.scale, w0.y * a.scale);     // the output scale rides on the twist ...
             const float2 sc = f2bc(a.scale);                                  // ... and on one fma per component
