@@ -278,6 +278,11 @@ long long frs_launch_count(const frs_ctx* ctx);
  * synchronises and returns accumulated milliseconds and launch counts per pass kind:
  * 0 rows_fwd (conv), 1 conv_cols, 2 rows_inv, 3 rows_fwd (Hartley), 4 hart_cols.  Resets on read. */
 int frs_profile_enable(frs_ctx* ctx, int on);
+/* Debug aid (compute-sanitizer is not available on every pool): with the environment variable FRS_GUARD=1 set when
+ * frs_create runs, every array the context owns is allocated between two 4 KB guard zones filled with a byte pattern.
+ * Returns the number of arrays whose guard zones have been written to (0 = clean; -1 on error), *n_arrays (may be NULL) the
+ * number of arrays under guard (0 without FRS_GUARD).  Synchronises the device. */
+int frs_debug_check_guards(frs_ctx* ctx, int* n_arrays);
 int frs_profile_read(frs_ctx* ctx, double ms[5], long long launches[5]);
 
 /* ---- self-test of host-replayable index logic (no GPU needed) -------------------------------- */

@@ -69,6 +69,7 @@ EXPORTS = {
     "frs_sky_metric_apply_host_batch": (_i, [_vp, _i, C.POINTER(_vp), C.POINTER(_vp)]),
     "frs_launch_count": (C.c_longlong, [_vp]),
     "frs_profile_enable": (_i, [_vp, _i]),
+    "frs_debug_check_guards": (_i, [_vp, C.POINTER(_i)]),
     "frs_profile_read": (_i, [_vp, C.POINTER(_d), C.POINTER(C.c_longlong)]),
     "frs_selftest_fft_host": (_i, [_i, _i, _vp, _vp]),
     "frs_selftest_tma_geometry": (_i, [_i, _i, C.POINTER(_i)]),
@@ -475,6 +476,14 @@ class Context:
     def psf_apply_host(self, x_host, y_host):
         self._ck(lib().frs_psf_apply_host(self._h, _vp(x_host.data_ptr()), _vp(y_host.data_ptr())))
         return y_host
+
+    def check_guards(self):
+        """(arrays with a corrupted guard zone, arrays under guard); needs FRS_GUARD=1 in the environment at construction."""
+        n = _i(0)
+        bad = lib().frs_debug_check_guards(self._h, C.byref(n))
+        if bad < 0:
+            raise FrsError(-1, "frs_debug_check_guards")
+        return bad, n.value
 
     # ---- instrumentation
     def launch_count(self):

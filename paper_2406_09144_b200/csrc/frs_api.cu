@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <vector>
@@ -54,6 +55,9 @@ struct frs_ctx {
     cudaEvent_t ev_in[2] = {}, ev_comp[2] = {}, ev_out[2] = {};
     double *partials = nullptr, *scal = nullptr;   // scal: [0..7] CG, [8] sum s.c, [9] sum j.s, [10] <xi,xi>, [11] E
     int* flag = nullptr;
+    bool guard = false;                // FRS_GUARD=1: guard zones around every ctx-owned array
+    struct Guard { char* base; size_t used, padded; };
+    std::vector<Guard> guards;
     bool have_psf = false, have_dirty = false, have_amp = false, have_s = false;
     long long launches = 0;
     // one CG iteration captured as a CUDA graph (cg_solve_impl): replayed while the key (every frozen argument) matches
@@ -121,11 +125,32 @@ struct Prof {
     }
 };
 
+// Guard zones (debug; the environment variable FRS_GUARD=1 at frs_create): every ctx-owned array gets kGuardBytes of a
+// byte pattern in front of and behind it, and frs_debug_check_guards counts the arrays whose pattern was touched -- the
+// stand-in for compute-sanitizer memcheck, which is closed on the GPU pool (profiles/r2_sanitizer.md).
+constexpr size_t kGuardBytes = 4096;
+constexpr int kGuardByte = 0xA5;
 template <typename T>
 int dev_alloc(frs_ctx* ctx, T** p, size_t count) {
     if (*p) return FRS_OK;
-    CK(cudaMalloc(reinterpret_cast<void**>(p), count * sizeof(T)));
+    if (!ctx->guard) {
+        CK(cudaMalloc(reinterpret_cast<void**>(p), count * sizeof(T)));
+        return FRS_OK;
+    }
+    const size_t bytes = (count * sizeof(T) + 255) & ~(size_t)255;
+    char* base = nullptr;
+    CK(cudaMalloc(reinterpret_cast<void**>(&base), bytes + 2 * kGuardBytes));
+    CK(cudaMemset(base, kGuardByte, kGuardBytes));
+    CK(cudaMemset(base + kGuardBytes + count * sizeof(T), kGuardByte, bytes - count * sizeof(T) + kGuardBytes));
+    *p = reinterpret_cast<T*>(base + kGuardBytes);
+    ctx->guards.push_back({base, count * sizeof(T), bytes});
     return FRS_OK;
+}
+void dev_free(frs_ctx* ctx, void* p) {
+    if (!p) return;
+    for (auto& g : ctx->guards)
+        if (g.base + kGuardBytes == p) { cudaFree(g.base); g.base = nullptr; return; }
+    cudaFree(p);
 }
 
 int ensure_tables(frs_ctx* ctx, int n) {
@@ -499,6 +524,7 @@ int frs_create(int ny, int nx, int nchan, int device, void* stream, frs_ctx** ou
     frs_ctx* ctx = new frs_ctx();
     ctx->ny = ny; ctx->nx = nx; ctx->nchan = nchan; ctx->device = device;
     ctx->stream = reinterpret_cast<cudaStream_t>(stream);
+    { const char* e = getenv("FRS_GUARD"); ctx->guard = e && e[0] == '1'; }
     ctx->npix = (size_t)ny * nx;
     ctx->ntile = nx / 2 + 1;
     ctx->ntile_h = nx / 4 + 1;
@@ -533,24 +559,24 @@ void frs_destroy(frs_ctx* ctx) {
     for (auto& kv : ctx->twist) cudaFree(kv.second);
     void* ptrs[] = {ctx->visbuf, ctx->kern, ctx->kinvN, ctx->kinvT, ctx->kisqN, ctx->lat1, ctx->lat2, ctx->img2, ctx->img3, ctx->wt, ctx->wtT, ctx->dirty, ctx->dirtyT, ctx->amp, ctx->s, ctx->sT, ctx->d_mu, ctx->d_lognu, ctx->T, ctx->T2, ctx->Th, ctx->lin, ctx->img,
                     ctx->acc, ctx->cg_r, ctx->cg_p, ctx->cg_q, ctx->hx, ctx->hy, ctx->partials, ctx->scal, ctx->flag};
-    for (void* p : ptrs) if (p) cudaFree(p);
+    for (void* p : ptrs) dev_free(ctx, p);
     for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     if (ctx->cg_exec) cudaGraphExecDestroy(ctx->cg_exec);
     {
         AmpModel& m = ctx->am;
         PointSources& ps = ctx->pts;
         void* pp[] = {ps.idx, ps.xi, ps.out, ps.flux, ps.dflux, ps.sdiff, ps.stot};
-        for (void* q : pp) if (q) cudaFree(q);
+        for (void* q : pp) dev_free(ctx, q);
         void* mp[] = {m.pindex, m.mult, m.d_hyper, m.theta, m.ab, m.wn, m.abf, m.dabf, m.gbin, m.work, m.sc, m.xi};
-        for (void* q : mp) if (q) cudaFree(q);
+        for (void* q : mp) dev_free(ctx, q);
     }
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     if (ctx->s_in) {
         cudaStreamDestroy(ctx->s_in); cudaStreamDestroy(ctx->s_out);
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(ctx->ev_in[i]); cudaEventDestroy(ctx->ev_comp[i]); cudaEventDestroy(ctx->ev_out[i]); }
     }
-    if (ctx->hx2) cudaFree(ctx->hx2);
-    if (ctx->hy2) cudaFree(ctx->hy2);
+    dev_free(ctx, ctx->hx2);
+    dev_free(ctx, ctx->hy2);
     delete ctx;
 }
 
@@ -1414,7 +1440,7 @@ int frs_major_cycle_residual(frs_ctx* ctx, const float* uv, const float* wgt, in
     if (!wgt || !dirty_full || !sky || !d_next) return fail(ctx, FRS_EINVAL, "frs_major_cycle_residual: bad argument");
     CK(cudaSetDevice(ctx->device));
     if (ctx->visbuf_n < (size_t)nvis) {
-        if (ctx->visbuf) CK(cudaFree(ctx->visbuf));
+        if (ctx->visbuf) dev_free(ctx, ctx->visbuf);
         ctx->visbuf = nullptr;
         CK(cudaMalloc(reinterpret_cast<void**>(&ctx->visbuf), (size_t)nvis * 2 * sizeof(float)));
         ctx->visbuf_n = (size_t)nvis;
@@ -1576,6 +1602,28 @@ int frs_sky_metric_apply_host_batch(frs_ctx* ctx, int n, const float* const* x_h
     return FRS_OK;
 }
 int frs_psf_apply_host(frs_ctx* ctx, const float* x_host, float* y_host) { return host_apply(ctx, x_host, y_host, false); }
+
+// number of ctx-owned arrays whose guard zones were written to (0 without FRS_GUARD=1); *n_arrays: arrays under guard
+int frs_debug_check_guards(frs_ctx* ctx, int* n_arrays) {
+    if (!ctx) return -1;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaDeviceSynchronize());
+    int bad = 0, n = 0;
+    std::vector<unsigned char> h;
+    for (const auto& g : ctx->guards) {
+        if (!g.base) continue;
+        ++n;
+        const size_t tail = g.padded - g.used + kGuardBytes;
+        h.resize(kGuardBytes + tail);
+        if (cudaMemcpy(h.data(), g.base, kGuardBytes, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+        if (cudaMemcpy(h.data() + kGuardBytes, g.base + kGuardBytes + g.used, tail, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+        bool ok = true;
+        for (unsigned char c : h) ok = ok && c == (unsigned char)kGuardByte;
+        if (!ok) ++bad;
+    }
+    if (n_arrays) *n_arrays = n;
+    return bad;
+}
 
 int frs_profile_enable(frs_ctx* ctx, int on) {
     if (!ctx) return FRS_EINVAL;

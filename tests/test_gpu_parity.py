@@ -468,10 +468,12 @@ def _check_l2_apply_and_one_cg_step(frs, ctx, w, xi, s32):
 
 # ---------------------------------------------------------------------------------- full-size configs
 @pytest.mark.parametrize("cfg", [3, 4])
-def test_full_size_config_parity(frs, cfg):
+def test_full_size_config_parity(frs, cfg, monkeypatch):
     """BASELINE.json configs 3 and 4 at full size, in the launch configuration bench.py times:
-    sky, C s (through the L1 apply) and gradient against the full fp64 oracle."""
+    sky, C s (through the L1 apply) and gradient against the full fp64 oracle.  The context runs with guard zones around
+    every array it owns (FRS_GUARD, the stand-in for memcheck): none may be touched at these launch shapes."""
     import torch
+    monkeypatch.setenv("FRS_GUARD", "1")
     w = wl.make_config(cfg)
     ctx = make_ctx(frs, w)
     xi = (0.5 * np.random.default_rng(6).normal(size=(1, w.ny, w.nx))).astype(np.float32)
@@ -491,12 +493,15 @@ def test_full_size_config_parity(frs, cfg):
     assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
     assert rel(g.cpu().numpy(), g_ref) <= TOL
     _check_l2_apply_and_one_cg_step(frs, ctx, w, xi, s32)
+    bad, n = ctx.check_guards()
+    assert bad == 0 and n >= 10, (bad, n)
     del ctx
     torch.cuda.empty_cache()
 
 
-def test_config5_multichannel_parity(frs):
-    """config 5 (16 x 1024^2, two latent fields): per-channel L1 apply and the gradient."""
+def test_config5_multichannel_parity(frs, monkeypatch):
+    """config 5 (16 x 1024^2, two latent fields): per-channel L1 apply and the gradient (guard zones on, as above)."""
+    monkeypatch.setenv("FRS_GUARD", "1")
     w = wl.make_config(5)
     ctx = make_ctx(frs, w)
     xi = (0.5 * np.random.default_rng(8).normal(size=(2, w.ny, w.nx))).astype(np.float32)
@@ -517,6 +522,8 @@ def test_config5_multichannel_parity(frs):
     assert abs(e - e_ref) <= 1e-5 * abs(e_ref)
     assert rel(g.cpu().numpy(), g_ref) <= TOL
     _check_l2_apply_and_one_cg_step(frs, ctx, w, xi, s32)
+    bad, n = ctx.check_guards()
+    assert bad == 0 and n >= 10, (bad, n)
 
 
 def test_config2_as_stated_outer_steps_teacher_forced(frs):
