@@ -6,6 +6,14 @@
  * Citations `P:<n>` are lines of the paper text; `R<k>` are the
  * readings listed in DESIGN.md for points the paper leaves open.
  *
+ * That energy is Eq. 9 of the paper in the limit N' = R' (likelihood mode 0, the default and the one the headline
+ * benchmark times: one padded PSF convolution per metric apply).  The paper's literal likelihood with the separately
+ * fitted noise kernel (Eq. 15-18: three convolutions per metric apply) is mode 1, frs_set_likelihood.  Further families of
+ * calls, each in its own section below: MGVI samples and the sample-averaged KL; the major-cycle residual with an exact
+ * response on uv points; the learned amplitude spectrum with the joint latent vector (xi, theta) and inverse-gamma
+ * point-source pixels; building blocks for several Gaussian processes on patches; images that are not a power of two by
+ * embedding; host-buffer entry points; instrumentation and self-tests.
+ *
  * Conventions (all calls)
  *   - frs_ctx owns the PSF spectrum, dirty image, amplitude spectra, the cached sky of the current
  *     position and all scratch.  The caller owns every array it passes; set_* calls COPY.
