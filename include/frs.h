@@ -127,6 +127,11 @@ int frs_cg_solve(frs_ctx* ctx, const float* b, float* x, int max_iter, float rto
  * launches throughout: what the profiling events of frs_profile_enable need, and the comparison arm of bench.py).
  * The results are the same kernels on the same data either way.  Default: on. */
 int frs_set_cuda_graphs(frs_ctx* ctx, int on);
+/* In the latent-space calls (single channel, one field, no point sources, row length 1024 .. 4096) the last pass of the
+ * convolution and the row pass of the Hartley transform that follows run as ONE kernel: s . C(...) goes from registers
+ * straight into the half-length row transform instead of through memory.  on = 0: the two separate passes (same
+ * arithmetic; the fp64 energy sums are added in another order).  Default: on. */
+int frs_set_fused_passes(frs_ctx* ctx, int on);
 /* Copy out the CG state of the last frs_cg_solve / frs_cg_step: r, p, q (DEVICE pointers,
  * [nfield][ny][nx] each, any may be NULL) and the scalar block scal_host (HOST double[8], may be NULL:
  * rr, pq, rr_new, alpha, beta, breakdown, bb, -).  Synchronises. */

@@ -42,6 +42,7 @@ EXPORTS = {
     "frs_ninv_apply": (_i, [_vp, _vp, _vp]),
     "frs_set_likelihood": (_i, [_vp, _i]),
     "frs_set_cuda_graphs": (_i, [_vp, _i]),
+    "frs_set_fused_passes": (_i, [_vp, _i]),
     "frs_sky_energy_grad": (_i, [_vp, _vp, C.POINTER(_d), _vp]),
     "frs_dot": (_i, [_vp, _vp, _vp, C.c_longlong, C.POINTER(_d)]),
     "frs_latent_jvp": (_i, [_vp, _vp, _vp]),
@@ -348,6 +349,9 @@ class Context:
         nyp, nxp = patch.shape[-2], patch.shape[-1]
         self._ck(lib().frs_patch_crop(self._h, _ptr(field, self.f32, self.npix, "field"), nyp, nxp, int(y0), int(x0),
                                       _ptr(patch, self.f32, nyp * nxp, "patch")))
+
+    def set_fused_passes(self, on):
+        self._ck(lib().frs_set_fused_passes(self._h, int(bool(on))))
 
     def set_cuda_graphs(self, on):
         self._ck(lib().frs_set_cuda_graphs(self._h, int(bool(on))))

@@ -67,6 +67,7 @@ struct frs_ctx {
     cudaStream_t cap_stream = nullptr;  // capture runs on a stream of the ctx's own (the caller's may be the legacy default stream)
     long long cg_graph_launches = 0;   // kernels per replay
     int use_graphs = 1;
+    int fuse_inv_hart = 1;             // latent-space path: rows_inv and the following Hartley row pass as one kernel
     // NEXT-3: learned amplitude spectrum (prior.h).  plain_latent: the joint calls run the latent-space passes without
     // the fused (.A, + v) prologue / epilogue and apply their own
     AmpModel am;
@@ -271,10 +272,27 @@ int conv_rows_inv(frs_ctx* ctx, const Orient& o, float* out, int mode, const flo
 // The row pass leaves column tiles, and the column pass of column x produces H[.][x] for all y, which is
 // one contiguous run of the transposed output -- so the transform transposes for free, and the
 // latent-space path keeps its sky-space arrays transposed instead of paying for scattered stores.
+// second half of hartley_t: the column pass over ctx->Th
+int hartley_cols(frs_ctx* ctx, int n1, int n2, float* out, const float* mul, const float* add, const float* offset_dev, int nb,
+                 double* d_dot = nullptr, bool exp_out = false) {
+    Prof pr(ctx, kPassHartCols);
+    HartColsArgs a{};
+    a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = n2; a.exp_out = exp_out ? 1 : 0;
+    a.img_bstride = ctx->npix;
+    a.tw = ctx->tw[n1];
+    a.dot_partials = (d_dot && add) ? ctx->partials : nullptr;   // <add, out> fused into the epilogue (fp64)
+    int gx = 0;
+    CKL(launch_hart_cols(ctx->stream, n1, a, nb, &gx));
+    ctx->launches++;
+    if (a.dot_partials) {
+        reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, gx, 1, 0, d_dot);
+        ctx->launches++;
+    }
+    return FRS_OK;
+}
 int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul, float* out, const float* mul,
               const float* add, const float* offset_dev, int nb, double* d_dot = nullptr, float sign = 1.0f,
               bool exp_out = false) {
-    const int ntile_h = n2 / 4 + 1;
     {
         Prof pr(ctx, kPassHartRows);
         RowsFwdArgs a{};
@@ -285,21 +303,27 @@ int hartley_t(frs_ctx* ctx, const float* in, int n1, int n2, const float* premul
         CKL(launch_rows_fwd(ctx->stream, n2 / 2, false, a, nb));
         ctx->launches++;
     }
-    {
-        Prof pr(ctx, kPassHartCols);
-        HartColsArgs a{};
-        a.t = ctx->Th; a.out = out; a.mul = mul; a.add = add; a.offset = offset_dev; a.nx = n2; a.exp_out = exp_out ? 1 : 0;
-        a.img_bstride = ctx->npix;
-        a.tw = ctx->tw[n1];
-        a.dot_partials = (d_dot && add) ? ctx->partials : nullptr;   // <add, out> fused into the epilogue (fp64)
-        int gx = 0;
-        CKL(launch_hart_cols(ctx->stream, n1, a, nb, &gx));
-        ctx->launches++;
-        if (a.dot_partials) {
-            reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, gx, 1, 0, d_dot);
-            ctx->launches++;
-        }
-    }
+    return hartley_cols(ctx, n1, n2, out, mul, add, offset_dev, nb, d_dot, exp_out);
+}
+
+// The inverse row pass of the convolution fused with the row pass of the Hartley transform of its result
+// (kernels_inv_hart.inl): T2 -> Th without the image in between.  mode: kMulS or kEnergy.  Follow with hartley_cols.
+bool fused_inv_hart_ok(const frs_ctx* ctx, const Orient& o) {
+    return ctx->fuse_inv_hart && rows_inv_hart_ok(o.len) && ctx->nchan == 1 && ctx->nfield == 1 && !ctx->profiling &&
+           !(ctx->pts.n > 0 && ctx->pts.in_sky);
+}
+int conv_rows_inv_hart(frs_ctx* ctx, const Orient& o, int mode, const float* s, const float* j, float sign, int* grid_x) {
+    RowsInvHartArgs h{};
+    RowsInvArgs& a = h.inv;
+    a.t = ctx->T2; a.out = nullptr; a.s = s; a.j = j; a.partials = ctx->partials;
+    a.ny = o.rows; a.mode = mode; a.cols = 2 * o.ntile;
+    RET(spectrum_maps(ctx, ctx->T, o.rows, o.len, ctx->nchan, &a.tmap, nullptr));
+    a.img_bstride = ctx->npix;
+    a.tw = ctx->tw[o.len]; a.twist = ctx->twist[o.len];
+    h.th = ctx->Th; h.scale = 0.5f * sign;
+    h.tw2 = ctx->tw[o.len / 2]; h.twist2 = ctx->twist[o.len / 2];
+    CKL(launch_rows_inv_hart(ctx->stream, o.len, h, ctx->nchan, grid_x));
+    ctx->launches++;
     return FRS_OK;
 }
 
@@ -406,6 +430,14 @@ int metric_apply9_impl(frs_ctx* ctx, const float* v, int with_prior, float* out,
     RET(ninv_transposed(ctx, ctx->img2, ctx->img));                                       // N'^-1 C J v
     RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
     RET(conv_cols(ctx, o));
+    if (simple && fused_inv_hart_ok(ctx, o)) {
+        RET(conv_rows_inv_hart(ctx, o, kMulS, ctx->sT, nullptr, 1.0f, nullptr));
+        RET(hartley_cols(ctx, ctx->nx, ctx->ny, out, ctx->plain_latent ? nullptr : ctx->amp,
+                         (with_prior && !ctx->plain_latent) ? v : nullptr, nullptr, ctx->nfield,
+                         (with_prior && !ctx->plain_latent) ? d_vmv : nullptr));
+        CK(cudaGetLastError());
+        return FRS_OK;
+    }
     if (simple) {
         RET(conv_rows_inv(ctx, o, ctx->acc, kMulS, ctx->sT, nullptr, nullptr));
         RET(points_post(ctx, ctx->acc, 1.0, nullptr));
@@ -440,6 +472,15 @@ int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, 
         RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
     }
     RET(conv_cols(ctx, o));
+    if (simple && fused_inv_hart_ok(ctx, o)) {
+        // acc = s . C(...) never reaches memory: its rows go straight into the row pass of the transform below
+        RET(conv_rows_inv_hart(ctx, o, kMulS, ctx->sT, nullptr, 1.0f, nullptr));
+        RET(hartley_cols(ctx, ctx->nx, ctx->ny, out, ctx->plain_latent ? nullptr : ctx->amp,
+                         (with_prior && !ctx->plain_latent) ? v : nullptr, nullptr, ctx->nfield,
+                         (with_prior && !ctx->plain_latent) ? d_vmv : nullptr));
+        CK(cudaGetLastError());
+        return FRS_OK;
+    }
     if (simple) {
         RET(conv_rows_inv(ctx, o, ctx->acc, kMulS, ctx->sT, nullptr, nullptr));      // acc = s . C(...)
         RET(points_post(ctx, ctx->acc, 1.0, nullptr));
@@ -825,6 +866,12 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
         RET(conv_rows_fwd(ctx, o, ctx->img, nullptr));
         RET(conv_cols(ctx, o));
         const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
+        const bool fused = simple && fused_inv_hart_ok(ctx, o);
+        if (fused) {
+            RET(conv_rows_inv_hart(ctx, o, kMulS, ctx->sT, nullptr, -1.0f, nullptr));
+            RET(hartley_cols(ctx, ctx->nx, ctx->ny, grad, ctx->plain_latent ? nullptr : ctx->amp,
+                             (with_prior && !ctx->plain_latent) ? xi : nullptr, nullptr, ctx->nfield));
+        } else {
         RET(conv_rows_inv(ctx, o, simple ? ctx->acc : ctx->img, kMulS, ctx->sT, nullptr, nullptr));   // s . C u
         if (simple) RET(points_post(ctx, ctx->acc, -1.0, ctx->scal + 11));
         if (!simple) {
@@ -834,6 +881,7 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
         }
         RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, grad, ctx->plain_latent ? nullptr : ctx->amp,
                       (with_prior && !ctx->plain_latent) ? xi : nullptr, nullptr, ctx->nfield, nullptr, -1.0f));
+        }
         CK(cudaGetLastError());
         if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
         if (h_energy) {
@@ -845,6 +893,9 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
     RET(conv_rows_fwd(ctx, o, ctx->sT, nullptr));
     RET(conv_cols(ctx, o));
     int gx = 0;
+    const bool fused0 = fused_inv_hart_ok(ctx, o);
+    if (fused0) RET(conv_rows_inv_hart(ctx, o, kEnergy, ctx->sT, ctx->dirtyT, 1.0f, &gx));   // s (C s - j) goes straight into Th
+    else
     RET(conv_rows_inv(ctx, o, ctx->img, kEnergy, ctx->sT, ctx->dirtyT, &gx));   // img_c = s_c (C s_c - j_c), partial sums
     const int np = gx;      // one (sum s.c, sum j.s) pair per persistent CTA
     reduce_final_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->partials, np, 2, 0, ctx->scal + 8);
@@ -853,6 +904,17 @@ static int energy_grad_impl(frs_ctx* ctx, const float* xi, int with_prior, doubl
     if (with_prior) RET(dot(ctx, xi, xi, (size_t)ctx->nfield * ctx->npix, ctx->scal + 10));
     energy_final_kernel<<<1, 1, 0, ctx->stream>>>(ctx->scal + 8, ctx->scal + 9, ctx->scal + 10, with_prior, ctx->scal + 11);
     ctx->launches++;
+    if (fused0) {
+        RET(hartley_cols(ctx, ctx->nx, ctx->ny, grad, ctx->plain_latent ? nullptr : ctx->amp,
+                         (with_prior && !ctx->plain_latent) ? xi : nullptr, nullptr, ctx->nfield));
+        CK(cudaGetLastError());
+        if (d_energy) CK(cudaMemcpyAsync(d_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+        if (h_energy) {
+            CK(cudaMemcpyAsync(h_energy, ctx->scal + 11, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+        }
+        return FRS_OK;
+    }
     const float* accp = ctx->img;
     if (ctx->nchan == 1 && ctx->nfield == 1) RET(points_post(ctx, ctx->img, 1.0, ctx->scal + 11));
     if (!(ctx->nchan == 1 && ctx->nfield == 1)) {
@@ -941,6 +1003,13 @@ int frs_cg_step_end(frs_ctx* ctx, float* x, int with_prior) {
 
 static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, float rtol, int with_prior, int* h_iters,
                          double* h_resnorm, double* d_res_history);
+
+int frs_set_fused_passes(frs_ctx* ctx, int on) {
+    if (!ctx) return FRS_EINVAL;
+    ctx->fuse_inv_hart = on ? 1 : 0;
+    ctx->cfg_epoch++;
+    return FRS_OK;
+}
 
 int frs_set_cuda_graphs(frs_ctx* ctx, int on) {
     if (!ctx) return FRS_EINVAL;

@@ -247,5 +247,6 @@ rows_fwd_kernel(RowsFwdArgs a) {
 #include "kernels_cols.inl"
 #include "kernels_cols_dif.inl"
 #include "kernels_inv.inl"
+#include "kernels_inv_hart.inl"
 
 }  // namespace frs

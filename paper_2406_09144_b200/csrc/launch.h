@@ -15,6 +15,9 @@ int launch_rows_fwd(cudaStream_t st, int nf, bool pad, const RowsFwdArgs& a, int
 int launch_conv_cols(cudaStream_t st, int nf, const ConvColsArgs& a, int nb);
 inline bool conv_cols_uses_dif(int nf) { return nf >= 256; }
 int launch_rows_inv(cudaStream_t st, int nf, const RowsInvArgs& a, int nb, int* grid_x);
+// the inverse row pass fused with the row pass of the Hartley transform that follows (a.inv.mode: kMulS or kEnergy)
+inline bool rows_inv_hart_ok(int nf) { return nf == 1024 || nf == 2048 || nf == 4096; }
+int launch_rows_inv_hart(cudaStream_t st, int nf, const RowsInvHartArgs& a, int nb, int* grid_x);
 int launch_hart_cols(cudaStream_t st, int nf, const HartColsArgs& a, int nb, int* grid_x = nullptr);
 
 struct PsfColsArgs {

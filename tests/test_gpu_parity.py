@@ -604,3 +604,29 @@ def test_host_batch_apply_equals_single_calls(frs):
     y_dev = ctx.new_image()
     ctx.sky_metric_apply(xs[4].cuda(), y_dev)
     assert torch.equal(y_dev.cpu(), ref[4])
+
+
+@pytest.mark.parametrize("key", [("sq", 2, 1024), ("rect", 2048, 1024), ("rect", 1024, 4096)])
+def test_fused_inverse_and_hartley_row_pass_equals_separate_passes(frs, key):
+    """The fused kernel (rows_inv + the row pass of the following Hartley transform) against the two separate passes:
+    same arithmetic on the same data, so gradient and metric agree to rounding (1e-6), the energy to fp64 summation order;
+    both likelihood modes.  (Against the oracle the fused path is the default of every other test.)"""
+    w = workload(key)
+    ctx = make_ctx(frs, w)
+    rng = np.random.default_rng(3)
+    xi = dev(0.3 * rng.normal(size=(1, w.ny, w.nx)))
+    v = dev(rng.normal(size=(1, w.ny, w.nx)))
+    for mode in (0, 1):
+        if mode == 1:
+            ctx.set_noise_kernel(1e-2 * float(o.psf_from_weights(w.w_half[0])[0, 0]))
+            ctx.set_likelihood(1)
+        res = {}
+        for fused in (1, 0):
+            ctx.set_fused_passes(fused)
+            g, out = ctx.new_latent(), ctx.new_latent()
+            e = ctx.energy_grad(xi, g, with_prior=True)
+            ctx.metric_apply(v, out, with_prior=True)
+            res[fused] = (e, g.cpu().numpy(), out.cpu().numpy())
+        assert abs(res[1][0] - res[0][0]) <= 1e-10 * abs(res[0][0])
+        assert rel(res[1][1], res[0][1]) <= 1e-6 and rel(res[1][2], res[0][2]) <= 1e-6
+        assert not np.array_equal(res[1][1], np.zeros_like(res[1][1]))
