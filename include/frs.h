@@ -283,6 +283,42 @@ int frs_sky_metric_apply_host_batch(frs_ctx* ctx, int n, const float* const* x_h
 /* y = C x with HOST buffers. */
 int frs_psf_apply_host(frs_ctx* ctx, const float* x_host, float* y_host);
 
+/* ---- an entry point that allocates nothing ------------------------------------------------------
+ * Everything above needs a frs_ctx, and a context allocates device memory: tables in frs_create, the scratch arrays on
+ * first use.  Some callers cannot afford a single cudaMalloc: a process whose framework allocator (PyTorch's caching
+ * allocator, say) has already taken the GPU's memory for itself, so that an allocation made behind its back fails or
+ * eats into what it planned with; and a latency-bound loop -- a sharded CG between two all-reduces -- in which
+ * cudaMalloc / cudaFree would hold up every stream of the device.  For them the inner product of frs_dot (the prior
+ * terms 1/2 <xi_k, xi_k> of a composed model, the scalars of a CG written by the caller) exists in a second form that
+ * needs no context and calls no cudaMalloc, cudaFree or other allocating routine.  Its only scratch, one fp64 partial sum
+ * per CTA, is a fixed 9 472-byte array inside the library's device code; every GPU that loads libfrs.so holds that array
+ * until the process exits. */
+
+/* Largest n frs_dot_noalloc accepts: 2^28 floats = 1 GiB per operand, 8 x the largest latent vector of this library
+ * (2 fields x 4096^2).  The scratch itself never overflows -- at most 1184 CTAs stride over the data, whatever n -- so
+ * this is the range the entry point is specified and tested for, and anything larger is refused rather than run. */
+#define FRS_DOT_NOALLOC_MAX_N (1LL << 28)
+
+/* *d_out = <a, b> over n floats, products and sums in fp64 in the fixed order of frs_dot (the same bits).
+ *   device : CUDA device ordinal (0 .. 63) that holds a, b and d_out; made current on the calling thread, as every frs_*
+ *            call does with its context's device.
+ *   stream : cudaStream_t on that device (NULL = the legacy default stream).  The two kernels are enqueued there and the
+ *            call returns without synchronising; d_out is valid once the stream reaches that point.
+ *   a, b   : DEVICE float32 [n], 16-byte aligned, owned by the caller, read only.  n: positive multiple of 4.
+ *   d_out  : DEVICE double, 8-byte aligned, owned by the caller.
+ * Set-up: the FIRST call on each device looks up where the scratch array lives on that device (once, under a lock).
+ * Make that first call during initialisation, before any stream capture is begun on the thread.
+ * Sharing: every call on a device uses the same scratch array, on whatever stream.  The array keeps what the last call
+ * wrote; no slot is read before the same call has written it, so nothing has to be cleared between calls.  But two calls
+ * whose kernels can overlap on the GPU (different streams without an event between them, or two host threads) race on
+ * it and both results are garbage: order them on one stream or with events.
+ * Errors (text via frs_dot_noalloc_last_error): FRS_EINVAL for a NULL or misaligned pointer, n <= 0, n not a multiple
+ * of 4, n > FRS_DOT_NOALLOC_MAX_N ("beyond the maximum"), device outside 0 .. 63; FRS_ECUDA for a CUDA error.  Nothing
+ * is enqueued when an error is returned. */
+int frs_dot_noalloc(int device, void* stream, const float* a, const float* b, long long n, double* d_out);
+/* Text of the calling thread's last frs_dot_noalloc error (static thread-local storage, never NULL). */
+const char* frs_dot_noalloc_last_error(void);
+
 /* ---- instrumentation ---------------------------------------------------------------------------- */
 
 /* Number of kernels this ctx has launched since creation (monotone). */

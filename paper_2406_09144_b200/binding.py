@@ -45,6 +45,8 @@ EXPORTS = {
     "frs_set_fused_passes": (_i, [_vp, _i]),
     "frs_sky_energy_grad": (_i, [_vp, _vp, C.POINTER(_d), _vp]),
     "frs_dot": (_i, [_vp, _vp, _vp, C.c_longlong, C.POINTER(_d)]),
+    "frs_dot_noalloc": (_i, [_i, _vp, _vp, _vp, C.c_longlong, _vp]),
+    "frs_dot_noalloc_last_error": (C.c_char_p, []),
     "frs_latent_jvp": (_i, [_vp, _vp, _vp]),
     "frs_latent_vjp": (_i, [_vp, _vp, _vp, _vp]),
     "frs_patch_insert_add": (_i, [_vp, _vp, _i, _i, _i, _i, _vp]),
@@ -167,6 +169,28 @@ def selftest_tma_geometry(nf, rows):
     if rc != 0:
         raise FrsError(rc, "selftest_tma_geometry")
     return tuple(int(v) for v in out)
+
+
+FRS_DOT_NOALLOC_MAX_N = 1 << 28
+
+
+def dot_noalloc(a, b, d_out, stream=None):
+    """frs_dot_noalloc: d_out[0] = <a, b> in fp64 for callers that must not allocate on the device (a framework allocator
+    owns the GPU's memory, or a cudaMalloc would stall the other streams of a latency-bound loop).  Needs no Context; the
+    library's only scratch is a fixed array in its device code, shared by every call on the device -- so calls that can
+    overlap on the GPU race.  a, b: CUDA float32 tensors of equal length (a multiple of 4, at most FRS_DOT_NOALLOC_MAX_N);
+    d_out: a CUDA float64 tensor of one element on the same device, written on `stream` (default: torch's current
+    stream) without synchronising.  Marshalling only."""
+    import torch
+    pa, pb = _ptr(a, torch.float32, None, "a"), _ptr(b, torch.float32, a.numel(), "b")
+    po = _ptr(d_out, torch.float64, 1, "d_out")
+    if b.device != a.device or d_out.device != a.device:
+        raise ValueError("a, b and d_out must live on one device")
+    if stream is None:
+        stream = torch.cuda.current_stream(a.device)
+    rc = lib().frs_dot_noalloc(a.device.index, stream.cuda_stream, pa, pb, a.numel(), po)
+    if rc != 0:
+        raise FrsError(rc, lib().frs_dot_noalloc_last_error().decode())
 
 
 class _DevicePtr:
