@@ -60,6 +60,11 @@ const char* frs_version(void);
  * requires max|Im W| <= 1e-5 max W and min Re W >= -1e-5 max W, else FRS_ENOTPSD (R4; P:191:
  * a covariance kernel must be real and positive).  Stores max(Re W, 0).  Synchronises. */
 int frs_set_psf(frs_ctx* ctx, const float* psf);
+/* PSF given as its real, non-negative half spectrum W [nchan][2ny][nx+1] (the gridded, Hermitian-
+ * symmetrised visibility weights; P:180 'FFT[I^PSF]', R3: (C x)[n] = sum_k W[k] xhat[k] e^{+2 pi i k.n/M},
+ * so the PSF peak equals sum W).  Negative entries -> FRS_ENOTPSD.  Synchronises. */
+int frs_set_psf_weights(frs_ctx* ctx, const float* w_half);
+
 /* ---- images that are not a power of two (3600^2) by embedding; reading R19 ----
  * Eq. 14 is a LINEAR convolution of the ny_img x nx_img image with a PSF twice its size: any padded grid of at least
  * twice the image computes it exactly.  The context is created on the next power of two (ny, nx); every image-sized
@@ -76,10 +81,6 @@ int frs_set_psf_embedded(frs_ctx* ctx, const float* psf_img, int ny_img, int nx_
  * given as weights on the context's own padded grid.  Invalidates the cached position. */
 int frs_set_field_of_view(frs_ctx* ctx, int ny_img, int nx_img);
 
-/* PSF given as its real, non-negative half spectrum W [nchan][2ny][nx+1] (the gridded, Hermitian-
- * symmetrised visibility weights; P:180 'FFT[I^PSF]', R3: (C x)[n] = sum_k W[k] xhat[k] e^{+2 pi i k.n/M},
- * so the PSF peak equals sum W).  Negative entries -> FRS_ENOTPSD.  Synchronises. */
-int frs_set_psf_weights(frs_ctx* ctx, const float* w_half);
 /* Dirty image j = I^D [nchan][ny][nx]  (Eq. 6, Eq. 8).  For major cycles pass
  * j_eff = d_i + C s_{i-1} (Eq. 21, R13). */
 int frs_set_dirty(frs_ctx* ctx, const float* j);
@@ -201,7 +202,8 @@ int frs_amplitude_vjp(frs_ctx* ctx, const float* g_amp, float* g_theta);
  * With point sources set, theta of the joint calls below is [amplitude part (frs_amp_model_size) | xi_p, p < npts] and
  * so are grad_theta, dtheta, out_theta; frs_sky_forward adds the fluxes of the last joint position (xi_p = 0 before
  * one), and every latent-space call uses the diffuse sky as the Jacobian of the diffuse part at those pixels.
- * Errors: FRS_EINVAL (pixel outside the field, repeated pixel, alpha or q <= 0), FRS_ESTATE for nchan != 1. */
+ * Errors: FRS_EINVAL (pixel outside the field of view, repeated pixel, alpha or q <= 0), FRS_ESTATE for nchan != 1.
+ * frs_set_field_of_view / frs_set_psf_embedded return FRS_EINVAL, changing nothing, if a point set earlier would fall outside. */
 int frs_set_point_sources(frs_ctx* ctx, int npts, const int* yx_host, float alpha, float q);
 /* Energy of the likelihood in use (frs_set_likelihood) at the joint position (xi, theta), prior 1/2 <xi,xi> + 1/2
  * <theta,theta> if with_prior, and its gradient with respect to both (grad_xi [ny][nx], grad_theta [ntheta]).

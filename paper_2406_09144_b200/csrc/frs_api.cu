@@ -61,7 +61,7 @@ struct frs_ctx {
     bool have_psf = false, have_dirty = false, have_amp = false, have_s = false;
     long long launches = 0;
     // one CG iteration captured as a CUDA graph (cg_solve_impl): replayed while the key (every frozen argument) matches
-    struct CgGraphKey { const float* x; int with_prior, nfield, lik_mode; double* hist; double rtol2; bool sT_ok; long long epoch; } cg_key = {};
+    struct CgGraphKey { const float* x; int with_prior, nfield, lik_mode; double* hist; double rtol2; bool sT_ok, pts_in_sky; long long epoch; } cg_key = {};
     long long cfg_epoch = 0;           // bumped by every setter that can change the launch sequence of an iteration
     cudaGraphExec_t cg_exec = nullptr;
     cudaStream_t cap_stream = nullptr;  // capture runs on a stream of the ctx's own (the caller's may be the legacy default stream)
@@ -75,6 +75,7 @@ struct frs_ctx {
     // inverse-gamma point-source pixels (reading R18): fluxes added to the cached sky; the latent-space passes patch the
     // few pixels where the Jacobian of the diffuse part differs from the total sky (points_pre / points_post)
     PointSources pts;
+    std::vector<int> pts_yx;            // host copy of the point pixels (y, x), re-validated when the field of view changes
     int fov_y = 0, fov_x = 0;           // image smaller than the grid (reading R19): the sky is zero outside [0,fov_y) x [0,fov_x); 0 = whole grid
     const float* pts_dv = nullptr;      // tangent of the point latents (joint metric), else null = 0
     const float* pts_add = nullptr;     // prior term added to the point outputs (joint calls with the prior), else null
@@ -499,11 +500,9 @@ int metric_apply_impl(frs_ctx* ctx, const float* v, int with_prior, float* out, 
 }
 
 int cg_alloc(frs_ctx* ctx) {
-    const size_t n = (size_t)ctx->nfield * ctx->npix;
-    RET(dev_alloc(ctx, &ctx->cg_r, 2 * ctx->npix));
+    RET(dev_alloc(ctx, &ctx->cg_r, 2 * ctx->npix));     // sized for two fields whatever nfield is now
     RET(dev_alloc(ctx, &ctx->cg_p, 2 * ctx->npix));
     RET(dev_alloc(ctx, &ctx->cg_q, 2 * ctx->npix));
-    (void)n;
     return FRS_OK;
 }
 
@@ -549,7 +548,7 @@ int for_each_position(frs_ctx* ctx, const float* xi, const float* samples, int n
 // =================================================================================================
 extern "C" {
 
-const char* frs_version(void) { return "frs 0.1 (sm_100a; register-Stockham FFT passes)"; }
+const char* frs_version(void) { return "frs 0.3 (sm_100a; packed-pair register FFT passes: sorting core for the row and Hartley passes, DIF/DIT core for the column convolution)"; }
 
 const char* frs_last_error(const frs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 
@@ -667,10 +666,20 @@ int frs_set_psf(frs_ctx* ctx, const float* psf) {
     return set_psf_impl(ctx, psf, true);
 }
 
+// every point-source pixel inside [0, ly) x [0, lx)?  (a point outside the field of view would have its flux masked to zero
+// while the bookkeeping of the latent-space passes kept the unmasked values)
+static bool points_inside(const frs_ctx* ctx, int ly, int lx) {
+    for (size_t i = 0; i + 1 < ctx->pts_yx.size(); i += 2)
+        if (ctx->pts_yx[i] >= ly || ctx->pts_yx[i + 1] >= lx) return false;
+    return true;
+}
+
 int frs_set_field_of_view(frs_ctx* ctx, int ny_img, int nx_img) {
     if (ctx) ctx->cfg_epoch++;
     if (!ctx || ny_img < 1 || nx_img < 1 || ny_img > ctx->ny || nx_img > ctx->nx)
         return fail(ctx, FRS_EINVAL, "frs_set_field_of_view: bad argument");
+    if (!points_inside(ctx, ny_img, nx_img))
+        return fail(ctx, FRS_EINVAL, "frs_set_field_of_view: a point source lies outside the new field of view (frs_set_point_sources first)");
     const bool whole = ny_img == ctx->ny && nx_img == ctx->nx;
     ctx->fov_y = whole ? 0 : ny_img;
     ctx->fov_x = whole ? 0 : nx_img;
@@ -683,6 +692,8 @@ int frs_set_psf_embedded(frs_ctx* ctx, const float* psf_img, int ny_img, int nx_
     if (ctx) ctx->cfg_epoch++;
     if (!ctx || !psf_img || !aligned16(psf_img) || ny_img < 1 || nx_img < 1 || ny_img > ctx->ny || nx_img > ctx->nx)
         return fail(ctx, FRS_EINVAL, "frs_set_psf_embedded: bad argument");
+    if (!points_inside(ctx, ny_img, nx_img))
+        return fail(ctx, FRS_EINVAL, "frs_set_psf_embedded: a point source lies outside the new field of view (frs_set_point_sources first)");
     CK(cudaSetDevice(ctx->device));
     float* big = nullptr;
     CK(cudaMalloc(reinterpret_cast<void**>(&big), (size_t)ctx->nchan * 4 * ctx->npix * sizeof(float)));
@@ -745,6 +756,7 @@ static int set_psf_impl(frs_ctx* ctx, const float* psf, bool covariance) {
         return FRS_ENOTPSD;
     }
     ctx->have_psf = true;
+    ctx->have_kern = false; ctx->lik_mode = 0;    // a kernel fitted to the previous PSF no longer applies (frs.h, frs_set_noise_kernel)
     return FRS_OK;
 }
 
@@ -1054,10 +1066,15 @@ static int cg_solve_impl(frs_ctx* ctx, const float* b, float* x, int max_iter, f
     }
     const bool graphs = ctx->use_graphs && !ctx->profiling && max_iter - it >= 2;
     if (graphs) {
-        const frs_ctx::CgGraphKey key = {x, with_prior, ctx->nfield, ctx->lik_mode, d_res_history, rtol2, ctx->sT_ok, ctx->cfg_epoch};
+        // pts_in_sky: whether the cached sky carries point fluxes decides between the fused and the patched launch
+        // sequence (points_pre / points_post, fused_inv_hart_ok), and frs_sky_forward / frs_energy_grad flip it
+        // without touching the epoch
+        const frs_ctx::CgGraphKey key = {x, with_prior, ctx->nfield, ctx->lik_mode, d_res_history, rtol2, ctx->sT_ok,
+                                         ctx->pts.n > 0 && ctx->pts.in_sky, ctx->cfg_epoch};
         const frs_ctx::CgGraphKey& k0 = ctx->cg_key;
         const bool same = ctx->cg_exec && k0.x == key.x && k0.with_prior == key.with_prior && k0.nfield == key.nfield &&
-                          k0.lik_mode == key.lik_mode && k0.hist == key.hist && k0.rtol2 == key.rtol2 && k0.sT_ok == key.sT_ok && k0.epoch == key.epoch;
+                          k0.lik_mode == key.lik_mode && k0.hist == key.hist && k0.rtol2 == key.rtol2 && k0.sT_ok == key.sT_ok &&
+                          k0.pts_in_sky == key.pts_in_sky && k0.epoch == key.epoch;
         if (!same) {
             if (ctx->cg_exec) { cudaGraphExecDestroy(ctx->cg_exec); ctx->cg_exec = nullptr; }
             cudaGraph_t g = nullptr;
@@ -1203,9 +1220,10 @@ int frs_set_point_sources(frs_ctx* ctx, int npts, const int* yx_host, float alph
     if (ctx->nchan != 1) return fail(ctx, FRS_ESTATE, "frs_set_point_sources: single-channel contexts only");
     CK(cudaSetDevice(ctx->device));
     std::vector<int> idx((size_t)npts);
+    const int ly = ctx->fov_y ? ctx->fov_y : ctx->ny, lx = ctx->fov_y ? ctx->fov_x : ctx->nx;   // the field of view, not the grid
     for (int i = 0; i < npts; ++i) {
         const int y = yx_host[2 * i], x = yx_host[2 * i + 1];
-        if (y < 0 || y >= ctx->ny || x < 0 || x >= ctx->nx) return fail(ctx, FRS_EINVAL, "frs_set_point_sources: pixel outside the field");
+        if (y < 0 || y >= ly || x < 0 || x >= lx) return fail(ctx, FRS_EINVAL, "frs_set_point_sources: pixel outside the field of view");
         idx[i] = x * ctx->ny + y;                       // the latent-space path keeps the sky transposed
         for (int k = 0; k < i; ++k)
             if (idx[k] == idx[i]) return fail(ctx, FRS_EINVAL, "frs_set_point_sources: the same pixel twice");
@@ -1222,6 +1240,7 @@ int frs_set_point_sources(frs_ctx* ctx, int npts, const int* yx_host, float alph
     CK(cudaMemsetAsync(p.xi, 0, (size_t)kMaxPoints * sizeof(float), ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     p.n = npts; p.alpha = alpha; p.q = q; p.in_sky = false;
+    ctx->pts_yx.assign(yx_host, yx_host + 2 * (size_t)npts);
     ctx->have_s = ctx->s_ok = ctx->sT_ok = false;
     ctx->am.have_xi = false;
     return FRS_OK;
@@ -1420,7 +1439,11 @@ int frs_draw_sample(frs_ctx* ctx, const float* eta_xi, const float* eta_d, int m
     RET(conv_cols(ctx, o));
     const bool simple = ctx->nchan == 1 && ctx->nfield == 1;
     RET(conv_rows_inv(ctx, o, simple ? ctx->acc : ctx->img, kMulS, ctx->sT, nullptr, nullptr));
-    if (!simple) {
+    if (simple) {
+        // J^T of the metric the CG below inverts is the DIFFUSE Jacobian at the point-source pixels (metric_apply_impl):
+        // the source must be formed with the same one, or Cov m != M there
+        RET(points_post(ctx, ctx->acc, 1.0, nullptr));
+    } else {
         vjp_combine_kernel<<<ew_grid(ctx->npix), kEwThreads, 0, ctx->stream>>>(ctx->img, ctx->d_lognu, ctx->acc, ctx->npix,
                                                                                ctx->nfield, ctx->nchan);
         ctx->launches++;

@@ -213,3 +213,28 @@ def test_mgvi_sample_and_kl_average(frs, key):
     g0 = ctx.new_latent()
     e1 = ctx.energy_grad(dev(xi), g0, with_prior=True)
     assert e0 == e1 and torch.equal(g, g0)
+
+
+def test_a_new_psf_discards_the_fitted_noise_kernel(frs):
+    """frs.h (frs_set_noise_kernel): a later frs_set_psf* discards the kernel and returns to mode 0 -- for the image-space
+    setter too, not only for frs_set_psf_weights: K was fitted to the old PSF."""
+    w = WORKLOADS["c1"]()
+    for setter in ("weights", "image"):
+        ctx, eps = setup(frs, w)
+        ctx.set_likelihood(1)
+        if setter == "weights":
+            ctx.set_psf_weights(dev(2.0 * w.w_half))
+        else:
+            psf = np.stack([o.psf_from_weights(2.0 * w.w_half[c]) for c in range(w.nchan)])
+            ctx.set_psf(dev(psf))
+        with pytest.raises(frs.FrsError) as ei:
+            ctx.set_likelihood(1)                                            # no kernel any more
+        assert ei.value.code == frs.binding.FRS_ESTATE
+        with pytest.raises(frs.FrsError):
+            ctx.get_noise_kernel()
+        # mode 0 is in force again: the energy is that of the N' = R' limit with the new PSF
+        xi = np.zeros((1, w.ny, w.nx), np.float32)
+        g = ctx.new_latent()
+        e = ctx.energy_grad(dev(xi), g, with_prior=True)
+        e_ref, g_ref = o.energy_grad(2.0 * w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, True)
+        assert abs(e - e_ref) <= TOL * abs(e_ref) and rel(g.cpu().numpy(), g_ref) <= TOL

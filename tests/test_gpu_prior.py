@@ -229,6 +229,26 @@ def test_point_source_argument_errors(frs):
     with pytest.raises(frs.FrsError):
         ctx.set_point_sources([[1, 1]], 0.0, 1.0)
     ctx.set_point_sources([], 0.5, 1.0)
+    # the field of view, not the grid, bounds the pixels -- in either order of the two calls
+    ctx.set_field_of_view(48, 40)
+    with pytest.raises(frs.FrsError, match="field of view"):
+        ctx.set_point_sources([[10, 40]], 0.5, 1.0)
+    with pytest.raises(frs.FrsError, match="field of view"):
+        ctx.set_point_sources([[48, 3]], 0.5, 1.0)
+    ctx.set_point_sources([[47, 39]], 0.5, 1.0)
+    with pytest.raises(frs.FrsError, match="field of view"):
+        ctx.set_field_of_view(47, 40)
+    ctx.set_field_of_view(64, 64)
+    ctx.set_point_sources([[63, 63]], 0.5, 1.0)
+    with pytest.raises(frs.FrsError, match="field of view"):
+        ctx.set_field_of_view(48, 40)
+    with pytest.raises(frs.FrsError, match="field of view"):
+        ctx.set_psf_embedded(torch_zeros_psf(24, 20), 24, 20)
+
+
+def torch_zeros_psf(ny_img, nx_img):
+    import torch
+    return torch.zeros(1, 2 * ny_img, 2 * nx_img, device="cuda")
 
 
 def test_cg_graph_is_rebuilt_when_the_model_changes(frs):
@@ -257,3 +277,75 @@ def test_cg_graph_is_rebuilt_when_the_model_changes(frs):
     x.zero_()
     ctx.cg_solve(b, x, 8)
     assert torch.equal(x, x2) and not torch.equal(x1, x2)
+
+
+def test_cg_graph_is_rebuilt_when_point_fluxes_enter_the_cached_sky(frs):
+    """Whether the cached sky carries point fluxes decides the launch sequence of an iteration (two patch kernels, no fused
+    inverse pass), and frs_set_sky / frs_sky_forward flip that without any setter being called: set_sky -> solve (graph
+    without the patch kernels) -> sky_forward -> solve into the same x must match plain launches bit for bit."""
+    import torch
+    w, hyper, xi, th, rng = _problem(128)
+    ctx = frs.Context(w.ny, w.nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    ctx.set_amplitude_model(hyper)
+    ctx.set_point_sources([[64, 64], [10, 100]], 0.5, 0.05 * float(np.median(w.sky_true)))
+    theta = torch.cat([dev(th), dev(np.array([1.5, 2.0], np.float32))])
+    gx, gt = torch.empty(1, w.ny, w.nx, device="cuda"), torch.empty(theta.numel(), device="cuda")
+    ctx.energy_grad_joint(dev(xi[None]), theta, gx, gt)
+    b = (-gx).contiguous()
+    s = ctx.new_image()
+    ctx.sky_forward(dev(xi[None]), s)
+    ctx.set_sky(s)                             # a caller's sky: no point bookkeeping, fused launch sequence
+    x = torch.zeros_like(b)
+    ctx.cg_solve(b, x, 8)
+    x_plain_sky = x.clone()
+    ctx.sky_forward(dev(xi[None]))             # fluxes back in the cached sky; no setter ran in between
+    x.zero_()
+    ctx.cg_solve(b, x, 8)                      # same x pointer, same arguments
+    x_graph = x.clone()
+    ctx.set_cuda_graphs(False)
+    x.zero_()
+    ctx.cg_solve(b, x, 8)
+    assert torch.equal(x, x_graph) and not torch.equal(x_plain_sky, x_graph)
+
+
+def test_mgvi_sample_with_point_sources_uses_the_diffuse_jacobian(frs):
+    """frs_draw_sample with point fluxes in the cached sky: the source m = eta_xi + J^T C N'^-1/2 eta_d is formed with the
+    Jacobian of the DIFFUSE sky at the point pixels, the one the metric of the CG that follows uses (Cov m = M)."""
+    from oracle import frs_oracle as fo
+    w, hyper, xi, th, rng = _problem(128)
+    ny, nx = w.ny, w.nx
+    yx = np.array([[ny // 2, nx // 2], [ny // 2 + 1, nx // 2 - 2], [0, nx - 1]])
+    alpha, q = 0.5, 0.05 * float(np.median(w.sky_true))
+    pts, xp = (yx, alpha, q), np.array([0.8, 2.5, -1.0], np.float32)
+    ctx = frs.Context(ny, nx, 1)
+    ctx.set_psf_weights(dev(w.w_half))
+    ctx.set_dirty(dev(w.dirty))
+    ctx.set_amplitude_model(hyper)
+    ctx.set_point_sources(yx, alpha, q)
+    ctx.set_noise_kernel(1e-2 * float(fo.psf_from_weights(w.w_half[0])[0, 0]))
+    ctx.set_likelihood(1)
+    kern = ctx.get_noise_kernel().cpu().numpy().astype(np.float64)
+    theta = np.concatenate([th, xp]).astype(np.float32)
+    import torch
+    gx, gt = torch.empty(1, ny, nx, device="cuda"), torch.empty(theta.size, device="cuda")
+    ctx.energy_grad_joint(dev(xi[None]), dev(theta), gx, gt, True)          # joint position: fluxes in the cached sky
+    eta_xi = rng.normal(size=(1, ny, nx)).astype(np.float32)
+    eta_d = rng.normal(size=(1, ny, nx)).astype(np.float32)
+    sample = ctx.new_latent()
+    assert ctx.draw_sample(dev(eta_xi), dev(eta_d), sample, 4) == 4
+    amp = po.amplitude(th.astype(np.float64), hyper, ny, nx)
+    s_diff = po.sky_joint(None, hyper, xi, th)[0][None]
+    s_tot = po.sky_full(hyper, xi, th, pts, xp)[0][None]
+    lognu = np.zeros(1)
+    m_ref = fo.sample_source_eq9(w.w_half, kern, amp[None], lognu, s_diff, eta_xi, eta_d)
+    m_wrong = fo.sample_source_eq9(w.w_half, kern, amp[None], lognu, s_tot, eta_xi, eta_d)
+    assert rel(m_wrong, m_ref) > 1e-3                                        # the two Jacobians are told apart here
+    zt, zp = np.zeros_like(th), np.zeros(len(xp))
+    apply = lambda v: po.metric_apply_full(w.w_half[0], hyper, xi, th, pts, xp, v[0], zt, zp, True, kern[0])[0][None]  # noqa: E731
+    sol = fo.cg(apply, m_ref, max_iter=4)
+    r, p, qq, sc = ctx.cg_read_state()
+    resid = m_ref - apply(sample.cpu().numpy().astype(np.float64))          # r_4 = m - M sigma_4 pins the GPU's m
+    assert np.linalg.norm(r.cpu().numpy() - resid) <= 1e-4 * np.linalg.norm(m_ref)
+    assert rel(sample.cpu().numpy(), sol["x"]) <= 1e-4
