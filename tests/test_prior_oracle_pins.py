@@ -264,3 +264,101 @@ def test_patch_model_gradient_metric_and_reduction():
     e1, g1 = po.energy_grad_patches(w.w_half[0], w.dirty[0], comps[:1], xis[:1])
     e0, g0 = fo.energy_grad(w.w_half, w.dirty, comps[0][0][None], [comps[0][1]], w.lognu, xis[0][None])
     assert abs(e1 - e0) <= 1e-12 * abs(e0) and np.max(np.abs(g1[0] - g0[0])) <= 1e-12 * np.max(np.abs(g0))
+
+
+# ---------------------------------------------------------------------------------- the metrics against the Jacobian of their own sky
+# Symmetry, M >= 1 and the reduction to a simpler model leave room for a consistent mistake in J and J^T together (the total
+# instead of the diffuse sky at the point pixels; a dropped da . xi term).  Here J is assembled column by column from central
+# differences of the very sky function the metric belongs to, M = J^T C J + 1 (Eq. 9 mode: J^T C N'^-1 C J + 1) is formed
+# densely with frs_oracle's psf_apply / ninv_apply, and every column of it is compared with the metric applied to a unit vector.
+def _dense_jacobian(sky_of, z, h=1e-3):
+    """Five-point central differences (error O(h^4), rounding ~ 1e-16 / h): good to ~1e-10 of the sky's scale."""
+    cols = []
+    for i in range(z.size):
+        e = np.zeros_like(z)
+        e[i] = h
+        d = (8.0 * (sky_of(z + e) - sky_of(z - e)) - (sky_of(z + 2 * e) - sky_of(z - 2 * e))) / (12.0 * h)
+        cols.append(d.ravel())
+    return np.stack(cols, axis=1)                                   # [npix, nlatent]
+
+
+def _dense_metric(w_half_c, shape, jac, kern):
+    def mid(col):
+        c = fo.psf_apply(w_half_c, col.reshape(shape))
+        if kern is not None:
+            c = fo.psf_apply(w_half_c, fo.ninv_apply(kern, c))
+        return c.ravel()
+    cj = np.stack([mid(jac[:, i]) for i in range(jac.shape[1])], axis=1)
+    return jac.T @ cj + np.eye(jac.shape[1])
+
+
+def _kernels(w):
+    return (None, fo.noise_kernel_from_psf(w.w_half[0], 1e-2 * float(fo.psf_from_weights(w.w_half[0])[0, 0])))
+
+
+def test_full_model_metric_is_the_dense_jacobian_form_of_sky_full():
+    n = 8
+    w, hyper, xi, th, rng = _problem(n)
+    pts = (np.array([[4, 4], [0, 7]]), 0.5, 0.05 * float(np.median(w.sky_true)))
+    xp = np.array([0.8, -0.4])
+    nx_, nt = xi.size, th.size
+    z0 = np.concatenate([xi.ravel(), th, xp])
+    sky_of = lambda z: po.sky_full(hyper, z[:nx_].reshape(n, n), z[nx_:nx_ + nt], pts, z[nx_ + nt:])[0]  # noqa: E731
+    jac = _dense_jacobian(sky_of, z0)
+    # the point columns of J are the flux derivative at the pixel and nothing else; the diffuse columns do NOT see the fluxes
+    s, s_diff, _ = po.sky_full(hyper, xi, th, pts, xp)
+    assert np.count_nonzero(np.abs(jac[:, nx_ + nt:]) > 1e-9 * np.max(np.abs(jac))) == 2
+    for kern in _kernels(w):
+        dense = _dense_metric(w.w_half[0], (n, n), jac, kern)
+        for i in range(z0.size):
+            e = np.zeros(z0.size)
+            e[i] = 1.0
+            ox, ot, op = po.metric_apply_full(w.w_half[0], hyper, xi, th, pts, xp, e[:nx_].reshape(n, n), e[nx_:nx_ + nt],
+                                              e[nx_ + nt:], True, kern)
+            col = np.concatenate([ox.ravel(), ot, op])
+            assert np.max(np.abs(col - dense[:, i])) <= 1e-6 * np.max(np.abs(dense[:, i])), (i, kern is None)
+    # the pin has teeth: the total sky in place of the diffuse one at the point pixels moves the metric far beyond the bound
+    jbad = jac.copy()
+    for (y, x), st, sd in zip(pts[0], [s[4, 4], s[0, 7]], [s_diff[4, 4], s_diff[0, 7]]):
+        jbad[y * n + x, :nx_ + nt] *= st / sd
+    bad = _dense_metric(w.w_half[0], (n, n), jbad, None)
+    good = _dense_metric(w.w_half[0], (n, n), jac, None)
+    assert np.max(np.abs(bad - good)) > 1e-3 * np.max(np.abs(good))
+
+
+def test_joint_metric_is_the_dense_jacobian_form_of_sky_joint():
+    n = 8
+    w, hyper, xi, th, rng = _problem(n)
+    nx_ = xi.size
+    z0 = np.concatenate([xi.ravel(), th])
+    sky_of = lambda z: po.sky_joint(None, hyper, z[:nx_].reshape(n, n), z[nx_:])[0]  # noqa: E731
+    jac = _dense_jacobian(sky_of, z0)
+    assert np.max(np.abs(jac[:, nx_:])) > 1e-3 * np.max(np.abs(jac))            # the theta columns (the da . xi term) are not small
+    for kern in _kernels(w):
+        dense = _dense_metric(w.w_half[0], (n, n), jac, kern)
+        for i in range(z0.size):
+            e = np.zeros(z0.size)
+            e[i] = 1.0
+            ox, ot = po.metric_apply_joint(w.w_half[0], hyper, xi, th, e[:nx_].reshape(n, n), e[nx_:], True, kern)
+            col = np.concatenate([ox.ravel(), ot])
+            assert np.max(np.abs(col - dense[:, i])) <= 1e-6 * np.max(np.abs(dense[:, i])), (i, kern is None)
+
+
+def test_patch_metric_is_the_dense_jacobian_form_of_sky_patches():
+    w = wl.make_config(1, n=16, seed=4)
+    rng = np.random.default_rng(9)
+    mu = float(np.log(np.median(w.sky_true)))
+    comps = [(w.amp[0], mu - 1.0, 0, 0), (wl.make_config(1, n=8, seed=4).amp[0], mu, 4, 6)]       # the patch overlaps the background
+    xis = [0.3 * rng.normal(size=c[0].shape) for c in comps]
+    sizes = [x.size for x in xis]
+    split = lambda z: [z[:sizes[0]].reshape(xis[0].shape), z[sizes[0]:].reshape(xis[1].shape)]  # noqa: E731
+    z0 = np.concatenate([x.ravel() for x in xis])
+    jac = _dense_jacobian(lambda z: po.sky_patches(comps, split(z), 16, 16)[0], z0)
+    for kern in _kernels(w):
+        dense = _dense_metric(w.w_half[0], (16, 16), jac, kern)
+        for i in range(0, z0.size, 3):                                             # every third unit vector: both components
+            e = np.zeros(z0.size)
+            e[i] = 1.0
+            outs = po.metric_apply_patches(w.w_half[0], 16, 16, comps, xis, split(e), True, kern)
+            col = np.concatenate([o_.ravel() for o_ in outs])
+            assert np.max(np.abs(col - dense[:, i])) <= 1e-6 * np.max(np.abs(dense[:, i])), (i, kern is None)
