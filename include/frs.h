@@ -327,7 +327,10 @@ const char* frs_dot_noalloc_last_error(void);
 long long frs_launch_count(const frs_ctx* ctx);
 /* When enabled, every FFT pass is bracketed by CUDA events on the ctx's stream.  frs_profile_read
  * synchronises and returns accumulated milliseconds and launch counts per pass kind:
- * 0 rows_fwd (conv), 1 conv_cols, 2 rows_inv, 3 rows_fwd (Hartley), 4 hart_cols.  Resets on read. */
+ * 0 rows_fwd (conv), 1 conv_cols, 2 rows_inv, 3 rows_fwd (Hartley), 4 hart_cols.  Resets on read.
+ * While enabled, CG iterations run as plain launches and the latent-space calls use the two separate passes instead of the
+ * fused inverse + Hartley row pass (frs_set_fused_passes), so that every pass has its own bracket: the per-pass times are
+ * those of the unfused sequence, not of the production path (time that one from outside, as bench.py does). */
 int frs_profile_enable(frs_ctx* ctx, int on);
 /* Debug aid (compute-sanitizer is not available on every pool): with the environment variable FRS_GUARD=1 set when
  * frs_create runs, every array the context owns is allocated between two 4 KB guard zones filled with a byte pattern.

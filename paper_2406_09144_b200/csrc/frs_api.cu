@@ -799,7 +799,9 @@ int frs_set_channel_lognu(frs_ctx* ctx, const float* lognu_host) {
 }
 
 int frs_set_sky(frs_ctx* ctx, const float* sky) {
-    if (ctx) ctx->cfg_epoch++;
+    // no epoch bump: what a new sky can change in the launch sequence of a CG iteration -- the orientation that is valid
+    // (sT_ok) and whether point fluxes are in it (pts.in_sky) -- is part of the graph key itself, so a composed model
+    // that calls frs_sky_energy_grad every step keeps its captured iteration
     if (!ctx || !sky || !aligned16(sky)) return fail(ctx, FRS_EINVAL, "frs_set_sky: bad argument");
     CK(cudaSetDevice(ctx->device));
     RET(ensure_scratch(ctx));
@@ -1449,9 +1451,15 @@ int frs_draw_sample(frs_ctx* ctx, const float* eta_xi, const float* eta_d, int m
         ctx->launches++;
     }
     RET(hartley_t(ctx, ctx->acc, ctx->nx, ctx->ny, nullptr, ctx->lat1, ctx->amp, eta_xi, nullptr, ctx->nfield));
-    // sigma = M^-1 m by CG from 0
-    CK(cudaMemsetAsync(sample, 0, (size_t)ctx->nfield * ctx->npix * sizeof(float), ctx->stream));
-    return cg_solve_impl(ctx, ctx->lat1, sample, max_iter, rtol, 1, h_iters, nullptr, nullptr);
+    // sigma = M^-1 m by CG from 0.  The solve runs in a buffer of the context's own and is copied out: the captured CG
+    // iteration is keyed on the solution pointer, and callers hand in a fresh `sample` buffer per draw
+    // (SampleShard.draw), which would re-capture the graph on every sample
+    const size_t nbytes = (size_t)ctx->nfield * ctx->npix * sizeof(float);
+    CK(cudaMemsetAsync(ctx->lat2, 0, nbytes, ctx->stream));
+    const int rc = cg_solve_impl(ctx, ctx->lat1, ctx->lat2, max_iter, rtol, 1, h_iters, nullptr, nullptr);
+    CK(cudaMemcpyAsync(sample, ctx->lat2, nbytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return rc;
 }
 
 int frs_kl_energy_grad(frs_ctx* ctx, const float* xi, const float* samples, int nsamples, int mirrored, double* d_energy,

@@ -238,3 +238,29 @@ def test_a_new_psf_discards_the_fitted_noise_kernel(frs):
         e = ctx.energy_grad(dev(xi), g, with_prior=True)
         e_ref, g_ref = o.energy_grad(2.0 * w.w_half, w.dirty, w.amp, w.mu, w.lognu, xi, True)
         assert abs(e - e_ref) <= TOL * abs(e_ref) and rel(g.cpu().numpy(), g_ref) <= TOL
+
+
+def test_draws_into_fresh_buffers_agree_with_plain_launches(frs):
+    """frs_draw_sample solves in a buffer of the context's own and copies the result out, so a caller that hands in a new
+    `sample` buffer per draw (SampleShard.draw) replays one captured CG iteration instead of re-capturing it per draw; the
+    samples are the same bits as with plain launches."""
+    import torch
+    w = WORKLOADS["c1"]()
+    ctx, eps = setup(frs, w)
+    ctx.set_likelihood(1)
+    rng = np.random.default_rng(77)
+    xi = (0.2 * rng.normal(size=(w.nfield, w.ny, w.nx))).astype(np.float32)
+    ctx.sky_forward(dev(xi))
+    etas = [(dev(rng.normal(size=xi.shape)), dev(rng.normal(size=(w.nchan, w.ny, w.nx)))) for _ in range(3)]
+    graph = []
+    for ex, ed in etas:
+        out = torch.full_like(ex, float("nan"))                                  # a fresh buffer per draw
+        assert ctx.draw_sample(ex, ed, out, 6) == 6
+        graph.append(out)
+    ctx.set_cuda_graphs(False)
+    for (ex, ed), g in zip(etas, graph):
+        out = torch.empty_like(ex)
+        ctx.draw_sample(ex, ed, out, 6)
+        assert torch.equal(out, g)
+    assert not torch.equal(graph[0], graph[1])
+
