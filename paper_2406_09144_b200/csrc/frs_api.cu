@@ -548,7 +548,15 @@ int for_each_position(frs_ctx* ctx, const float* xi, const float* samples, int n
 // =================================================================================================
 extern "C" {
 
-const char* frs_version(void) { return "frs 0.3 (sm_100a; packed-pair register FFT passes: sorting core for the row and Hartley passes, DIF/DIT core for the column convolution)"; }
+#define FRS_STR_(x) #x
+#define FRS_STR(x) FRS_STR_(x)
+const char* frs_version(void) {
+    return "frs 0.3 (sm_100a; packed-pair register FFT passes: sorting core for the row and Hartley passes, DIF/DIT core for the column convolution)"
+#if defined(FRS_STRIP) && FRS_STRIP != 0
+           " ATTRIBUTION BUILD FRS_STRIP=" FRS_STR(FRS_STRIP) ": conv_cols_dif results are wrong by construction"
+#endif
+        ;
+}
 
 const char* frs_last_error(const frs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 

@@ -6,6 +6,18 @@
 // slots the thread has just read, and one exchange of each transform stays inside C neighbouring lanes.  Per
 // column a group passes TWO blocking barriers (eight in the sorting core).  The staging buffer holds columns only
 // (the next one is in flight for a whole column time); the weights come from L2 straight into registers.
+//
+// Attribution builds (profiles/r3_conv_cols_attribution.md): compiling with -DFRS_STRIP=<mask> removes ingredients of this
+// kernel so that the time of what is left can be read; the results are then WRONG by construction (frs_version() says so and
+// bench.py marks its line).  Bits: 1 output stores, 2 weight loads (constant weights), 4 column fetch and its wait (stale
+// staging data), 8 staging reads, 16 the FFT stages (memory skeleton), 32 twist-table loads.  Default 0: the product kernel,
+// token for token.
+#ifndef FRS_STRIP
+#define FRS_STRIP 0
+#endif
+constexpr bool kStripStore = (FRS_STRIP & 1) != 0, kStripWeights = (FRS_STRIP & 2) != 0, kStripFetch = (FRS_STRIP & 4) != 0,
+               kStripStage = (FRS_STRIP & 8) != 0, kStripFft = (FRS_STRIP & 16) != 0, kStripTwist = (FRS_STRIP & 32) != 0;
+
 template <int NF> struct ColsDifGeo {
     using D = Dif<NF>;
     static constexpr int P = D::P;
@@ -39,6 +51,7 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
     // twist^n for the thread's samples n = t + e P, from the exactly rounded table.  Only its first half is read
     // (twist^(NF-m) = -conj twist^m), so that it stays resident in the few KB of L1 this kernel leaves
     auto twist_e = [&](int e) {
+        if (kStripTwist) return make_float2(0.6f + 1e-3f * (float)e, 0.8f);
         if (e < kE / 2) return __ldg(a.twist + t + e * P);
         const float2 c = __ldg(a.twist + (NF - e * P) - t);
         return make_float2(-c.x, c.y);
@@ -55,9 +68,10 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
     // (one bulk prefetch) and read from there straight into registers, so that the staging buffer belongs to the
     // columns alone and the NEXT column is in flight for a whole column time
     auto prefetch_weights = [&](const void* src, bool live) {
-        if (t == 0 && live) bulk_prefetch_l2(src, NF * 8);
+        if (t == 0 && live && !kStripWeights) bulk_prefetch_l2(src, NF * 8);
     };
     auto fetch_column = [&](int b, int kx, bool live) {          // column kx lands as NF contiguous samples
+        if (kStripFetch) return;
         if (t == 0 && live) {
             fence_proxy_async();
             mbar_expect_tx(bar, NF * 8);
@@ -81,18 +95,18 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
 
         C2 v[kE];
         if (live) {
-            mbar_wait(bar, parity);
+            if (!kStripFetch) mbar_wait(bar, parity);
             parity ^= 1u;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 x = stage[t + e * P];
+                const float2 x = kStripStage ? make_float2(1e-3f * (float)(t + e), 1.0f - 1e-3f * (float)item) : stage[t + e * P];
                 v[e] = c2make(x, cmul(x, twist_e(e)));                 // even bins: x, odd bins: x twist^n
             }
         } else {
 #pragma unroll
             for (int e = 0; e < kE; ++e) v[e] = c2zero();
         }
-        dif_fwd_0<NF>(v, t, X, tws);
+        if (!kStripFft) dif_fwd_0<NF>(v, t, X, tws);
         gb.sync();                                  // X1 written; and every thread has picked up its samples:
         {                                           // the next column may land
             bool nlive; int nb_, nkx; const float* nw;
@@ -100,24 +114,31 @@ conv_cols_dif_kernel(const __grid_constant__ ConvColsArgs a) {
             fetch_column(nb_, nkx, nlive);
             prefetch_weights(nw, nlive);
         }
-        dif_fwd_1<NF>(v, t, X, tws);
-        dif_warp_sync();
-        dif_fwd_2<NF>(v, t, X);
+        if (!kStripFft) {
+            dif_fwd_1<NF>(v, t, X, tws);
+            dif_warp_sync();
+            dif_fwd_2<NF>(v, t, X);
+        }
         if (live) {
             const float* wp = w + 2 * t;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
-                const float2 ww = ldg2(wp + 2 * e * P);               // (even-bin weight, odd-bin weight) of register e
+                const float2 ww = kStripWeights ? make_float2(1.0001f, 0.9999f - 1e-4f * (float)e)
+                                                : ldg2(wp + 2 * e * P);   // (even-bin weight, odd-bin weight) of register e
                 v[e].re = f2mul(v[e].re, ww);
                 v[e].im = f2mul(v[e].im, ww);
             }
         }
-        dif_inv_0<NF>(v, t, X);
-        dif_warp_sync();
-        dif_inv_1<NF>(v, t, X, tws);
+        if (!kStripFft) {
+            dif_inv_0<NF>(v, t, X);
+            dif_warp_sync();
+            dif_inv_1<NF>(v, t, X, tws);
+        }
         gb.sync();
-        dif_inv_2<NF>(v, t, X, tws);
-        if (live) {
+        if (!kStripFft) dif_inv_2<NF>(v, t, X, tws);
+        // without the stores the condition is still evaluated at run time (ncols is never negative), so that what
+        // feeds them cannot be optimised away
+        if (live && (!kStripStore || a.ncols < 0)) {
             float2* col = a.out + ((size_t)b * 2 * a.ntile + kx) * NF + t;
 #pragma unroll
             for (int e = 0; e < kE; ++e) {
